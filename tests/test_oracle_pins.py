@@ -1,0 +1,338 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix.
+
+None of these compares the oracle with itself or with the CUDA path: every expected value is a closed form, an
+invariant, a brute-force recomputation written differently (numpy all-pairs), or the paper's worked example.
+"""
+import numpy as np
+import pytest
+
+from conftest import golden
+from lsm_inputs import FIXED, MOVE, config1, triangular_lattice, two_phase_spring_params, blob_image
+from lsm_inputs.generators import SQ3_2
+from oracle.olsm import OracleSim
+
+
+def _two_particles(x1, k, r0, rc, dt, gamma=0.0, m=1.0, fix0=True, sample_every=0):
+    x = np.array([[0.0, 0.0], [x1, 0.0]])
+    s = OracleSim(x, [0], [1], [k], [r0], [rc], dt, gamma, mass=m, sample_every=sample_every)
+    if fix0:
+        s.set_boundary(0, [0], FIXED)
+    return s
+
+
+def test_P1_paper_oscillator_example():
+    """fixed end + free end, closed-form Verlet trajectory and analytic ODE solution."""
+    g = golden("paper_sho_example.txt")
+    s = _two_particles(g["x0"], g["k"], g["r0"], 100.0, g["dt"], m=g["m"])
+    th = np.arccos(1.0 - g["k"] * g["dt"] ** 2 / (2.0 * g["m"]))
+    w = np.sqrt(g["k"] / g["m"])
+    err_cf, err_an = 0.0, 0.0
+    for n in range(1, int(g["n_steps"]) + 1):
+        s.step(1)
+        x, v = s.read_state()
+        assert x[0, 0] == 0.0 and x[0, 1] == 0.0 and x[1, 1] == 0.0
+        amp = g["x0"] - g["r0"]
+        err_cf = max(err_cf, abs(x[1, 0] - (g["r0"] + amp * np.cos(n * th))))
+        if n % int(g["output_every"]) == 0:
+            err_an = max(err_an, abs(x[1, 0] - (g["r0"] + amp * np.cos(w * n * g["dt"]))))
+    assert err_cf <= 1e-11
+    assert err_an <= 2e-4            # "accurate ... without error accumulation" (L127)
+    assert abs(x[1, 0] - 5.804755697) < 1e-8
+
+
+def test_P1_velocity_closed_form():
+    """Full-step velocity of velocity Verlet on a linear spring: v_n = -(A sin(theta)/dt) sin(n theta)."""
+    k, r0, dt = 1e-4, 10.0, 1.0
+    s = _two_particles(15.0, k, r0, 100.0, dt)
+    th = np.arccos(1.0 - k * dt * dt / 2.0)
+    for n in range(1, 400):
+        s.step(1)
+        _, v = s.read_state()
+        assert abs(v[1, 0] + 5.0 * np.sin(th) / dt * np.sin(n * th)) < 1e-12
+
+
+def test_P2_two_free_particles_reduced_mass():
+    """Period 2 pi sqrt(m_red/k) (north_star closed form): separation = r0 + A cos(n theta2), COM at rest."""
+    k, r0, dt, m = 1e-4, 10.0, 1.0, 1.0
+    s = _two_particles(15.0, k, r0, 100.0, dt, fix0=False, m=m)
+    mred = m / 2.0
+    th2 = np.arccos(1.0 - (k / mred) * dt * dt / 2.0)
+    assert abs(2 * np.pi / th2 * dt - 2 * np.pi * np.sqrt(mred / k)) < 2e-3 * 444.288   # discrete vs continuous period
+    for n in range(1, 1001):
+        s.step(1)
+        x, v = s.read_state()
+        assert abs((x[1, 0] - x[0, 0]) - (r0 + 5.0 * np.cos(n * th2))) <= 1e-11
+        assert abs(0.5 * (x[1, 0] + x[0, 0]) - 7.5) <= 1e-12
+        assert abs(v[0, 0] + v[1, 0]) <= 1e-15
+
+
+@pytest.mark.parametrize("eps", [1e-3, 1e-5])
+def test_P3_affine_uniaxial_stress_state(eps):
+    """Young's modulus 2k/sqrt(3) and Poisson's ratio 1/3 of the triangular lattice (north_star), exact finite-strain
+    forms: under x -> x(1-eps/3), y -> y(1+eps) interior forces vanish and each interior top-row particle carries
+    f_y = -2 k (L - r0)/L * (sqrt3/2)(1+eps) r0 with L = r0 sqrt((1-eps/3)^2/4 + 3(1+eps)^2/4)."""
+    nx = ny = 64
+    kk = 1.7
+    x, si, sj, site, kind = triangular_lattice(nx, ny)
+    xa = x * np.array([1.0 - eps / 3.0, 1.0 + eps])
+    M = si.size
+    s = OracleSim(xa, si, sj, np.full(M, kk), np.ones(M), np.full(M, 2.0), 0.01)
+    f = s.read_forces()
+    row, col = site // nx, site % nx
+    interior = (row > 0) & (row < ny - 1) & (col > 0) & (col < nx - 1)
+    L = np.sqrt((1 - eps / 3) ** 2 / 4 + 3 * (1 + eps) ** 2 / 4)
+    fmag_d = kk * (L - 1.0)          # force magnitude of one diagonal spring
+    # Poisson's ratio 1/3: lateral contraction eps/3 leaves interior particles force-free to first order; the exact
+    # residual is second order in eps and cancels by symmetry -> zero to rounding
+    # (rounding: coordinates up to 64 carry ulp 1.4e-14, so differences carry that absolute error times k)
+    assert np.abs(f[interior]).max() <= 8 * np.finfo(float).eps * np.abs(xa).max() * kk < 1e-7 * fmag_d
+    top_int = (row == ny - 1) & (col > 0) & (col < nx - 1)
+    fy_expect = -2.0 * fmag_d / L * SQ3_2 * (1 + eps)
+    assert np.allclose(f[top_int, 1], fy_expect, rtol=1e-9 / max(eps / 1e-5, 1), atol=0)
+    # E = 2k/sqrt3 per unit thickness: stress per unit width / strain -> 2k/sqrt3 as eps -> 0
+    E_lat = -fy_expect / eps
+    assert abs(E_lat / (2 * kk / np.sqrt(3)) - 1) < 2 * eps
+    # energy (Eq. 1): n_h horizontal springs stretched by -eps/3, n_d diagonal springs of length L
+    n_h, n_d = ny * (nx - 1), (ny - 1) * (2 * nx - 1)
+    assert (kind == 0).sum() == n_h and (kind != 0).sum() == n_d
+    U, _ = s.read_energy()
+    U_expect = 0.5 * kk * (n_h * (eps / 3) ** 2 + n_d * (L - 1.0) ** 2)
+    assert abs(U[0] / U_expect - 1) < 1e-9
+
+
+def _random_state(nx, ny, seed, amp=0.05):
+    x, si, sj, site, kind = triangular_lattice(nx, ny)
+    rng = np.random.default_rng(seed)
+    x = x + rng.uniform(-amp, amp, x.shape)
+    M = si.size
+    k = rng.uniform(0.5, 2.0, M)
+    r0 = rng.uniform(0.9, 1.1, M)
+    return x, si, sj, k, r0
+
+
+def test_P4_zero_net_force_and_torque():
+    x, si, sj, k, r0 = _random_state(24, 20, 1)
+    s = OracleSim(x, si, sj, k, r0, np.full(si.size, 5.0), 0.01)
+    f = s.read_forces()
+    # scale: sum of |contributions|
+    d = x[sj] - x[si]
+    r = np.linalg.norm(d, axis=1)
+    scale = 2 * np.sum(np.abs(k * (r - r0)))
+    assert np.abs(f.sum(axis=0)).max() <= 1e-13 * scale
+    torque = np.sum(x[:, 0] * f[:, 1] - x[:, 1] * f[:, 0])
+    assert abs(torque) <= 1e-13 * scale * np.abs(x).max()
+
+
+@pytest.mark.parametrize("nx,ny", [(4, 3), (8, 8), (5, 7)])
+def test_P5_brute_force_all_pairs(nx, ny):
+    """O(N^2) recomputation: every particle pair whose INITIAL distance is r0 (within 1e-9) is a spring."""
+    x0, si, sj, _, _ = triangular_lattice(nx, ny)
+    N = x0.shape[0]
+    rng = np.random.default_rng(nx * 100 + ny)
+    x = x0 + rng.uniform(-0.08, 0.08, x0.shape)
+    kk = 1.3
+    s = OracleSim(x, si, sj, np.full(si.size, kk), np.ones(si.size), np.full(si.size, 9.0), 0.01)
+    f = s.read_forces()
+    fb = np.zeros_like(x)
+    npairs = 0
+    for a in range(N):
+        for b in range(N):
+            if a == b or abs(np.hypot(*(x0[a] - x0[b])) - 1.0) > 1e-9:
+                continue
+            npairs += 1
+            rab = np.hypot(*(x[a] - x[b]))
+            fb[a] += -kk * (rab - 1.0) * (x[a] - x[b]) / rab      # Eq. 2 as printed (L55)
+    assert npairs == 2 * si.size
+    assert np.abs(f - fb).max() <= 1e-14
+
+
+def test_P6_energy_conservation_and_scaling():
+    """gamma=0, grips FIXED, 1 % affine pre-stretch released: |dE/E0| < 1e-8 over 10^4 steps at dt = 1e-3;
+    fluctuation scales as dt^2 (halving dt divides it by 4)."""
+    nx = ny = 32
+    x, si, sj, site, _ = triangular_lattice(nx, ny)
+    row = site // nx
+    M = si.size
+    xa = x * np.array([1.0, 1.01])
+    def run(dt, nsteps, every):
+        s = OracleSim(xa, si, sj, np.ones(M), np.ones(M), np.full(M, 2.0), dt)
+        s.set_boundary(0, np.flatnonzero(row == 0), FIXED)
+        s.set_boundary(1, np.flatnonzero(row == ny - 1), FIXED)
+        U, KE = s.read_energy(); E0 = U[0] + KE[0]; dev = 0.0
+        for _ in range(nsteps // every):
+            s.step(every)
+            U, KE = s.read_energy()
+            dev = max(dev, abs(U[0] + KE[0] - E0) / E0)
+        return dev
+    d1 = run(1e-3, 10000, 100)
+    assert d1 < 1e-8
+    d_a, d_b = run(0.02, 2000, 10), run(0.01, 4000, 20)
+    assert 3.6 < d_a / d_b < 4.4
+
+
+def test_P6_momentum_conservation_free_lattice():
+    x, si, sj, k, r0 = _random_state(16, 16, 7)
+    rng = np.random.default_rng(3)
+    v = rng.normal(0, 0.01, x.shape)
+    s = OracleSim(x, si, sj, k, r0, np.full(si.size, 9.0), 0.01, v=v)
+    p0 = v.sum(axis=0)
+    s.step(2000)
+    _, v1 = s.read_state()
+    assert np.abs(v1.sum(axis=0) - p0).max() <= 1e-13
+
+
+def test_P7_strict_greater_than_dyadic():
+    """Q1: r == rc exactly survives; all numbers dyadic so every operation is exact."""
+    x = np.array([[0.0, 0.0], [1.0, 0.0]])
+    s = OracleSim(x, [0], [1], [1.0], [1.0], [1.0 + 2.0 ** -3], 1.0)
+    s.set_boundary(0, [0], FIXED)
+    s.set_boundary(1, [1], MOVE, [2.0 ** -10, 0.0])
+    s.step(128)
+    xx, _ = s.read_state()
+    assert xx[1, 0] == 1.125
+    b, bs, nb = s.read_broken()
+    assert nb == 0 and not b[0] and bs[0] == -1
+    assert s.read_forces()[1, 0] == -0.125 / 1.125 * 1.125       # -k (r - r0) (x1-x0)/r
+    s.step(1)
+    b, bs, nb = s.read_broken()
+    assert nb == 1 and b[0] and bs[0] == 129
+    assert np.all(s.read_forces() == 0.0)
+
+
+def test_P8_irreversible_breakage():
+    """Q2/Q3/Q18: once broken, force and energy stay zero even when r drops below rc again."""
+    x = np.array([[0.0, 0.0], [1.0, 0.0]])
+    s = OracleSim(x, [0], [1], [1.0], [1.0], [1.25], 1.0, sample_every=1)
+    s.set_boundary(0, [0], FIXED)
+    s.set_boundary(1, [1], MOVE, [0.0625, 0.0])
+    s.step(6)                                  # r = 1.375 > 1.25 -> broke at step 5 (1.3125)
+    b, bs, nb = s.read_broken()
+    assert nb == 1 and bs[0] == 5
+    s.set_boundary(1, [1], MOVE, [-0.0625, 0.0])
+    s.step(6)                                  # back to r = 1.0
+    xx, _ = s.read_state()
+    assert xx[1, 0] == 1.0
+    assert np.all(s.read_forces() == 0.0)
+    U, _ = s.read_energy()
+    assert U[0] == 0.0
+    h = s.read_stress()
+    assert list(h["n_broken"][:, 0]) == [0, 0, 0, 0, 1, 1, 1, 1, 1, 1, 1, 1]
+    assert np.all(h["U"][4:, 0] == 0.0) and h["U"][3, 0] == 0.5 * 0.25 ** 2
+
+
+def test_P9_time_reversibility():
+    """PAPER.md:L76 claims time reversibility: n steps, v -> -v, n steps returns to the start."""
+    x, si, sj, k, r0 = _random_state(16, 16, 11, amp=0.03)
+    s = OracleSim(x, si, sj, k, r0, np.full(si.size, 9.0), 0.01)
+    s.step(1000)
+    x1, v1 = s.read_state()
+    s2 = OracleSim(x1, si, sj, k, r0, np.full(si.size, 9.0), 0.01, v=-v1)
+    s2.step(1000)
+    x2, v2 = s2.read_state()
+    assert np.abs(x2 - x).max() <= 1e-10
+    assert np.abs(v2).max() <= 1e-10
+
+
+def test_P10_force_is_minus_grad_U():
+    x, si, sj, k, r0 = _random_state(8, 8, 5)
+    rc = np.full(si.size, 9.0)
+    f = OracleSim(x, si, sj, k, r0, rc, 0.01).read_forces()
+    h = 1e-6
+    rng = np.random.default_rng(0)
+    for _ in range(24):
+        p, c = rng.integers(x.shape[0]), rng.integers(2)
+        xp, xm = x.copy(), x.copy()
+        xp[p, c] += h; xm[p, c] -= h
+        Up = OracleSim(xp, si, sj, k, r0, rc, 0.01).read_energy()[0][0]
+        Um = OracleSim(xm, si, sj, k, r0, rc, 0.01).read_energy()[0][0]
+        assert abs(-(Up - Um) / (2 * h) - f[p, c]) <= 1e-7 * max(1.0, abs(f[p, c]))
+
+
+def test_P12_damping_closed_form():
+    """Q7: with c = gamma dt/m the step reduces to u_{n+2} - (2 - c - w^2 dt^2) u_{n+1} + (1 - c) u_n = 0."""
+    m = k = r0 = 1.0
+    dt, gamma, u0 = 0.01, 0.01, 0.05
+    s = _two_particles(r0 + u0, k, r0, 10.0, dt, gamma=gamma, m=m)
+    c, w2 = gamma * dt / m, k / m * dt * dt
+    rho = np.sqrt(1 - c)
+    cphi = (2 - c - w2) / (2 * rho)
+    phi = np.arccos(cphi)
+    A, u1 = u0, u0 * (1 - w2 / 2)
+    B = (u1 / rho - A * cphi) / np.sin(phi)
+    err = 0.0
+    for blk in range(100):
+        s.step(100)
+        n = (blk + 1) * 100
+        x, _ = s.read_state()
+        err = max(err, abs((x[1, 0] - r0) - rho ** n * (A * np.cos(n * phi) + B * np.sin(n * phi))))
+    assert err <= 1e-11
+    assert abs(rho ** 10000 - np.exp(-gamma * 100.0 / (2 * m))) < 2e-5
+
+
+def test_boundary_reaction_and_sampling_static():
+    """Reaction sums R_g = sum of spring forces on the group's particles (north_star item 4): static affine state,
+    R_top,y = -R_bot,y = sum over top-row particles of the closed-form per-particle force (edge particles differ)."""
+    nx = ny = 16
+    eps = 1e-3
+    x, si, sj, site, _ = triangular_lattice(nx, ny)
+    xa = x * np.array([1.0 - eps / 3, 1.0 + eps])
+    M = si.size
+    row = site // nx
+    s = OracleSim(xa, si, sj, np.ones(M), np.ones(M), np.full(M, 2.0), 1e-3, gamma=0.0, sample_every=1)
+    s.set_boundary(0, np.flatnonzero(row == 0), FIXED)
+    s.set_boundary(1, np.flatnonzero(row == ny - 1), FIXED)
+    s.step(1)
+    h = s.read_stress()
+    L = np.sqrt((1 - eps / 3) ** 2 / 4 + 3 * (1 + eps) ** 2 / 4)
+    n_diag_top = 2 * nx - 1                      # diagonal/vertical springs hanging from the top row
+    fy = -(L - 1.0) / L * SQ3_2 * (1 + eps)
+    # the interior moved by O(eps^2 dt^2): reaction equals the static value to ~1e-9 relative
+    assert abs(h["R"][0, 0, 1, 1] / (n_diag_top * fy) - 1) < 1e-6
+    assert abs(h["R"][0, 0, 0, 1] / (-n_diag_top * fy) - 1) < 1e-6
+    assert h["step"][0] == 1
+
+
+def test_batched_equals_individual():
+    """Batched layout (a9): a disjoint union evolves each specimen exactly as it evolves alone."""
+    from lsm_inputs import config4, single_specimen
+    pb = config4(B=3, n=16)
+    sb = OracleSim.from_problem(pb, sample_every=50)
+    sb.step(200)
+    xb, vb = sb.read_state()
+    hb = sb.read_stress()
+    for b in range(3):
+        p1 = single_specimen(b, 16)
+        s1 = OracleSim.from_problem(p1, sample_every=50)
+        s1.step(200)
+        x1, v1 = s1.read_state()
+        sl = slice(pb.particle_offsets[b], pb.particle_offsets[b + 1])
+        assert np.array_equal(xb[sl], x1) and np.array_equal(vb[sl], v1)
+        h1 = s1.read_stress()
+        assert np.array_equal(hb["U"][:, b], h1["U"][:, 0]) and np.array_equal(hb["R"][:, b], h1["R"][:, 0])
+
+
+def test_config1_reference_values():
+    """SURVEY.md S2 (an independent numpy scratch run of config 1 at survey time): no breakage in 10^4 steps,
+    sigma_top = 1.742e-2, sigma_bot = 2.208e-2, U = 0.7073, KE = 0.0278 at step 10^4."""
+    p = config1()
+    s = OracleSim.from_problem(p)
+    s.step(10000)
+    h = s.read_stress()
+    assert h["n_broken"][-1, 0] == 0
+    assert abs(-h["R"][-1, 0, 1, 1] / p.meta["W0"] - 1.742e-2) < 5e-6
+    assert abs(h["R"][-1, 0, 0, 1] / p.meta["W0"] - 2.208e-2) < 5e-6
+    assert abs(h["U"][-1, 0] - 0.7073) < 5e-5 and abs(h["KE"][-1, 0] - 0.0278) < 5e-5
+
+
+def test_generators_match_paper_shapes():
+    g = golden("paper_table1_table2.txt")
+    lo, hi = g["t2_springs_min"] / g["t2_particles_min"], g["t2_springs_max"] / g["t2_particles_max"]
+    p = config1()
+    assert p.M == 64 * 63 + 63 * 127 == 12033
+    assert lo - 0.1 < p.M / p.N < 3.0                      # Table 2: M/N = 2.885 .. 2.941
+    deg = np.bincount(np.concatenate([p.spring_i, p.spring_j]), minlength=p.N)
+    assert deg.max() == 6 and (deg == 6).sum() == 3844     # "six springs"
+    d = np.linalg.norm(p.x[p.spring_j] - p.x[p.spring_i], axis=1)
+    assert np.abs(d - 1.0).max() < 1e-14
+    # Table 1: rc/r0 between 1.01 and 1.10; the synthetic configs stay in a comparable range
+    assert 1.0 < g["t1_stiff_rc"] / g["t1_stiff_r0"] < p.rc[0] / p.r0[0] + 1e-12 <= g["t1_soft_rc"] / g["t1_soft_r0"] + 1e-12
