@@ -1,0 +1,156 @@
+/* lsm.h -- C ABI of the B200-native lattice-spring-model (LSM) step library, liblsm_b200.so.
+ *
+ * What it is: the hot path of CuLSM (arXiv 2201.04565, "ImageMech"): one time step of a bonded particle-spring
+ * network, parallelised over the spring list, i.e.
+ *   (1) truncated-harmonic spring forces  F_i = -sum_j k (r_ij - r0_ij) (r_i - r_j)/|r_i - r_j|   (Eq. 2)
+ *   (2) the irreversible breakage test    r_ij > r_c  => the spring is dead for good
+ *   (3) velocity Verlet in half-step-velocity form with fixed / displacement-controlled boundary rows
+ *                                                                                    (Eq. 3-5)
+ *   (4) device-side reductions: boundary reaction force, elastic energy U (Eq. 1), kinetic energy,
+ *       broken-spring count (the paper sums U and KE on the CPU, and names "parallel reduction" as
+ *       future work, L198).
+ * Everything between lsm_create and lsm_read_* runs in hand-written CUDA kernels for sm_100a.  There is no CPU
+ * fallback: without a CUDA device every compute entry point returns LSM_E_CUDA.
+ *
+ * Conventions
+ *   - plain C; no exceptions or C++ types cross the boundary; every function returns lsm_status unless noted.
+ *   - dim = 2 only (all configurations of the paper and of BASELINE.json are 2-D; the paper's listing is 3-D AoS,
+ *     PAPER.md:L93-L97 -> LSM_E_UNSUPPORTED for dim = 3 in this round).
+ *   - HOST pointers unless a parameter says DEVICE.  Vector arrays are interleaved [N*dim] (x0 y0 x1 y1 ...) as in the
+ *     paper's flattened 1-D arrays.  Inputs are borrowed for the duration of the call and copied;
+ *     outputs are caller-allocated buffers of the documented size.  The handle owns all device memory.
+ *   - particle ids / spring ids seen by the caller are ALWAYS the caller's own numbering, whatever renumbering
+ *     (`reorder`) or compaction the library applies internally.
+ *   - lsm_step only enqueues work on `stream`; lsm_read_* and lsm_sync synchronise it.  Errors are sticky: after a
+ *     failure every later call on the handle returns the same code; lsm_last_error gives the text.
+ *   - one handle may be used by one host thread at a time.
+ */
+#ifndef LSM_B200_H
+#define LSM_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LSM_MAX_GROUPS 8
+#define LSM_ABI_VERSION 1
+
+typedef struct lsm_sim lsm_sim; /* opaque */
+
+typedef enum {
+    LSM_OK = 0,
+    LSM_E_INVALID = -1,     /* null pointer, bad enum, n < 0, dt <= 0, gamma < 0, wrong struct_size               */
+    LSM_E_RANGE = -2,       /* spring endpoint outside [0,N), i == j, spring crossing two specimens, bad group id  */
+    LSM_E_NONFINITE = -3,   /* NaN/Inf in x, v, m, k, r0, rc; m <= 0; r0 <= 0; k < 0; rc <= 0                      */
+    LSM_E_CUDA = -4,        /* CUDA runtime error, or no CUDA device                                               */
+    LSM_E_NOMEM = -5,       /* host or device allocation failed                                                    */
+    LSM_E_STATE = -6,       /* the simulation failed earlier (e.g. non-finite energy detected on the device)       */
+    LSM_E_UNSUPPORTED = -7  /* dim = 3, reorder = 2 (RCM), exact arithmetic with the scatter kernel                */
+} lsm_status;
+
+enum { LSM_FIXED = 0, LSM_MOVE = 1 };                      /* boundary group modes */
+enum { LSM_FORCE_AUTO = 0, LSM_FORCE_SCATTER = 1, LSM_FORCE_GATHER = 2 };
+enum { LSM_REORDER_NONE = 0, LSM_REORDER_MORTON = 1, LSM_REORDER_RCM = 2 };
+
+/* Optional device allocator (the Python binding passes PyTorch's caching allocator). */
+typedef void *(*lsm_alloc_fn)(size_t bytes, void *user);  /* returns a DEVICE pointer, NULL on failure */
+typedef void (*lsm_free_fn)(void *dptr, void *user);
+
+typedef struct lsm_desc {
+    uint32_t struct_size;             /* = sizeof(lsm_desc): ABI check                                           */
+    int32_t dim;                      /* 2                                                                        */
+    int64_t n_particles, n_springs;   /* N >= 1, M >= 0, both < 2^31 - 1                                          */
+    int32_t n_batch;                  /* B >= 1 independent specimens stored as one disjoint union                */
+    int32_t _pad0;
+    const int64_t *particle_offsets;  /* [B+1] ascending, [0] = 0, [B] = N; NULL allowed when B == 1              */
+    const int64_t *spring_offsets;    /* [B+1]; springs of specimen b are [off[b], off[b+1]) and join its own
+                                         particles only                                                          */
+    const double *x;                  /* [N*dim] initial positions                                                */
+    const double *v;                  /* [N*dim] initial velocities, NULL = zeros                                 */
+    const double *mass;               /* [N] or NULL -> mass_uniform ("particle masses ... by type") */
+    double mass_uniform;
+    const int32_t *spring_i, *spring_j; /* [M] endpoints, the paper's atom_i / atom_j          */
+    const double *k, *r0, *rc;        /* [M] stiffness, rest length, breaking LENGTH (absolute, Table 1
+                                         PAPER.md:L137-L141); a NULL pointer takes the *_uniform scalar          */
+    double k_uniform, r0_uniform, rc_uniform;
+    double dt, gamma;                 /* time step; viscous damping coefficient (force -gamma*v, Q7)    */
+    int32_t sample_every;             /* record {step, R_g, U, KE, n_broken} when step % sample_every == 0; 0 off */
+    int32_t history_capacity;         /* samples kept in the device ring (0 -> 1024); oldest overwritten          */
+    int32_t compact_every;            /* drop dead springs from the device lists every this many steps; 0 never   */
+    int32_t reorder;                  /* LSM_REORDER_*: internal particle renumbering for gather locality         */
+    int32_t force_mode;               /* LSM_FORCE_*: AUTO = GATHER                                               */
+    int32_t exact;                    /* 1: IEEE sqrt/divide, no FMA contraction, each particle sums its springs in
+                                         ascending caller spring id -> bit-identical to a serial loop over the
+                                         spring list (GATHER only).  0: fast arithmetic (FMA, rsqrt)              */
+    int32_t use_graph;                /* 1: replay the step loop from CUDA graphs (small, launch-bound problems)  */
+    int32_t device;                   /* CUDA device ordinal                                                      */
+    void *stream;                     /* cudaStream_t, NULL = the default stream                                  */
+    lsm_alloc_fn alloc;               /* NULL -> cudaMalloc / cudaFree                                            */
+    lsm_free_fn free_;
+    void *alloc_user;
+} lsm_desc;
+
+/* Layout / traffic facts about a handle (for benchmarks and tests). */
+typedef struct lsm_info {
+    int64_t n_particles, n_springs;
+    int64_t n_half_edges_stored;      /* gather: ELL slots incl. padding; scatter: list length                    */
+    int64_t bytes_per_half_edge;      /* id + parameter bytes read per stored slot                                */
+    int32_t param_mode;               /* 0 uniform, 1 typed (1 B), 2 k,r0 uniform + rc fp64, 3 k,r0 typed + rc fp64,
+                                         4 k, r0, rc all fp64                                                     */
+    int32_t n_types;
+    int32_t force_mode, exact, reorder, n_batch;
+    int64_t device_bytes;             /* device memory owned by the handle                                        */
+    int64_t kernels_launched;         /* cumulative count of kernels this handle enqueued                         */
+    int64_t current_step;
+} lsm_info;
+
+/* Build a simulation from particle / spring arrays.  Copies everything (the caller may free its inputs afterwards),
+ * validates, renumbers, builds the device layout, evaluates forces once at step 0 (so f, U are defined and a spring
+ * already longer than rc is broken at step 0).  On failure *out = NULL and lsm_last_error(NULL) has the reason. */
+lsm_status lsm_create(const lsm_desc *desc, lsm_sim **out);
+
+/* Define boundary group `group` in [0, LSM_MAX_GROUPS): its particles become kinematic from now on
+ * (never integrated; position = position at this call + (steps since this call) * disp_per_step; FIXED ignores
+ * disp_per_step).  particle_ids: [n] caller numbering; a particle may be in at most one group.  Calling it again for
+ * the same group releases the old members first.  ("boundary displacements are first applied".) */
+lsm_status lsm_set_boundary(lsm_sim *sim, int32_t group, const int32_t *particle_ids, int64_t n, int32_t mode,
+                            const double *disp_per_step /* [dim] */);
+
+/* Advance n_steps velocity-Verlet steps (kick - drift - force+breakage - kick).  Asynchronous. */
+lsm_status lsm_step(lsm_sim *sim, int64_t n_steps);
+
+/* Overwrite positions and velocities (restart / perturbation); forces are re-evaluated at the current step and
+ * kinematic particles take the new position as their origin.  v NULL = zeros. */
+lsm_status lsm_write_state(lsm_sim *sim, const double *x, const double *v);
+
+lsm_status lsm_read_state(lsm_sim *sim, double *x /* [N*dim] or NULL */, double *v /* [N*dim] or NULL */);
+/* Spring force on every particle at the current positions (no damping term). */
+lsm_status lsm_read_forces(lsm_sim *sim, double *f /* [N*dim] */);
+/* broken[s] = 1 if spring s is dead; break_step[s] = step of the force evaluation that broke it, -1 if alive. */
+lsm_status lsm_read_broken(lsm_sim *sim, uint8_t *broken /* [M] or NULL */, int64_t *break_step /* [M] or NULL */,
+                           int64_t *n_broken /* scalar or NULL */);
+/* Per-specimen energies of the current state: U (Eq. 1) and KE of the free particles. */
+lsm_status lsm_read_energy(lsm_sim *sim, double *U /* [B] or NULL */, double *KE /* [B] or NULL */);
+/* Copy out (and clear) the samples recorded since the last call, oldest first, at most `capacity`:
+ * step[n], reaction[n][B][LSM_MAX_GROUPS][dim] (raw sums of spring forces over each group's particles; the caller
+ * divides by a cross-section to get stress), U[n][B], KE[n][B], n_broken[n][B] (cumulative).  NULL outputs skipped. */
+lsm_status lsm_read_stress(lsm_sim *sim, int64_t capacity, int64_t *n_samples, int64_t *step, double *reaction,
+                           double *U, double *KE, int64_t *n_broken);
+
+/* Drop dead springs from the device lists now (also done every compact_every steps). Results never change. */
+lsm_status lsm_compact(lsm_sim *sim);
+lsm_status lsm_sync(lsm_sim *sim);
+lsm_status lsm_get_info(lsm_sim *sim, lsm_info *info);
+/* Device pointers of the current state in INTERNAL numbering, for zero-copy consumers (may change after lsm_step). */
+lsm_status lsm_device_state(lsm_sim *sim, const double **pos_xy /* DEVICE [N*2] */, const double **vel_xy);
+const char *lsm_last_error(const lsm_sim *sim); /* sim NULL: error of the last failed lsm_create on this thread */
+void lsm_destroy(lsm_sim *sim);
+int32_t lsm_abi_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LSM_B200_H */

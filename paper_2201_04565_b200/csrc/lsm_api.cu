@@ -1,0 +1,841 @@
+// lsm_api.cu -- host side of liblsm_b200.so: the C ABI of include/lsm.h.
+// Validation, renumbering (a8), layout construction, the step loop (launch sequencing / CUDA graphs), sampling ring,
+// compaction scheduling, numbering translation at the boundary.  All arithmetic of the method runs in the kernels of
+// lsm_kernels.cuh; nothing here computes a force or integrates.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <unordered_map>
+#include <vector>
+
+#include "../../include/lsm.h"
+#include "lsm_kernels.cuh"
+
+using namespace lsmk;
+
+static thread_local std::string g_create_error;
+
+namespace {
+
+struct Group {
+    bool set = false;
+    int mode = 0;
+    double du[2] = {0, 0};
+    long long n0 = 0;
+    std::vector<int32_t> ids;  // internal ids, sorted
+    int32_t *d_ids = nullptr;
+    long long *d_seg = nullptr;  // [B+1]
+};
+
+}  // namespace
+
+struct lsm_sim {
+    // configuration
+    long long N = 0, M = 0;
+    int B = 1;
+    double dt = 0, gamma = 0, mass_u = 1;
+    int sample_every = 0, hist_cap = 1024, compact_every = 0, reorder = 0, force_mode = LSM_FORCE_GATHER, exact = 0, use_graph = 0;
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    lsm_alloc_fn alloc = nullptr;
+    lsm_free_fn free_ = nullptr;
+    void *alloc_user = nullptr;
+    std::vector<void *> dev_allocs;
+    long long device_bytes = 0;
+    // numbering
+    std::vector<int32_t> perm, inv;  // internal -> caller, caller -> internal (empty = identity)
+    std::vector<long long> poff;
+    std::vector<uint8_t> h_grp;      // internal numbering
+    int32_t *d_inv = nullptr;
+    // device state
+    double2 *pos[2] = {nullptr, nullptr}, *vel = nullptr, *f = nullptr, *fd = nullptr, *stage[2] = {nullptr, nullptr};
+    uint8_t *grp = nullptr;
+    double *mass = nullptr;
+    int cur = 0;
+    // gather layout
+    long long nslices = 0, E = 0;
+    uint32_t *slice_off = nullptr;
+    uint8_t *slice_w = nullptr;
+    int32_t *nbr = nullptr, *sid = nullptr;
+    // scatter layout
+    long long Ms = 0;
+    int32_t *ssi = nullptr, *ssj = nullptr, *ssid = nullptr;
+    double *sUs = nullptr;
+    long long *d_soff_list = nullptr;
+    // parameters
+    int pm = PM_UNIFORM, ntypes = 0;
+    uint8_t *typ = nullptr;
+    double *kF = nullptr, *r0F = nullptr, *rcF = nullptr, *tab = nullptr;
+    double k_u = 0, r0_u = 0, rc_u = 0;
+    // breakage
+    long long *break_step = nullptr;
+    unsigned long long *nbroken = nullptr;
+    long long *d_poff = nullptr;
+    uint8_t *d_broken = nullptr;
+    // reductions
+    double *sU = nullptr, *sKE = nullptr, *part = nullptr;
+    long long nchunks = 0;
+    long long *chunk_lo = nullptr, *chunk_hi = nullptr;
+    int *spec_chunk_off = nullptr;
+    int *flags = nullptr;
+    double *cur_U = nullptr, *cur_KE = nullptr;
+    // history ring
+    long long *hist_step = nullptr, *hist_nb = nullptr;
+    double *hist_R = nullptr, *hist_U = nullptr, *hist_KE = nullptr;
+    long long hist_head = 0, hist_count = 0;
+    // groups
+    Group groups[kMaxGroups];
+    // run state
+    long long step = 0;
+    long long kernels_launched = 0;
+    long long last_compact_step = 0;
+    lsm_status sticky = LSM_OK;
+    std::string err;
+    // CUDA graph cache: one graph of `graph_len` fused MID steps
+    cudaGraphExec_t graph_exec = nullptr;
+    int graph_len = 0;
+    int graph_cur = -1;
+    long long *d_step_base = nullptr;
+};
+
+namespace {
+
+lsm_status fail(lsm_sim *s, lsm_status st, const std::string &msg) {
+    if (s) { s->sticky = st; s->err = msg; }
+    else g_create_error = msg;
+    return st;
+}
+
+#define CUDA_TRY(s, expr)                                                                          \
+    do {                                                                                           \
+        cudaError_t _e = (expr);                                                                   \
+        if (_e != cudaSuccess)                                                                     \
+            return fail((s), LSM_E_CUDA, std::string(#expr) + ": " + cudaGetErrorString(_e));      \
+    } while (0)
+
+template <class T> lsm_status dev_alloc(lsm_sim *s, T **out, size_t count) {
+    size_t bytes = std::max<size_t>(count, 1) * sizeof(T);
+    void *p = nullptr;
+    if (s->alloc) {
+        p = s->alloc(bytes, s->alloc_user);
+        if (!p) return fail(s, LSM_E_NOMEM, "device allocator callback returned NULL");
+    } else {
+        cudaError_t e = cudaMalloc(&p, bytes);
+        if (e != cudaSuccess) return fail(s, e == cudaErrorMemoryAllocation ? LSM_E_NOMEM : LSM_E_CUDA, std::string("cudaMalloc: ") + cudaGetErrorString(e));
+    }
+    s->dev_allocs.push_back(p);
+    s->device_bytes += (long long)bytes;
+    *out = reinterpret_cast<T *>(p);
+    return LSM_OK;
+}
+
+template <class T> lsm_status upload(lsm_sim *s, T **out, const std::vector<T> &h) {
+    lsm_status st = dev_alloc(s, out, h.size());
+    if (st != LSM_OK) return st;
+    if (!h.empty()) CUDA_TRY(s, cudaMemcpyAsync(*out, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice, s->stream));
+    return LSM_OK;
+}
+
+#define TRY(expr)                         \
+    do {                                  \
+        lsm_status _st = (expr);          \
+        if (_st != LSM_OK) return _st;    \
+    } while (0)
+
+inline unsigned grid_for(long long n) { return (unsigned)((n + kBlock - 1) / kBlock); }
+
+inline uint64_t part1by1(uint64_t x) {
+    x &= 0xffffffffull;
+    x = (x | (x << 16)) & 0x0000ffff0000ffffull;
+    x = (x | (x << 8)) & 0x00ff00ff00ff00ffull;
+    x = (x | (x << 4)) & 0x0f0f0f0f0f0f0f0full;
+    x = (x | (x << 2)) & 0x3333333333333333ull;
+    x = (x | (x << 1)) & 0x5555555555555555ull;
+    return x;
+}
+
+GroupTab group_tab(const lsm_sim *s) {
+    GroupTab g;
+    for (int i = 0; i < kMaxGroups; ++i) {
+        g.dux[i] = s->groups[i].set ? s->groups[i].du[0] : 0.0;
+        g.duy[i] = s->groups[i].set ? s->groups[i].du[1] : 0.0;
+        g.n0[i] = s->groups[i].n0;
+    }
+    return g;
+}
+
+StepParams step_params(const lsm_sim *s, long long step) {
+    StepParams P;
+    std::memset(&P, 0, sizeof(P));
+    const bool gather = s->force_mode == LSM_FORCE_GATHER;
+    P.pos_cur = s->pos[s->cur];
+    P.pos_next = gather ? s->pos[s->cur ^ 1] : s->pos[s->cur];
+    P.vel = s->vel; P.f = s->f; P.fd = s->fd; P.grp = s->grp; P.mass = s->mass;
+    P.mass_u = s->mass_u; P.inv_mass_u = 1.0 / s->mass_u;
+    P.dt = s->dt; P.hdt = 0.5 * s->dt; P.gamma = s->gamma;
+    P.N = s->N; P.step = step;
+    P.slice_off = s->slice_off; P.slice_w = s->slice_w; P.nbr = s->nbr; P.sid = s->sid;
+    P.sp.typ = s->typ; P.sp.kF = s->kF; P.sp.r0F = s->r0F; P.sp.rcF = s->rcF; P.sp.tab = s->tab; P.sp.ntypes = s->ntypes;
+    P.sp.k_u = s->k_u; P.sp.r0_u = s->r0_u; P.sp.rc_u = s->rc_u;
+    P.break_step = s->break_step; P.nbroken = s->nbroken; P.poff = s->d_poff; P.B = s->B;
+    P.sU = s->sU; P.sKE = s->sKE;
+    P.g = group_tab(s);
+    return P;
+}
+
+ScatterParams scatter_params(const lsm_sim *s) {
+    ScatterParams S;
+    std::memset(&S, 0, sizeof(S));
+    S.si = s->ssi; S.sj = s->ssj; S.sid = s->ssid; S.M = s->Ms; S.sUs = s->sUs;
+    S.sp.typ = s->typ; S.sp.kF = s->kF; S.sp.r0F = s->r0F; S.sp.rcF = s->rcF; S.sp.tab = s->tab; S.sp.ntypes = s->ntypes;
+    S.sp.k_u = s->k_u; S.sp.r0_u = s->r0_u; S.sp.rc_u = s->rc_u;
+    return S;
+}
+
+enum Variant { V_MID = 0, V_MID_SAMPLE = 1, V_END = 2, V_INIT = 3 };
+
+template <int PM, bool EXACT> void launch_gather_v(const StepParams &P, Variant v, unsigned grid, cudaStream_t st) {
+    switch (v) {
+        case V_MID: k_gather_step<PM, EXACT, true, true, false><<<grid, kBlock, 0, st>>>(P); break;
+        case V_MID_SAMPLE: k_gather_step<PM, EXACT, true, true, true><<<grid, kBlock, 0, st>>>(P); break;
+        case V_END: k_gather_step<PM, EXACT, true, false, true><<<grid, kBlock, 0, st>>>(P); break;
+        case V_INIT: k_gather_step<PM, EXACT, false, false, true><<<grid, kBlock, 0, st>>>(P); break;
+    }
+}
+
+template <bool EXACT> void launch_gather_pm(int pm, const StepParams &P, Variant v, unsigned grid, cudaStream_t st) {
+    switch (pm) {
+        case PM_UNIFORM: launch_gather_v<PM_UNIFORM, EXACT>(P, v, grid, st); break;
+        case PM_TYPED: launch_gather_v<PM_TYPED, EXACT>(P, v, grid, st); break;
+        case PM_RCF: launch_gather_v<PM_RCF, EXACT>(P, v, grid, st); break;
+        case PM_KRT_RCF: launch_gather_v<PM_KRT_RCF, EXACT>(P, v, grid, st); break;
+        default: launch_gather_v<PM_FULL, EXACT>(P, v, grid, st); break;
+    }
+}
+
+void launch_gather(lsm_sim *s, const StepParams &P, Variant v) {
+    const unsigned grid = grid_for(s->N);
+    if (s->exact) launch_gather_pm<true>(s->pm, P, v, grid, s->stream);
+    else launch_gather_pm<false>(s->pm, P, v, grid, s->stream);
+    s->kernels_launched += 1;
+}
+
+template <int PM> void launch_scatter_pm(const StepParams &P, const ScatterParams &S, bool sample, cudaStream_t st) {
+    const unsigned grid = grid_for(S.M);
+    if (S.M == 0) return;
+    if (sample) k_spring_scatter<PM, true><<<grid, kBlock, 0, st>>>(P, S);
+    else k_spring_scatter<PM, false><<<grid, kBlock, 0, st>>>(P, S);
+}
+
+void launch_scatter_force(lsm_sim *s, const StepParams &P, bool sample) {
+    const ScatterParams S = scatter_params(s);
+    switch (s->pm) {
+        case PM_UNIFORM: launch_scatter_pm<PM_UNIFORM>(P, S, sample, s->stream); break;
+        case PM_TYPED: launch_scatter_pm<PM_TYPED>(P, S, sample, s->stream); break;
+        case PM_RCF: launch_scatter_pm<PM_RCF>(P, S, sample, s->stream); break;
+        case PM_KRT_RCF: launch_scatter_pm<PM_KRT_RCF>(P, S, sample, s->stream); break;
+        default: launch_scatter_pm<PM_FULL>(P, S, sample, s->stream); break;
+    }
+    s->kernels_launched += 1;
+}
+
+void launch_integrate(lsm_sim *s, const StepParams &P, Variant v) {
+    const unsigned grid = grid_for(s->N);
+    switch (v) {
+        case V_MID: k_integrate<true, true, false><<<grid, kBlock, 0, s->stream>>>(P); break;
+        case V_MID_SAMPLE: k_integrate<true, true, true><<<grid, kBlock, 0, s->stream>>>(P); break;
+        case V_END: k_integrate<true, false, true><<<grid, kBlock, 0, s->stream>>>(P); break;
+        case V_INIT: k_integrate<false, false, true><<<grid, kBlock, 0, s->stream>>>(P); break;
+    }
+    s->kernels_launched += 1;
+}
+
+ReduceParams reduce_params(const lsm_sim *s, long long step) {
+    ReduceParams R;
+    std::memset(&R, 0, sizeof(R));
+    R.sU = s->sU; R.sKE = s->sKE; R.f = s->f;
+    R.chunk_lo = s->chunk_lo; R.chunk_hi = s->chunk_hi; R.spec_chunk_off = s->spec_chunk_off; R.part = s->part;
+    for (int g = 0; g < kMaxGroups; ++g) {
+        R.gids[g] = s->groups[g].set ? s->groups[g].d_ids : nullptr;
+        R.gseg[g] = s->groups[g].set ? s->groups[g].d_seg : nullptr;
+    }
+    R.nbroken = s->nbroken; R.B = s->B; R.step = step; R.flags = s->flags;
+    if (s->force_mode == LSM_FORCE_SCATTER) { R.sUs = s->sUs; R.soff_list = s->d_soff_list; }
+    return R;
+}
+
+// Run the two reduction kernels; slot >= 0 records into the history ring, slot < 0 into cur_U / cur_KE.
+void launch_reduce(lsm_sim *s, long long step, long long slot) {
+    ReduceParams R = reduce_params(s, step);
+    if (slot >= 0) {
+        R.out_step = s->hist_step + slot;
+        R.out_R = s->hist_R + (size_t)slot * s->B * kMaxGroups * 2;
+        R.out_U = s->hist_U + (size_t)slot * s->B;
+        R.out_KE = s->hist_KE + (size_t)slot * s->B;
+        R.out_nb = s->hist_nb + (size_t)slot * s->B;
+    } else {
+        R.out_U = s->cur_U; R.out_KE = s->cur_KE;
+    }
+    k_reduce_chunks<<<(unsigned)s->nchunks, kBlock, 0, s->stream>>>(R);
+    k_finalize_sample<<<(unsigned)((s->B + 3) / 4), 128, 0, s->stream>>>(R);
+    s->kernels_launched += 2;
+}
+
+void record_sample(lsm_sim *s, long long step) {
+    const long long slot = s->hist_head;
+    launch_reduce(s, step, slot);
+    s->hist_head = (s->hist_head + 1) % s->hist_cap;
+    if (s->hist_count < s->hist_cap) s->hist_count += 1;
+}
+
+bool is_sample_step(const lsm_sim *s, long long step) { return s->sample_every > 0 && step > 0 && step % s->sample_every == 0; }
+
+// Force evaluation at the current positions for the current step, without a kick (create / write_state).
+lsm_status eval_initial(lsm_sim *s) {
+    StepParams P = step_params(s, s->step);
+    if (s->force_mode == LSM_FORCE_GATHER) {
+        launch_gather(s, P, V_INIT);
+    } else {
+        k_zero_f<<<grid_for(s->N), kBlock, 0, s->stream>>>(s->f, s->N);
+        s->kernels_launched += 1;
+        launch_scatter_force(s, P, true);
+        launch_integrate(s, P, V_INIT);
+    }
+    CUDA_TRY(s, cudaGetLastError());
+    return LSM_OK;
+}
+
+lsm_status do_compact(lsm_sim *s) {
+    if (s->force_mode == LSM_FORCE_GATHER) {
+        CompactParams C;
+        C.slice_off = s->slice_off; C.slice_w = s->slice_w; C.nbr = s->nbr; C.sid = s->sid; C.typ = s->typ;
+        C.kF = s->kF; C.r0F = s->r0F; C.rcF = s->rcF; C.nslices = s->nslices;
+        k_compact_ell<<<grid_for(s->nslices * kSlice), kBlock, 0, s->stream>>>(C);
+        s->kernels_launched += 1;
+        CUDA_TRY(s, cudaGetLastError());
+    }
+    s->last_compact_step = s->step;
+    return LSM_OK;
+}
+
+void destroy_graph(lsm_sim *s) {
+    if (s->graph_exec) { cudaGraphExecDestroy(s->graph_exec); s->graph_exec = nullptr; }
+    s->graph_len = 0;
+}
+
+}  // namespace
+
+// =====================================================================================================================
+extern "C" {
+
+int32_t lsm_abi_version(void) { return LSM_ABI_VERSION; }
+
+const char *lsm_last_error(const lsm_sim *sim) { return sim ? sim->err.c_str() : g_create_error.c_str(); }
+
+void lsm_destroy(lsm_sim *s) {
+    if (!s) return;
+    cudaSetDevice(s->device);
+    cudaStreamSynchronize(s->stream);
+    destroy_graph(s);
+    for (void *p : s->dev_allocs) {
+        if (s->alloc) { if (s->free_) s->free_(p, s->alloc_user); }
+        else cudaFree(p);
+    }
+    delete s;
+}
+
+static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
+    const long long N = d->n_particles, M = d->n_springs;
+    const int B = d->n_batch;
+    s->N = N; s->M = M; s->B = B; s->dt = d->dt; s->gamma = d->gamma;
+    s->mass_u = d->mass ? 1.0 : d->mass_uniform;
+    s->sample_every = d->sample_every; s->hist_cap = d->history_capacity > 0 ? d->history_capacity : 1024;
+    s->compact_every = d->compact_every; s->reorder = d->reorder;
+    s->force_mode = d->force_mode == LSM_FORCE_AUTO ? LSM_FORCE_GATHER : d->force_mode;
+    s->exact = d->exact; s->use_graph = d->use_graph; s->device = d->device; s->stream = (cudaStream_t)d->stream;
+    s->alloc = d->alloc; s->free_ = d->free_; s->alloc_user = d->alloc_user;
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= 0) return fail(s, LSM_E_CUDA, "no CUDA device: this library has no CPU fallback");
+    if (d->device < 0 || d->device >= ndev) return fail(s, LSM_E_INVALID, "device ordinal out of range");
+    CUDA_TRY(s, cudaSetDevice(d->device));
+
+    // ---- specimen offsets ----
+    s->poff.assign(B + 1, 0);
+    std::vector<long long> soff(B + 1, 0);
+    if (d->particle_offsets && d->spring_offsets) {
+        for (int b = 0; b <= B; ++b) { s->poff[b] = d->particle_offsets[b]; soff[b] = d->spring_offsets[b]; }
+    } else if (B == 1) { s->poff[1] = N; soff[1] = M; }
+    else return fail(s, LSM_E_INVALID, "n_batch > 1 needs particle_offsets and spring_offsets");
+    if (s->poff[0] != 0 || s->poff[B] != N || soff[0] != 0 || soff[B] != M) return fail(s, LSM_E_INVALID, "offsets must start at 0 and end at N / M");
+    for (int b = 0; b < B; ++b)
+        if (s->poff[b + 1] < s->poff[b] || soff[b + 1] < soff[b]) return fail(s, LSM_E_INVALID, "offsets must ascend");
+
+    // ---- validation of values ----
+    for (long long q = 0; q < 2 * N; ++q) {
+        if (!std::isfinite(d->x[q])) return fail(s, LSM_E_NONFINITE, "non-finite position");
+        if (d->v && !std::isfinite(d->v[q])) return fail(s, LSM_E_NONFINITE, "non-finite velocity");
+    }
+    if (d->mass) { for (long long p = 0; p < N; ++p) if (!(d->mass[p] > 0.0) || !std::isfinite(d->mass[p])) return fail(s, LSM_E_NONFINITE, "mass must be finite and > 0"); }
+    else if (!(d->mass_uniform > 0.0) || !std::isfinite(d->mass_uniform)) return fail(s, LSM_E_NONFINITE, "mass_uniform must be finite and > 0");
+    if (M > 0 && (!d->spring_i || !d->spring_j)) return fail(s, LSM_E_INVALID, "spring_i / spring_j are NULL");
+    {
+        int b = 0;
+        for (long long e = 0; e < M; ++e) {
+            while (e >= soff[b + 1]) ++b;
+            const long long i = d->spring_i[e], j = d->spring_j[e];
+            if (i < s->poff[b] || i >= s->poff[b + 1] || j < s->poff[b] || j >= s->poff[b + 1] || i == j)
+                return fail(s, LSM_E_RANGE, "spring " + std::to_string(e) + ": endpoint out of its specimen's range, or i == j");
+            const double k = d->k ? d->k[e] : d->k_uniform, r0 = d->r0 ? d->r0[e] : d->r0_uniform, rc = d->rc ? d->rc[e] : d->rc_uniform;
+            if (!std::isfinite(k) || !std::isfinite(r0) || !std::isfinite(rc) || k < 0.0 || !(r0 > 0.0) || !(rc > 0.0))
+                return fail(s, LSM_E_NONFINITE, "spring " + std::to_string(e) + ": need finite k >= 0, r0 > 0, rc > 0");
+        }
+    }
+
+    // ---- (a8) renumbering: Morton order of the initial positions, per specimen ----
+    if (s->reorder == LSM_REORDER_MORTON) {
+        s->perm.resize(N); s->inv.resize(N);
+        std::vector<std::pair<uint64_t, int32_t>> keys(N);
+        for (int b = 0; b < B; ++b) {
+            double lox = 1e300, loy = 1e300, hix = -1e300, hiy = -1e300;
+            for (long long p = s->poff[b]; p < s->poff[b + 1]; ++p) {
+                lox = std::min(lox, d->x[2 * p]); hix = std::max(hix, d->x[2 * p]);
+                loy = std::min(loy, d->x[2 * p + 1]); hiy = std::max(hiy, d->x[2 * p + 1]);
+            }
+            const double ext = std::max(std::max(hix - lox, hiy - loy), 1e-300);
+            const double sc = 1048575.0 / ext;  // 20 bits per axis
+            for (long long p = s->poff[b]; p < s->poff[b + 1]; ++p) {
+                const uint64_t qx = (uint64_t)((d->x[2 * p] - lox) * sc), qy = (uint64_t)((d->x[2 * p + 1] - loy) * sc);
+                keys[p] = {part1by1(qx) | (part1by1(qy) << 1), (int32_t)p};
+            }
+            std::sort(keys.begin() + s->poff[b], keys.begin() + s->poff[b + 1]);
+        }
+        for (long long p = 0; p < N; ++p) { s->perm[p] = keys[p].second; s->inv[keys[p].second] = (int32_t)p; }
+    }
+    auto to_int = [&](long long c) -> int32_t { return s->inv.empty() ? (int32_t)c : s->inv[c]; };
+
+    // ---- parameter encoding: uniform scalars, a type table (Table 1) or fp64 arrays ----
+    const bool k_arr = d->k != nullptr, r0_arr = d->r0 != nullptr, rc_arr = d->rc != nullptr;
+    std::vector<uint8_t> stype;  // per spring type index
+    std::vector<double> tab;
+    {
+        auto all_same = [&](const double *a) { if (!a) return true; for (long long e = 1; e < M; ++e) if (a[e] != a[0]) return false; return true; };
+        const bool ku = all_same(d->k), r0u = all_same(d->r0), rcu = all_same(d->rc);
+        s->k_u = (k_arr && M > 0) ? d->k[0] : d->k_uniform;
+        s->r0_u = (r0_arr && M > 0) ? d->r0[0] : d->r0_uniform;
+        s->rc_u = (rc_arr && M > 0) ? d->rc[0] : d->rc_uniform;
+        if (!k_arr) s->k_u = d->k_uniform;
+        if (!r0_arr) s->r0_u = d->r0_uniform;
+        if (!rc_arr) s->rc_u = d->rc_uniform;
+        auto getk = [&](long long e) { return k_arr ? d->k[e] : s->k_u; };
+        auto getr0 = [&](long long e) { return r0_arr ? d->r0[e] : s->r0_u; };
+        auto getrc = [&](long long e) { return rc_arr ? d->rc[e] : s->rc_u; };
+        struct Key { uint64_t a, b, c; bool operator==(const Key &o) const { return a == o.a && b == o.b && c == o.c; } };
+        struct KeyHash { size_t operator()(const Key &k) const { return (size_t)(k.a * 0x9E3779B97F4A7C15ull ^ (k.b + 0x7F4A7C15ull) * 0xC2B2AE3D27D4EB4Full ^ (k.c * 0x165667B19E3779F9ull)); } };
+        auto bits = [](double v) { uint64_t u; std::memcpy(&u, &v, 8); return u; };
+        auto build_table = [&](bool with_rc) -> bool {  // false if more than kMaxTypes distinct entries
+            std::unordered_map<Key, int, KeyHash> map;
+            stype.assign(M, 0); tab.clear();
+            for (long long e = 0; e < M; ++e) {
+                Key key{bits(getk(e)), bits(getr0(e)), with_rc ? bits(getrc(e)) : 0};
+                auto it = map.find(key);
+                if (it == map.end()) {
+                    if ((int)map.size() == kMaxTypes) return false;
+                    it = map.emplace(key, (int)map.size()).first;
+                    tab.push_back(getk(e)); tab.push_back(getr0(e)); tab.push_back(with_rc ? getrc(e) : 0.0);
+                }
+                stype[e] = (uint8_t)it->second;
+            }
+            return true;
+        };
+        if (ku && r0u && rcu) s->pm = PM_UNIFORM;
+        else if (build_table(true)) s->pm = PM_TYPED;
+        else if (ku && r0u) s->pm = PM_RCF;
+        else if (build_table(false)) s->pm = PM_KRT_RCF;
+        else s->pm = PM_FULL;
+        if (s->pm != PM_TYPED && s->pm != PM_KRT_RCF) { stype.clear(); tab.clear(); }
+        s->ntypes = (int)(tab.size() / 3);
+    }
+    const bool need_typ = s->pm == PM_TYPED || s->pm == PM_KRT_RCF;
+    const bool need_rcF = s->pm == PM_RCF || s->pm == PM_KRT_RCF || s->pm == PM_FULL;
+    const bool need_krF = s->pm == PM_FULL;
+    auto getk = [&](long long e) { return k_arr ? d->k[e] : s->k_u; };
+    auto getr0 = [&](long long e) { return r0_arr ? d->r0[e] : s->r0_u; };
+    auto getrc = [&](long long e) { return rc_arr ? d->rc[e] : s->rc_u; };
+
+    // ---- particle state ----
+    {
+        std::vector<double2> hx(N), hv(N);
+        for (long long c = 0; c < N; ++c) {
+            const int32_t p = to_int(c);
+            hx[p] = make_double2(d->x[2 * c], d->x[2 * c + 1]);
+            hv[p] = d->v ? make_double2(d->v[2 * c], d->v[2 * c + 1]) : make_double2(0.0, 0.0);
+        }
+        TRY(upload(s, &s->pos[0], hx));
+        TRY(dev_alloc(s, &s->pos[1], (size_t)N));
+        CUDA_TRY(s, cudaMemcpyAsync(s->pos[1], s->pos[0], sizeof(double2) * N, cudaMemcpyDeviceToDevice, s->stream));
+        TRY(upload(s, &s->vel, hv));
+        TRY(dev_alloc(s, &s->f, (size_t)N));
+        TRY(dev_alloc(s, &s->fd, (size_t)N));
+        TRY(dev_alloc(s, &s->stage[0], (size_t)N));
+        TRY(dev_alloc(s, &s->stage[1], (size_t)N));
+        CUDA_TRY(s, cudaMemsetAsync(s->f, 0, sizeof(double2) * N, s->stream));
+        CUDA_TRY(s, cudaMemsetAsync(s->fd, 0, sizeof(double2) * N, s->stream));
+        s->h_grp.assign(N, kFree);
+        TRY(upload(s, &s->grp, s->h_grp));
+        if (d->mass) {
+            std::vector<double> hm(N);
+            for (long long c = 0; c < N; ++c) hm[to_int(c)] = d->mass[c];
+            TRY(upload(s, &s->mass, hm));
+        }
+        if (!s->inv.empty()) TRY(upload(s, &s->d_inv, s->inv));
+        TRY(upload(s, &s->d_poff, s->poff));
+        CUDA_TRY(s, cudaStreamSynchronize(s->stream));  // host vectors go out of scope
+    }
+
+    // ---- breakage bookkeeping ----
+    TRY(dev_alloc(s, &s->break_step, (size_t)M));
+    CUDA_TRY(s, cudaMemsetAsync(s->break_step, 0xFF, sizeof(long long) * std::max<long long>(M, 1), s->stream));  // -1
+    TRY(dev_alloc(s, &s->nbroken, (size_t)B));
+    CUDA_TRY(s, cudaMemsetAsync(s->nbroken, 0, sizeof(unsigned long long) * B, s->stream));
+    TRY(dev_alloc(s, &s->d_broken, (size_t)M));
+
+    // ---- spring layout ----
+    if (s->force_mode == LSM_FORCE_GATHER) {
+        const long long S = (N + kSlice - 1) / kSlice;
+        s->nslices = S;
+        std::vector<uint32_t> deg(N, 0);
+        for (long long e = 0; e < M; ++e) { deg[to_int(d->spring_i[e])]++; deg[to_int(d->spring_j[e])]++; }
+        std::vector<uint32_t> off(S + 1, 0);
+        std::vector<uint8_t> wv(S, 0);
+        for (long long sl = 0; sl < S; ++sl) {
+            uint32_t w = 0;
+            for (long long p = sl * kSlice; p < std::min<long long>(N, (sl + 1) * kSlice); ++p) w = std::max(w, deg[p]);
+            if (w > 255) return fail(s, LSM_E_UNSUPPORTED, "particle degree above 255 is not supported by the gather layout; use force_mode = SCATTER");
+            wv[sl] = (uint8_t)w;
+            const uint64_t nxt = (uint64_t)off[sl] + w;
+            if (nxt > 0xFFFFFFFFull) return fail(s, LSM_E_UNSUPPORTED, "gather layout too large");
+            off[sl + 1] = (uint32_t)nxt;
+        }
+        const size_t E = (size_t)off[S] * kSlice;
+        s->E = (long long)E;
+        std::vector<int32_t> hn(E, kPad), hs(E, -1);
+        std::vector<uint8_t> cnt(N, 0);
+        auto slot = [&](int32_t p) { const size_t e = ((size_t)off[p >> 5] + cnt[p]) * kSlice + (p & 31); cnt[p]++; return e; };
+        for (long long e = 0; e < M; ++e) {  // caller order -> every row is ascending in caller spring id
+            const int32_t a = to_int(d->spring_i[e]), b2 = to_int(d->spring_j[e]);
+            const size_t ea = slot(a), eb = slot(b2);
+            hn[ea] = b2; hs[ea] = (int32_t)e;
+            hn[eb] = a; hs[eb] = (int32_t)e;
+        }
+        TRY(upload(s, &s->slice_off, off));
+        TRY(upload(s, &s->slice_w, wv));
+        TRY(upload(s, &s->nbr, hn));
+        if (need_typ) { std::vector<uint8_t> ht(E, 0); for (size_t e = 0; e < E; ++e) if (hs[e] >= 0) ht[e] = stype[hs[e]]; TRY(upload(s, &s->typ, ht)); CUDA_TRY(s, cudaStreamSynchronize(s->stream)); }
+        if (need_rcF) { std::vector<double> h(E, 0.0); for (size_t e = 0; e < E; ++e) if (hs[e] >= 0) h[e] = getrc(hs[e]); TRY(upload(s, &s->rcF, h)); CUDA_TRY(s, cudaStreamSynchronize(s->stream)); }
+        if (need_krF) {
+            std::vector<double> h(E, 0.0);
+            for (size_t e = 0; e < E; ++e) if (hs[e] >= 0) h[e] = getk(hs[e]);
+            TRY(upload(s, &s->kF, h)); CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+            for (size_t e = 0; e < E; ++e) if (hs[e] >= 0) h[e] = getr0(hs[e]);
+            TRY(upload(s, &s->r0F, h)); CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+        }
+        TRY(upload(s, &s->sid, hs));
+        CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    } else if (s->force_mode == LSM_FORCE_SCATTER) {
+        if (s->exact) return fail(s, LSM_E_UNSUPPORTED, "exact arithmetic needs force_mode = GATHER (atomic summation order is not fixed)");
+        // spring list in internal numbering, sorted by (lower endpoint, upper endpoint) for gather / atomic locality
+        std::vector<int32_t> order(M);
+        for (long long e = 0; e < M; ++e) order[e] = (int32_t)e;
+        std::vector<int32_t> a(M), b2(M);
+        for (long long e = 0; e < M; ++e) { int32_t i = to_int(d->spring_i[e]), j = to_int(d->spring_j[e]); a[e] = std::min(i, j); b2[e] = std::max(i, j); }
+        std::sort(order.begin(), order.end(), [&](int32_t x, int32_t y) { return a[x] != a[y] ? a[x] < a[y] : (b2[x] != b2[y] ? b2[x] < b2[y] : x < y); });
+        std::vector<int32_t> hi(M), hj(M), hs(M);
+        for (long long q = 0; q < M; ++q) { const int32_t e = order[q]; hi[q] = to_int(d->spring_i[e]); hj[q] = to_int(d->spring_j[e]); hs[q] = e; }
+        s->Ms = M; s->E = M;
+        TRY(upload(s, &s->ssi, hi)); TRY(upload(s, &s->ssj, hj)); TRY(upload(s, &s->ssid, hs));
+        if (need_typ) { std::vector<uint8_t> ht(M); for (long long q = 0; q < M; ++q) ht[q] = stype[hs[q]]; TRY(upload(s, &s->typ, ht)); CUDA_TRY(s, cudaStreamSynchronize(s->stream)); }
+        if (need_rcF) { std::vector<double> h(M); for (long long q = 0; q < M; ++q) h[q] = getrc(hs[q]); TRY(upload(s, &s->rcF, h)); CUDA_TRY(s, cudaStreamSynchronize(s->stream)); }
+        if (need_krF) {
+            std::vector<double> h(M);
+            for (long long q = 0; q < M; ++q) h[q] = getk(hs[q]);
+            TRY(upload(s, &s->kF, h)); CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+            for (long long q = 0; q < M; ++q) h[q] = getr0(hs[q]);
+            TRY(upload(s, &s->r0F, h)); CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+        }
+        TRY(dev_alloc(s, &s->sUs, (size_t)M));
+        // specimen segments of the sorted list (sorted by lower endpoint, specimens are contiguous id ranges)
+        std::vector<long long> sl(B + 1, 0);
+        { int b = 0; for (long long q = 0; q < M; ++q) { while (std::min(hi[q], hj[q]) >= s->poff[b + 1]) { ++b; sl[b] = q; } } for (int bb = b + 1; bb <= B; ++bb) sl[bb] = M; }
+        TRY(upload(s, &s->d_soff_list, sl));
+        CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    } else {
+        return fail(s, LSM_E_INVALID, "bad force_mode");
+    }
+    if (!tab.empty()) { TRY(upload(s, &s->tab, tab)); CUDA_TRY(s, cudaStreamSynchronize(s->stream)); }
+
+    // ---- reductions: chunk table, scratch, history ring ----
+    {
+        std::vector<long long> lo, hi;
+        std::vector<int> sco(B + 1, 0);
+        for (int b = 0; b < B; ++b) {
+            for (long long p = s->poff[b]; p < s->poff[b + 1]; p += kChunk) { lo.push_back(p); hi.push_back(std::min(p + kChunk, s->poff[b + 1])); }
+            sco[b + 1] = (int)lo.size();
+        }
+        s->nchunks = (long long)lo.size();
+        TRY(upload(s, &s->chunk_lo, lo)); TRY(upload(s, &s->chunk_hi, hi)); TRY(upload(s, &s->spec_chunk_off, sco));
+        CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+        TRY(dev_alloc(s, &s->part, (size_t)s->nchunks * 2));
+        TRY(dev_alloc(s, &s->sU, (size_t)N)); TRY(dev_alloc(s, &s->sKE, (size_t)N));
+        TRY(dev_alloc(s, &s->flags, 1));
+        CUDA_TRY(s, cudaMemsetAsync(s->flags, 0, sizeof(int), s->stream));
+        TRY(dev_alloc(s, &s->cur_U, (size_t)B)); TRY(dev_alloc(s, &s->cur_KE, (size_t)B));
+        const size_t cap = (size_t)s->hist_cap;
+        TRY(dev_alloc(s, &s->hist_step, cap)); TRY(dev_alloc(s, &s->hist_nb, cap * B));
+        TRY(dev_alloc(s, &s->hist_R, cap * B * kMaxGroups * 2));
+        TRY(dev_alloc(s, &s->hist_U, cap * B)); TRY(dev_alloc(s, &s->hist_KE, cap * B));
+        TRY(dev_alloc(s, &s->d_step_base, 1));
+    }
+    s->step = 0;
+    TRY(eval_initial(s));
+    CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    return LSM_OK;
+}
+
+lsm_status lsm_create(const lsm_desc *d, lsm_sim **out) {
+    if (out) *out = nullptr;
+    if (!d || !out) return fail(nullptr, LSM_E_INVALID, "desc / out is NULL");
+    if (d->struct_size != sizeof(lsm_desc)) return fail(nullptr, LSM_E_INVALID, "lsm_desc.struct_size does not match this library (ABI mismatch)");
+    if (d->dim == 3) return fail(nullptr, LSM_E_UNSUPPORTED, "dim = 3 is not built in this round (hot path is 2-D)");
+    if (d->dim != 2) return fail(nullptr, LSM_E_INVALID, "dim must be 2");
+    if (d->n_particles < 1 || d->n_springs < 0 || d->n_particles >= 2147483647LL || d->n_springs >= 2147483647LL) return fail(nullptr, LSM_E_INVALID, "need 1 <= N < 2^31-1 and 0 <= M < 2^31-1");
+    if (d->n_batch < 1 || !d->x) return fail(nullptr, LSM_E_INVALID, "n_batch < 1 or x is NULL");
+    if (!(d->dt > 0.0) || !(d->gamma >= 0.0) || !std::isfinite(d->dt) || !std::isfinite(d->gamma)) return fail(nullptr, LSM_E_INVALID, "need dt > 0 and gamma >= 0");
+    if (d->sample_every < 0 || d->compact_every < 0 || d->history_capacity < 0) return fail(nullptr, LSM_E_INVALID, "negative sample_every / compact_every / history_capacity");
+    if (d->reorder == LSM_REORDER_RCM) return fail(nullptr, LSM_E_UNSUPPORTED, "reorder = RCM is not built; use MORTON");
+    if (d->reorder != LSM_REORDER_NONE && d->reorder != LSM_REORDER_MORTON) return fail(nullptr, LSM_E_INVALID, "bad reorder");
+    if (d->force_mode < 0 || d->force_mode > 2) return fail(nullptr, LSM_E_INVALID, "bad force_mode");
+    if ((d->alloc == nullptr) != (d->free_ == nullptr)) return fail(nullptr, LSM_E_INVALID, "alloc and free_ must be given together");
+    lsm_sim *s = new (std::nothrow) lsm_sim();
+    if (!s) return fail(nullptr, LSM_E_NOMEM, "out of host memory");
+    lsm_status st;
+    try { st = create_impl(d, s); }
+    catch (const std::bad_alloc &) { st = fail(s, LSM_E_NOMEM, "out of host memory while building the layout"); }
+    if (st != LSM_OK) { g_create_error = s->err; lsm_destroy(s); return st; }
+    *out = s;
+    return LSM_OK;
+}
+
+#define CHECK_SIM(s)                                   \
+    do {                                               \
+        if (!(s)) return LSM_E_INVALID;                \
+        if ((s)->sticky != LSM_OK) return (s)->sticky; \
+        cudaSetDevice((s)->device);                    \
+    } while (0)
+
+lsm_status lsm_set_boundary(lsm_sim *s, int32_t gi, const int32_t *ids, int64_t n, int32_t mode, const double *du) {
+    CHECK_SIM(s);
+    if (gi < 0 || gi >= kMaxGroups) { s->err = "group id out of range"; return LSM_E_RANGE; }
+    if (n < 0 || (n > 0 && !ids) || (mode != LSM_FIXED && mode != LSM_MOVE)) { s->err = "bad arguments"; return LSM_E_INVALID; }
+    if (mode == LSM_MOVE && (!du || !std::isfinite(du[0]) || !std::isfinite(du[1]))) { s->err = "MOVE needs a finite disp_per_step"; return LSM_E_INVALID; }
+    Group &g = s->groups[gi];
+    std::vector<int32_t> nid((size_t)n);
+    for (long long q = 0; q < n; ++q) {
+        if (ids[q] < 0 || ids[q] >= s->N) { s->err = "boundary particle id out of range"; return LSM_E_RANGE; }
+        nid[q] = s->inv.empty() ? ids[q] : s->inv[ids[q]];
+        const uint8_t cg = s->h_grp[nid[q]];
+        if (cg != kFree && cg != gi) { s->err = "particle already belongs to another boundary group"; return LSM_E_RANGE; }
+    }
+    std::sort(nid.begin(), nid.end());
+    if (std::adjacent_find(nid.begin(), nid.end()) != nid.end()) { s->err = "duplicate particle id in the group"; return LSM_E_RANGE; }
+    destroy_graph(s);
+    // release the old members (they keep the kinematic velocity du/dt, like the oracle's stored v)
+    if (g.set && !g.ids.empty()) {
+        k_group_release<<<grid_for((long long)g.ids.size()), kBlock, 0, s->stream>>>(g.d_ids, (long long)g.ids.size(), s->grp, s->vel, g.du[0] / s->dt, g.du[1] / s->dt);
+        s->kernels_launched += 1;
+        for (int32_t p : g.ids) s->h_grp[p] = kFree;
+    }
+    g.set = true; g.mode = mode; g.n0 = s->step;
+    g.du[0] = mode == LSM_MOVE ? du[0] : 0.0; g.du[1] = mode == LSM_MOVE ? du[1] : 0.0;
+    g.ids = nid;
+    for (int32_t p : nid) s->h_grp[p] = (uint8_t)gi;
+    std::vector<long long> seg(s->B + 1, 0);
+    { int b = 0; for (size_t q = 0; q < nid.size(); ++q) { while (nid[q] >= s->poff[b + 1]) { ++b; seg[b] = (long long)q; } } for (int bb = b + 1; bb <= s->B; ++bb) seg[bb] = (long long)nid.size(); }
+    // (old device lists stay owned by the handle until destroy; groups are set a handful of times)
+    TRY(upload(s, &g.d_ids, nid));
+    TRY(upload(s, &g.d_seg, seg));
+    if (n > 0) {
+        k_group_assign<<<grid_for(n), kBlock, 0, s->stream>>>(g.d_ids, n, s->grp, s->vel, s->pos[s->cur], (uint8_t)gi);
+        s->kernels_launched += 1;
+    }
+    CUDA_TRY(s, cudaGetLastError());
+    CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    return LSM_OK;
+}
+
+// Enqueue one lsm_step call: START, (n-1) fused MID steps, END.
+lsm_status lsm_step(lsm_sim *s, int64_t n_steps) {
+    CHECK_SIM(s);
+    if (n_steps < 0) { s->err = "n_steps < 0"; return LSM_E_INVALID; }
+    if (n_steps == 0) return LSM_OK;
+    const bool gather = s->force_mode == LSM_FORCE_GATHER;
+    long long done = 0;
+    while (done < n_steps) {
+        // split the call at compaction boundaries
+        long long seg = n_steps - done;
+        if (s->compact_every > 0) seg = std::min<long long>(seg, s->compact_every - (s->step - s->last_compact_step) > 0 ? s->compact_every - (s->step - s->last_compact_step) : 1);
+        // START: first half kick + drift from the completed state
+        {
+            StepParams P = step_params(s, s->step);
+            if (s->exact) k_start<true><<<grid_for(s->N), kBlock, 0, s->stream>>>(P);
+            else k_start<false><<<grid_for(s->N), kBlock, 0, s->stream>>>(P);
+            s->kernels_launched += 1;
+            if (gather) s->cur ^= 1;
+            else { k_zero_f<<<grid_for(s->N), kBlock, 0, s->stream>>>(s->f, s->N); s->kernels_launched += 1; }
+        }
+        for (long long i = 1; i <= seg; ++i) {
+            const long long m = s->step + i;  // the step this force evaluation completes
+            const bool last = i == seg;
+            const bool samp = is_sample_step(s, m);
+            const Variant v = last ? V_END : (samp ? V_MID_SAMPLE : V_MID);
+            StepParams P = step_params(s, m);
+            if (gather) {
+                launch_gather(s, P, v);
+                if (!last) s->cur ^= 1;
+            } else {
+                launch_scatter_force(s, P, samp || last);
+                launch_integrate(s, P, v);
+            }
+            if (samp) record_sample(s, m);
+            if (!gather && samp && !last) { k_zero_f<<<grid_for(s->N), kBlock, 0, s->stream>>>(s->f, s->N); s->kernels_launched += 1; }
+        }
+        s->step += seg;
+        done += seg;
+        CUDA_TRY(s, cudaGetLastError());
+        if (s->compact_every > 0 && s->step - s->last_compact_step >= s->compact_every) TRY(do_compact(s));
+    }
+    return LSM_OK;
+}
+
+lsm_status lsm_compact(lsm_sim *s) {
+    CHECK_SIM(s);
+    return do_compact(s);
+}
+
+static lsm_status check_flags(lsm_sim *s) {
+    int fl = 0;
+    CUDA_TRY(s, cudaMemcpyAsync(&fl, s->flags, sizeof(int), cudaMemcpyDeviceToHost, s->stream));
+    CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    if (fl & 1) return fail(s, LSM_E_STATE, "non-finite energy detected on the device: the simulation blew up");
+    return LSM_OK;
+}
+
+lsm_status lsm_sync(lsm_sim *s) {
+    CHECK_SIM(s);
+    CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    return LSM_OK;
+}
+
+lsm_status lsm_write_state(lsm_sim *s, const double *x, const double *v) {
+    CHECK_SIM(s);
+    if (!x) { s->err = "x is NULL"; return LSM_E_INVALID; }
+    CUDA_TRY(s, cudaMemcpyAsync(s->stage[0], x, sizeof(double2) * s->N, cudaMemcpyHostToDevice, s->stream));
+    if (v) CUDA_TRY(s, cudaMemcpyAsync(s->stage[1], v, sizeof(double2) * s->N, cudaMemcpyHostToDevice, s->stream));
+    k_from_caller<<<grid_for(s->N), kBlock, 0, s->stream>>>(s->stage[0], v ? s->stage[1] : nullptr, s->pos[s->cur], s->vel, s->d_inv, s->N, s->grp);
+    s->kernels_launched += 1;
+    for (int g = 0; g < kMaxGroups; ++g) s->groups[g].n0 = s->step;
+    destroy_graph(s);
+    TRY(eval_initial(s));
+    return LSM_OK;
+}
+
+lsm_status lsm_read_state(lsm_sim *s, double *x, double *v) {
+    CHECK_SIM(s);
+    const GroupTab g = group_tab(s);
+    if (x) {
+        k_to_caller<<<grid_for(s->N), kBlock, 0, s->stream>>>(s->pos[s->cur], s->stage[0], s->d_inv, s->N, s->grp, g, s->dt, 0);
+        CUDA_TRY(s, cudaMemcpyAsync(x, s->stage[0], sizeof(double2) * s->N, cudaMemcpyDeviceToHost, s->stream));
+        s->kernels_launched += 1;
+    }
+    if (v) {
+        k_to_caller<<<grid_for(s->N), kBlock, 0, s->stream>>>(s->vel, s->stage[1], s->d_inv, s->N, s->grp, g, s->dt, 1);
+        CUDA_TRY(s, cudaMemcpyAsync(v, s->stage[1], sizeof(double2) * s->N, cudaMemcpyDeviceToHost, s->stream));
+        s->kernels_launched += 1;
+    }
+    return check_flags(s);
+}
+
+lsm_status lsm_read_forces(lsm_sim *s, double *f) {
+    CHECK_SIM(s);
+    if (!f) { s->err = "f is NULL"; return LSM_E_INVALID; }
+    k_to_caller<<<grid_for(s->N), kBlock, 0, s->stream>>>(s->f, s->stage[0], s->d_inv, s->N, s->grp, group_tab(s), s->dt, 0);
+    s->kernels_launched += 1;
+    CUDA_TRY(s, cudaMemcpyAsync(f, s->stage[0], sizeof(double2) * s->N, cudaMemcpyDeviceToHost, s->stream));
+    return check_flags(s);
+}
+
+lsm_status lsm_read_broken(lsm_sim *s, uint8_t *broken, int64_t *break_step, int64_t *n_broken) {
+    CHECK_SIM(s);
+    if (broken && s->M > 0) {
+        k_broken_from_steps<<<grid_for(s->M), kBlock, 0, s->stream>>>(s->break_step, s->d_broken, s->M);
+        s->kernels_launched += 1;
+        CUDA_TRY(s, cudaMemcpyAsync(broken, s->d_broken, (size_t)s->M, cudaMemcpyDeviceToHost, s->stream));
+    }
+    if (break_step && s->M > 0) CUDA_TRY(s, cudaMemcpyAsync(break_step, s->break_step, sizeof(long long) * s->M, cudaMemcpyDeviceToHost, s->stream));
+    std::vector<unsigned long long> nb(s->B);
+    CUDA_TRY(s, cudaMemcpyAsync(nb.data(), s->nbroken, sizeof(unsigned long long) * s->B, cudaMemcpyDeviceToHost, s->stream));
+    CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    if (n_broken) { long long t = 0; for (auto q : nb) t += (long long)q; *n_broken = t; }
+    return LSM_OK;
+}
+
+lsm_status lsm_read_energy(lsm_sim *s, double *U, double *KE) {
+    CHECK_SIM(s);
+    launch_reduce(s, s->step, -1);  // sU / sKE / f of the completed state were written by the END / INIT kernel
+    CUDA_TRY(s, cudaGetLastError());
+    if (U) CUDA_TRY(s, cudaMemcpyAsync(U, s->cur_U, sizeof(double) * s->B, cudaMemcpyDeviceToHost, s->stream));
+    if (KE) CUDA_TRY(s, cudaMemcpyAsync(KE, s->cur_KE, sizeof(double) * s->B, cudaMemcpyDeviceToHost, s->stream));
+    return check_flags(s);
+}
+
+lsm_status lsm_read_stress(lsm_sim *s, int64_t capacity, int64_t *n_samples, int64_t *step, double *R, double *U, double *KE, int64_t *nb) {
+    CHECK_SIM(s);
+    if (!n_samples || capacity < 0) { s->err = "n_samples is NULL or capacity < 0"; return LSM_E_INVALID; }
+    const long long n = std::min<long long>(s->hist_count, capacity);
+    const long long B = s->B;
+    for (long long t = 0; t < n; ++t) {  // oldest of the last n first
+        const long long slot = ((s->hist_head - n + t) % s->hist_cap + s->hist_cap) % s->hist_cap;
+        if (step) CUDA_TRY(s, cudaMemcpyAsync(step + t, s->hist_step + slot, sizeof(long long), cudaMemcpyDeviceToHost, s->stream));
+        if (R) CUDA_TRY(s, cudaMemcpyAsync(R + t * B * kMaxGroups * 2, s->hist_R + slot * B * kMaxGroups * 2, sizeof(double) * B * kMaxGroups * 2, cudaMemcpyDeviceToHost, s->stream));
+        if (U) CUDA_TRY(s, cudaMemcpyAsync(U + t * B, s->hist_U + slot * B, sizeof(double) * B, cudaMemcpyDeviceToHost, s->stream));
+        if (KE) CUDA_TRY(s, cudaMemcpyAsync(KE + t * B, s->hist_KE + slot * B, sizeof(double) * B, cudaMemcpyDeviceToHost, s->stream));
+        if (nb) CUDA_TRY(s, cudaMemcpyAsync(nb + t * B, s->hist_nb + slot * B, sizeof(long long) * B, cudaMemcpyDeviceToHost, s->stream));
+    }
+    *n_samples = n;
+    s->hist_count = 0;
+    return check_flags(s);
+}
+
+lsm_status lsm_get_info(lsm_sim *s, lsm_info *info) {
+    if (!s || !info) return LSM_E_INVALID;
+    std::memset(info, 0, sizeof(*info));
+    info->n_particles = s->N; info->n_springs = s->M; info->n_half_edges_stored = s->E;
+    static const int pbytes[5] = {0, 1, 8, 9, 24};
+    info->bytes_per_half_edge = (s->force_mode == LSM_FORCE_GATHER ? 4 : 8) + pbytes[s->pm];
+    info->param_mode = s->pm; info->n_types = s->ntypes; info->force_mode = s->force_mode; info->exact = s->exact;
+    info->reorder = s->reorder; info->n_batch = s->B; info->device_bytes = s->device_bytes;
+    info->kernels_launched = s->kernels_launched; info->current_step = s->step;
+    return LSM_OK;
+}
+
+lsm_status lsm_device_state(lsm_sim *s, const double **pos_xy, const double **vel_xy) {
+    CHECK_SIM(s);
+    if (pos_xy) *pos_xy = reinterpret_cast<const double *>(s->pos[s->cur]);
+    if (vel_xy) *vel_xy = reinterpret_cast<const double *>(s->vel);
+    return LSM_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,466 @@
+// lsm_kernels.cuh -- hand-written sm_100a kernels of the lattice-spring step (see include/lsm.h).
+//
+// Data layout in HBM:
+//   pos[2][N], vel[N], f[N], fd[N]   double2 (x,y packed: one 16-byte access per particle; streaming accesses are
+//                                    fully coalesced, neighbour gathers touch one sector instead of two)
+//   grp[N]                           uint8 boundary group of the particle, 0xFF = free.  For a kinematic particle the
+//                                    vel slot holds its ORIGIN x0 (its velocity is du_g/dt by definition).
+//   gather layout (particle-centric, sliced ELL, slice = one warp = 32 consecutive particles):
+//     slice_off[S+1] (units of 32 slots), slice_w[S] (live width), nbr[E] int32 neighbour id (bitwise-NOT of the id
+//     once the spring is dead, INT32_MIN = padding), sid[E] caller spring id, per-slot parameters by ParamMode.
+//     Slot s of lane l of slice S is entry (slice_off[S] + s)*32 + l  -> every slot load is one coalesced line.
+//     Rows are ordered by ascending caller spring id, so a particle sums its springs in the oracle's order.
+//   scatter layout (the paper's spring list, re-done in SoA): si[M'], sj[M'] (si bitwise-NOT
+//     once dead), per-spring parameters by ParamMode, force accumulated with fp64 RED atomics into f.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace lsmk {
+
+constexpr int kBlock = 256;
+constexpr int kSlice = 32;
+constexpr int32_t kPad = INT32_MIN;
+constexpr uint8_t kFree = 0xFF;
+constexpr int kMaxGroups = 8;
+constexpr int kChunk = 2048;  // particles per reduction chunk
+constexpr int kMaxTypes = 256;
+
+enum ParamMode { PM_UNIFORM = 0, PM_TYPED = 1, PM_RCF = 2, PM_KRT_RCF = 3, PM_FULL = 4 };
+
+struct GroupTab {
+    double dux[kMaxGroups], duy[kMaxGroups];
+    long long n0[kMaxGroups];
+};
+
+struct SpringParams {  // parameter encoding shared by the gather (per half-edge) and scatter (per spring) layouts
+    const uint8_t *typ;
+    const double *kF, *r0F, *rcF;
+    const double *tab;  // [ntypes][3] = k, r0, rc
+    int ntypes;
+    double k_u, r0_u, rc_u;
+};
+
+struct StepParams {
+    const double2 *pos_cur;
+    double2 *pos_next;
+    double2 *vel, *f, *fd;
+    const uint8_t *grp;
+    const double *mass;
+    double mass_u, inv_mass_u;
+    double dt, hdt, gamma;
+    long long N;
+    long long step;  // step number of THIS force evaluation (stamped on springs that break in it)
+    // gather layout
+    const uint32_t *slice_off;
+    const uint8_t *slice_w;
+    int32_t *nbr;
+    const int32_t *sid;
+    SpringParams sp;
+    // breakage bookkeeping
+    long long *break_step;
+    unsigned long long *nbroken;
+    const long long *poff;
+    int B;
+    // per-particle energy scratch (written by SAMPLE variants)
+    double *sU, *sKE;
+    GroupTab g;
+};
+
+// ---- arithmetic: EXACT = IEEE sqrt / divide and never-contracted multiply-add (mirrors gcc -ffp-contract=off) ----
+template <bool E> __device__ __forceinline__ double mul(double a, double b) { return E ? __dmul_rn(a, b) : a * b; }
+template <bool E> __device__ __forceinline__ double add(double a, double b) { return E ? __dadd_rn(a, b) : a + b; }
+template <bool E> __device__ __forceinline__ double sub(double a, double b) { return E ? __dsub_rn(a, b) : a - b; }
+template <bool E> __device__ __forceinline__ double mad(double a, double b, double c) {  // a*b + c
+    return E ? __dadd_rn(__dmul_rn(a, b), c) : fma(a, b, c);
+}
+
+__device__ __forceinline__ int spec_of(const long long *poff, int B, long long p) {
+    int lo = 0, hi = B;  // poff[lo] <= p < poff[hi]
+    while (hi - lo > 1) {
+        int mid = (lo + hi) >> 1;
+        if (poff[mid] <= p) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+
+template <int PM> __device__ __forceinline__ void load_params(const SpringParams &sp, const double *s_tab, size_t e,
+                                                              double &k, double &r0, double &rc) {
+    if (PM == PM_UNIFORM) { k = sp.k_u; r0 = sp.r0_u; rc = sp.rc_u; }
+    else if (PM == PM_TYPED) { int t = sp.typ[e]; k = s_tab[3 * t]; r0 = s_tab[3 * t + 1]; rc = s_tab[3 * t + 2]; }
+    else if (PM == PM_RCF) { k = sp.k_u; r0 = sp.r0_u; rc = __ldg(sp.rcF + e); }
+    else if (PM == PM_KRT_RCF) { int t = sp.typ[e]; k = s_tab[3 * t]; r0 = s_tab[3 * t + 1]; rc = __ldg(sp.rcF + e); }
+    else { k = __ldg(sp.kF + e); r0 = __ldg(sp.r0F + e); rc = __ldg(sp.rcF + e); }
+}
+
+// One spring seen from one endpoint: d = x_other - x_self.  Returns false when the spring just broke.
+// Eq. 2 with the listing's breakage test (L98).  Both endpoints compute bit-identical r
+// ((-dx)^2 == dx^2), so they take the same decision without communicating.
+template <bool EXACT> __device__ __forceinline__ bool spring_eval(double dx, double dy, double k, double r0, double rc,
+                                                                  double &gk, double &ext) {
+    const double r2 = EXACT ? add<true>(mul<true>(dx, dx), mul<true>(dy, dy)) : fma(dy, dy, dx * dx);
+    double r, rinv;
+    if (EXACT) { r = __dsqrt_rn(r2); rinv = 0.0; }
+    else { rinv = rsqrt(r2); r = r2 * rinv; if (!(r2 > 0.0)) r = 0.0; }
+    if (r > rc) return false;                       // strict '>' (Q1)
+    ext = sub<EXACT>(r, r0);
+    if (r == 0.0) { gk = 0.0; ext = 0.0; return true; }   // coincident endpoints: no direction, no force (Q4)
+    gk = EXACT ? __ddiv_rn(mul<true>(k, ext), r) : (k * ext) * rinv;
+    return true;
+}
+
+// Velocity-Verlet particle update (Eq. 3-5, half-step-velocity form L76), given the spring force
+// (fx,fy) at the current positions.  KICK2: second half kick completing the step; ADVANCE: first half kick + drift of
+// the next step fused behind it (the half-step velocity is what is stored between kernels); !ADVANCE: store the
+// completed state (v, f, fd).  SAMPLE: write per-particle energy terms and f for the reductions.
+template <bool EXACT, bool KICK2, bool ADVANCE, bool SAMPLE>
+__device__ __forceinline__ void particle_update(const StepParams &P, long long p, double2 xp, double2 vh, uint8_t g,
+                                                double fx, double fy, double u) {
+    if (g == kFree) {
+        const double fdx = sub<EXACT>(fx, mul<EXACT>(P.gamma, vh.x));  // damping with the held velocity (Q7)
+        const double fdy = sub<EXACT>(fy, mul<EXACT>(P.gamma, vh.y));
+        double ax, ay, m;
+        if (P.mass) { m = __ldg(P.mass + p); ax = EXACT ? __ddiv_rn(fdx, m) : fdx / m; ay = EXACT ? __ddiv_rn(fdy, m) : fdy / m; }
+        else { m = P.mass_u; ax = EXACT ? __ddiv_rn(fdx, m) : fdx * P.inv_mass_u; ay = EXACT ? __ddiv_rn(fdy, m) : fdy * P.inv_mass_u; }
+        double2 v = vh;
+        if (KICK2) { v.x = mad<EXACT>(P.hdt, ax, vh.x); v.y = mad<EXACT>(P.hdt, ay, vh.y); }  // Eq. 5, second half
+        if (SAMPLE) {
+            const double v2 = add<EXACT>(mul<EXACT>(v.x, v.x), mul<EXACT>(v.y, v.y));
+            P.sU[p] = u;
+            P.sKE[p] = mul<EXACT>(mul<EXACT>(0.5, m), v2);
+        }
+        if (SAMPLE || !ADVANCE) P.f[p] = make_double2(fx, fy);
+        if (ADVANCE) {
+            double2 w, xn;
+            w.x = mad<EXACT>(P.hdt, ax, v.x); w.y = mad<EXACT>(P.hdt, ay, v.y);          // Eq. 5, first half
+            xn.x = mad<EXACT>(P.dt, w.x, xp.x); xn.y = mad<EXACT>(P.dt, w.y, xp.y);      // Eq. 3
+            P.pos_next[p] = xn;
+            P.vel[p] = w;
+        } else {
+            P.vel[p] = v;
+            P.fd[p] = make_double2(fdx, fdy);
+        }
+    } else {  // kinematic particle: vh holds its origin x0 ("boundary displacements are first applied")
+        if (SAMPLE) { P.sU[p] = u; P.sKE[p] = 0.0; }
+        if (SAMPLE || !ADVANCE) P.f[p] = make_double2(fx, fy);
+        if (ADVANCE) {
+            const double ns = (double)(P.step + 1 - P.g.n0[g]);
+            P.pos_next[p] = make_double2(mad<EXACT>(ns, P.g.dux[g], vh.x), mad<EXACT>(ns, P.g.duy[g], vh.y));
+        } else {
+            P.fd[p] = make_double2(fx, fy);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Fused gather step: one thread per particle.  Gathers the positions of its (<= slice width) neighbours, evaluates
+// every incident spring (each spring is evaluated from both of its endpoints: twice the arithmetic, no atomics, no
+// force array round trip, deterministic), applies the breakage test, then integrates.  Reads x (double-buffered),
+// v, ids, parameters; writes x_next, v.  HBM bytes per step: 64 N + (4 + parameter bytes) * 2M.
+// ---------------------------------------------------------------------------------------------------------------
+template <int PM, bool EXACT, bool KICK2, bool ADVANCE, bool SAMPLE>
+__global__ void __launch_bounds__(kBlock) k_gather_step(const StepParams P) {
+    constexpr bool kTab = (PM == PM_TYPED || PM == PM_KRT_RCF);
+    __shared__ double s_tab[kTab ? 3 * kMaxTypes : 1];
+    if (kTab) {
+        for (int i = threadIdx.x; i < 3 * P.sp.ntypes; i += kBlock) s_tab[i] = P.sp.tab[i];
+        __syncthreads();
+    }
+    const long long p = (long long)blockIdx.x * kBlock + threadIdx.x;
+    if (p >= P.N) return;
+    const unsigned sl = (unsigned)(p >> 5);
+    const unsigned w = P.slice_w[sl];
+    const size_t e0 = (size_t)P.slice_off[sl] * kSlice + (threadIdx.x & 31);
+    const double2 xp = P.pos_cur[p];
+    const double2 vh = P.vel[p];
+    const uint8_t g = P.grp[p];
+
+    double fx = 0.0, fy = 0.0, u = 0.0;
+    constexpr int CH = 6;
+    for (unsigned s0 = 0; s0 < w; s0 += CH) {
+        int nb[CH];
+        double2 xq[CH];
+        double pk[CH], pr0[CH], prc[CH];
+#pragma unroll
+        for (int c = 0; c < CH; ++c) nb[c] = (s0 + c < w) ? P.nbr[e0 + (size_t)(s0 + c) * kSlice] : kPad;
+#pragma unroll
+        for (int c = 0; c < CH; ++c) {
+            if (nb[c] >= 0) {
+                xq[c] = P.pos_cur[nb[c]];
+                load_params<PM>(P.sp, s_tab, e0 + (size_t)(s0 + c) * kSlice, pk[c], pr0[c], prc[c]);
+            }
+        }
+#pragma unroll
+        for (int c = 0; c < CH; ++c) {
+            if (nb[c] >= 0) {
+                const double dx = sub<EXACT>(xq[c].x, xp.x), dy = sub<EXACT>(xq[c].y, xp.y);
+                double gk, ext;
+                if (spring_eval<EXACT>(dx, dy, pk[c], pr0[c], prc[c], gk, ext)) {
+                    fx = mad<EXACT>(gk, dx, fx);
+                    fy = mad<EXACT>(gk, dy, fy);
+                    if (SAMPLE && p < nb[c])   // each spring's energy is counted once, by its lower endpoint (Eq. 1)
+                        u = add<EXACT>(u, mul<EXACT>(mul<EXACT>(mul<EXACT>(0.5, pk[c]), ext), ext));
+                } else {  // broke in this evaluation: dead from now on, zero force already in this step (Q2, Q3)
+                    const size_t e = e0 + (size_t)(s0 + c) * kSlice;
+                    P.nbr[e] = ~nb[c];
+                    if (p < nb[c]) {
+                        P.break_step[P.sid[e]] = P.step;
+                        atomicAdd(P.nbroken + spec_of(P.poff, P.B, p), 1ULL);
+                    }
+                }
+            }
+        }
+    }
+    particle_update<EXACT, KICK2, ADVANCE, SAMPLE>(P, p, xp, vh, g, fx, fy, u);
+}
+
+// First half kick + drift from a completed state (v, fd): the first kernel of every lsm_step call.
+template <bool EXACT>
+__global__ void __launch_bounds__(kBlock) k_start(const StepParams P) {
+    const long long p = (long long)blockIdx.x * kBlock + threadIdx.x;
+    if (p >= P.N) return;
+    const double2 xp = P.pos_cur[p];
+    const double2 v = P.vel[p];
+    const uint8_t g = P.grp[p];
+    if (g == kFree) {
+        const double2 fd = P.fd[p];
+        double ax, ay;
+        if (P.mass) { const double m = __ldg(P.mass + p); ax = EXACT ? __ddiv_rn(fd.x, m) : fd.x / m; ay = EXACT ? __ddiv_rn(fd.y, m) : fd.y / m; }
+        else { ax = EXACT ? __ddiv_rn(fd.x, P.mass_u) : fd.x * P.inv_mass_u; ay = EXACT ? __ddiv_rn(fd.y, P.mass_u) : fd.y * P.inv_mass_u; }
+        double2 w, xn;
+        w.x = mad<EXACT>(P.hdt, ax, v.x); w.y = mad<EXACT>(P.hdt, ay, v.y);
+        xn.x = mad<EXACT>(P.dt, w.x, xp.x); xn.y = mad<EXACT>(P.dt, w.y, xp.y);
+        P.pos_next[p] = xn;
+        P.vel[p] = w;
+    } else {
+        const double ns = (double)(P.step + 1 - P.g.n0[g]);
+        P.pos_next[p] = make_double2(mad<EXACT>(ns, P.g.dux[g], v.x), mad<EXACT>(ns, P.g.duy[g], v.y));
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Scatter path = the paper's design (one thread per spring, atomicAdd into f: PAPER.md:L88-L111) re-done with
+// packed fp64 positions, a dead bit instead of k = 0, and RED.ADD.F64 (no return value).  Kept as the measured
+// "paper design" row; the fused gather kernel above is the product path.
+// ---------------------------------------------------------------------------------------------------------------
+struct ScatterParams {
+    int32_t *si;
+    const int32_t *sj;
+    const int32_t *sid;
+    SpringParams sp;
+    long long M;
+    double *sUs;  // per-spring energy scratch (SAMPLE)
+};
+
+template <int PM, bool SAMPLE>
+__global__ void __launch_bounds__(kBlock) k_spring_scatter(const StepParams P, const ScatterParams S) {
+    constexpr bool kTab = (PM == PM_TYPED || PM == PM_KRT_RCF);
+    __shared__ double s_tab[kTab ? 3 * kMaxTypes : 1];
+    if (kTab) {
+        for (int i = threadIdx.x; i < 3 * S.sp.ntypes; i += kBlock) s_tab[i] = S.sp.tab[i];
+        __syncthreads();
+    }
+    const long long e = (long long)blockIdx.x * kBlock + threadIdx.x;
+    if (e >= S.M) return;
+    const int i = S.si[e];
+    if (i < 0) { if (SAMPLE) S.sUs[e] = 0.0; return; }
+    const int j = S.sj[e];
+    const double2 xi = P.pos_cur[i], xj = P.pos_cur[j];
+    double k, r0, rc;
+    load_params<PM>(S.sp, s_tab, (size_t)e, k, r0, rc);
+    const double dx = xj.x - xi.x, dy = xj.y - xi.y;
+    double gk, ext;
+    if (spring_eval<false>(dx, dy, k, r0, rc, gk, ext)) {
+        const double gx = gk * dx, gy = gk * dy;
+        double *fi = reinterpret_cast<double *>(P.f + i), *fj = reinterpret_cast<double *>(P.f + j);
+        atomicAdd(fi, gx); atomicAdd(fi + 1, gy);       // REDG.E.ADD.F64 (result unused)
+        atomicAdd(fj, -gx); atomicAdd(fj + 1, -gy);
+        if (SAMPLE) S.sUs[e] = 0.5 * k * ext * ext;
+    } else {
+        S.si[e] = ~i;
+        P.break_step[S.sid[e]] = P.step;
+        atomicAdd(P.nbroken + spec_of(P.poff, P.B, i), 1ULL);
+        if (SAMPLE) S.sUs[e] = 0.0;
+    }
+}
+
+// Integrate pass of the scatter path: consumes f (and zeroes it for the next spring pass when ADVANCE).
+template <bool KICK2, bool ADVANCE, bool SAMPLE>
+__global__ void __launch_bounds__(kBlock) k_integrate(const StepParams P) {
+    const long long p = (long long)blockIdx.x * kBlock + threadIdx.x;
+    if (p >= P.N) return;
+    const double2 xp = P.pos_cur[p];
+    const double2 vh = P.vel[p];
+    const uint8_t g = P.grp[p];
+    const double2 f = P.f[p];
+    // in-place variant: pos_next == pos_cur for this path
+    particle_update<false, KICK2, ADVANCE, SAMPLE>(P, p, xp, vh, g, f.x, f.y, 0.0);
+    if (ADVANCE && !SAMPLE) P.f[p] = make_double2(0.0, 0.0);
+}
+
+__global__ void __launch_bounds__(kBlock) k_zero_f(double2 *f, long long N) {
+    const long long p = (long long)blockIdx.x * kBlock + threadIdx.x;
+    if (p < N) f[p] = make_double2(0.0, 0.0);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Reductions (a6): deterministic two-level sums.  Level 1: one block per chunk of <= kChunk particles of one
+// specimen.  Level 2: one warp per specimen sums its chunk partials and its boundary groups' forces in a fixed order.
+// ---------------------------------------------------------------------------------------------------------------
+struct ReduceParams {
+    const double *sU, *sKE;
+    const double2 *f;
+    const long long *chunk_lo, *chunk_hi;  // [nchunks]
+    const int *spec_chunk_off;             // [B+1]
+    double *part;                          // [nchunks][2]
+    const int32_t *gids[kMaxGroups];       // members of each group, internal ids, sorted
+    const long long *gseg[kMaxGroups];     // [B+1] segment of each specimen inside gids[g]
+    const unsigned long long *nbroken;
+    int B;
+    long long step;
+    // outputs
+    long long *out_step;                   // scalar or NULL
+    double *out_R;                         // [B][8][2] or NULL
+    double *out_U, *out_KE;                // [B]
+    long long *out_nb;                     // [B] or NULL
+    int *flags;                            // bit 0: non-finite energy
+    // scatter path: per-spring energies summed per specimen
+    const double *sUs;
+    const long long *soff_list;            // [B+1] specimen segments of the (sorted) spring list, or NULL
+};
+
+__global__ void __launch_bounds__(kBlock) k_reduce_chunks(const ReduceParams R) {
+    __shared__ double sh[2][kBlock];
+    const int c = blockIdx.x;
+    const long long lo = R.chunk_lo[c], hi = R.chunk_hi[c];
+    double u = 0.0, ke = 0.0;
+    for (long long p = lo + threadIdx.x; p < hi; p += kBlock) { u += R.sU[p]; ke += R.sKE[p]; }
+    sh[0][threadIdx.x] = u; sh[1][threadIdx.x] = ke;
+    __syncthreads();
+    for (int s = kBlock / 2; s > 0; s >>= 1) {
+        if (threadIdx.x < s) { sh[0][threadIdx.x] += sh[0][threadIdx.x + s]; sh[1][threadIdx.x] += sh[1][threadIdx.x + s]; }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) { R.part[2 * c] = sh[0][0]; R.part[2 * c + 1] = sh[1][0]; }
+}
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+__global__ void __launch_bounds__(128) k_finalize_sample(const ReduceParams R) {
+    const int b = blockIdx.x * 4 + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
+    if (b >= R.B) return;
+    double u = 0.0, ke = 0.0;
+    for (int c = R.spec_chunk_off[b] + lane; c < R.spec_chunk_off[b + 1]; c += 32) { u += R.part[2 * c]; ke += R.part[2 * c + 1]; }
+    if (R.sUs) for (long long e = R.soff_list[b] + lane; e < R.soff_list[b + 1]; e += 32) u += R.sUs[e];
+    u = warp_sum(u); ke = warp_sum(ke);
+    if (lane == 0) {
+        R.out_U[b] = u; R.out_KE[b] = ke;
+        if (R.out_nb) R.out_nb[b] = (long long)R.nbroken[b];
+        if (!isfinite(u + ke)) atomicOr(R.flags, 1);
+        if (b == 0 && R.out_step) *R.out_step = R.step;
+    }
+    if (R.out_R) {
+        for (int g = 0; g < kMaxGroups; ++g) {
+            double rx = 0.0, ry = 0.0;
+            if (R.gids[g]) {
+                for (long long q = R.gseg[g][b] + lane; q < R.gseg[g][b + 1]; q += 32) {
+                    const double2 f = R.f[R.gids[g][q]];
+                    rx += f.x; ry += f.y;
+                }
+            }
+            rx = warp_sum(rx); ry = warp_sum(ry);
+            if (lane == 0) { R.out_R[((size_t)b * kMaxGroups + g) * 2] = rx; R.out_R[((size_t)b * kMaxGroups + g) * 2 + 1] = ry; }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Stream compaction of dead springs (a7).  Gather layout: every row is compacted in place, stably (the summation
+// order of the survivors is unchanged, so results are bit-identical), and the slice's live width shrinks to the
+// longest surviving row: dead columns are no longer read at all.
+// ---------------------------------------------------------------------------------------------------------------
+struct CompactParams {
+    const uint32_t *slice_off;
+    uint8_t *slice_w;
+    int32_t *nbr, *sid;
+    uint8_t *typ;
+    double *kF, *r0F, *rcF;
+    long long nslices;
+};
+
+__global__ void __launch_bounds__(kBlock) k_compact_ell(const CompactParams C) {
+    const long long sl = ((long long)blockIdx.x * kBlock + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (sl >= C.nslices) return;
+    const unsigned w = C.slice_w[sl];
+    const size_t e0 = (size_t)C.slice_off[sl] * kSlice + lane;
+    unsigned j = 0;
+    for (unsigned s = 0; s < w; ++s) {
+        const size_t e = e0 + (size_t)s * kSlice;
+        const int nb = C.nbr[e];
+        if (nb >= 0) {
+            if (j != s) {
+                const size_t d = e0 + (size_t)j * kSlice;
+                C.nbr[d] = nb; C.sid[d] = C.sid[e];
+                if (C.typ) C.typ[d] = C.typ[e];
+                if (C.kF) C.kF[d] = C.kF[e];
+                if (C.r0F) C.r0F[d] = C.r0F[e];
+                if (C.rcF) C.rcF[d] = C.rcF[e];
+            }
+            ++j;
+        }
+    }
+    for (unsigned s = j; s < w; ++s) C.nbr[e0 + (size_t)s * kSlice] = kPad;
+    unsigned wmax = j;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) wmax = max(wmax, __shfl_xor_sync(0xffffffffu, wmax, o));
+    if (lane == 0) C.slice_w[sl] = (uint8_t)wmax;
+}
+
+// ---- small utility kernels (numbering translation at the API boundary, boundary-group bookkeeping) ----
+// dst[perm_dst[q]] <- src[q] style copies.  inv: caller id -> internal id.
+__global__ void __launch_bounds__(kBlock) k_to_caller(const double2 *src, double2 *dst, const int32_t *inv, long long N,
+                                                      const uint8_t *grp, GroupTab g, double dt, int synth_vel) {
+    const long long c = (long long)blockIdx.x * kBlock + threadIdx.x;  // caller id
+    if (c >= N) return;
+    const int p = inv ? inv[c] : (int)c;
+    double2 v = src[p];
+    if (synth_vel) { const uint8_t gg = grp[p]; if (gg != kFree) v = make_double2(g.dux[gg] / dt, g.duy[gg] / dt); }
+    dst[c] = v;
+}
+
+__global__ void __launch_bounds__(kBlock) k_from_caller(const double2 *srcx, const double2 *srcv, double2 *pos, double2 *vel,
+                                                        const int32_t *inv, long long N, const uint8_t *grp) {
+    const long long c = (long long)blockIdx.x * kBlock + threadIdx.x;
+    if (c >= N) return;
+    const int p = inv ? inv[c] : (int)c;
+    const double2 x = srcx[c];
+    pos[p] = x;
+    vel[p] = (grp[p] != kFree) ? x : (srcv ? srcv[c] : make_double2(0.0, 0.0));  // kinematic: vel slot = origin
+}
+
+__global__ void __launch_bounds__(kBlock) k_group_release(const int32_t *ids, long long n, uint8_t *grp, double2 *vel, double vx, double vy) {
+    const long long q = (long long)blockIdx.x * kBlock + threadIdx.x;
+    if (q >= n) return;
+    grp[ids[q]] = kFree;
+    vel[ids[q]] = make_double2(vx, vy);
+}
+
+__global__ void __launch_bounds__(kBlock) k_group_assign(const int32_t *ids, long long n, uint8_t *grp, double2 *vel, const double2 *pos, uint8_t g) {
+    const long long q = (long long)blockIdx.x * kBlock + threadIdx.x;
+    if (q >= n) return;
+    grp[ids[q]] = g;
+    vel[ids[q]] = pos[ids[q]];
+}
+
+__global__ void __launch_bounds__(kBlock) k_broken_from_steps(const long long *break_step, uint8_t *broken, long long M) {
+    const long long e = (long long)blockIdx.x * kBlock + threadIdx.x;
+    if (e < M) broken[e] = break_step[e] >= 0;
+}
+
+}  // namespace lsmk

@@ -1,0 +1,363 @@
+"""GPU parity: the CUDA path through the C ABI vs the CPU oracle on the same seeded inputs.
+
+Tolerances (north_star): forces 1e-12 relative (Q11 norms); positions 1e-9 after 10^4 pre-fracture steps; broken sets
+bit-exact up to the first breakage; stress-strain curve 1e-6 up to the first breakage, peak stress / failure strain 1 %
+after; exact mode bit-identical throughout.
+"""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+import paper_2201_04565_b200 as lsm
+from paper_2201_04565_b200.binding import lsm_create_from_problem
+from lsm_inputs import (FIXED, MOVE, config1, config2, config3, config4, single_specimen, shuffle_ids,
+                        triangular_lattice)
+from oracle.olsm import OracleSim
+from parity import check_forces, force_scale
+
+MODES = [dict(force_mode=lsm.FORCE_GATHER, exact=False), dict(force_mode=lsm.FORCE_GATHER, exact=True),
+         dict(force_mode=lsm.FORCE_SCATTER, exact=False)]
+MODE_IDS = ["gather-fast", "gather-exact", "scatter"]
+
+
+@pytest.fixture(autouse=True)
+def _need_gpu():
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device: the product path has no CPU fallback")
+
+
+def _perturbed(p, amp, seed):
+    rng = np.random.default_rng(seed)
+    p.x = p.x + rng.uniform(-amp, amp, p.x.shape)
+    return p
+
+
+def _fracture_problem(n=64, du_y=4.4e-4, seed=7):
+    p = config2(n=n, seed=seed, n_blobs=24, du_y=du_y)
+    p.sample_every = 100
+    return p
+
+
+# ---------------------------------------------------------------- T1: single force evaluation
+@pytest.mark.parametrize("mode", MODES, ids=MODE_IDS)
+@pytest.mark.parametrize("reorder", [0, 1])
+@pytest.mark.parametrize("make", [lambda: _perturbed(config1(), 0.03, 1), lambda: _perturbed(config2(n=96, n_blobs=20), 0.02, 2),
+                                  lambda: _perturbed(config3(n=160), 0.02, 3), lambda: _perturbed(config4(B=3, n=24), 0.02, 4)],
+                         ids=["cfg1", "cfg2-96", "cfg3-160", "cfg4-3x24"])
+def test_T1_forces_single_evaluation(make, mode, reorder):
+    p = make()
+    o = OracleSim.from_problem(p)
+    g = lsm_create_from_problem(p, reorder=reorder, **mode)
+    fo, fg = o.read_forces(), g.read_forces()
+    bo, _, nbo = o.read_broken()
+    bg, _, nbg = g.read_broken()
+    assert nbo == nbg and np.array_equal(bo, bg)          # perturbation may break a few brittle springs at step 0
+    sc = force_scale(p.x, p.spring_i, p.spring_j, p.k, p.r0, ~bo)
+    if mode["exact"]:
+        assert np.array_equal(fo, fg)
+    else:
+        check_forces(fg, fo, sc)
+    Uo, KEo = o.read_energy(); Ug, KEg = g.read_energy()
+    assert np.allclose(Ug, Uo, rtol=1e-12, atol=0) and np.allclose(KEg, KEo, rtol=1e-12, atol=1e-300)
+    g.close()
+
+
+# ---------------------------------------------------------------- T2: 10^4 pre-fracture steps of config 1
+@pytest.mark.parametrize("mode", MODES, ids=MODE_IDS)
+def test_T2_config1_positions_after_1e4_steps(mode):
+    p = config1()
+    o = OracleSim.from_problem(p); o.step(10000)
+    g = lsm_create_from_problem(p, **mode); g.step(10000)
+    xo, vo = o.read_state(); xg, vg = g.read_state()
+    assert o.read_broken()[2] == 0 and g.n_broken() == 0
+    if mode["exact"]:
+        assert np.array_equal(xo, xg) and np.array_equal(vo, vg)
+    else:
+        assert np.abs(xg - xo).max() <= 1e-9 and np.abs(vg - vo).max() <= 1e-9
+    ho, hg = o.read_stress(), g.read_stress()
+    assert np.array_equal(ho["step"], hg["step"]) and len(hg["step"]) == 100
+    for key in ("R", "U", "KE"):
+        den = np.abs(ho[key]).max()
+        assert np.abs(hg[key] - ho[key]).max() <= 1e-9 * den, key
+    fo, fg = o.read_forces(), g.read_forces()
+    assert np.abs(fg - fo).max() <= 1e-10 * np.abs(fo).max()
+    g.close()
+
+
+# ---------------------------------------------------------------- T3/T4/T5: fracture run, fast modes
+def _curve(h, p):
+    sig = -h["R"][:, 0, 1, 1] / p.meta["W0"]
+    return sig
+
+
+def _peak_and_failure(step, sig, du_y, H0):
+    ip = int(np.argmax(sig))
+    after = np.flatnonzero(sig[ip:] < 0.1 * sig[ip])
+    eps_f = (step[ip + after[0]] * du_y / H0) if after.size else None
+    return sig[ip], step[ip] * du_y / H0, eps_f
+
+
+@pytest.mark.parametrize("mode", [MODES[0], MODES[2]], ids=["gather-fast", "scatter"])
+def test_T3_T4_T5_fracture_curve(mode):
+    p = _fracture_problem()
+    nsteps = 9000
+    o = OracleSim.from_problem(p); o.step(nsteps)
+    g = lsm_create_from_problem(p, **mode); g.step(nsteps)
+    ho, hg = o.read_stress(), g.read_stress()
+    bo, bso, nbo = o.read_broken(); bg, bsg, nbg = g.read_broken()
+    assert nbo > 10, "the test problem must actually fracture"
+    first = bso[bso >= 0].min()
+    # T3: identical first breakage (same spring, same step)
+    assert bsg[bsg >= 0].min() == first
+    assert np.array_equal(np.flatnonzero(bso == first), np.flatnonzero(bsg == first))
+    # T4: curve up to the first breakage within 1e-6 (relative to the curve's max)
+    pre = ho["step"] < first
+    so, sg = _curve(ho, p), _curve(hg, p)
+    assert np.abs(sg[pre] - so[pre]).max() <= 1e-6 * np.abs(so[pre]).max()
+    for key in ("U", "KE"):
+        assert np.abs(hg[key][pre] - ho[key][pre]).max() <= 1e-6 * np.abs(ho[key][pre]).max()
+    assert np.array_equal(hg["n_broken"][pre], ho["n_broken"][pre])
+    # T5: after the first breakage: peak stress and failure strain within 1 %
+    du_y, H0 = p.groups[1].du[1], p.meta["H0"]
+    pk_o, ep_o, ef_o = _peak_and_failure(ho["step"], so, du_y, H0)
+    pk_g, ep_g, ef_g = _peak_and_failure(hg["step"], sg, du_y, H0)
+    assert abs(pk_g / pk_o - 1) <= 0.01 and abs(ep_g / ep_o - 1) <= 0.01
+    if ef_o is not None:
+        assert ef_g is not None and abs(ef_g / ef_o - 1) <= 0.01
+    assert abs(nbg - nbo) <= max(5, 0.05 * nbo)
+    g.close()
+
+
+# ---------------------------------------------------------------- T6: exact mode is bit-identical through fracture
+@pytest.mark.parametrize("reorder,compact", [(0, 0), (1, 500)])
+def test_T6_exact_mode_bit_identical_fracture(reorder, compact):
+    p = _fracture_problem()
+    o = OracleSim.from_problem(p); o.step(9000)
+    g = lsm_create_from_problem(p, force_mode=lsm.FORCE_GATHER, exact=True, reorder=reorder, compact_every=compact)
+    g.step(4000); g.step(1); g.step(4999)                 # also crosses lsm_step call boundaries
+    xo, vo = o.read_state(); xg, vg = g.read_state()
+    bo, bso, nbo = o.read_broken(); bg, bsg, nbg = g.read_broken()
+    assert nbo > 10
+    assert np.array_equal(bso, bsg) and np.array_equal(bo, bg) and nbo == nbg
+    assert np.array_equal(xo, xg) and np.array_equal(vo, vg)
+    assert np.array_equal(o.read_forces(), g.read_forces())
+    ho, hg = o.read_stress(), g.read_stress()
+    assert np.array_equal(ho["n_broken"], hg["n_broken"]) and np.array_equal(ho["step"], hg["step"])
+    for key in ("R", "U", "KE"):
+        assert np.abs(hg[key] - ho[key]).max() <= 1e-12 * np.abs(ho[key]).max(), key
+    g.close()
+
+
+# ---------------------------------------------------------------- T7: renumbering / compaction / shuffled input order
+@pytest.mark.parametrize("mode", MODES, ids=MODE_IDS)
+def test_T7_reorder_compaction_shuffle_transparent(mode):
+    p = _fracture_problem(n=48, du_y=6e-4)
+    q = shuffle_ids(p, 99)
+    nsteps = 6000
+    o = OracleSim.from_problem(p); o.step(nsteps)
+    xo, vo = o.read_state(); bo, bso, nbo = o.read_broken()
+    assert nbo > 0
+    first = bso[bso >= 0].min()
+    for prob, reorder, compact in [(p, 1, 0), (p, 0, 300), (q, 1, 300), (q, 0, 0)]:
+        g = lsm_create_from_problem(prob, reorder=reorder, compact_every=compact, **mode)
+        g.step(nsteps)
+        xg, vg = g.read_state(); bg, bsg, nbg = g.read_broken()
+        if prob is q:       # translate back to p's numbering
+            xg2 = np.empty_like(xg); xg2[q.meta["perm"]] = xg; xg = xg2
+            bs2 = np.empty_like(bsg); bs2[q.meta["spring_perm"]] = bsg; bsg = bs2
+        if mode["exact"] and prob is p:
+            assert np.array_equal(xg, xo) and np.array_equal(bsg, bso)
+        else:               # a shuffled spring order changes the oracle's own summation order: tolerance tier
+            assert bsg[bsg >= 0].min() == first
+            assert abs(nbg - nbo) <= max(3, 0.1 * nbo)
+        g.close()
+
+
+# ---------------------------------------------------------------- T8: batch independence
+@pytest.mark.parametrize("mode", MODES, ids=MODE_IDS)
+def test_T8_batch_equals_individual(mode):
+    B, n, nsteps = 5, 32, 3000
+    pb = config4(B=B, n=n)
+    pb.sample_every = 100
+    g = lsm_create_from_problem(pb, reorder=1, **mode); g.step(nsteps)
+    xg, vg = g.read_state(); hg = g.read_stress(); bg, bsg, nbg = g.read_broken()
+    ob = OracleSim.from_problem(pb); ob.step(nsteps)
+    hb = ob.read_stress()
+    for b in range(B):
+        p1 = single_specimen(b, n); p1.sample_every = 100
+        o = OracleSim.from_problem(p1); o.step(nsteps)
+        xo, vo = o.read_state(); ho = o.read_stress(); bo, bso, nbo = o.read_broken()
+        sl = slice(pb.particle_offsets[b], pb.particle_offsets[b + 1])
+        ss = slice(pb.spring_offsets[b], pb.spring_offsets[b + 1])
+        if mode["exact"]:
+            assert np.array_equal(xg[sl], xo) and np.array_equal(vg[sl], vo) and np.array_equal(bsg[ss], bso)
+            assert np.array_equal(hg["n_broken"][:, b], ho["n_broken"][:, 0])
+        elif nbo == 0:
+            assert np.abs(xg[sl] - xo).max() <= 1e-9 and np.abs(vg[sl] - vo).max() <= 1e-9
+        pre = ho["n_broken"][:, 0] == 0
+        for key in ("R", "U", "KE"):
+            a, r = hg[key][:, b][pre], ho[key][:, 0][pre]
+            assert np.abs(a - r).max() <= 1e-6 * np.abs(r).max(), (key, b)
+    g.close()
+
+
+# ---------------------------------------------------------------- paper example and pins re-run on the GPU
+@pytest.mark.parametrize("mode", MODES, ids=MODE_IDS)
+def test_paper_oscillator_on_gpu(mode):
+    """PAPER.md:L123-L127 through the CUDA path: closed form of velocity Verlet, 1e-11."""
+    x = np.array([[0.0, 0.0], [15.0, 0.0]])
+    g = lsm.lsm_create(x, [0], [1], 1e-4, 10.0, 100.0, 1.0, **mode)
+    g.set_boundary(0, [0], FIXED)
+    th = np.arccos(1.0 - 1e-4 / 2.0)
+    for n in range(1, 1001):
+        g.step(1)
+        if n % 10 == 0:
+            xx, _ = g.read_state()
+            assert abs(xx[1, 0] - (10.0 + 5.0 * np.cos(n * th))) <= 1e-11
+            assert xx[0, 0] == 0.0
+    g.close()
+
+
+@pytest.mark.parametrize("mode", MODES, ids=MODE_IDS)
+def test_strict_greater_and_irreversible_on_gpu(mode):
+    """P7/P8 on the GPU: r == rc survives (dyadic, exact in every mode), breakage is irreversible."""
+    x = np.array([[0.0, 0.0], [1.0, 0.0]])
+    g = lsm.lsm_create(x, [0], [1], 1.0, 1.0, 1.125, 1.0, sample_every=1, **mode)
+    g.set_boundary(0, [0], FIXED)
+    g.set_boundary(1, [1], MOVE, [2.0 ** -10, 0.0])
+    g.step(128)
+    b, bs, nb = g.read_broken()
+    assert nb == 0 and bs[0] == -1 and g.read_state()[0][1, 0] == 1.125
+    assert abs(g.read_forces()[1, 0] + 0.125) < 1e-15
+    g.step(1)
+    b, bs, nb = g.read_broken()
+    assert nb == 1 and b[0] and bs[0] == 129 and np.all(g.read_forces() == 0.0)
+    g.set_boundary(1, [1], MOVE, [-2.0 ** -10, 0.0])
+    g.step(129)
+    assert g.read_state()[0][1, 0] == 1.0 and np.all(g.read_forces() == 0.0) and g.read_energy()[0][0] == 0.0
+    h = g.read_stress()
+    assert h["n_broken"][127, 0] == 0 and h["n_broken"][128, 0] == 1 and h["n_broken"][-1, 0] == 1
+    g.close()
+
+
+# ---------------------------------------------------------------- edge cases
+def test_edge_cases_degenerate_inputs():
+    # no springs at all; N = 1; N not a multiple of the slice width; free flight
+    x = np.array([[0.0, 0.0]])
+    g = lsm.lsm_create(x, [], [], 1.0, 1.0, 2.0, 0.5, v=np.array([[1.0, -2.0]]))
+    g.step(4)
+    xx, vv = g.read_state()
+    assert np.array_equal(xx, [[2.0, -4.0]]) and np.array_equal(vv, [[1.0, -2.0]])
+    assert g.read_broken()[2] == 0
+    g.close()
+    # a star with a degree-40 hub (beyond any lattice degree), an isolated particle and a coincident pair (r = 0)
+    n = 40
+    ang = np.linspace(0, 2 * np.pi, n, endpoint=False)
+    x = np.concatenate([[[0.0, 0.0]], np.stack([1.2 * np.cos(ang), 1.2 * np.sin(ang)], 1), [[5.0, 5.0]], [[7.0, 7.0]], [[7.0, 7.0]]])
+    si = np.concatenate([np.zeros(n, dtype=np.int32), [n + 2]]).astype(np.int32)
+    sj = np.concatenate([np.arange(1, n + 1), [n + 3]]).astype(np.int32)
+    k = np.linspace(0.5, 1.5, n + 1); r0 = np.ones(n + 1); rc = np.full(n + 1, 3.0)
+    for mode in MODES:
+        o = OracleSim(x, si, sj, k, r0, rc, 0.01); gg = lsm.lsm_create(x, si, sj, k, r0, rc, 0.01, **mode)
+        o.step(50); gg.step(50)
+        xo, vo = o.read_state(); xg, vg = gg.read_state()
+        assert np.all(np.isfinite(xg)) and np.abs(xg - xo).max() <= 1e-12 and np.abs(vg - vo).max() <= 1e-12
+        assert np.array_equal(xg[n + 1], [5.0, 5.0]) and np.array_equal(xg[n + 2], [7.0, 7.0])
+        gg.close()
+
+
+def test_invalid_inputs_are_rejected():
+    x = np.array([[0.0, 0.0], [1.0, 0.0], [2.0, 0.0]])
+    for args, status in [((x, [0], [0], 1.0, 1.0, 2.0, 0.01), -2), ((x, [0], [3], 1.0, 1.0, 2.0, 0.01), -2),
+                         ((x, [0], [1], -1.0, 1.0, 2.0, 0.01), -3), ((x, [0], [1], 1.0, np.nan, 2.0, 0.01), -3),
+                         ((x, [0], [1], 1.0, 1.0, 2.0, 0.0), -1)]:
+        with pytest.raises(lsm.LsmError) as ei:
+            lsm.lsm_create(*args)
+        assert ei.value.status == status
+    xb = x.copy(); xb[1, 1] = np.inf
+    with pytest.raises(lsm.LsmError) as ei:
+        lsm.lsm_create(xb, [0], [1], 1.0, 1.0, 2.0, 0.01)
+    assert ei.value.status == -3
+    g = lsm.lsm_create(x, [0, 1], [1, 2], 1.0, 1.0, 2.0, 0.01)
+    g.set_boundary(0, [0], FIXED)
+    with pytest.raises(lsm.LsmError):
+        g.set_boundary(1, [0], FIXED)                      # already in group 0
+    with pytest.raises(lsm.LsmError):
+        g.set_boundary(9, [1], FIXED)
+    g.close()
+    # springs must not cross specimens
+    with pytest.raises(lsm.LsmError) as ei:
+        lsm.lsm_create(x, [0, 1], [1, 2], 1.0, 1.0, 2.0, 0.01, n_batch=2, particle_offsets=[0, 2, 3], spring_offsets=[0, 1, 2])
+    assert ei.value.status == -2
+
+
+def test_nonfinite_state_is_detected_and_sticky():
+    p = config1(16, 16)
+    g = lsm_create_from_problem(p, gamma=0.0)
+    g2 = lsm.lsm_create(p.x, p.spring_i, p.spring_j, 1.0, 1.0, 1e9, 5.0, sample_every=10)   # dt far above stability
+    rng = np.random.default_rng(0)
+    g2.write_state(p.x + rng.uniform(-0.1, 0.1, p.x.shape))
+    g2.step(4000)
+    with pytest.raises(lsm.LsmError) as ei:
+        g2.read_energy()
+    assert ei.value.status == -6
+    with pytest.raises(lsm.LsmError):
+        g2.step(1)
+    g.close(); g2.close()
+
+
+def test_history_ring_wraps_and_restart_resumes():
+    p = config1(24, 24); p.sample_every = 10
+    g = lsm_create_from_problem(p, history_capacity=8)
+    g.step(200)
+    h = g.read_stress()
+    assert list(h["step"]) == list(range(130, 201, 10))     # the latest 8 samples, oldest first
+    assert len(g.read_stress()["step"]) == 0
+    # checkpoint / resume: read_state -> fresh handle -> same continuation as the uninterrupted run (exact mode)
+    a = lsm_create_from_problem(p, exact=True); a.step(300)
+    b = lsm_create_from_problem(p, exact=True); b.step(120)
+    xb, vb = b.read_state()
+    c = lsm.lsm_create(xb, p.spring_i, p.spring_j, p.k, p.r0, p.rc, p.dt, gamma=p.gamma, v=vb, exact=True)
+    for gi, gr in enumerate(p.groups):
+        c.set_boundary(gi, gr.ids, gr.mode, gr.du)
+    c.step(180)
+    xa, va = a.read_state(); xc, vc = c.read_state()
+    # the restarted run re-derives fd from the FULL-step velocity (the half-step one is not part of the public state):
+    # agreement is to rounding of the damping term, not bit-exact
+    assert np.abs(xa - xc).max() <= 1e-9 and np.abs(va - vc).max() <= 1e-9
+    for s in (g, a, b, c):
+        s.close()
+
+
+def test_write_state_matches_oracle():
+    p = _perturbed(config1(20, 20), 0.0, 0)
+    o = OracleSim.from_problem(p); g = lsm_create_from_problem(p, exact=True)
+    o.step(50); g.step(50)
+    rng = np.random.default_rng(5)
+    xn = p.x + rng.uniform(-0.02, 0.02, p.x.shape); vn = rng.normal(0, 1e-3, p.x.shape)
+    o.write_state(xn, vn); g.write_state(xn, vn)
+    assert np.array_equal(o.read_forces(), g.read_forces())
+    o.step(100); g.step(100)
+    assert np.array_equal(o.read_state()[0], g.read_state()[0]) and np.array_equal(o.read_state()[1], g.read_state()[1])
+    g.close()
+
+
+# ---------------------------------------------------------------- full-size check in the bench launch configuration
+def test_full_size_config3_bench_configuration():
+    """BASELINE.json configs[2] at full size, default (bench) launch configuration: 20 steps against the oracle on all
+    particles, plus size-independent properties (zero net internal force)."""
+    p = config3()
+    o = OracleSim.from_problem(p)
+    g = lsm_create_from_problem(p)
+    inf = g.info()
+    assert inf["param_mode"] == 2 and inf["force_mode"] == lsm.FORCE_GATHER
+    o.step(20); g.step(20)
+    xo, vo = o.read_state(); xg, vg = g.read_state()
+    assert np.abs(xg - xo).max() <= 1e-12 and np.abs(vg - vo).max() <= 1e-12
+    fo, fg = o.read_forces(), g.read_forces()
+    assert np.abs(fg - fo).max() <= 1e-12 * np.abs(fo).max()
+    assert np.abs(fg.sum(axis=0)).max() <= 1e-9 * np.abs(fg).sum()
+    assert g.n_broken() == o.read_broken()[2]
+    g.close()
