@@ -672,6 +672,9 @@ lsm_status lsm_set_boundary(lsm_sim *s, int32_t gi, const int32_t *ids, int64_t 
         s->kernels_launched += 1;
     }
     CUDA_TRY(s, cudaGetLastError());
+    // membership changed: refresh fd (released particles are damped again) and the per-particle energy terms
+    // (kinematic particles carry no KE).  Positions are unchanged, so no spring can break here.
+    TRY(eval_initial(s));
     CUDA_TRY(s, cudaStreamSynchronize(s->stream));
     return LSM_OK;
 }
