@@ -1,0 +1,314 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the lattice-spring step on B200 (BASELINE.json metric: spring-updates/s).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--inner S] [--workload cfg3|cfg2|cfg4|cfg5|cfg1]
+    python bench.py --impl reference ...          # the CPU oracle, as it stands, on the host cores
+
+Workload (config.workload): BASELINE.json configs[2], the 2048x2048 porous lattice -- the configuration north_star's
+target ("the 4M-particle lattice", >= 60 % of HBM) is quoted on.  Synthetic and seeded (lsm_inputs.config3).
+
+A bench "step" is one lsm_step(S) call: S = --inner consecutive time steps of the whole hot path (boundary
+displacement, kick + drift, spring forces + breakage, damping + kick, the sample reductions every 100 time steps and
+the scheduled compaction), on state already resident in HBM.  value = live springs x time steps / second over all
+ranks.  The per-step traffic (~400 MB) is larger than the 126 MB L2, so consecutive time steps cannot serve each other
+from cache (config.l2: "inputs larger than L2").
+
+e2e: the same K bench steps through the C ABI with HOST buffers inside the timed region: lsm_write_state from pinned
+host memory (x, v) -> lsm_step(S) -> lsm_read_state into pinned host memory + lsm_read_stress.
+
+N > 1 (torchrun): the path runs on one GPU by construction (north_star; replicas only), so each
+rank steps an independent replica of the workload; no data-path collective; scaling = "weak".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "spring_updates_per_s"
+UNIT = "springs*steps/s"
+SAMPLE_EVERY = 100
+
+
+def make_problem(name):
+    import lsm_inputs as gen
+    if name == "cfg3":
+        return gen.config3(), "BASELINE.json configs[2]: 2048x2048 porous lattice, 30 % seeded circular voids, k=1, rc~U[1.05,1.15] per spring, fp64"
+    if name == "cfg2":
+        return gen.config2(), "BASELINE.json configs[1]: 512x512 two-phase composite (L2-resident)"
+    if name == "cfg1":
+        return gen.config1(), "BASELINE.json configs[0]: 64x64 lattice (latency-bound)"
+    if name == "cfg4":
+        return gen.config4(), "BASELINE.json configs[3]: 1024 x 128x128 two-phase specimens, batched"
+    if name == "cfg4s":
+        return gen.config4(B=128), "BASELINE.json configs[3] reduced to 128 specimens"
+    if name == "cfg5":
+        return gen.config5(), "BASELINE.json configs[4]: 8192x8192 notched lattice"
+    if name == "cfg5s":
+        return gen.config5(n=4096), "BASELINE.json configs[4] reduced to 4096x4096"
+    raise SystemExit("unknown workload " + name)
+
+
+def counted_bytes(N, M_alive, p_var):
+    """SURVEY.md 8(d) / DESIGN.md "Counted bytes": x and v read and written once, two int32 ids per live spring, fp64
+    parameters that truly vary per spring, one alive bit."""
+    return 64.0 * N + M_alive * (8.0 + 8.0 * p_var) + M_alive / 8.0
+
+
+def p_var_of(p):
+    """Number of spring parameters with more than 256 distinct values (a smaller set is a type table)."""
+    return int(sum(1 for a in (p.k, p.r0, p.rc) if np.unique(a[: min(a.size, 2_000_000)]).size > 256))
+
+
+class ClockSampler:
+    """nvidia-smi sampler (the profiling recipe's clocks line); samples are stamped on receipt."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.samples = []
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits", "-lms", "50"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.samples.append((time.monotonic(), [t.strip() for t in line.split(",")]))
+
+    def wait_first(self, timeout=10.0):
+        t0 = time.monotonic()
+        while self.proc and not self.samples and time.monotonic() - t0 < timeout:
+            time.sleep(0.05)
+
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=5)
+            except Exception:
+                self.proc.kill()
+
+    def summary(self, t0, t1):
+        rows = [r for (t, r) in self.samples if t0 <= t <= t1 and len(r) >= 8] or [r for (_, r) in self.samples[-3:] if len(r) >= 8]
+        if not rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        sm = [float(r[0]) for r in rows]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(r[4 + i].lower().startswith("active") for r in rows)]
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": float(rows[0][1]), "reasons": reasons, "samples": len(rows),
+                "power_w_max": max(float(r[2]) for r in rows)}
+
+
+def time_oracle(p, n_steps, warm=1):
+    """Time the CPU oracle as it stands (serial, 1 thread) on `n_steps` time steps of problem p."""
+    from oracle.olsm import OracleSim
+    o = OracleSim.from_problem(p)
+    o.step(warm)
+    t0 = time.perf_counter()
+    o.step(n_steps)
+    dt = time.perf_counter() - t0
+    nb = o.read_broken()[2]
+    o.close()
+    return dt, nb
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, same config / metric / unit; each step a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    p, desc = make_problem(args.workload)
+    from oracle.olsm import OracleSim
+    inner = args.ref_inner
+    o = OracleSim.from_problem(p)
+    for _ in range(args.warmup):
+        o.step(inner)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        o.step(inner)
+    dt = time.perf_counter() - t0
+    o.close()
+    val = p.M * inner * args.steps / dt
+    sample = "%d bench steps of %d time steps each of the full workload (serial oracle, 1 thread)" % (args.steps, inner)
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": desc, "N": p.N, "M": p.M, "time_steps_per_bench_step": inner},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--inner", type=int, default=500, help="time steps per bench step (one lsm_step call)")
+    ap.add_argument("--ref-inner", type=int, default=2, help="time steps per bench step of --impl reference")
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--workload", default="cfg3")
+    ap.add_argument("--force-mode", default="auto", choices=["auto", "gather", "scatter", "tile"])
+    ap.add_argument("--reorder", type=int, default=0)
+    ap.add_argument("--compact-every", type=int, default=1000)
+    ap.add_argument("--exact", type=int, default=0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-steps", type=int, default=0, help="oracle time steps for cpu_baseline (0 = sized to ~15 s)")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "b200":
+        args.warmup = 3                        # timing rule: W >= 3
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import paper_2201_04565_b200 as lsm
+    from paper_2201_04565_b200.binding import lsm_create_from_problem
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    p, desc = make_problem(args.workload)
+    p.sample_every = SAMPLE_EVERY
+    fm = {"auto": lsm.FORCE_AUTO, "gather": lsm.FORCE_GATHER, "scatter": lsm.FORCE_SCATTER, "tile": getattr(lsm, "FORCE_TILE", 3)}[args.force_mode]
+    sim = lsm_create_from_problem(p, device=local, force_mode=fm, reorder=args.reorder, compact_every=args.compact_every,
+                                  exact=bool(args.exact), history_capacity=64)
+    inf0 = sim.info()
+    M_alive0 = p.M - sim.n_broken()
+    S, K, W = args.inner, args.steps, args.warmup
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    sampler = ClockSampler(local) if rank == 0 else None
+    if sampler:
+        sampler.wait_first()
+
+    # ---------------- device-resident throughput ----------------
+    for _ in range(W):
+        sim.step(S)
+    sim.read_stress()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    l0 = sim.info()["kernels_launched"]
+    tw0 = time.monotonic()
+    ev0.record()                               # the library enqueues on torch's current stream
+    for _ in range(K):
+        sim.step(S)
+    ev1.record()
+    barrier()
+    tw1 = time.monotonic()
+    ms = ev0.elapsed_time(ev1)
+    launches = sim.info()["kernels_launched"] - l0
+    nb_after = sim.n_broken()
+
+    # ---------------- end to end through the C ABI with host buffers ----------------
+    xh = torch.empty((p.N, 2), dtype=torch.float64, pin_memory=True)
+    vh = torch.empty((p.N, 2), dtype=torch.float64, pin_memory=True)
+    xo = torch.empty((p.N, 2), dtype=torch.float64, pin_memory=True)
+    vo = torch.empty((p.N, 2), dtype=torch.float64, pin_memory=True)
+    sim.read_state(xh.numpy(), vh.numpy())
+    d2h_hist = 0
+    for it in range(2 + K):                    # 2 untimed warm-up rounds
+        if it == 2:
+            barrier()
+            te0 = time.perf_counter()
+        sim.write_state(xh, vh)
+        sim.step(S)
+        sim.read_state(xo.numpy(), vo.numpy())
+        h = sim.read_stress()
+        d2h_hist = sum(a.nbytes for a in h.values())
+        xh, xo = xo, xh
+        vh, vo = vo, vh
+    barrier()
+    te = time.perf_counter() - te0
+    assert np.isfinite(h["U"]).all()
+
+    t_all = torch.tensor([ms, te * 1e3], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(t_all, op=dist.ReduceOp.MAX)
+    ms_max, te_ms_max = float(t_all[0]), float(t_all[1])
+    if sampler:
+        sampler.stop()
+
+    if rank == 0:
+        peaks = {}
+        try:
+            peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        except Exception:
+            pass
+        peak = float(peaks.get("hbm_gbs", 6650.0))
+        peak_src = "measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
+        pv = p_var_of(p)
+        bc = counted_bytes(p.N, M_alive0, pv)
+        t_launch = ms_max * 1e-3 / (K * S)     # upper bound of the step kernel's mean duration: every other launch in
+        ach = bc / t_launch / 1e9              # the region (start/end, reductions, compaction) is charged to it
+        value = world * M_alive0 * S * K / (ms_max * 1e-3)
+        e2e = world * M_alive0 * S * K / (te_ms_max * 1e-3)
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": desc, "N": p.N, "M": p.M, "M_alive_at_start": M_alive0, "broken_at_end": nb_after,
+                       "time_steps_per_bench_step": S, "ns_per_time_step": 1e6 * ms_max / (K * S), "sample_every": SAMPLE_EVERY,
+                       "compact_every": args.compact_every, "force_mode": inf0["force_mode"], "param_mode": inf0["param_mode"],
+                       "exact": inf0["exact"], "reorder": inf0["reorder"], "bytes_per_half_edge": inf0["bytes_per_half_edge"],
+                       "half_edges_stored": inf0["n_half_edges_stored"], "device_bytes": inf0["device_bytes"],
+                       "l2": "inputs larger than L2 (%.0f MB touched per time step vs 126 MB L2)" % (bc / 1e6),
+                       "parallelism": "replicas x%d" % world if world > 1 else "1 GPU"},
+            "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 2 * xh.numel() * 8, "d2h_bytes_per_step": 2 * xh.numel() * 8 + d2h_hist,
+                    "ms_per_step": te_ms_max / K},
+            "gpu_launches": int(launches),
+            "roofline": {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": None,
+                         "peak_source": peak_src, "frac_of_nominal_8TBs": ach / 8000.0, "counted_bytes_per_time_step": bc,
+                         "p_var": pv, "kernel": "fused step kernel (one launch per time step)",
+                         "duration_us": t_launch * 1e6},
+            "clocks": sampler.summary(tw0, tw1) if sampler else None,
+        }
+        tr = os.path.join(ROOT, "profiles", "traffic_%s.json" % args.workload)
+        if os.path.exists(tr):                 # per-launch DRAM bytes of the step kernel from the committed ncu --set full capture
+            try:
+                line["roofline"]["traffic"] = json.load(open(tr)).get("dram_bytes_per_launch")
+            except Exception:
+                pass
+        if not args.no_cpu_baseline:
+            import lsm_inputs as gen
+            n_cpu = args.cpu_steps or max(2, int(15.0 * 4.0e7 / max(p.M, 1)))
+            dt_o, _ = time_oracle(p, n_cpu)
+            line["cpu_baseline"] = {"value": p.M * n_cpu / dt_o, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                    "sample": "first %d time steps of the same workload (after 1 warm-up step), serial oracle" % n_cpu,
+                                    "seconds": dt_o}
+        print(json.dumps(line))
+    sim.close()
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
