@@ -36,7 +36,7 @@ extern "C" {
 #endif
 
 #define LSM_MAX_GROUPS 8
-#define LSM_ABI_VERSION 1
+#define LSM_ABI_VERSION 2
 
 typedef struct lsm_sim lsm_sim; /* opaque */
 
@@ -54,6 +54,9 @@ typedef enum {
 enum { LSM_FIXED = 0, LSM_MOVE = 1 };                      /* boundary group modes */
 enum { LSM_FORCE_AUTO = 0, LSM_FORCE_SCATTER = 1, LSM_FORCE_GATHER = 2 };
 enum { LSM_REORDER_NONE = 0, LSM_REORDER_MORTON = 1, LSM_REORDER_RCM = 2 };
+/* kernels of the gather path: DIRECT = one thread per particle reading global memory; STREAMED = persistent CTAs,
+ * bulk-async-copy (TMA engine) staging of the tile streams through a shared-memory mbarrier pipeline */
+enum { LSM_GATHER_AUTO = 0, LSM_GATHER_DIRECT = 1, LSM_GATHER_STREAMED = 2 };
 
 /* Optional device allocator (the Python binding passes PyTorch's caching allocator). */
 typedef void *(*lsm_alloc_fn)(size_t bytes, void *user);  /* returns a DEVICE pointer, NULL on failure */
@@ -86,7 +89,9 @@ typedef struct lsm_desc {
                                          ascending caller spring id -> bit-identical to a serial loop over the
                                          spring list (GATHER only).  0: fast arithmetic (FMA, rsqrt)              */
     int32_t use_graph;                /* 1: replay the step loop from CUDA graphs (small, launch-bound problems)  */
+    int32_t gather_variant;           /* LSM_GATHER_*: AUTO = STREAMED when a tile's rows fit in shared memory    */
     int32_t device;                   /* CUDA device ordinal                                                      */
+    int32_t _pad1;
     void *stream;                     /* cudaStream_t, NULL = the default stream                                  */
     lsm_alloc_fn alloc;               /* NULL -> cudaMalloc / cudaFree                                            */
     lsm_free_fn free_;
@@ -98,13 +103,18 @@ typedef struct lsm_info {
     int64_t n_particles, n_springs;
     int64_t n_half_edges_stored;      /* gather: ELL slots incl. padding; scatter: list length                    */
     int64_t bytes_per_half_edge;      /* id + parameter bytes read per stored slot                                */
-    int32_t param_mode;               /* 0 uniform, 1 typed (1 B), 2 k,r0 uniform + rc fp64, 3 k,r0 typed + rc fp64,
-                                         4 k, r0, rc all fp64                                                     */
+    int32_t param_mode;               /* 0 uniform, 1 typed (1 B), 2 k,r0 uniform + rc per spring, 3 k,r0 typed + rc per
+                                         spring, 4 k, r0, rc all per spring.  Gather layout: a per-spring rc costs 4 B
+                                         per half-edge (fp32 lower bound; the exact fp64 rc is read only when r is
+                                         within one fp32 ulp of it, so the decision is always the fp64 one)       */
     int32_t n_types;
     int32_t force_mode, exact, reorder, n_batch;
     int64_t device_bytes;             /* device memory owned by the handle                                        */
     int64_t kernels_launched;         /* cumulative count of kernels this handle enqueued                         */
     int64_t current_step;
+    int32_t gather_variant;           /* resolved LSM_GATHER_* (0 for the scatter path)                           */
+    int32_t pipeline_stages;          /* streamed variant: stages of the shared-memory pipeline                   */
+    int64_t stage_bytes;              /* streamed variant: bytes per stage                                        */
 } lsm_info;
 
 /* Build a simulation from particle / spring arrays.  Copies everything (the caller may free its inputs afterwards),

@@ -56,10 +56,15 @@ struct lsm_sim {
     double *mass = nullptr;
     int cur = 0;
     // gather layout
-    long long nslices = 0, E = 0;
-    uint32_t *slice_off = nullptr;
-    uint8_t *slice_w = nullptr;
+    long long nslices = 0, E = 0, T = 0, Npad = 0;
+    TileHdr *hdr = nullptr;
     int32_t *nbr = nullptr, *sid = nullptr;
+    float *rc32 = nullptr;
+    double *rcS = nullptr;
+    int gather_variant = 0;          // resolved: 1 direct, 2 streamed
+    StageLayout L;
+    int stream_smem = 0, stream_grid = 0;
+    uint32_t max_tile_slots = 0;
     // scatter layout
     long long Ms = 0;
     int32_t *ssi = nullptr, *ssj = nullptr, *ssid = nullptr;
@@ -177,8 +182,9 @@ StepParams step_params(const lsm_sim *s, long long step) {
     P.mass_u = s->mass_u; P.inv_mass_u = 1.0 / s->mass_u;
     P.dt = s->dt; P.hdt = 0.5 * s->dt; P.gamma = s->gamma;
     P.N = s->N; P.step = step;
-    P.slice_off = s->slice_off; P.slice_w = s->slice_w; P.nbr = s->nbr; P.sid = s->sid;
+    P.hdr = s->hdr; P.T = s->T; P.nbr = s->nbr; P.sid = s->sid;
     P.sp.typ = s->typ; P.sp.kF = s->kF; P.sp.r0F = s->r0F; P.sp.rcF = s->rcF; P.sp.tab = s->tab; P.sp.ntypes = s->ntypes;
+    P.sp.rc32 = s->rc32; P.sp.rcS = s->rcS;
     P.sp.k_u = s->k_u; P.sp.r0_u = s->r0_u; P.sp.rc_u = s->rc_u;
     P.break_step = s->break_step; P.nbroken = s->nbroken; P.poff = s->d_poff; P.B = s->B;
     P.sU = s->sU; P.sKE = s->sKE;
@@ -216,10 +222,44 @@ template <bool EXACT> void launch_gather_pm(int pm, const StepParams &P, Variant
     }
 }
 
+template <int PM, bool EXACT, bool KICK2, bool ADVANCE, bool SAMPLE> void launch_stream_one(const lsm_sim *s, const StepParams &P) {
+    auto kern = k_gather_stream<PM, EXACT, KICK2, ADVANCE, SAMPLE>;
+    static thread_local int configured_for = -1;   // opt in to > 48 KB of dynamic shared memory once per kernel
+    if (configured_for < s->stream_smem) {
+        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, s->stream_smem);
+        configured_for = s->stream_smem;
+    }
+    kern<<<s->stream_grid, kTile + 32, s->stream_smem, s->stream>>>(P, s->L);
+}
+
+template <int PM, bool EXACT> void launch_stream_v(const lsm_sim *s, const StepParams &P, Variant v) {
+    switch (v) {
+        case V_MID: launch_stream_one<PM, EXACT, true, true, false>(s, P); break;
+        case V_MID_SAMPLE: launch_stream_one<PM, EXACT, true, true, true>(s, P); break;
+        case V_END: launch_stream_one<PM, EXACT, true, false, true>(s, P); break;
+        case V_INIT: launch_stream_one<PM, EXACT, false, false, true>(s, P); break;
+    }
+}
+
+template <bool EXACT> void launch_stream_pm(const lsm_sim *s, const StepParams &P, Variant v) {
+    switch (s->pm) {
+        case PM_UNIFORM: launch_stream_v<PM_UNIFORM, EXACT>(s, P, v); break;
+        case PM_TYPED: launch_stream_v<PM_TYPED, EXACT>(s, P, v); break;
+        case PM_RCF: launch_stream_v<PM_RCF, EXACT>(s, P, v); break;
+        case PM_KRT_RCF: launch_stream_v<PM_KRT_RCF, EXACT>(s, P, v); break;
+        default: launch_stream_v<PM_FULL, EXACT>(s, P, v); break;
+    }
+}
+
 void launch_gather(lsm_sim *s, const StepParams &P, Variant v) {
-    const unsigned grid = grid_for(s->N);
-    if (s->exact) launch_gather_pm<true>(s->pm, P, v, grid, s->stream);
-    else launch_gather_pm<false>(s->pm, P, v, grid, s->stream);
+    if (s->gather_variant == 2) {
+        if (s->exact) launch_stream_pm<true>(s, P, v);
+        else launch_stream_pm<false>(s, P, v);
+    } else {
+        const unsigned grid = (unsigned)s->T;
+        if (s->exact) launch_gather_pm<true>(s->pm, P, v, grid, s->stream);
+        else launch_gather_pm<false>(s->pm, P, v, grid, s->stream);
+    }
     s->kernels_launched += 1;
 }
 
@@ -311,8 +351,8 @@ lsm_status eval_initial(lsm_sim *s) {
 lsm_status do_compact(lsm_sim *s) {
     if (s->force_mode == LSM_FORCE_GATHER) {
         CompactParams C;
-        C.slice_off = s->slice_off; C.slice_w = s->slice_w; C.nbr = s->nbr; C.sid = s->sid; C.typ = s->typ;
-        C.kF = s->kF; C.r0F = s->r0F; C.rcF = s->rcF; C.nslices = s->nslices;
+        C.hdr = s->hdr; C.nbr = s->nbr; C.sid = s->sid; C.typ = s->typ; C.rc32 = s->rc32;
+        C.kF = s->kF; C.r0F = s->r0F; C.nslices = s->nslices;
         k_compact_ell<<<grid_for(s->nslices * kSlice), kBlock, 0, s->stream>>>(C);
         s->kernels_launched += 1;
         CUDA_TRY(s, cudaGetLastError());
@@ -355,7 +395,7 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
     s->sample_every = d->sample_every; s->hist_cap = d->history_capacity > 0 ? d->history_capacity : 1024;
     s->compact_every = d->compact_every; s->reorder = d->reorder;
     s->force_mode = d->force_mode == LSM_FORCE_AUTO ? LSM_FORCE_GATHER : d->force_mode;
-    s->exact = d->exact; s->use_graph = d->use_graph; s->device = d->device; s->stream = (cudaStream_t)d->stream;
+    s->exact = d->exact; s->use_graph = d->use_graph; s->gather_variant = d->gather_variant; s->device = d->device; s->stream = (cudaStream_t)d->stream;
     s->alloc = d->alloc; s->free_ = d->free_; s->alloc_user = d->alloc_user;
 
     int ndev = 0;
@@ -468,15 +508,18 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
 
     // ---- particle state ----
     {
-        std::vector<double2> hx(N), hv(N);
+        s->T = (N + kTile - 1) / kTile;
+        s->Npad = s->T * kTile;                       // the streamed kernel copies whole tiles: pad the tail tile
+        const long long Np = s->Npad;
+        std::vector<double2> hx(Np, make_double2(0.0, 0.0)), hv(Np, make_double2(0.0, 0.0));
         for (long long c = 0; c < N; ++c) {
             const int32_t p = to_int(c);
             hx[p] = make_double2(d->x[2 * c], d->x[2 * c + 1]);
             hv[p] = d->v ? make_double2(d->v[2 * c], d->v[2 * c + 1]) : make_double2(0.0, 0.0);
         }
         TRY(upload(s, &s->pos[0], hx));
-        TRY(dev_alloc(s, &s->pos[1], (size_t)N));
-        CUDA_TRY(s, cudaMemcpyAsync(s->pos[1], s->pos[0], sizeof(double2) * N, cudaMemcpyDeviceToDevice, s->stream));
+        TRY(dev_alloc(s, &s->pos[1], (size_t)Np));
+        CUDA_TRY(s, cudaMemcpyAsync(s->pos[1], s->pos[0], sizeof(double2) * Np, cudaMemcpyDeviceToDevice, s->stream));
         TRY(upload(s, &s->vel, hv));
         TRY(dev_alloc(s, &s->f, (size_t)N));
         TRY(dev_alloc(s, &s->fd, (size_t)N));
@@ -484,8 +527,9 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
         TRY(dev_alloc(s, &s->stage[1], (size_t)N));
         CUDA_TRY(s, cudaMemsetAsync(s->f, 0, sizeof(double2) * N, s->stream));
         CUDA_TRY(s, cudaMemsetAsync(s->fd, 0, sizeof(double2) * N, s->stream));
-        s->h_grp.assign(N, kFree);
+        s->h_grp.assign(Np, kFree);
         TRY(upload(s, &s->grp, s->h_grp));
+        s->h_grp.resize(N);
         if (d->mass) {
             std::vector<double> hm(N);
             for (long long c = 0; c < N; ++c) hm[to_int(c)] = d->mass[c];
@@ -506,21 +550,28 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
     // ---- spring layout ----
     if (s->force_mode == LSM_FORCE_GATHER) {
         const long long S = (N + kSlice - 1) / kSlice;
+        const long long T = s->T;
         s->nslices = S;
         std::vector<uint32_t> deg(N, 0);
         for (long long e = 0; e < M; ++e) { deg[to_int(d->spring_i[e])]++; deg[to_int(d->spring_j[e])]++; }
-        std::vector<uint32_t> off(S + 1, 0);
-        std::vector<uint8_t> wv(S, 0);
-        for (long long sl = 0; sl < S; ++sl) {
+        std::vector<uint32_t> off(T * kTileSlices + 1, 0);
+        std::vector<TileHdr> hh(T);
+        std::memset(hh.data(), 0, sizeof(TileHdr) * T);
+        for (long long sl = 0; sl < T * kTileSlices; ++sl) {
             uint32_t w = 0;
             for (long long p = sl * kSlice; p < std::min<long long>(N, (sl + 1) * kSlice); ++p) w = std::max(w, deg[p]);
             if (w > 255) return fail(s, LSM_E_UNSUPPORTED, "particle degree above 255 is not supported by the gather layout; use force_mode = SCATTER");
-            wv[sl] = (uint8_t)w;
             const uint64_t nxt = (uint64_t)off[sl] + w;
-            if (nxt > 0xFFFFFFFFull) return fail(s, LSM_E_UNSUPPORTED, "gather layout too large");
+            if (nxt > 0x07FFFFFFull) return fail(s, LSM_E_UNSUPPORTED, "gather layout too large");
             off[sl + 1] = (uint32_t)nxt;
+            TileHdr &h = hh[sl / kTileSlices];
+            h.off[sl % kTileSlices] = off[sl];
+            h.off[sl % kTileSlices + 1] = off[sl + 1];
+            h.w[sl % kTileSlices] = (uint8_t)w;
         }
-        const size_t E = (size_t)off[S] * kSlice;
+        s->max_tile_slots = 0;
+        for (long long t = 0; t < T; ++t) s->max_tile_slots = std::max(s->max_tile_slots, hh[t].off[kTileSlices] - hh[t].off[0]);
+        const size_t E = (size_t)off[T * kTileSlices] * kSlice;
         s->E = (long long)E;
         std::vector<int32_t> hn(E, kPad), hs(E, -1);
         std::vector<uint8_t> cnt(N, 0);
@@ -531,11 +582,23 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
             hn[ea] = b2; hs[ea] = (int32_t)e;
             hn[eb] = a; hs[eb] = (int32_t)e;
         }
-        TRY(upload(s, &s->slice_off, off));
-        TRY(upload(s, &s->slice_w, wv));
+        TRY(upload(s, &s->hdr, hh));
         TRY(upload(s, &s->nbr, hn));
         if (need_typ) { std::vector<uint8_t> ht(E, 0); for (size_t e = 0; e < E; ++e) if (hs[e] >= 0) ht[e] = stype[hs[e]]; TRY(upload(s, &s->typ, ht)); CUDA_TRY(s, cudaStreamSynchronize(s->stream)); }
-        if (need_rcF) { std::vector<double> h(E, 0.0); for (size_t e = 0; e < E; ++e) if (hs[e] >= 0) h[e] = getrc(hs[e]); TRY(upload(s, &s->rcF, h)); CUDA_TRY(s, cudaStreamSynchronize(s->stream)); }
+        if (need_rcF) {
+            // rc32 = the largest fp32 <= rc: "r <= rc32" proves "r <= rc"; anything closer is settled by the exact rcS
+            std::vector<float> h(E, 0.0f);
+            for (size_t e = 0; e < E; ++e) if (hs[e] >= 0) {
+                const double rc = getrc(hs[e]);
+                float f = (float)rc;
+                if ((double)f > rc) f = std::nextafterf(f, -INFINITY);
+                h[e] = f;
+            }
+            TRY(upload(s, &s->rc32, h)); CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+            std::vector<double> hr(M);
+            for (long long e = 0; e < M; ++e) hr[e] = getrc(e);
+            TRY(upload(s, &s->rcS, hr)); CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+        }
         if (need_krF) {
             std::vector<double> h(E, 0.0);
             for (size_t e = 0; e < E; ++e) if (hs[e] >= 0) h[e] = getk(hs[e]);
@@ -545,6 +608,36 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
         }
         TRY(upload(s, &s->sid, hs));
         CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+        // ---- streamed-kernel stage layout: pipeline depth from the largest tile ----
+        {
+            StageLayout &L = s->L;
+            std::memset(&L, 0, sizeof(L));
+            auto up = [](int x) { return (x + 127) & ~127; };
+            const int cap = (int)s->max_tile_slots;
+            int o = 0;
+            L.pos = o; o += kTile * 16;
+            L.vel = o; o += kTile * 16;
+            L.hdr = o; o += 128;
+            L.grp = o; o += kTile;
+            L.nbr = o; o += up(cap * kSlice * 4);
+            L.rc32 = o; if (need_rcF) o += up(cap * kSlice * 4);
+            L.typ = o; if (need_typ) o += up(cap * kSlice);
+            L.kF = o; if (need_krF) o += up(cap * kSlice * 8);
+            L.r0F = o; if (need_krF) o += up(cap * kSlice * 8);
+            L.bytes = up(o);
+            L.first = 128 + (need_typ ? 3 * kMaxTypes * 8 : 0);
+            int dev_smem = 0, n_sm = 0;
+            CUDA_TRY(s, cudaDeviceGetAttribute(&dev_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, d->device));
+            CUDA_TRY(s, cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, d->device));
+            const int ctas_per_sm = 2;
+            const int budget = std::min(dev_smem, (dev_smem + 1024) / ctas_per_sm - 1024) - L.first;   // 1 KB reserved per CTA
+            L.stages = std::min<int>(kMaxStages, std::min<int>(4, budget / std::max(L.bytes, 1)));
+            const bool can_stream = L.stages >= 2;
+            if (s->gather_variant == 0) s->gather_variant = can_stream ? 2 : 1;
+            if (s->gather_variant == 2 && !can_stream) return fail(s, LSM_E_UNSUPPORTED, "gather_variant = streamed: a tile's rows do not fit in shared memory (degree too high); use the direct variant");
+            s->stream_smem = L.first + L.stages * L.bytes;
+            s->stream_grid = (int)std::min<long long>(T, (long long)ctas_per_sm * n_sm);
+        }
     } else if (s->force_mode == LSM_FORCE_SCATTER) {
         if (s->exact) return fail(s, LSM_E_UNSUPPORTED, "exact arithmetic needs force_mode = GATHER (atomic summation order is not fixed)");
         // spring list in internal numbering, sorted by (lower endpoint, upper endpoint) for gather / atomic locality
@@ -618,6 +711,7 @@ lsm_status lsm_create(const lsm_desc *d, lsm_sim **out) {
     if (d->reorder == LSM_REORDER_RCM) return fail(nullptr, LSM_E_UNSUPPORTED, "reorder = RCM is not built; use MORTON");
     if (d->reorder != LSM_REORDER_NONE && d->reorder != LSM_REORDER_MORTON) return fail(nullptr, LSM_E_INVALID, "bad reorder");
     if (d->force_mode < 0 || d->force_mode > 2) return fail(nullptr, LSM_E_INVALID, "bad force_mode");
+    if (d->gather_variant < 0 || d->gather_variant > 2) return fail(nullptr, LSM_E_INVALID, "bad gather_variant");
     if ((d->alloc == nullptr) != (d->free_ == nullptr)) return fail(nullptr, LSM_E_INVALID, "alloc and free_ must be given together");
     lsm_sim *s = new (std::nothrow) lsm_sim();
     if (!s) return fail(nullptr, LSM_E_NOMEM, "out of host memory");
@@ -826,8 +920,11 @@ lsm_status lsm_get_info(lsm_sim *s, lsm_info *info) {
     if (!s || !info) return LSM_E_INVALID;
     std::memset(info, 0, sizeof(*info));
     info->n_particles = s->N; info->n_springs = s->M; info->n_half_edges_stored = s->E;
-    static const int pbytes[5] = {0, 1, 8, 9, 24};
-    info->bytes_per_half_edge = (s->force_mode == LSM_FORCE_GATHER ? 4 : 8) + pbytes[s->pm];
+    static const int pbytes_scatter[5] = {0, 1, 8, 9, 24}, pbytes_gather[5] = {0, 1, 4, 5, 20};
+    info->bytes_per_half_edge = s->force_mode == LSM_FORCE_GATHER ? 4 + pbytes_gather[s->pm] : 8 + pbytes_scatter[s->pm];
+    info->gather_variant = s->force_mode == LSM_FORCE_GATHER ? s->gather_variant : 0;
+    info->pipeline_stages = s->gather_variant == 2 ? s->L.stages : 0;
+    info->stage_bytes = s->gather_variant == 2 ? s->L.bytes : 0;
     info->param_mode = s->pm; info->n_types = s->ntypes; info->force_mode = s->force_mode; info->exact = s->exact;
     info->reorder = s->reorder; info->n_batch = s->B; info->device_bytes = s->device_bytes;
     info->kernels_launched = s->kernels_launched; info->current_step = s->step;

@@ -5,10 +5,15 @@
 //                                    fully coalesced, neighbour gathers touch one sector instead of two)
 //   grp[N]                           uint8 boundary group of the particle, 0xFF = free.  For a kinematic particle the
 //                                    vel slot holds its ORIGIN x0 (its velocity is du_g/dt by definition).
-//   gather layout (particle-centric, sliced ELL, slice = one warp = 32 consecutive particles):
-//     slice_off[S+1] (units of 32 slots), slice_w[S] (live width), nbr[E] int32 neighbour id (bitwise-NOT of the id
-//     once the spring is dead, INT32_MIN = padding), sid[E] caller spring id, per-slot parameters by ParamMode.
-//     Slot s of lane l of slice S is entry (slice_off[S] + s)*32 + l  -> every slot load is one coalesced line.
+//   gather layout (particle-centric, sliced ELL, slice = one warp = 32 consecutive particles, tile = 8 slices = 256
+//   particles = one CTA's unit of work):
+//     hdr[T] (64 B per tile: slot offset of each of its 8 slices + end, live width of each slice),
+//     nbr[E] int32 neighbour id (bitwise-NOT of the id once the spring is dead, INT32_MIN = padding),
+//     sid[E] caller spring id (cold: read only when a spring breaks or sits within one fp32 ulp of rc),
+//     per-slot parameters by ParamMode: typ[E] uint8, rc32[E] float = the largest fp32 <= rc (a conservative filter:
+//     r <= rc32 proves r <= rc; otherwise the exact fp64 rcS[sid] decides, so the decision is the fp64 one), kF/r0F[E].
+//     Slot s of lane l of slice S is entry (off[S] + s)*32 + l  -> every slot load is one coalesced 128-byte line, and
+//     the slots of one tile are one contiguous range per array -> one bulk async copy per array per tile.
 //     Rows are ordered by ascending caller spring id, so a particle sums its springs in the oracle's order.
 //   scatter layout (the paper's spring list, re-done in SoA): si[M'], sj[M'] (si bitwise-NOT
 //     once dead), per-spring parameters by ParamMode, force accumulated with fp64 RED atomics into f.
@@ -20,6 +25,9 @@ namespace lsmk {
 
 constexpr int kBlock = 256;
 constexpr int kSlice = 32;
+constexpr int kTile = 256;            // particles per tile (= kBlock): 8 slices
+constexpr int kTileSlices = kTile / kSlice;
+constexpr int kMaxStages = 8;
 constexpr int32_t kPad = INT32_MIN;
 constexpr uint8_t kFree = 0xFF;
 constexpr int kMaxGroups = 8;
@@ -28,6 +36,13 @@ constexpr int kMaxTypes = 256;
 
 enum ParamMode { PM_UNIFORM = 0, PM_TYPED = 1, PM_RCF = 2, PM_KRT_RCF = 3, PM_FULL = 4 };
 
+struct __align__(16) TileHdr {          // 64 bytes per tile of 256 particles
+    uint32_t off[kTileSlices + 1];     // slot offset (units of 32 entries) of each slice, and the end of the tile
+    uint8_t w[kTileSlices];            // live width of each slice (shrinks under compaction)
+    uint8_t pad[20];
+};
+static_assert(sizeof(TileHdr) == 64, "TileHdr must be 64 bytes");
+
 struct GroupTab {
     double dux[kMaxGroups], duy[kMaxGroups];
     long long n0[kMaxGroups];
@@ -35,7 +50,9 @@ struct GroupTab {
 
 struct SpringParams {  // parameter encoding shared by the gather (per half-edge) and scatter (per spring) layouts
     const uint8_t *typ;
-    const double *kF, *r0F, *rcF;
+    const double *kF, *r0F, *rcF;      // rcF: scatter layout only
+    const float *rc32;                 // gather layout: fp32 lower bound of rc per half-edge
+    const double *rcS;                 // gather layout: exact rc per spring, caller numbering
     const double *tab;  // [ntypes][3] = k, r0, rc
     int ntypes;
     double k_u, r0_u, rc_u;
@@ -52,8 +69,8 @@ struct StepParams {
     long long N;
     long long step;  // step number of THIS force evaluation (stamped on springs that break in it)
     // gather layout
-    const uint32_t *slice_off;
-    const uint8_t *slice_w;
+    const TileHdr *hdr;
+    long long T;  // tiles
     int32_t *nbr;
     const int32_t *sid;
     SpringParams sp;
@@ -157,7 +174,88 @@ __device__ __forceinline__ void particle_update(const StepParams &P, long long p
 // every incident spring (each spring is evaluated from both of its endpoints: twice the arithmetic, no atomics, no
 // force array round trip, deterministic), applies the breakage test, then integrates.  Reads x (double-buffered),
 // v, ids, parameters; writes x_next, v.  HBM bytes per step: 64 N + (4 + parameter bytes) * 2M.
+// Two kernels share the row evaluation below: k_gather_step reads the slot streams straight from global memory;
+// k_gather_stream (the product path) stages them tile by tile through shared memory with bulk async copies.
 // ---------------------------------------------------------------------------------------------------------------
+struct RowSrc {            // where one particle's row lives: pointers already offset to (slice offset)*32 + lane
+    const int32_t *nbr;    // slot s at nbr[s*32]  (global memory, or the staged shared-memory copy)
+    const float *rc32;
+    const uint8_t *typ;
+    const double *kF, *r0F;
+    const double2 *tile_pos;  // staged positions of the tile's own 256 particles (STAGED only)
+    int p0;                   // first particle of the tile
+    size_t e0;                // global entry index of slot 0 of this lane (for the cold paths)
+};
+
+template <int PM, bool EXACT, bool SAMPLE, bool STAGED>
+__device__ __forceinline__ void row_forces(const StepParams &P, const RowSrc &R, const double *s_tab, long long p, unsigned w,
+                                           double2 xp, double &fx, double &fy, double &u) {
+    constexpr int CH = 6;
+    constexpr bool kHasRc32 = (PM == PM_RCF || PM == PM_KRT_RCF || PM == PM_FULL);
+    for (unsigned s0 = 0; s0 < w; s0 += CH) {
+        int nb[CH];
+        double2 xq[CH];
+#pragma unroll
+        for (int c = 0; c < CH; ++c) nb[c] = (s0 + c < w) ? R.nbr[(s0 + c) * kSlice] : kPad;
+#pragma unroll
+        for (int c = 0; c < CH; ++c) {
+            if (nb[c] >= 0) {
+                if (STAGED) {
+                    const unsigned rel = (unsigned)(nb[c] - R.p0);
+                    if (rel < (unsigned)kTile) xq[c] = R.tile_pos[rel];
+                    else xq[c] = __ldg(P.pos_cur + nb[c]);
+                } else {
+                    xq[c] = __ldg(P.pos_cur + nb[c]);
+                }
+            }
+        }
+#pragma unroll
+        for (int c = 0; c < CH; ++c) {
+            if (nb[c] >= 0) {
+                const unsigned so = (s0 + c) * kSlice;
+                double k, r0, rc = 0.0;
+                if (PM == PM_UNIFORM) { k = P.sp.k_u; r0 = P.sp.r0_u; rc = P.sp.rc_u; }
+                else if (PM == PM_TYPED) { const int t = R.typ[so]; k = s_tab[3 * t]; r0 = s_tab[3 * t + 1]; rc = s_tab[3 * t + 2]; }
+                else if (PM == PM_RCF) { k = P.sp.k_u; r0 = P.sp.r0_u; }
+                else if (PM == PM_KRT_RCF) { const int t = R.typ[so]; k = s_tab[3 * t]; r0 = s_tab[3 * t + 1]; }
+                else { k = R.kF[so]; r0 = R.r0F[so]; }
+                const double dx = sub<EXACT>(xq[c].x, xp.x), dy = sub<EXACT>(xq[c].y, xp.y);
+                const double r2 = EXACT ? add<true>(mul<true>(dx, dx), mul<true>(dy, dy)) : fma(dy, dy, dx * dx);
+                double r, rinv = 0.0;
+                if (EXACT) r = __dsqrt_rn(r2);
+                else { rinv = rsqrt(r2); r = r2 * rinv; if (!(r2 > 0.0)) r = 0.0; }
+                // breakage test, strict '>' (Q1).  Both endpoints compute bit-identical r ((-dx)^2 == dx^2) and read
+                // the same rc, so they take the same decision without communicating.
+                bool broke;
+                if (kHasRc32) {
+                    broke = false;
+                    if (r > (double)R.rc32[so]) broke = r > __ldg(P.sp.rcS + __ldg(P.sid + R.e0 + so));  // within 1 fp32 ulp: exact rc decides
+                } else {
+                    broke = r > rc;
+                }
+                if (!broke) {
+                    const double ext = sub<EXACT>(r, r0);
+                    if (r != 0.0) {  // coincident endpoints: no direction, no force (Q4)
+                        const double gk = EXACT ? __ddiv_rn(mul<true>(k, ext), r) : (k * ext) * rinv;
+                        fx = mad<EXACT>(gk, dx, fx);
+                        fy = mad<EXACT>(gk, dy, fy);
+                        if (SAMPLE && p < nb[c])  // each spring's energy is counted once, by its lower endpoint (Eq. 1)
+                            u = add<EXACT>(u, mul<EXACT>(mul<EXACT>(mul<EXACT>(0.5, k), ext), ext));
+                    }
+                } else {  // broke in this evaluation: dead from now on, zero force already in this step (Q2, Q3)
+                    const size_t e = R.e0 + so;
+                    P.nbr[e] = ~nb[c];
+                    if (p < nb[c]) {
+                        P.break_step[P.sid[e]] = P.step;
+                        atomicAdd(P.nbroken + spec_of(P.poff, P.B, p), 1ULL);
+                    }
+                }
+            }
+        }
+    }
+}
+
+// Direct variant: block = tile, every stream read from global memory by the thread that needs it.
 template <int PM, bool EXACT, bool KICK2, bool ADVANCE, bool SAMPLE>
 __global__ void __launch_bounds__(kBlock) k_gather_step(const StepParams P) {
     constexpr bool kTab = (PM == PM_TYPED || PM == PM_KRT_RCF);
@@ -168,50 +266,139 @@ __global__ void __launch_bounds__(kBlock) k_gather_step(const StepParams P) {
     }
     const long long p = (long long)blockIdx.x * kBlock + threadIdx.x;
     if (p >= P.N) return;
-    const unsigned sl = (unsigned)(p >> 5);
-    const unsigned w = P.slice_w[sl];
-    const size_t e0 = (size_t)P.slice_off[sl] * kSlice + (threadIdx.x & 31);
+    const int wi = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const TileHdr *h = P.hdr + blockIdx.x;
+    const unsigned w = h->w[wi];
+    const size_t e0 = (size_t)h->off[wi] * kSlice + lane;
     const double2 xp = P.pos_cur[p];
     const double2 vh = P.vel[p];
     const uint8_t g = P.grp[p];
-
+    RowSrc R;
+    R.nbr = P.nbr + e0; R.rc32 = P.sp.rc32 + e0; R.typ = P.sp.typ + e0; R.kF = P.sp.kF + e0; R.r0F = P.sp.r0F + e0;
+    R.tile_pos = nullptr; R.p0 = 0; R.e0 = e0;
     double fx = 0.0, fy = 0.0, u = 0.0;
-    constexpr int CH = 6;
-    for (unsigned s0 = 0; s0 < w; s0 += CH) {
-        int nb[CH];
-        double2 xq[CH];
-        double pk[CH], pr0[CH], prc[CH];
-#pragma unroll
-        for (int c = 0; c < CH; ++c) nb[c] = (s0 + c < w) ? P.nbr[e0 + (size_t)(s0 + c) * kSlice] : kPad;
-#pragma unroll
-        for (int c = 0; c < CH; ++c) {
-            if (nb[c] >= 0) {
-                xq[c] = P.pos_cur[nb[c]];
-                load_params<PM>(P.sp, s_tab, e0 + (size_t)(s0 + c) * kSlice, pk[c], pr0[c], prc[c]);
-            }
-        }
-#pragma unroll
-        for (int c = 0; c < CH; ++c) {
-            if (nb[c] >= 0) {
-                const double dx = sub<EXACT>(xq[c].x, xp.x), dy = sub<EXACT>(xq[c].y, xp.y);
-                double gk, ext;
-                if (spring_eval<EXACT>(dx, dy, pk[c], pr0[c], prc[c], gk, ext)) {
-                    fx = mad<EXACT>(gk, dx, fx);
-                    fy = mad<EXACT>(gk, dy, fy);
-                    if (SAMPLE && p < nb[c])   // each spring's energy is counted once, by its lower endpoint (Eq. 1)
-                        u = add<EXACT>(u, mul<EXACT>(mul<EXACT>(mul<EXACT>(0.5, pk[c]), ext), ext));
-                } else {  // broke in this evaluation: dead from now on, zero force already in this step (Q2, Q3)
-                    const size_t e = e0 + (size_t)(s0 + c) * kSlice;
-                    P.nbr[e] = ~nb[c];
-                    if (p < nb[c]) {
-                        P.break_step[P.sid[e]] = P.step;
-                        atomicAdd(P.nbroken + spec_of(P.poff, P.B, p), 1ULL);
+    row_forces<PM, EXACT, SAMPLE, false>(P, R, s_tab, p, w, xp, fx, fy, u);
+    particle_update<EXACT, KICK2, ADVANCE, SAMPLE>(P, p, xp, vh, g, fx, fy, u);
+}
+
+// ---- mbarrier / bulk-copy primitives (PTX; sm_90+ async proxy: the copy engine moves the bytes, no registers) ----
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity) {
+    const uint32_t a = smem_u32(bar);
+    uint32_t ok;
+    do {
+        asm volatile("{\n\t.reg .pred q;\n\tmbarrier.try_wait.parity.shared::cta.b64 q, [%1], %2;\n\tselp.u32 %0, 1, 0, q;\n\t}"
+                     : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned bytes, uint64_t *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+struct StageLayout {      // byte offsets of the staged arrays inside one pipeline stage (all multiples of 128)
+    int pos, vel, hdr, grp, nbr, rc32, typ, kF, r0F;
+    int bytes;            // stage size
+    int stages;           // pipeline depth
+    int first;            // offset of stage 0 in dynamic shared memory (after the barriers and the type table)
+};
+
+// Streamed variant (product path).  Persistent CTAs (grid = CTAs/SM x SMs) walk the tiles round-robin.  Warp 8 is the
+// producer: one lane arms the stage's mbarrier with the byte count and issues one bulk async copy per array
+// (own x, own v, group bytes, tile header, neighbour ids, parameters); warps 0..7 are the consumers (one thread per
+// particle).  The bytes in flight per SM are (stages - 1) x stage size x CTAs/SM, independent of registers and
+// occupancy; the only latency the consumers see is the neighbour-position gather (L2 / L1 hits, or the staged tile).
+template <int PM, bool EXACT, bool KICK2, bool ADVANCE, bool SAMPLE>
+__global__ void __launch_bounds__(kTile + 32, 2) k_gather_stream(const StepParams P, const StageLayout L) {
+    constexpr bool kTab = (PM == PM_TYPED || PM == PM_KRT_RCF);
+    constexpr bool kHasRc32 = (PM == PM_RCF || PM == PM_KRT_RCF || PM == PM_FULL);
+    constexpr bool kHasTyp = kTab;
+    constexpr bool kHasKR = (PM == PM_FULL);
+    extern __shared__ __align__(128) unsigned char smem[];
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem);          // [kMaxStages]
+    uint64_t *empty = full + kMaxStages;                            // [kMaxStages]
+    double *s_tab = reinterpret_cast<double *>(smem + 128);         // [3*kMaxTypes] when kTab
+    unsigned char *stage0 = smem + L.first;
+    const int tid = threadIdx.x, wi = tid >> 5, lane = tid & 31;
+    if (tid == 0) {
+        for (int s = 0; s < L.stages; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, kTileSlices); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (kTab) for (int i = tid; i < 3 * P.sp.ntypes; i += kTile + 32) s_tab[i] = P.sp.tab[i];
+    __syncthreads();
+
+    if (wi == kTileSlices) {  // ---------------- producer warp ----------------
+        if (lane == 0) {
+            int s = 0; unsigned u = 0;
+            for (long long t = blockIdx.x; t < P.T; t += gridDim.x) {
+                if (u > 0) mbar_wait(empty + s, (u - 1) & 1);
+                const TileHdr *h = P.hdr + t;
+                const uint32_t o0 = __ldg(&h->off[0]);
+                const uint32_t ns = __ldg(&h->off[kTileSlices]) - o0;
+                unsigned bytes = 2 * kTile * 16 + kTile + 64 + ns * (kSlice * 4);
+                if (kHasRc32) bytes += ns * (kSlice * 4);
+                if (kHasTyp) bytes += ns * kSlice;
+                if (kHasKR) bytes += 2 * ns * (kSlice * 8);
+                unsigned char *b = stage0 + (size_t)s * L.bytes;
+                mbar_expect_tx(full + s, bytes);
+                bulk_g2s(b + L.pos, P.pos_cur + t * kTile, kTile * 16, full + s);
+                bulk_g2s(b + L.vel, P.vel + t * kTile, kTile * 16, full + s);
+                bulk_g2s(b + L.grp, P.grp + t * kTile, kTile, full + s);
+                bulk_g2s(b + L.hdr, h, 64, full + s);
+                if (ns) {
+                    const size_t e = (size_t)o0 * kSlice;
+                    bulk_g2s(b + L.nbr, P.nbr + e, ns * (kSlice * 4), full + s);
+                    if (kHasRc32) bulk_g2s(b + L.rc32, P.sp.rc32 + e, ns * (kSlice * 4), full + s);
+                    if (kHasTyp) bulk_g2s(b + L.typ, P.sp.typ + e, ns * kSlice, full + s);
+                    if (kHasKR) {
+                        bulk_g2s(b + L.kF, P.sp.kF + e, ns * (kSlice * 8), full + s);
+                        bulk_g2s(b + L.r0F, P.sp.r0F + e, ns * (kSlice * 8), full + s);
                     }
                 }
+                if (++s == L.stages) { s = 0; ++u; }
             }
         }
+        return;
     }
-    particle_update<EXACT, KICK2, ADVANCE, SAMPLE>(P, p, xp, vh, g, fx, fy, u);
+    // ---------------- consumer warps: thread = particle ----------------
+    int s = 0; unsigned u = 0;
+    for (long long t = blockIdx.x; t < P.T; t += gridDim.x) {
+        mbar_wait(full + s, u & 1);
+        const unsigned char *b = stage0 + (size_t)s * L.bytes;
+        const TileHdr *h = reinterpret_cast<const TileHdr *>(b + L.hdr);
+        const long long p = t * kTile + tid;
+        if (p < P.N) {
+            const unsigned w = h->w[wi];
+            const unsigned rel = (h->off[wi] - h->off[0]) * kSlice + lane;
+            const double2 xp = reinterpret_cast<const double2 *>(b + L.pos)[tid];
+            const double2 vh = reinterpret_cast<const double2 *>(b + L.vel)[tid];
+            const uint8_t g = (b + L.grp)[tid];
+            RowSrc R;
+            R.nbr = reinterpret_cast<const int32_t *>(b + L.nbr) + rel;
+            R.rc32 = reinterpret_cast<const float *>(b + L.rc32) + rel;
+            R.typ = (b + L.typ) + rel;
+            R.kF = reinterpret_cast<const double *>(b + L.kF) + rel;
+            R.r0F = reinterpret_cast<const double *>(b + L.r0F) + rel;
+            R.tile_pos = reinterpret_cast<const double2 *>(b + L.pos);
+            R.p0 = (int)(t * kTile);
+            R.e0 = (size_t)h->off[wi] * kSlice + lane;
+            double fx = 0.0, fy = 0.0, uu = 0.0;
+            row_forces<PM, EXACT, SAMPLE, true>(P, R, s_tab, p, w, xp, fx, fy, uu);
+            particle_update<EXACT, KICK2, ADVANCE, SAMPLE>(P, p, xp, vh, g, fx, fy, uu);
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(empty + s);
+        if (++s == L.stages) { s = 0; ++u; }
+    }
 }
 
 // First half kick + drift from a completed state (v, fd): the first kernel of every lsm_step call.
@@ -385,11 +572,11 @@ __global__ void __launch_bounds__(128) k_finalize_sample(const ReduceParams R) {
 // longest surviving row: dead columns are no longer read at all.
 // ---------------------------------------------------------------------------------------------------------------
 struct CompactParams {
-    const uint32_t *slice_off;
-    uint8_t *slice_w;
+    TileHdr *hdr;
     int32_t *nbr, *sid;
     uint8_t *typ;
-    double *kF, *r0F, *rcF;
+    float *rc32;
+    double *kF, *r0F;
     long long nslices;
 };
 
@@ -397,8 +584,10 @@ __global__ void __launch_bounds__(kBlock) k_compact_ell(const CompactParams C) {
     const long long sl = ((long long)blockIdx.x * kBlock + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
     if (sl >= C.nslices) return;
-    const unsigned w = C.slice_w[sl];
-    const size_t e0 = (size_t)C.slice_off[sl] * kSlice + lane;
+    TileHdr *h = C.hdr + sl / kTileSlices;
+    const int wi = (int)(sl % kTileSlices);
+    const unsigned w = h->w[wi];
+    const size_t e0 = (size_t)h->off[wi] * kSlice + lane;
     unsigned j = 0;
     for (unsigned s = 0; s < w; ++s) {
         const size_t e = e0 + (size_t)s * kSlice;
@@ -408,9 +597,9 @@ __global__ void __launch_bounds__(kBlock) k_compact_ell(const CompactParams C) {
                 const size_t d = e0 + (size_t)j * kSlice;
                 C.nbr[d] = nb; C.sid[d] = C.sid[e];
                 if (C.typ) C.typ[d] = C.typ[e];
+                if (C.rc32) C.rc32[d] = C.rc32[e];
                 if (C.kF) C.kF[d] = C.kF[e];
                 if (C.r0F) C.r0F[d] = C.r0F[e];
-                if (C.rcF) C.rcF[d] = C.rcF[e];
             }
             ++j;
         }
@@ -419,7 +608,7 @@ __global__ void __launch_bounds__(kBlock) k_compact_ell(const CompactParams C) {
     unsigned wmax = j;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) wmax = max(wmax, __shfl_xor_sync(0xffffffffu, wmax, o));
-    if (lane == 0) C.slice_w[sl] = (uint8_t)wmax;
+    if (lane == 0) h->w[wi] = (uint8_t)wmax;
 }
 
 // ---- small utility kernels (numbering translation at the API boundary, boundary-group bookkeeping) ----
