@@ -187,6 +187,10 @@ struct RowSrc {            // where one particle's row lives: pointers already o
     size_t e0;                // global entry index of slot 0 of this lane (for the cold paths)
 };
 
+// The hot part is branch-free (padding slots, dead springs and coincident endpoints contribute an exact 0 through
+// selects, so the six springs of a row interleave in the fp64 pipe); the rare events -- a spring within one fp32 ulp
+// of rc, a spring breaking -- are handled after it under one warp-level branch.  Accumulation stays in slot order
+// (ascending caller spring id): adding +-0.0 for the skipped slots leaves every partial sum bit-identical.
 template <int PM, bool EXACT, bool SAMPLE, bool STAGED>
 __device__ __forceinline__ void row_forces(const StepParams &P, const RowSrc &R, const double *s_tab, long long p, unsigned w,
                                            double2 xp, double &fx, double &fy, double &u) {
@@ -195,62 +199,80 @@ __device__ __forceinline__ void row_forces(const StepParams &P, const RowSrc &R,
     for (unsigned s0 = 0; s0 < w; s0 += CH) {
         int nb[CH];
         double2 xq[CH];
+        double gk[CH], dx[CH], dy[CH], ue[CH];
+        unsigned hot = 0;  // bit c: slot c needs the rare path (may have broken)
 #pragma unroll
         for (int c = 0; c < CH; ++c) nb[c] = (s0 + c < w) ? R.nbr[(s0 + c) * kSlice] : kPad;
 #pragma unroll
         for (int c = 0; c < CH; ++c) {
-            if (nb[c] >= 0) {
-                if (STAGED) {
-                    const unsigned rel = (unsigned)(nb[c] - R.p0);
-                    if (rel < (unsigned)kTile) xq[c] = R.tile_pos[rel];
-                    else xq[c] = __ldg(P.pos_cur + nb[c]);
-                } else {
-                    xq[c] = __ldg(P.pos_cur + nb[c]);
+            const int j = nb[c] >= 0 ? nb[c] : (int)p;   // padding / dead: gather the own position (always legal)
+            if (STAGED) {
+                const unsigned rel = (unsigned)(j - R.p0);
+                if (rel < (unsigned)kTile) xq[c] = R.tile_pos[rel];
+                else xq[c] = __ldg(P.pos_cur + j);
+            } else {
+                xq[c] = __ldg(P.pos_cur + j);
+            }
+        }
+#pragma unroll
+        for (int c = 0; c < CH; ++c) {
+            const unsigned so = (s0 + c < w) ? (s0 + c) * kSlice : 0u;
+            const bool valid = nb[c] >= 0;
+            double k, r0, rc = 0.0;
+            if (PM == PM_UNIFORM) { k = P.sp.k_u; r0 = P.sp.r0_u; rc = P.sp.rc_u; }
+            else if (PM == PM_TYPED) { const int t = R.typ[so]; k = s_tab[3 * t]; r0 = s_tab[3 * t + 1]; rc = s_tab[3 * t + 2]; }
+            else if (PM == PM_RCF) { k = P.sp.k_u; r0 = P.sp.r0_u; rc = (double)R.rc32[so]; }
+            else if (PM == PM_KRT_RCF) { const int t = R.typ[so]; k = s_tab[3 * t]; r0 = s_tab[3 * t + 1]; rc = (double)R.rc32[so]; }
+            else { k = R.kF[so]; r0 = R.r0F[so]; rc = (double)R.rc32[so]; }
+            dx[c] = sub<EXACT>(xq[c].x, xp.x); dy[c] = sub<EXACT>(xq[c].y, xp.y);
+            const double r2 = EXACT ? add<true>(mul<true>(dx[c], dx[c]), mul<true>(dy[c], dy[c])) : fma(dy[c], dy[c], dx[c] * dx[c]);
+            double r, g;
+            if (EXACT) {
+                r = __dsqrt_rn(r2);
+                const double ext = sub<true>(r, r0);
+                g = __ddiv_rn(mul<true>(k, ext), r);
+                ue[c] = mul<true>(mul<true>(mul<true>(0.5, k), ext), ext);
+            } else {
+                const double rinv = rsqrt(r2);
+                r = r2 * rinv;
+                const double ext = r - r0;
+                g = (k * ext) * rinv;
+                ue[c] = (0.5 * k) * ext * ext;
+            }
+            // coincident endpoints (r2 == 0: no direction, no force, Q4) and padding / dead slots contribute 0
+            const bool live = valid && r2 > 0.0;
+            gk[c] = live ? g : 0.0;
+            ue[c] = (SAMPLE && live && p < nb[c]) ? ue[c] : 0.0;  // energy counted once, by the lower endpoint (Eq. 1)
+            // strict '>' (Q1).  With a per-spring rc, rc holds its fp32 lower bound here: r <= rc32 proves r <= rc.
+            if (live && r > rc) hot |= 1u << c;
+        }
+        if (hot) {  // rare: settle with the exact rc, mark the broken (Q2, Q3: zero force already in this step)
+#pragma unroll
+            for (int c = 0; c < CH; ++c) {
+                if (hot & (1u << c)) {
+                    const size_t e = R.e0 + (size_t)(s0 + c) * kSlice;
+                    bool broke = true;
+                    if (kHasRc32) {
+                        const double r2 = EXACT ? add<true>(mul<true>(dx[c], dx[c]), mul<true>(dy[c], dy[c])) : fma(dy[c], dy[c], dx[c] * dx[c]);
+                        const double r = EXACT ? __dsqrt_rn(r2) : r2 * rsqrt(r2);
+                        broke = r > __ldg(P.sp.rcS + __ldg(P.sid + e));
+                    }
+                    if (broke) {
+                        gk[c] = 0.0; ue[c] = 0.0;
+                        P.nbr[e] = ~nb[c];
+                        if (p < nb[c]) {
+                            P.break_step[P.sid[e]] = P.step;
+                            atomicAdd(P.nbroken + spec_of(P.poff, P.B, p), 1ULL);
+                        }
+                    }
                 }
             }
         }
 #pragma unroll
         for (int c = 0; c < CH; ++c) {
-            if (nb[c] >= 0) {
-                const unsigned so = (s0 + c) * kSlice;
-                double k, r0, rc = 0.0;
-                if (PM == PM_UNIFORM) { k = P.sp.k_u; r0 = P.sp.r0_u; rc = P.sp.rc_u; }
-                else if (PM == PM_TYPED) { const int t = R.typ[so]; k = s_tab[3 * t]; r0 = s_tab[3 * t + 1]; rc = s_tab[3 * t + 2]; }
-                else if (PM == PM_RCF) { k = P.sp.k_u; r0 = P.sp.r0_u; }
-                else if (PM == PM_KRT_RCF) { const int t = R.typ[so]; k = s_tab[3 * t]; r0 = s_tab[3 * t + 1]; }
-                else { k = R.kF[so]; r0 = R.r0F[so]; }
-                const double dx = sub<EXACT>(xq[c].x, xp.x), dy = sub<EXACT>(xq[c].y, xp.y);
-                const double r2 = EXACT ? add<true>(mul<true>(dx, dx), mul<true>(dy, dy)) : fma(dy, dy, dx * dx);
-                double r, rinv = 0.0;
-                if (EXACT) r = __dsqrt_rn(r2);
-                else { rinv = rsqrt(r2); r = r2 * rinv; if (!(r2 > 0.0)) r = 0.0; }
-                // breakage test, strict '>' (Q1).  Both endpoints compute bit-identical r ((-dx)^2 == dx^2) and read
-                // the same rc, so they take the same decision without communicating.
-                bool broke;
-                if (kHasRc32) {
-                    broke = false;
-                    if (r > (double)R.rc32[so]) broke = r > __ldg(P.sp.rcS + __ldg(P.sid + R.e0 + so));  // within 1 fp32 ulp: exact rc decides
-                } else {
-                    broke = r > rc;
-                }
-                if (!broke) {
-                    const double ext = sub<EXACT>(r, r0);
-                    if (r != 0.0) {  // coincident endpoints: no direction, no force (Q4)
-                        const double gk = EXACT ? __ddiv_rn(mul<true>(k, ext), r) : (k * ext) * rinv;
-                        fx = mad<EXACT>(gk, dx, fx);
-                        fy = mad<EXACT>(gk, dy, fy);
-                        if (SAMPLE && p < nb[c])  // each spring's energy is counted once, by its lower endpoint (Eq. 1)
-                            u = add<EXACT>(u, mul<EXACT>(mul<EXACT>(mul<EXACT>(0.5, k), ext), ext));
-                    }
-                } else {  // broke in this evaluation: dead from now on, zero force already in this step (Q2, Q3)
-                    const size_t e = R.e0 + so;
-                    P.nbr[e] = ~nb[c];
-                    if (p < nb[c]) {
-                        P.break_step[P.sid[e]] = P.step;
-                        atomicAdd(P.nbroken + spec_of(P.poff, P.B, p), 1ULL);
-                    }
-                }
-            }
+            fx = mad<EXACT>(gk[c], dx[c], fx);
+            fy = mad<EXACT>(gk[c], dy[c], fy);
+            if (SAMPLE) u = add<EXACT>(u, ue[c]);
         }
     }
 }
