@@ -33,7 +33,8 @@ def stale() -> bool:
 
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or stale():
-        cmd = [nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", SO] + SOURCES
+        extra = os.environ.get("LSM_NVCC_FLAGS", "").split()          # e.g. -DLSM_STREAM_MINB=3 for tuning sweeps
+        cmd = [nvcc()] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", SO] + SOURCES
         subprocess.run(cmd, check=True)
     return SO
 

@@ -5,6 +5,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -59,7 +60,7 @@ struct lsm_sim {
     long long nslices = 0, E = 0, T = 0, Npad = 0;
     TileHdr *hdr = nullptr;
     int32_t *nbr = nullptr, *sid = nullptr;
-    float *rc32 = nullptr;
+    uint32_t *thr = nullptr;
     double *rcS = nullptr;
     int gather_variant = 0;          // resolved: 1 direct, 2 streamed
     StageLayout L;
@@ -162,6 +163,14 @@ inline uint64_t part1by1(uint64_t x) {
     return x;
 }
 
+// Breakage filter word of a breaking length rc: (high 32 bits of rc*rc) - 1 (lsm_kernels.cuh, row_chunk).
+uint32_t thr_of(double rc) {
+    const double rc2 = rc * rc;
+    uint64_t u; std::memcpy(&u, &rc2, 8);
+    const uint32_t hi = (uint32_t)(u >> 32);
+    return hi > 0 ? hi - 1 : 0;
+}
+
 GroupTab group_tab(const lsm_sim *s) {
     GroupTab g;
     for (int i = 0; i < kMaxGroups; ++i) {
@@ -184,7 +193,7 @@ StepParams step_params(const lsm_sim *s, long long step) {
     P.N = s->N; P.step = step;
     P.hdr = s->hdr; P.T = s->T; P.nbr = s->nbr; P.sid = s->sid;
     P.sp.typ = s->typ; P.sp.kF = s->kF; P.sp.r0F = s->r0F; P.sp.rcF = s->rcF; P.sp.tab = s->tab; P.sp.ntypes = s->ntypes;
-    P.sp.rc32 = s->rc32; P.sp.rcS = s->rcS;
+    P.sp.thr = s->thr; P.sp.rcS = s->rcS; P.sp.kr0_u = s->k_u * s->r0_u; P.sp.thr_u = thr_of(s->rc_u);
     P.sp.k_u = s->k_u; P.sp.r0_u = s->r0_u; P.sp.rc_u = s->rc_u;
     P.break_step = s->break_step; P.nbroken = s->nbroken; P.poff = s->d_poff; P.B = s->B;
     P.sU = s->sU; P.sKE = s->sKE;
@@ -351,7 +360,7 @@ lsm_status eval_initial(lsm_sim *s) {
 lsm_status do_compact(lsm_sim *s) {
     if (s->force_mode == LSM_FORCE_GATHER) {
         CompactParams C;
-        C.hdr = s->hdr; C.nbr = s->nbr; C.sid = s->sid; C.typ = s->typ; C.rc32 = s->rc32;
+        C.hdr = s->hdr; C.nbr = s->nbr; C.sid = s->sid; C.typ = s->typ; C.thr = s->thr;
         C.kF = s->kF; C.r0F = s->r0F; C.nslices = s->nslices;
         k_compact_ell<<<grid_for(s->nslices * kSlice), kBlock, 0, s->stream>>>(C);
         s->kernels_launched += 1;
@@ -586,15 +595,9 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
         TRY(upload(s, &s->nbr, hn));
         if (need_typ) { std::vector<uint8_t> ht(E, 0); for (size_t e = 0; e < E; ++e) if (hs[e] >= 0) ht[e] = stype[hs[e]]; TRY(upload(s, &s->typ, ht)); CUDA_TRY(s, cudaStreamSynchronize(s->stream)); }
         if (need_rcF) {
-            // rc32 = the largest fp32 <= rc: "r <= rc32" proves "r <= rc"; anything closer is settled by the exact rcS
-            std::vector<float> h(E, 0.0f);
-            for (size_t e = 0; e < E; ++e) if (hs[e] >= 0) {
-                const double rc = getrc(hs[e]);
-                float f = (float)rc;
-                if ((double)f > rc) f = std::nextafterf(f, -INFINITY);
-                h[e] = f;
-            }
-            TRY(upload(s, &s->rc32, h)); CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+            std::vector<uint32_t> h(E, 0xFFFFFFFFu);
+            for (size_t e = 0; e < E; ++e) if (hs[e] >= 0) h[e] = thr_of(getrc(hs[e]));
+            TRY(upload(s, &s->thr, h)); CUDA_TRY(s, cudaStreamSynchronize(s->stream));
             std::vector<double> hr(M);
             for (long long e = 0; e < M; ++e) hr[e] = getrc(e);
             TRY(upload(s, &s->rcS, hr)); CUDA_TRY(s, cudaStreamSynchronize(s->stream));
@@ -620,18 +623,20 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
             L.hdr = o; o += 128;
             L.grp = o; o += kTile;
             L.nbr = o; o += up(cap * kSlice * 4);
-            L.rc32 = o; if (need_rcF) o += up(cap * kSlice * 4);
+            L.thr = o; if (need_rcF) o += up(cap * kSlice * 4);
             L.typ = o; if (need_typ) o += up(cap * kSlice);
             L.kF = o; if (need_krF) o += up(cap * kSlice * 8);
             L.r0F = o; if (need_krF) o += up(cap * kSlice * 8);
             L.bytes = up(o);
-            L.first = 128 + (need_typ ? 3 * kMaxTypes * 8 : 0);
+            L.first = 128 + (need_typ ? 4 * kMaxTypes * 8 : 0);
             int dev_smem = 0, n_sm = 0;
             CUDA_TRY(s, cudaDeviceGetAttribute(&dev_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, d->device));
             CUDA_TRY(s, cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, d->device));
-            const int ctas_per_sm = 2;
+            int ctas_per_sm = kStreamMinB, max_stages = 4;
+            if (const char *e = std::getenv("LSM_STREAM_CTAS_PER_SM")) ctas_per_sm = std::max(1, std::min(4, std::atoi(e)));   // tuning overrides
+            if (const char *e = std::getenv("LSM_STREAM_STAGES")) max_stages = std::max(2, std::min<int>(kMaxStages, std::atoi(e)));
             const int budget = std::min(dev_smem, (dev_smem + 1024) / ctas_per_sm - 1024) - L.first;   // 1 KB reserved per CTA
-            L.stages = std::min<int>(kMaxStages, std::min<int>(4, budget / std::max(L.bytes, 1)));
+            L.stages = std::min<int>(max_stages, budget / std::max(L.bytes, 1));
             const bool can_stream = L.stages >= 2;
             if (s->gather_variant == 0) s->gather_variant = can_stream ? 2 : 1;
             if (s->gather_variant == 2 && !can_stream) return fail(s, LSM_E_UNSUPPORTED, "gather_variant = streamed: a tile's rows do not fit in shared memory (degree too high); use the direct variant");
@@ -668,7 +673,18 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
     } else {
         return fail(s, LSM_E_INVALID, "bad force_mode");
     }
-    if (!tab.empty()) { TRY(upload(s, &s->tab, tab)); CUDA_TRY(s, cudaStreamSynchronize(s->stream)); }
+    if (!tab.empty()) {
+        if (s->force_mode == LSM_FORCE_GATHER) {   // gather kernels: 4 doubles per type, the 4th carries the filter word
+            std::vector<double> t4(tab.size() / 3 * 4, 0.0);
+            for (size_t t = 0; t < tab.size() / 3; ++t) {
+                t4[4 * t] = tab[3 * t]; t4[4 * t + 1] = tab[3 * t + 1]; t4[4 * t + 2] = tab[3 * t + 2];
+                const uint64_t w = thr_of(tab[3 * t + 2]);
+                std::memcpy(&t4[4 * t + 3], &w, 8);
+            }
+            tab.swap(t4);
+        }
+        TRY(upload(s, &s->tab, tab)); CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    }
 
     // ---- reductions: chunk table, scratch, history ring ----
     {

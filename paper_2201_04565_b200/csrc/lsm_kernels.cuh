@@ -10,8 +10,8 @@
 //     hdr[T] (64 B per tile: slot offset of each of its 8 slices + end, live width of each slice),
 //     nbr[E] int32 neighbour id (bitwise-NOT of the id once the spring is dead, INT32_MIN = padding),
 //     sid[E] caller spring id (cold: read only when a spring breaks or sits within one fp32 ulp of rc),
-//     per-slot parameters by ParamMode: typ[E] uint8, rc32[E] float = the largest fp32 <= rc (a conservative filter:
-//     r <= rc32 proves r <= rc; otherwise the exact fp64 rcS[sid] decides, so the decision is the fp64 one), kF/r0F[E].
+//     per-slot parameters by ParamMode: typ[E] uint8, thr[E] uint32 = (high word of rc*rc) - 1 (a conservative integer
+//     filter on r^2; anything above it is decided by the exact fp64 rcS[sid], so the decision is the fp64 one), kF/r0F[E].
 //     Slot s of lane l of slice S is entry (off[S] + s)*32 + l  -> every slot load is one coalesced 128-byte line, and
 //     the slots of one tile are one contiguous range per array -> one bulk async copy per array per tile.
 //     Rows are ordered by ascending caller spring id, so a particle sums its springs in the oracle's order.
@@ -28,6 +28,13 @@ constexpr int kSlice = 32;
 constexpr int kTile = 256;            // particles per tile (= kBlock): 8 slices
 constexpr int kTileSlices = kTile / kSlice;
 constexpr int kMaxStages = 8;
+#ifndef LSM_STREAM_MINB
+#define LSM_STREAM_MINB 3      // resident CTAs per SM the streamed kernel is compiled for (register budget)
+#endif
+#ifndef LSM_ROW_CH
+#define LSM_ROW_CH 3           // springs of a row evaluated together (instruction-level parallelism vs registers)
+#endif
+constexpr int kStreamMinB = LSM_STREAM_MINB;
 constexpr int32_t kPad = INT32_MIN;
 constexpr uint8_t kFree = 0xFF;
 constexpr int kMaxGroups = 8;
@@ -51,11 +58,12 @@ struct GroupTab {
 struct SpringParams {  // parameter encoding shared by the gather (per half-edge) and scatter (per spring) layouts
     const uint8_t *typ;
     const double *kF, *r0F, *rcF;      // rcF: scatter layout only
-    const float *rc32;                 // gather layout: fp32 lower bound of rc per half-edge
+    const uint32_t *thr;               // gather layout: breakage filter per half-edge, (high word of rc*rc) - 1
     const double *rcS;                 // gather layout: exact rc per spring, caller numbering
-    const double *tab;  // [ntypes][3] = k, r0, rc
+    const double *tab;  // scatter: [ntypes][3] = k, r0, rc;  gather: [ntypes][4] = k, r0, rc, (thr in the low word)
     int ntypes;
-    double k_u, r0_u, rc_u;
+    double k_u, r0_u, rc_u, kr0_u;
+    uint32_t thr_u;
 };
 
 struct StepParams {
@@ -90,6 +98,19 @@ template <bool E> __device__ __forceinline__ double add(double a, double b) { re
 template <bool E> __device__ __forceinline__ double sub(double a, double b) { return E ? __dsub_rn(a, b) : a - b; }
 template <bool E> __device__ __forceinline__ double mad(double a, double b, double c) {  // a*b + c
     return E ? __dadd_rn(__dmul_rn(a, b), c) : fma(a, b, c);
+}
+
+// Fast-mode 1/sqrt(x) for normal x > 0: hardware seed (MUFU.RSQ64H, ~2^-20 relative) + one cubically convergent
+// correction y = y0 + y0*e*(1/2 + 3/8 e), e = 1 - x*y0^2  ->  ~2^-60 before rounding, 5 fp64 ops, no special-case
+// branch (the library rsqrt() carries a slow-path call per use that breaks the interleaving of a row's springs).
+// x = 0 gives inf / NaN: the callers select those lanes away.
+__device__ __forceinline__ double rsqrt_fast(double x) {
+    double y0;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(x));
+    const double t = x * y0;
+    const double e = fma(-t, y0, 1.0);
+    const double q = fma(0.375, e, 0.5);
+    return fma(y0 * e, q, y0);
 }
 
 __device__ __forceinline__ int spec_of(const long long *poff, int B, long long p) {
@@ -179,7 +200,7 @@ __device__ __forceinline__ void particle_update(const StepParams &P, long long p
 // ---------------------------------------------------------------------------------------------------------------
 struct RowSrc {            // where one particle's row lives: pointers already offset to (slice offset)*32 + lane
     const int32_t *nbr;    // slot s at nbr[s*32]  (global memory, or the staged shared-memory copy)
-    const float *rc32;
+    const uint32_t *thr;
     const uint8_t *typ;
     const double *kF, *r0F;
     const double2 *tile_pos;  // staged positions of the tile's own 256 particles (STAGED only)
@@ -188,102 +209,111 @@ struct RowSrc {            // where one particle's row lives: pointers already o
 };
 
 // The hot part is branch-free (padding slots, dead springs and coincident endpoints contribute an exact 0 through
-// selects, so the six springs of a row interleave in the fp64 pipe); the rare events -- a spring within one fp32 ulp
-// of rc, a spring breaking -- are handled after it under one warp-level branch.  Accumulation stays in slot order
-// (ascending caller spring id): adding +-0.0 for the skipped slots leaves every partial sum bit-identical.
-template <int PM, bool EXACT, bool SAMPLE, bool STAGED>
-__device__ __forceinline__ void row_forces(const StepParams &P, const RowSrc &R, const double *s_tab, long long p, unsigned w,
-                                           double2 xp, double &fx, double &fy, double &u) {
-    constexpr int CH = 6;
-    constexpr bool kHasRc32 = (PM == PM_RCF || PM == PM_KRT_RCF || PM == PM_FULL);
-    for (unsigned s0 = 0; s0 < w; s0 += CH) {
-        int nb[CH];
-        double2 xq[CH];
-        double gk[CH], dx[CH], dy[CH], ue[CH];
-        unsigned hot = 0;  // bit c: slot c needs the rare path (may have broken)
+// selects, so the springs of a chunk interleave in the fp64 pipe); the rare events -- a spring close to rc, a spring
+// breaking -- are handled after it under one warp-level branch.  Accumulation stays in slot order (ascending caller
+// spring id): adding +-0.0 for the skipped slots leaves every partial sum bit-identical.
+//
+// Breakage filter: thr = (high 32 bits of rc*rc) - 1.  For positive doubles the high word orders like the value, so
+// hi32(r2) < thr proves r2 < rc^2 (1 - 2^-20): alive, with one integer compare and no conversion.  Otherwise (r within
+// ~5e-7 of rc, relatively) the rare path takes the decision exactly as the oracle does: r = IEEE sqrt(r2) > rc in fp64.
+template <int PM, bool EXACT, bool SAMPLE, bool STAGED, int CH>
+__device__ __forceinline__ void row_chunk(const StepParams &P, const RowSrc &R, const double *s_tab, long long p, unsigned s0,
+                                          double2 xp, double &fx, double &fy, double &u) {
+    constexpr bool kPerSpringRc = (PM == PM_RCF || PM == PM_KRT_RCF || PM == PM_FULL);
+    int nb[CH];
+    double2 xq[CH];
+    double gk[CH], dx[CH], dy[CH], ue[CH], r2[CH];
+    unsigned hot = 0;  // bit c: slot c needs the rare path (may have broken)
 #pragma unroll
-        for (int c = 0; c < CH; ++c) nb[c] = (s0 + c < w) ? R.nbr[(s0 + c) * kSlice] : kPad;
+    for (int c = 0; c < CH; ++c) nb[c] = R.nbr[(s0 + c) * kSlice];
+#pragma unroll
+    for (int c = 0; c < CH; ++c) {
+        const int j = nb[c] >= 0 ? nb[c] : (int)p;   // padding / dead: gather the own position (always legal)
+        if (STAGED) {
+            const unsigned rel = (unsigned)(j - R.p0);
+            if (rel < (unsigned)kTile) xq[c] = R.tile_pos[rel];
+            else xq[c] = __ldg(P.pos_cur + j);
+        } else {
+            xq[c] = __ldg(P.pos_cur + j);
+        }
+    }
+#pragma unroll
+    for (int c = 0; c < CH; ++c) {
+        const unsigned so = (s0 + c) * kSlice;
+        const bool valid = nb[c] >= 0;
+        double k, r0, kr0;
+        uint32_t thr;
+        if (PM == PM_UNIFORM) { k = P.sp.k_u; r0 = P.sp.r0_u; kr0 = P.sp.kr0_u; thr = P.sp.thr_u; }
+        else if (PM == PM_TYPED) { const int t = R.typ[so]; k = s_tab[4 * t]; r0 = s_tab[4 * t + 1]; kr0 = k * r0; thr = reinterpret_cast<const uint32_t *>(s_tab)[8 * t + 6]; }
+        else if (PM == PM_RCF) { k = P.sp.k_u; r0 = P.sp.r0_u; kr0 = P.sp.kr0_u; thr = R.thr[so]; }
+        else if (PM == PM_KRT_RCF) { const int t = R.typ[so]; k = s_tab[4 * t]; r0 = s_tab[4 * t + 1]; kr0 = k * r0; thr = R.thr[so]; }
+        else { k = R.kF[so]; r0 = R.r0F[so]; kr0 = k * r0; thr = R.thr[so]; }
+        dx[c] = sub<EXACT>(xq[c].x, xp.x); dy[c] = sub<EXACT>(xq[c].y, xp.y);
+        r2[c] = EXACT ? add<true>(mul<true>(dx[c], dx[c]), mul<true>(dy[c], dy[c])) : fma(dy[c], dy[c], dx[c] * dx[c]);
+        const uint32_t hi = (uint32_t)__double2hiint(r2[c]);
+        double g;
+        bool live;
+        if (EXACT) {
+            const double r = __dsqrt_rn(r2[c]);
+            const double ext = sub<true>(r, r0);
+            g = __ddiv_rn(mul<true>(k, ext), r);
+            if (SAMPLE) ue[c] = mul<true>(mul<true>(mul<true>(0.5, k), ext), ext);
+            live = valid && r2[c] > 0.0;         // coincident endpoints: no direction, no force (Q4)
+        } else {
+            const double rinv = rsqrt_fast(r2[c]);
+            g = fma(-kr0, rinv, k);              // k (r - r0) / r = k - k r0 / r
+            if (SAMPLE) { const double ext = fma(r2[c], rinv, -r0); ue[c] = (0.5 * k) * ext * ext; }
+            live = valid && hi >= 0x00100000u;   // r2 zero (or denormal: treated as coincident, Q4)
+        }
+        gk[c] = live ? g : 0.0;
+        if (SAMPLE) ue[c] = (live && p < nb[c]) ? ue[c] : 0.0;  // energy counted once, by the lower endpoint (Eq. 1)
+        if (live && hi >= thr) hot |= 1u << c;
+    }
+    if (hot) {  // rare: decide with the exact rc, mark the broken (Q2, Q3: zero force already in this step)
 #pragma unroll
         for (int c = 0; c < CH; ++c) {
-            const int j = nb[c] >= 0 ? nb[c] : (int)p;   // padding / dead: gather the own position (always legal)
-            if (STAGED) {
-                const unsigned rel = (unsigned)(j - R.p0);
-                if (rel < (unsigned)kTile) xq[c] = R.tile_pos[rel];
-                else xq[c] = __ldg(P.pos_cur + j);
-            } else {
-                xq[c] = __ldg(P.pos_cur + j);
-            }
-        }
-#pragma unroll
-        for (int c = 0; c < CH; ++c) {
-            const unsigned so = (s0 + c < w) ? (s0 + c) * kSlice : 0u;
-            const bool valid = nb[c] >= 0;
-            double k, r0, rc = 0.0;
-            if (PM == PM_UNIFORM) { k = P.sp.k_u; r0 = P.sp.r0_u; rc = P.sp.rc_u; }
-            else if (PM == PM_TYPED) { const int t = R.typ[so]; k = s_tab[3 * t]; r0 = s_tab[3 * t + 1]; rc = s_tab[3 * t + 2]; }
-            else if (PM == PM_RCF) { k = P.sp.k_u; r0 = P.sp.r0_u; rc = (double)R.rc32[so]; }
-            else if (PM == PM_KRT_RCF) { const int t = R.typ[so]; k = s_tab[3 * t]; r0 = s_tab[3 * t + 1]; rc = (double)R.rc32[so]; }
-            else { k = R.kF[so]; r0 = R.r0F[so]; rc = (double)R.rc32[so]; }
-            dx[c] = sub<EXACT>(xq[c].x, xp.x); dy[c] = sub<EXACT>(xq[c].y, xp.y);
-            const double r2 = EXACT ? add<true>(mul<true>(dx[c], dx[c]), mul<true>(dy[c], dy[c])) : fma(dy[c], dy[c], dx[c] * dx[c]);
-            double r, g;
-            if (EXACT) {
-                r = __dsqrt_rn(r2);
-                const double ext = sub<true>(r, r0);
-                g = __ddiv_rn(mul<true>(k, ext), r);
-                ue[c] = mul<true>(mul<true>(mul<true>(0.5, k), ext), ext);
-            } else {
-                const double rinv = rsqrt(r2);
-                r = r2 * rinv;
-                const double ext = r - r0;
-                g = (k * ext) * rinv;
-                ue[c] = (0.5 * k) * ext * ext;
-            }
-            // coincident endpoints (r2 == 0: no direction, no force, Q4) and padding / dead slots contribute 0
-            const bool live = valid && r2 > 0.0;
-            gk[c] = live ? g : 0.0;
-            ue[c] = (SAMPLE && live && p < nb[c]) ? ue[c] : 0.0;  // energy counted once, by the lower endpoint (Eq. 1)
-            // strict '>' (Q1).  With a per-spring rc, rc holds its fp32 lower bound here: r <= rc32 proves r <= rc.
-            if (live && r > rc) hot |= 1u << c;
-        }
-        if (hot) {  // rare: settle with the exact rc, mark the broken (Q2, Q3: zero force already in this step)
-#pragma unroll
-            for (int c = 0; c < CH; ++c) {
-                if (hot & (1u << c)) {
-                    const size_t e = R.e0 + (size_t)(s0 + c) * kSlice;
-                    bool broke = true;
-                    if (kHasRc32) {
-                        const double r2 = EXACT ? add<true>(mul<true>(dx[c], dx[c]), mul<true>(dy[c], dy[c])) : fma(dy[c], dy[c], dx[c] * dx[c]);
-                        const double r = EXACT ? __dsqrt_rn(r2) : r2 * rsqrt(r2);
-                        broke = r > __ldg(P.sp.rcS + __ldg(P.sid + e));
-                    }
-                    if (broke) {
-                        gk[c] = 0.0; ue[c] = 0.0;
-                        P.nbr[e] = ~nb[c];
-                        if (p < nb[c]) {
-                            P.break_step[P.sid[e]] = P.step;
-                            atomicAdd(P.nbroken + spec_of(P.poff, P.B, p), 1ULL);
-                        }
+            if (hot & (1u << c)) {
+                const size_t e = R.e0 + (size_t)(s0 + c) * kSlice;
+                double rc;
+                if (PM == PM_UNIFORM) rc = P.sp.rc_u;
+                else if (PM == PM_TYPED) rc = s_tab[4 * R.typ[(s0 + c) * kSlice] + 2];
+                else rc = __ldg(P.sp.rcS + __ldg(P.sid + e));
+                if (__dsqrt_rn(r2[c]) > rc) {   // strict '>' (Q1); both endpoints see bit-identical r2 ((-dx)^2 == dx^2)
+                    gk[c] = 0.0;
+                    if (SAMPLE) ue[c] = 0.0;
+                    P.nbr[e] = ~nb[c];
+                    if (p < nb[c]) {
+                        P.break_step[P.sid[e]] = P.step;
+                        atomicAdd(P.nbroken + spec_of(P.poff, P.B, p), 1ULL);
                     }
                 }
             }
         }
-#pragma unroll
-        for (int c = 0; c < CH; ++c) {
-            fx = mad<EXACT>(gk[c], dx[c], fx);
-            fy = mad<EXACT>(gk[c], dy[c], fy);
-            if (SAMPLE) u = add<EXACT>(u, ue[c]);
-        }
     }
+#pragma unroll
+    for (int c = 0; c < CH; ++c) {
+        fx = mad<EXACT>(gk[c], dx[c], fx);
+        fy = mad<EXACT>(gk[c], dy[c], fy);
+        if (SAMPLE) u = add<EXACT>(u, ue[c]);
+    }
+}
+
+template <int PM, bool EXACT, bool SAMPLE, bool STAGED>
+__device__ __forceinline__ void row_forces(const StepParams &P, const RowSrc &R, const double *s_tab, long long p, unsigned w,
+                                           double2 xp, double &fx, double &fy, double &u) {
+    constexpr int CH = LSM_ROW_CH;
+    unsigned s0 = 0;
+    for (; s0 + CH <= w; s0 += CH) row_chunk<PM, EXACT, SAMPLE, STAGED, CH>(P, R, s_tab, p, s0, xp, fx, fy, u);
+    for (; s0 < w; ++s0) row_chunk<PM, EXACT, SAMPLE, STAGED, 1>(P, R, s_tab, p, s0, xp, fx, fy, u);
 }
 
 // Direct variant: block = tile, every stream read from global memory by the thread that needs it.
 template <int PM, bool EXACT, bool KICK2, bool ADVANCE, bool SAMPLE>
 __global__ void __launch_bounds__(kBlock) k_gather_step(const StepParams P) {
     constexpr bool kTab = (PM == PM_TYPED || PM == PM_KRT_RCF);
-    __shared__ double s_tab[kTab ? 3 * kMaxTypes : 1];
+    __shared__ double s_tab[kTab ? 4 * kMaxTypes : 1];
     if (kTab) {
-        for (int i = threadIdx.x; i < 3 * P.sp.ntypes; i += kBlock) s_tab[i] = P.sp.tab[i];
+        for (int i = threadIdx.x; i < 4 * P.sp.ntypes; i += kBlock) s_tab[i] = P.sp.tab[i];
         __syncthreads();
     }
     const long long p = (long long)blockIdx.x * kBlock + threadIdx.x;
@@ -296,7 +326,7 @@ __global__ void __launch_bounds__(kBlock) k_gather_step(const StepParams P) {
     const double2 vh = P.vel[p];
     const uint8_t g = P.grp[p];
     RowSrc R;
-    R.nbr = P.nbr + e0; R.rc32 = P.sp.rc32 + e0; R.typ = P.sp.typ + e0; R.kF = P.sp.kF + e0; R.r0F = P.sp.r0F + e0;
+    R.nbr = P.nbr + e0; R.thr = P.sp.thr + e0; R.typ = P.sp.typ + e0; R.kF = P.sp.kF + e0; R.r0F = P.sp.r0F + e0;
     R.tile_pos = nullptr; R.p0 = 0; R.e0 = e0;
     double fx = 0.0, fy = 0.0, u = 0.0;
     row_forces<PM, EXACT, SAMPLE, false>(P, R, s_tab, p, w, xp, fx, fy, u);
@@ -328,7 +358,7 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned by
 }
 
 struct StageLayout {      // byte offsets of the staged arrays inside one pipeline stage (all multiples of 128)
-    int pos, vel, hdr, grp, nbr, rc32, typ, kF, r0F;
+    int pos, vel, hdr, grp, nbr, thr, typ, kF, r0F;
     int bytes;            // stage size
     int stages;           // pipeline depth
     int first;            // offset of stage 0 in dynamic shared memory (after the barriers and the type table)
@@ -340,22 +370,22 @@ struct StageLayout {      // byte offsets of the staged arrays inside one pipeli
 // particle).  The bytes in flight per SM are (stages - 1) x stage size x CTAs/SM, independent of registers and
 // occupancy; the only latency the consumers see is the neighbour-position gather (L2 / L1 hits, or the staged tile).
 template <int PM, bool EXACT, bool KICK2, bool ADVANCE, bool SAMPLE>
-__global__ void __launch_bounds__(kTile + 32, 2) k_gather_stream(const StepParams P, const StageLayout L) {
+__global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const StepParams P, const StageLayout L) {
     constexpr bool kTab = (PM == PM_TYPED || PM == PM_KRT_RCF);
-    constexpr bool kHasRc32 = (PM == PM_RCF || PM == PM_KRT_RCF || PM == PM_FULL);
+    constexpr bool kHasThr = (PM == PM_RCF || PM == PM_KRT_RCF || PM == PM_FULL);
     constexpr bool kHasTyp = kTab;
     constexpr bool kHasKR = (PM == PM_FULL);
     extern __shared__ __align__(128) unsigned char smem[];
     uint64_t *full = reinterpret_cast<uint64_t *>(smem);          // [kMaxStages]
     uint64_t *empty = full + kMaxStages;                            // [kMaxStages]
-    double *s_tab = reinterpret_cast<double *>(smem + 128);         // [3*kMaxTypes] when kTab
+    double *s_tab = reinterpret_cast<double *>(smem + 128);         // [4*kMaxTypes] when kTab
     unsigned char *stage0 = smem + L.first;
     const int tid = threadIdx.x, wi = tid >> 5, lane = tid & 31;
     if (tid == 0) {
         for (int s = 0; s < L.stages; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, kTileSlices); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    if (kTab) for (int i = tid; i < 3 * P.sp.ntypes; i += kTile + 32) s_tab[i] = P.sp.tab[i];
+    if (kTab) for (int i = tid; i < 4 * P.sp.ntypes; i += kTile + 32) s_tab[i] = P.sp.tab[i];
     __syncthreads();
 
     if (wi == kTileSlices) {  // ---------------- producer warp ----------------
@@ -367,7 +397,7 @@ __global__ void __launch_bounds__(kTile + 32, 2) k_gather_stream(const StepParam
                 const uint32_t o0 = __ldg(&h->off[0]);
                 const uint32_t ns = __ldg(&h->off[kTileSlices]) - o0;
                 unsigned bytes = 2 * kTile * 16 + kTile + 64 + ns * (kSlice * 4);
-                if (kHasRc32) bytes += ns * (kSlice * 4);
+                if (kHasThr) bytes += ns * (kSlice * 4);
                 if (kHasTyp) bytes += ns * kSlice;
                 if (kHasKR) bytes += 2 * ns * (kSlice * 8);
                 unsigned char *b = stage0 + (size_t)s * L.bytes;
@@ -379,7 +409,7 @@ __global__ void __launch_bounds__(kTile + 32, 2) k_gather_stream(const StepParam
                 if (ns) {
                     const size_t e = (size_t)o0 * kSlice;
                     bulk_g2s(b + L.nbr, P.nbr + e, ns * (kSlice * 4), full + s);
-                    if (kHasRc32) bulk_g2s(b + L.rc32, P.sp.rc32 + e, ns * (kSlice * 4), full + s);
+                    if (kHasThr) bulk_g2s(b + L.thr, P.sp.thr + e, ns * (kSlice * 4), full + s);
                     if (kHasTyp) bulk_g2s(b + L.typ, P.sp.typ + e, ns * kSlice, full + s);
                     if (kHasKR) {
                         bulk_g2s(b + L.kF, P.sp.kF + e, ns * (kSlice * 8), full + s);
@@ -406,7 +436,7 @@ __global__ void __launch_bounds__(kTile + 32, 2) k_gather_stream(const StepParam
             const uint8_t g = (b + L.grp)[tid];
             RowSrc R;
             R.nbr = reinterpret_cast<const int32_t *>(b + L.nbr) + rel;
-            R.rc32 = reinterpret_cast<const float *>(b + L.rc32) + rel;
+            R.thr = reinterpret_cast<const uint32_t *>(b + L.thr) + rel;
             R.typ = (b + L.typ) + rel;
             R.kF = reinterpret_cast<const double *>(b + L.kF) + rel;
             R.r0F = reinterpret_cast<const double *>(b + L.r0F) + rel;
@@ -597,7 +627,7 @@ struct CompactParams {
     TileHdr *hdr;
     int32_t *nbr, *sid;
     uint8_t *typ;
-    float *rc32;
+    uint32_t *thr;
     double *kF, *r0F;
     long long nslices;
 };
@@ -619,7 +649,7 @@ __global__ void __launch_bounds__(kBlock) k_compact_ell(const CompactParams C) {
                 const size_t d = e0 + (size_t)j * kSlice;
                 C.nbr[d] = nb; C.sid[d] = C.sid[e];
                 if (C.typ) C.typ[d] = C.typ[e];
-                if (C.rc32) C.rc32[d] = C.rc32[e];
+                if (C.thr) C.thr[d] = C.thr[e];
                 if (C.kF) C.kF[d] = C.kF[e];
                 if (C.r0F) C.r0F[d] = C.r0F[e];
             }
