@@ -32,7 +32,7 @@ constexpr int kMaxStages = 8;
 #define LSM_STREAM_MINB 3      // resident CTAs per SM the streamed kernel is compiled for (register budget)
 #endif
 #ifndef LSM_ROW_CH
-#define LSM_ROW_CH 3           // springs of a row evaluated together (instruction-level parallelism vs registers)
+#define LSM_ROW_CH 6           // springs of a row evaluated together (instruction-level parallelism vs registers)
 #endif
 constexpr int kStreamMinB = LSM_STREAM_MINB;
 constexpr int32_t kPad = INT32_MIN;
@@ -208,103 +208,131 @@ struct RowSrc {            // where one particle's row lives: pointers already o
     size_t e0;                // global entry index of slot 0 of this lane (for the cold paths)
 };
 
-// The hot part is branch-free (padding slots, dead springs and coincident endpoints contribute an exact 0 through
-// selects, so the springs of a chunk interleave in the fp64 pipe); the rare events -- a spring close to rc, a spring
-// breaking -- are handled after it under one warp-level branch.  Accumulation stays in slot order (ascending caller
-// spring id): adding +-0.0 for the skipped slots leaves every partial sum bit-identical.
+// Row evaluation in two passes.  The FAST pass is branch-free: padding slots, dead springs and coincident endpoints
+// contribute an exact 0 through selects, every slot is accumulated at once in slot order (ascending caller spring
+// id; adding +-0.0 for skipped slots leaves each partial sum bit-identical), and nothing is kept per slot, so the
+// springs of a chunk interleave in the fp64 pipe with few registers.  It only notes whether any spring came close to
+// its breaking length.  If one did (rare), the CAREFUL pass redoes the whole row from zero, slot by slot in the
+// same order with the same arithmetic, deciding each near-rc spring exactly and marking the broken ones (Q2, Q3:
+// zero force already in the step they break).
 //
 // Breakage filter: thr = (high 32 bits of rc*rc) - 1.  For positive doubles the high word orders like the value, so
 // hi32(r2) < thr proves r2 < rc^2 (1 - 2^-20): alive, with one integer compare and no conversion.  Otherwise (r within
-// ~5e-7 of rc, relatively) the rare path takes the decision exactly as the oracle does: r = IEEE sqrt(r2) > rc in fp64.
+// ~5e-7 of rc, relatively) the careful pass decides exactly as the oracle does: r = IEEE sqrt(r2) > rc in fp64.
+template <int PM> __device__ __forceinline__ void slot_params(const StepParams &P, const RowSrc &R, const double *s_tab, unsigned so,
+                                                              double &k, double &r0, double &kr0, uint32_t &thr) {
+    if (PM == PM_UNIFORM) { k = P.sp.k_u; r0 = P.sp.r0_u; kr0 = P.sp.kr0_u; thr = P.sp.thr_u; }
+    else if (PM == PM_TYPED) { const int t = R.typ[so]; k = s_tab[4 * t]; r0 = s_tab[4 * t + 1]; kr0 = k * r0; thr = reinterpret_cast<const uint32_t *>(s_tab)[8 * t + 6]; }
+    else if (PM == PM_RCF) { k = P.sp.k_u; r0 = P.sp.r0_u; kr0 = P.sp.kr0_u; thr = R.thr[so]; }
+    else if (PM == PM_KRT_RCF) { const int t = R.typ[so]; k = s_tab[4 * t]; r0 = s_tab[4 * t + 1]; kr0 = k * r0; thr = R.thr[so]; }
+    else { k = R.kF[so]; r0 = R.r0F[so]; kr0 = k * r0; thr = R.thr[so]; }
+}
+
+template <bool STAGED> __device__ __forceinline__ double2 gather_pos(const StepParams &P, const RowSrc &R, int j) {
+    if (STAGED) {
+        const unsigned rel = (unsigned)(j - R.p0);
+        if (rel < (unsigned)kTile) return R.tile_pos[rel];
+    }
+    return __ldg(P.pos_cur + j);
+}
+
+// One spring seen from one endpoint (Eq. 2): d = x_other - x_self, g = k (r - r0) / r.
+// live: the slot holds a spring with a direction (valid and r2 > 0; coincident endpoints give no force, Q4);
+// near: r2 reaches the breakage filter (see above).  Both endpoints compute bit-identical r2 ((-dx)^2 == dx^2).
+template <bool EXACT, bool SAMPLE>
+__device__ __forceinline__ void slot_eval(double2 xq, double2 xp, bool valid, bool lower, double k, double r0, double kr0, uint32_t thr,
+                                          double &dx, double &dy, double &r2, double &g, double &ue, bool &near) {
+    dx = sub<EXACT>(xq.x, xp.x); dy = sub<EXACT>(xq.y, xp.y);
+    r2 = EXACT ? add<true>(mul<true>(dx, dx), mul<true>(dy, dy)) : fma(dy, dy, dx * dx);
+    const uint32_t hi = (uint32_t)__double2hiint(r2);
+    bool live;
+    ue = 0.0;
+    if (EXACT) {
+        const double r = __dsqrt_rn(r2);
+        const double ext = sub<true>(r, r0);
+        g = __ddiv_rn(mul<true>(k, ext), r);
+        if (SAMPLE) ue = mul<true>(mul<true>(mul<true>(0.5, k), ext), ext);
+        live = valid && r2 > 0.0;
+    } else {
+        const double rinv = rsqrt_fast(r2);
+        g = fma(-kr0, rinv, k);              // k (r - r0) / r = k - k r0 / r
+        if (SAMPLE) { const double ext = fma(r2, rinv, -r0); ue = (0.5 * k) * ext * ext; }
+        live = valid && hi >= 0x00100000u;   // r2 zero (or denormal: treated as coincident)
+    }
+    g = live ? g : 0.0;
+    if (SAMPLE) ue = (live && lower) ? ue : 0.0;  // energy counted once, by the lower endpoint (Eq. 1)
+    near = live && hi >= thr;
+}
+
 template <int PM, bool EXACT, bool SAMPLE, bool STAGED, int CH>
-__device__ __forceinline__ void row_chunk(const StepParams &P, const RowSrc &R, const double *s_tab, long long p, unsigned s0,
+__device__ __forceinline__ bool row_chunk(const StepParams &P, const RowSrc &R, const double *s_tab, int p, unsigned s0,
                                           double2 xp, double &fx, double &fy, double &u) {
-    constexpr bool kPerSpringRc = (PM == PM_RCF || PM == PM_KRT_RCF || PM == PM_FULL);
     int nb[CH];
     double2 xq[CH];
-    double gk[CH], dx[CH], dy[CH], ue[CH], r2[CH];
-    unsigned hot = 0;  // bit c: slot c needs the rare path (may have broken)
+    bool any_near = false;
 #pragma unroll
     for (int c = 0; c < CH; ++c) nb[c] = R.nbr[(s0 + c) * kSlice];
 #pragma unroll
-    for (int c = 0; c < CH; ++c) {
-        const int j = nb[c] >= 0 ? nb[c] : (int)p;   // padding / dead: gather the own position (always legal)
-        if (STAGED) {
-            const unsigned rel = (unsigned)(j - R.p0);
-            if (rel < (unsigned)kTile) xq[c] = R.tile_pos[rel];
-            else xq[c] = __ldg(P.pos_cur + j);
-        } else {
-            xq[c] = __ldg(P.pos_cur + j);
-        }
-    }
+    for (int c = 0; c < CH; ++c) xq[c] = gather_pos<STAGED>(P, R, nb[c] >= 0 ? nb[c] : p);  // padding / dead: own position
 #pragma unroll
     for (int c = 0; c < CH; ++c) {
-        const unsigned so = (s0 + c) * kSlice;
-        const bool valid = nb[c] >= 0;
-        double k, r0, kr0;
+        double k, r0, kr0, dx, dy, r2, g, ue;
         uint32_t thr;
-        if (PM == PM_UNIFORM) { k = P.sp.k_u; r0 = P.sp.r0_u; kr0 = P.sp.kr0_u; thr = P.sp.thr_u; }
-        else if (PM == PM_TYPED) { const int t = R.typ[so]; k = s_tab[4 * t]; r0 = s_tab[4 * t + 1]; kr0 = k * r0; thr = reinterpret_cast<const uint32_t *>(s_tab)[8 * t + 6]; }
-        else if (PM == PM_RCF) { k = P.sp.k_u; r0 = P.sp.r0_u; kr0 = P.sp.kr0_u; thr = R.thr[so]; }
-        else if (PM == PM_KRT_RCF) { const int t = R.typ[so]; k = s_tab[4 * t]; r0 = s_tab[4 * t + 1]; kr0 = k * r0; thr = R.thr[so]; }
-        else { k = R.kF[so]; r0 = R.r0F[so]; kr0 = k * r0; thr = R.thr[so]; }
-        dx[c] = sub<EXACT>(xq[c].x, xp.x); dy[c] = sub<EXACT>(xq[c].y, xp.y);
-        r2[c] = EXACT ? add<true>(mul<true>(dx[c], dx[c]), mul<true>(dy[c], dy[c])) : fma(dy[c], dy[c], dx[c] * dx[c]);
-        const uint32_t hi = (uint32_t)__double2hiint(r2[c]);
-        double g;
-        bool live;
-        if (EXACT) {
-            const double r = __dsqrt_rn(r2[c]);
-            const double ext = sub<true>(r, r0);
-            g = __ddiv_rn(mul<true>(k, ext), r);
-            if (SAMPLE) ue[c] = mul<true>(mul<true>(mul<true>(0.5, k), ext), ext);
-            live = valid && r2[c] > 0.0;         // coincident endpoints: no direction, no force (Q4)
-        } else {
-            const double rinv = rsqrt_fast(r2[c]);
-            g = fma(-kr0, rinv, k);              // k (r - r0) / r = k - k r0 / r
-            if (SAMPLE) { const double ext = fma(r2[c], rinv, -r0); ue[c] = (0.5 * k) * ext * ext; }
-            live = valid && hi >= 0x00100000u;   // r2 zero (or denormal: treated as coincident, Q4)
-        }
-        gk[c] = live ? g : 0.0;
-        if (SAMPLE) ue[c] = (live && p < nb[c]) ? ue[c] : 0.0;  // energy counted once, by the lower endpoint (Eq. 1)
-        if (live && hi >= thr) hot |= 1u << c;
+        bool near;
+        slot_params<PM>(P, R, s_tab, (s0 + c) * kSlice, k, r0, kr0, thr);
+        slot_eval<EXACT, SAMPLE>(xq[c], xp, nb[c] >= 0, p < nb[c], k, r0, kr0, thr, dx, dy, r2, g, ue, near);
+        fx = mad<EXACT>(g, dx, fx);
+        fy = mad<EXACT>(g, dy, fy);
+        if (SAMPLE) u = add<EXACT>(u, ue);
+        any_near |= near;
     }
-    if (hot) {  // rare: decide with the exact rc, mark the broken (Q2, Q3: zero force already in this step)
-#pragma unroll
-        for (int c = 0; c < CH; ++c) {
-            if (hot & (1u << c)) {
-                const size_t e = R.e0 + (size_t)(s0 + c) * kSlice;
-                double rc;
-                if (PM == PM_UNIFORM) rc = P.sp.rc_u;
-                else if (PM == PM_TYPED) rc = s_tab[4 * R.typ[(s0 + c) * kSlice] + 2];
-                else rc = __ldg(P.sp.rcS + __ldg(P.sid + e));
-                if (__dsqrt_rn(r2[c]) > rc) {   // strict '>' (Q1); both endpoints see bit-identical r2 ((-dx)^2 == dx^2)
-                    gk[c] = 0.0;
-                    if (SAMPLE) ue[c] = 0.0;
-                    P.nbr[e] = ~nb[c];
-                    if (p < nb[c]) {
-                        P.break_step[P.sid[e]] = P.step;
-                        atomicAdd(P.nbroken + spec_of(P.poff, P.B, p), 1ULL);
-                    }
+    return any_near;
+}
+
+template <int PM, bool EXACT, bool SAMPLE, bool STAGED>
+__device__ __forceinline__ void row_careful(const StepParams &P, const RowSrc &R, const double *s_tab, int p, unsigned w,
+                                         double2 xp, double &fx, double &fy, double &u) {
+    fx = 0.0; fy = 0.0; u = 0.0;
+#pragma unroll 1
+    for (unsigned s = 0; s < w; ++s) {
+        const unsigned so = s * kSlice;
+        const int nb = R.nbr[so];
+        const double2 xq = gather_pos<STAGED>(P, R, nb >= 0 ? nb : p);
+        double k, r0, kr0, dx, dy, r2, g, ue;
+        uint32_t thr;
+        bool near;
+        slot_params<PM>(P, R, s_tab, so, k, r0, kr0, thr);
+        slot_eval<EXACT, SAMPLE>(xq, xp, nb >= 0, p < nb, k, r0, kr0, thr, dx, dy, r2, g, ue, near);
+        if (near) {
+            const size_t e = R.e0 + so;
+            double rc;
+            if (PM == PM_UNIFORM) rc = P.sp.rc_u;
+            else if (PM == PM_TYPED) rc = s_tab[4 * R.typ[so] + 2];
+            else rc = __ldg(P.sp.rcS + __ldg(P.sid + e));
+            if (__dsqrt_rn(r2) > rc) {   // strict '>' (Q1)
+                P.nbr[e] = ~nb;
+                if (p < nb) {
+                    P.break_step[P.sid[e]] = P.step;
+                    atomicAdd(P.nbroken + spec_of(P.poff, P.B, p), 1ULL);
                 }
+                continue;
             }
         }
-    }
-#pragma unroll
-    for (int c = 0; c < CH; ++c) {
-        fx = mad<EXACT>(gk[c], dx[c], fx);
-        fy = mad<EXACT>(gk[c], dy[c], fy);
-        if (SAMPLE) u = add<EXACT>(u, ue[c]);
+        fx = mad<EXACT>(g, dx, fx);
+        fy = mad<EXACT>(g, dy, fy);
+        if (SAMPLE) u = add<EXACT>(u, ue);
     }
 }
 
 template <int PM, bool EXACT, bool SAMPLE, bool STAGED>
-__device__ __forceinline__ void row_forces(const StepParams &P, const RowSrc &R, const double *s_tab, long long p, unsigned w,
+__device__ __forceinline__ void row_forces(const StepParams &P, const RowSrc &R, const double *s_tab, int p, unsigned w,
                                            double2 xp, double &fx, double &fy, double &u) {
     constexpr int CH = LSM_ROW_CH;
     unsigned s0 = 0;
-    for (; s0 + CH <= w; s0 += CH) row_chunk<PM, EXACT, SAMPLE, STAGED, CH>(P, R, s_tab, p, s0, xp, fx, fy, u);
-    for (; s0 < w; ++s0) row_chunk<PM, EXACT, SAMPLE, STAGED, 1>(P, R, s_tab, p, s0, xp, fx, fy, u);
+    bool any_near = false;
+    for (; s0 + CH <= w; s0 += CH) any_near |= row_chunk<PM, EXACT, SAMPLE, STAGED, CH>(P, R, s_tab, p, s0, xp, fx, fy, u);
+    for (; s0 < w; ++s0) any_near |= row_chunk<PM, EXACT, SAMPLE, STAGED, 1>(P, R, s_tab, p, s0, xp, fx, fy, u);
+    if (any_near) row_careful<PM, EXACT, SAMPLE, STAGED>(P, R, s_tab, p, w, xp, fx, fy, u);
 }
 
 // Direct variant: block = tile, every stream read from global memory by the thread that needs it.
@@ -329,7 +357,7 @@ __global__ void __launch_bounds__(kBlock) k_gather_step(const StepParams P) {
     R.nbr = P.nbr + e0; R.thr = P.sp.thr + e0; R.typ = P.sp.typ + e0; R.kF = P.sp.kF + e0; R.r0F = P.sp.r0F + e0;
     R.tile_pos = nullptr; R.p0 = 0; R.e0 = e0;
     double fx = 0.0, fy = 0.0, u = 0.0;
-    row_forces<PM, EXACT, SAMPLE, false>(P, R, s_tab, p, w, xp, fx, fy, u);
+    row_forces<PM, EXACT, SAMPLE, false>(P, R, s_tab, (int)p, w, xp, fx, fy, u);
     particle_update<EXACT, KICK2, ADVANCE, SAMPLE>(P, p, xp, vh, g, fx, fy, u);
 }
 
@@ -391,11 +419,13 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
     if (wi == kTileSlices) {  // ---------------- producer warp ----------------
         if (lane == 0) {
             int s = 0; unsigned u = 0;
+            uint32_t o0n = 0, o8n = 0;
+            if ((long long)blockIdx.x < P.T) { o0n = __ldg(&P.hdr[blockIdx.x].off[0]); o8n = __ldg(&P.hdr[blockIdx.x].off[kTileSlices]); }
             for (long long t = blockIdx.x; t < P.T; t += gridDim.x) {
-                if (u > 0) mbar_wait(empty + s, (u - 1) & 1);
                 const TileHdr *h = P.hdr + t;
-                const uint32_t o0 = __ldg(&h->off[0]);
-                const uint32_t ns = __ldg(&h->off[kTileSlices]) - o0;
+                const uint32_t o0 = o0n, ns = o8n - o0n;
+                if (t + gridDim.x < P.T) { o0n = __ldg(&h[gridDim.x].off[0]); o8n = __ldg(&h[gridDim.x].off[kTileSlices]); }  // next tile's extent, ahead of the wait
+                if (u > 0) mbar_wait(empty + s, (u - 1) & 1);
                 unsigned bytes = 2 * kTile * 16 + kTile + 64 + ns * (kSlice * 4);
                 if (kHasThr) bytes += ns * (kSlice * 4);
                 if (kHasTyp) bytes += ns * kSlice;
@@ -432,8 +462,6 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
             const unsigned w = h->w[wi];
             const unsigned rel = (h->off[wi] - h->off[0]) * kSlice + lane;
             const double2 xp = reinterpret_cast<const double2 *>(b + L.pos)[tid];
-            const double2 vh = reinterpret_cast<const double2 *>(b + L.vel)[tid];
-            const uint8_t g = (b + L.grp)[tid];
             RowSrc R;
             R.nbr = reinterpret_cast<const int32_t *>(b + L.nbr) + rel;
             R.thr = reinterpret_cast<const uint32_t *>(b + L.thr) + rel;
@@ -444,7 +472,9 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
             R.p0 = (int)(t * kTile);
             R.e0 = (size_t)h->off[wi] * kSlice + lane;
             double fx = 0.0, fy = 0.0, uu = 0.0;
-            row_forces<PM, EXACT, SAMPLE, true>(P, R, s_tab, p, w, xp, fx, fy, uu);
+            row_forces<PM, EXACT, SAMPLE, true>(P, R, s_tab, (int)p, w, xp, fx, fy, uu);
+            const double2 vh = reinterpret_cast<const double2 *>(b + L.vel)[tid];
+            const uint8_t g = (b + L.grp)[tid];
             particle_update<EXACT, KICK2, ADVANCE, SAMPLE>(P, p, xp, vh, g, fx, fy, uu);
         }
         __syncwarp();
