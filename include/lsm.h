@@ -36,7 +36,7 @@ extern "C" {
 #endif
 
 #define LSM_MAX_GROUPS 8
-#define LSM_ABI_VERSION 2
+#define LSM_ABI_VERSION 3
 
 typedef struct lsm_sim lsm_sim; /* opaque */
 
@@ -48,7 +48,7 @@ typedef enum {
     LSM_E_CUDA = -4,        /* CUDA runtime error, or no CUDA device                                               */
     LSM_E_NOMEM = -5,       /* host or device allocation failed                                                    */
     LSM_E_STATE = -6,       /* the simulation failed earlier (e.g. non-finite energy detected on the device)       */
-    LSM_E_UNSUPPORTED = -7  /* dim = 3, reorder = 2 (RCM), exact arithmetic with the scatter kernel                */
+    LSM_E_UNSUPPORTED = -7  /* dim = 3, exact arithmetic with the scatter kernel, degree > 255 in the gather layout  */
 } lsm_status;
 
 enum { LSM_FIXED = 0, LSM_MOVE = 1 };                      /* boundary group modes */
@@ -57,6 +57,7 @@ enum { LSM_REORDER_NONE = 0, LSM_REORDER_MORTON = 1, LSM_REORDER_RCM = 2 };
 /* kernels of the gather path: DIRECT = one thread per particle reading global memory; STREAMED = persistent CTAs,
  * bulk-async-copy (TMA engine) staging of the tile streams through a shared-memory mbarrier pipeline */
 enum { LSM_GATHER_AUTO = 0, LSM_GATHER_DIRECT = 1, LSM_GATHER_STREAMED = 2 };
+enum { LSM_FUSION_AUTO = 0, LSM_FUSION_ON = 1, LSM_FUSION_OFF = 2 };
 
 /* Optional device allocator (the Python binding passes PyTorch's caching allocator). */
 typedef void *(*lsm_alloc_fn)(size_t bytes, void *user);  /* returns a DEVICE pointer, NULL on failure */
@@ -83,12 +84,14 @@ typedef struct lsm_desc {
     int32_t sample_every;             /* record {step, R_g, U, KE, n_broken} when step % sample_every == 0; 0 off */
     int32_t history_capacity;         /* samples kept in the device ring (0 -> 1024); oldest overwritten          */
     int32_t compact_every;            /* drop dead springs from the device lists every this many steps; 0 never   */
-    int32_t reorder;                  /* LSM_REORDER_*: internal particle renumbering for gather locality         */
+    int32_t reorder;                  /* LSM_REORDER_*: internal particle renumbering for gather locality: Morton order of
+                                         the initial positions, or reverse Cuthill-McKee on the spring graph        */
     int32_t force_mode;               /* LSM_FORCE_*: AUTO = GATHER                                               */
     int32_t exact;                    /* 1: IEEE sqrt/divide, no FMA contraction, each particle sums its springs in
                                          ascending caller spring id -> bit-identical to a serial loop over the
                                          spring list (GATHER only).  0: fast arithmetic (FMA, rsqrt)              */
-    int32_t use_graph;                /* 1: replay the step loop from CUDA graphs (small, launch-bound problems)  */
+    int32_t step_fusion;              /* LSM_FUSION_*: run several time steps per (cooperative) launch with a grid
+                                         barrier between steps; AUTO = ON for L2-resident, launch-bound problems    */
     int32_t gather_variant;           /* LSM_GATHER_*: AUTO = STREAMED when a tile's rows fit in shared memory    */
     int32_t device;                   /* CUDA device ordinal                                                      */
     int32_t _pad1;
@@ -115,6 +118,8 @@ typedef struct lsm_info {
     int32_t gather_variant;           /* resolved LSM_GATHER_* (0 for the scatter path)                           */
     int32_t pipeline_stages;          /* streamed variant: stages of the shared-memory pipeline                   */
     int64_t stage_bytes;              /* streamed variant: bytes per stage                                        */
+    int32_t step_fusion;              /* 1 if runs of plain time steps are fused into one launch                  */
+    int32_t _pad;
 } lsm_info;
 
 /* Build a simulation from particle / spring arrays.  Copies everything (the caller may free its inputs afterwards),

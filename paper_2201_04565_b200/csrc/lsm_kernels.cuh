@@ -35,6 +35,7 @@ constexpr int kMaxStages = 8;
 #define LSM_ROW_CH 6           // springs of a row evaluated together (instruction-level parallelism vs registers)
 #endif
 constexpr int kStreamMinB = LSM_STREAM_MINB;
+constexpr int kStreamHdrBytes = 256;   // mbarriers at the front of the streamed kernel's dynamic shared memory
 constexpr int32_t kPad = INT32_MIN;
 constexpr uint8_t kFree = 0xFF;
 constexpr int kMaxGroups = 8;
@@ -64,6 +65,12 @@ struct SpringParams {  // parameter encoding shared by the gather (per half-edge
     int ntypes;
     double k_u, r0_u, rc_u, kr0_u;
     uint32_t thr_u;
+};
+
+struct StepVar {        // what changes from one time step to the next inside a multi-step launch
+    const double2 *pos_cur;
+    double2 *pos_next;
+    long long step;     // step number of THIS force evaluation (stamped on springs that break in it)
 };
 
 struct StepParams {
@@ -176,7 +183,7 @@ template <bool EXACT> __device__ __forceinline__ bool spring_eval(double dx, dou
 // the next step fused behind it (the half-step velocity is what is stored between kernels); !ADVANCE: store the
 // completed state (v, f, fd).  SAMPLE: write per-particle energy terms and f for the reductions.
 template <bool EXACT, bool KICK2, bool ADVANCE, bool SAMPLE>
-__device__ __forceinline__ void particle_update(const StepParams &P, long long p, double2 xp, double2 vh, uint8_t g,
+__device__ __forceinline__ void particle_update(const StepParams &P, const StepVar &V, long long p, double2 xp, double2 vh, uint8_t g,
                                                 double fx, double fy, double u) {
     if (g == kFree) {
         const double fdx = sub<EXACT>(fx, mul<EXACT>(P.gamma, vh.x));  // damping with the held velocity (Q7)
@@ -196,7 +203,7 @@ __device__ __forceinline__ void particle_update(const StepParams &P, long long p
             double2 w, xn;
             w.x = mad<EXACT>(P.hdt, ax, v.x); w.y = mad<EXACT>(P.hdt, ay, v.y);          // Eq. 5, first half
             xn.x = mad<EXACT>(P.dt, w.x, xp.x); xn.y = mad<EXACT>(P.dt, w.y, xp.y);      // Eq. 3
-            store_pos(P.pos_next + p, xn, P.l2);
+            store_pos(V.pos_next + p, xn, P.l2);
             store_stream(P.vel + p, w, P.l2);
         } else {
             P.vel[p] = v;
@@ -206,8 +213,8 @@ __device__ __forceinline__ void particle_update(const StepParams &P, long long p
         if (SAMPLE) { P.sU[p] = u; P.sKE[p] = 0.0; }
         if (SAMPLE || !ADVANCE) P.f[p] = make_double2(fx, fy);
         if (ADVANCE) {
-            const double ns = (double)(P.step + 1 - P.g.n0[g]);
-            store_pos(P.pos_next + p, make_double2(mad<EXACT>(ns, P.g.dux[g], vh.x), mad<EXACT>(ns, P.g.duy[g], vh.y)), P.l2);
+            const double ns = (double)(V.step + 1 - P.g.n0[g]);
+            store_pos(V.pos_next + p, make_double2(mad<EXACT>(ns, P.g.dux[g], vh.x), mad<EXACT>(ns, P.g.duy[g], vh.y)), P.l2);
         } else {
             P.fd[p] = make_double2(fx, fy);
         }
@@ -227,8 +234,6 @@ struct RowSrc {            // where one particle's row lives: pointers already o
     const uint32_t *thr;
     const uint8_t *typ;
     const double *kF, *r0F;
-    uint32_t tile_pos_s;      // shared-memory address of the staged positions of the tile's own 256 particles (STAGED only)
-    int p0;                   // first particle of the tile
     size_t e0;                // global entry index of slot 0 of this lane (for the cold paths)
 };
 
@@ -252,24 +257,12 @@ template <int PM> __device__ __forceinline__ void slot_params(const StepParams &
     else { k = R.kF[so]; r0 = R.r0F[so]; kr0 = k * r0; thr = R.thr[so]; }
 }
 
-#ifndef LSM_GATHER_SMEM
-#define LSM_GATHER_SMEM 0      // 1: neighbours inside the staged tile are read from shared memory; 0 (default): always ld.global.nc --
-                               // measured equal on config 3 (58.0 vs 56.6 us) and 17 % faster on the 4096^2 full lattice (275 vs 322 us)
-#endif
-// Position of neighbour j.  STAGED: one predicated pair of loads (shared if j is one of the tile's own 256 particles,
-// else global through the read-only path) -- no branch, so the gathers of a chunk issue back to back.
-template <bool STAGED> __device__ __forceinline__ double2 gather_pos(const StepParams &P, const RowSrc &R, int j) {
-    if (STAGED && LSM_GATHER_SMEM) {
-        const unsigned rel = (unsigned)(j - R.p0);
-        double2 v;
-        asm("{\n\t.reg .pred q;\n\tsetp.lt.u32 q, %2, 256;\n\t"
-            "@q ld.shared.v2.f64 {%0, %1}, [%3];\n\t"
-            "@!q ld.global.nc.v2.f64 {%0, %1}, [%4];\n\t}"
-            : "=d"(v.x), "=d"(v.y)
-            : "r"(rel), "r"(R.tile_pos_s + rel * 16u), "l"(P.pos_cur + j));
-        return v;
-    }
-    return __ldg(P.pos_cur + j);
+// Position of neighbour j.  Always a global load (every position was just streamed in by some CTA, so these are
+// L1 / L2 hits); reading in-tile neighbours from the staged copy instead was measured equal on config 3 and 17 %
+// slower on full lattices (a per-slot branch).  COHERENT (multi-step launches): positions written by other CTAs
+// earlier in the same launch must not come from a stale L1 line -> ld.global.cg (L2 only).
+template <bool COHERENT> __device__ __forceinline__ double2 gather_pos(const StepVar &V, int j) {
+    return COHERENT ? __ldcg(V.pos_cur + j) : __ldg(V.pos_cur + j);
 }
 
 // One spring seen from one endpoint (Eq. 2): d = x_other - x_self, g = k (r - r0) / r.
@@ -300,8 +293,8 @@ __device__ __forceinline__ void slot_eval(double2 xq, double2 xp, bool valid, bo
     near = live && hi >= thr;
 }
 
-template <int PM, bool EXACT, bool SAMPLE, bool STAGED, int CH>
-__device__ __forceinline__ bool row_chunk(const StepParams &P, const RowSrc &R, const double *s_tab, int p, unsigned s0,
+template <int PM, bool EXACT, bool SAMPLE, bool COHERENT, int CH>
+__device__ __forceinline__ bool row_chunk(const StepParams &P, const StepVar &V, const RowSrc &R, const double *s_tab, int p, unsigned s0,
                                           double2 xp, double &fx, double &fy, double &u) {
     int nb[CH];
     double2 xq[CH];
@@ -309,7 +302,7 @@ __device__ __forceinline__ bool row_chunk(const StepParams &P, const RowSrc &R, 
 #pragma unroll
     for (int c = 0; c < CH; ++c) nb[c] = R.nbr[(s0 + c) * kSlice];
 #pragma unroll
-    for (int c = 0; c < CH; ++c) xq[c] = gather_pos<STAGED>(P, R, nb[c] >= 0 ? nb[c] : p);  // padding / dead: own position
+    for (int c = 0; c < CH; ++c) xq[c] = gather_pos<COHERENT>(V, nb[c] >= 0 ? nb[c] : p);  // padding / dead: own position
 #pragma unroll
     for (int c = 0; c < CH; ++c) {
         double k, r0, kr0, dx, dy, r2, g, ue;
@@ -325,15 +318,15 @@ __device__ __forceinline__ bool row_chunk(const StepParams &P, const RowSrc &R, 
     return any_near;
 }
 
-template <int PM, bool EXACT, bool SAMPLE, bool STAGED>
-__device__ __forceinline__ void row_careful(const StepParams &P, const RowSrc &R, const double *s_tab, int p, unsigned w,
+template <int PM, bool EXACT, bool SAMPLE, bool COHERENT>
+__device__ __forceinline__ void row_careful(const StepParams &P, const StepVar &V, const RowSrc &R, const double *s_tab, int p, unsigned w,
                                          double2 xp, double &fx, double &fy, double &u) {
     fx = 0.0; fy = 0.0; u = 0.0;
 #pragma unroll 1
     for (unsigned s = 0; s < w; ++s) {
         const unsigned so = s * kSlice;
         const int nb = R.nbr[so];
-        const double2 xq = gather_pos<STAGED>(P, R, nb >= 0 ? nb : p);
+        const double2 xq = gather_pos<COHERENT>(V, nb >= 0 ? nb : p);
         double k, r0, kr0, dx, dy, r2, g, ue;
         uint32_t thr;
         bool near;
@@ -348,7 +341,7 @@ __device__ __forceinline__ void row_careful(const StepParams &P, const RowSrc &R
             if (__dsqrt_rn(r2) > rc) {   // strict '>' (Q1)
                 P.nbr[e] = ~nb;
                 if (p < nb) {
-                    P.break_step[P.sid[e]] = P.step;
+                    P.break_step[P.sid[e]] = V.step;
                     atomicAdd(P.nbroken + spec_of(P.poff, P.B, p), 1ULL);
                 }
                 continue;
@@ -360,15 +353,15 @@ __device__ __forceinline__ void row_careful(const StepParams &P, const RowSrc &R
     }
 }
 
-template <int PM, bool EXACT, bool SAMPLE, bool STAGED>
-__device__ __forceinline__ void row_forces(const StepParams &P, const RowSrc &R, const double *s_tab, int p, unsigned w,
+template <int PM, bool EXACT, bool SAMPLE, bool COHERENT>
+__device__ __forceinline__ void row_forces(const StepParams &P, const StepVar &V, const RowSrc &R, const double *s_tab, int p, unsigned w,
                                            double2 xp, double &fx, double &fy, double &u) {
     constexpr int CH = LSM_ROW_CH;
     unsigned s0 = 0;
     bool any_near = false;
-    for (; s0 + CH <= w; s0 += CH) any_near |= row_chunk<PM, EXACT, SAMPLE, STAGED, CH>(P, R, s_tab, p, s0, xp, fx, fy, u);
-    for (; s0 < w; ++s0) any_near |= row_chunk<PM, EXACT, SAMPLE, STAGED, 1>(P, R, s_tab, p, s0, xp, fx, fy, u);
-    if (any_near) row_careful<PM, EXACT, SAMPLE, STAGED>(P, R, s_tab, p, w, xp, fx, fy, u);
+    for (; s0 + CH <= w; s0 += CH) any_near |= row_chunk<PM, EXACT, SAMPLE, COHERENT, CH>(P, V, R, s_tab, p, s0, xp, fx, fy, u);
+    for (; s0 < w; ++s0) any_near |= row_chunk<PM, EXACT, SAMPLE, COHERENT, 1>(P, V, R, s_tab, p, s0, xp, fx, fy, u);
+    if (any_near) row_careful<PM, EXACT, SAMPLE, COHERENT>(P, V, R, s_tab, p, w, xp, fx, fy, u);
 }
 
 // Direct variant: block = tile, every stream read from global memory by the thread that needs it.
@@ -391,10 +384,11 @@ __global__ void __launch_bounds__(kBlock) k_gather_step(const StepParams P) {
     const uint8_t g = P.grp[p];
     RowSrc R;
     R.nbr = P.nbr + e0; R.thr = P.sp.thr + e0; R.typ = P.sp.typ + e0; R.kF = P.sp.kF + e0; R.r0F = P.sp.r0F + e0;
-    R.tile_pos_s = 0; R.p0 = 0; R.e0 = e0;
+    R.e0 = e0;
     double fx = 0.0, fy = 0.0, u = 0.0;
-    row_forces<PM, EXACT, SAMPLE, false>(P, R, s_tab, (int)p, w, xp, fx, fy, u);
-    particle_update<EXACT, KICK2, ADVANCE, SAMPLE>(P, p, xp, vh, g, fx, fy, u);
+    const StepVar V{P.pos_cur, P.pos_next, P.step};
+    row_forces<PM, EXACT, SAMPLE, false>(P, V, R, s_tab, (int)p, w, xp, fx, fy, u);
+    particle_update<EXACT, KICK2, ADVANCE, SAMPLE>(P, V, p, xp, vh, g, fx, fy, u);
 }
 
 // ---- mbarrier / bulk-copy primitives (PTX; sm_90+ async proxy: the copy engine moves the bytes, no registers) ----
@@ -436,9 +430,22 @@ struct StageLayout {      // byte offsets of the staged arrays inside one pipeli
 // producer: one lane arms the stage's mbarrier with the byte count and issues one bulk async copy per array
 // (own x, own v, group bytes, tile header, neighbour ids, parameters); warps 0..7 are the consumers (one thread per
 // particle).  The bytes in flight per SM are (stages - 1) x stage size x CTAs/SM, independent of registers and
-// occupancy; the only latency the consumers see is the neighbour-position gather (L2 / L1 hits, or the staged tile).
-template <int PM, bool EXACT, bool KICK2, bool ADVANCE, bool SAMPLE>
-__global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const StepParams P, const StageLayout L) {
+// occupancy; the only latency the consumers see is the neighbour-position gather (L1 / L2 hits).
+//
+// MULTI: the launch advances M.nsteps time steps (cooperative launch, all CTAs resident).  Between two steps every
+// CTA passes a grid barrier: its consumer warps publish their stores (__threadfence) and arrive on a CTA-local
+// mbarrier; the producer lane waits for it, arrives on a global counter, spins until all CTAs of this step have
+// arrived, orders the generic-proxy writes before its next bulk copies (fence.proxy.async) and refills the pipeline
+// from the swapped position buffers.  Small (L2-resident, launch-bound) problems step ~2x faster this way.
+struct MultiParams {
+    int nsteps;                       // time steps in this launch (1 when !MULTI)
+    unsigned long long *gbar;         // global arrival counter (monotonic across launches)
+    unsigned long long gbar_base;     // its value before this launch
+    double2 *pos_a, *pos_b;           // step i reads pos_a / writes pos_b when i is even, the reverse when odd
+};
+
+template <int PM, bool EXACT, bool KICK2, bool ADVANCE, bool SAMPLE, bool MULTI>
+__global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const StepParams P, const StageLayout L, const MultiParams M) {
     constexpr bool kTab = (PM == PM_TYPED || PM == PM_KRT_RCF);
     constexpr bool kHasThr = (PM == PM_RCF || PM == PM_KRT_RCF || PM == PM_FULL);
     constexpr bool kHasTyp = kTab;
@@ -446,98 +453,122 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
     extern __shared__ __align__(128) unsigned char smem[];
     uint64_t *full = reinterpret_cast<uint64_t *>(smem);          // [kMaxStages]
     uint64_t *empty = full + kMaxStages;                            // [kMaxStages]
-    double *s_tab = reinterpret_cast<double *>(smem + 128);         // [4*kMaxTypes] when kTab
+    uint64_t *stepdone = empty + kMaxStages;                        // MULTI: all consumer warps of this CTA finished the step
+    double *s_tab = reinterpret_cast<double *>(smem + kStreamHdrBytes);         // [4*kMaxTypes] when kTab
     unsigned char *stage0 = smem + L.first;
     const int tid = threadIdx.x, wi = tid >> 5, lane = tid & 31;
     if (tid == 0) {
         for (int s = 0; s < L.stages; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, kTileSlices); }
+        if (MULTI) mbar_init(stepdone, kTileSlices);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (kTab) for (int i = tid; i < 4 * P.sp.ntypes; i += kTile + 32) s_tab[i] = P.sp.tab[i];
     __syncthreads();
+    const int nsteps = MULTI ? M.nsteps : 1;
 
     if (wi == kTileSlices) {  // ---------------- producer warp ----------------
         if (lane == 0) {
             int s = 0; unsigned u = 0;
             const uint64_t pol_keep = l2_policy_evict_last(), pol_stream = l2_policy_evict_first();
-            uint32_t o0n = 0, o8n = 0;
-            if ((long long)blockIdx.x < P.T) { o0n = __ldg(&P.hdr[blockIdx.x].off[0]); o8n = __ldg(&P.hdr[blockIdx.x].off[kTileSlices]); }
-            for (long long t = blockIdx.x; t < P.T; t += gridDim.x) {
-                const TileHdr *h = P.hdr + t;
-                const uint32_t o0 = o0n, ns = o8n - o0n;
-                if (t + gridDim.x < P.T) { o0n = __ldg(&h[gridDim.x].off[0]); o8n = __ldg(&h[gridDim.x].off[kTileSlices]); }  // next tile's extent, ahead of the wait
-                if (u > 0) mbar_wait(empty + s, (u - 1) & 1);
-                unsigned bytes = 2 * kTile * 16 + kTile + 64 + ns * (kSlice * 4);
-                if (kHasThr) bytes += ns * (kSlice * 4);
-                if (kHasTyp) bytes += ns * kSlice;
-                if (kHasKR) bytes += 2 * ns * (kSlice * 8);
-                unsigned char *b = stage0 + (size_t)s * L.bytes;
-                mbar_expect_tx(full + s, bytes);
-                if (P.l2 & 1) bulk_g2s_hint(b + L.pos, P.pos_cur + t * kTile, kTile * 16, full + s, pol_keep);
-                else bulk_g2s(b + L.pos, P.pos_cur + t * kTile, kTile * 16, full + s);
-                if (P.l2 & 2) {
-                    bulk_g2s_hint(b + L.vel, P.vel + t * kTile, kTile * 16, full + s, pol_stream);
-                    bulk_g2s_hint(b + L.grp, P.grp + t * kTile, kTile, full + s, pol_stream);
-                    bulk_g2s_hint(b + L.hdr, h, 64, full + s, pol_stream);
-                } else {
-                    bulk_g2s(b + L.vel, P.vel + t * kTile, kTile * 16, full + s);
-                    bulk_g2s(b + L.grp, P.grp + t * kTile, kTile, full + s);
-                    bulk_g2s(b + L.hdr, h, 64, full + s);
+            for (int it = 0; it < nsteps; ++it) {
+                const double2 *pos_cur = MULTI ? ((it & 1) ? M.pos_b : M.pos_a) : P.pos_cur;
+                if (MULTI && it > 0) {  // grid barrier: every CTA has finished (and published) step it-1
+                    mbar_wait(stepdone, (it - 1) & 1);
+                    __threadfence();
+                    atomicAdd(M.gbar, 1ULL);
+                    const unsigned long long target = M.gbar_base + (unsigned long long)it * gridDim.x;
+                    while (*reinterpret_cast<volatile unsigned long long *>(M.gbar) < target) { }
+                    __threadfence();
+                    asm volatile("fence.proxy.async;" ::: "memory");
                 }
-                if (ns) {
-                    const size_t e = (size_t)o0 * kSlice;
+                uint32_t o0n = 0, o8n = 0;
+                if ((long long)blockIdx.x < P.T) { o0n = __ldg(&P.hdr[blockIdx.x].off[0]); o8n = __ldg(&P.hdr[blockIdx.x].off[kTileSlices]); }
+                for (long long t = blockIdx.x; t < P.T; t += gridDim.x) {
+                    const TileHdr *h = P.hdr + t;
+                    const uint32_t o0 = o0n, ns = o8n - o0n;
+                    if (t + gridDim.x < P.T) { o0n = __ldg(&h[gridDim.x].off[0]); o8n = __ldg(&h[gridDim.x].off[kTileSlices]); }  // next tile's extent, ahead of the wait
+                    if (u > 0) mbar_wait(empty + s, (u - 1) & 1);
+                    unsigned bytes = 2 * kTile * 16 + kTile + 64 + ns * (kSlice * 4);
+                    if (kHasThr) bytes += ns * (kSlice * 4);
+                    if (kHasTyp) bytes += ns * kSlice;
+                    if (kHasKR) bytes += 2 * ns * (kSlice * 8);
+                    unsigned char *b = stage0 + (size_t)s * L.bytes;
+                    mbar_expect_tx(full + s, bytes);
+                    if (P.l2 & 1) bulk_g2s_hint(b + L.pos, pos_cur + t * kTile, kTile * 16, full + s, pol_keep);
+                    else bulk_g2s(b + L.pos, pos_cur + t * kTile, kTile * 16, full + s);
                     if (P.l2 & 2) {
-                        bulk_g2s_hint(b + L.nbr, P.nbr + e, ns * (kSlice * 4), full + s, pol_stream);
-                        if (kHasThr) bulk_g2s_hint(b + L.thr, P.sp.thr + e, ns * (kSlice * 4), full + s, pol_stream);
-                        if (kHasTyp) bulk_g2s_hint(b + L.typ, P.sp.typ + e, ns * kSlice, full + s, pol_stream);
-                        if (kHasKR) {
-                            bulk_g2s_hint(b + L.kF, P.sp.kF + e, ns * (kSlice * 8), full + s, pol_stream);
-                            bulk_g2s_hint(b + L.r0F, P.sp.r0F + e, ns * (kSlice * 8), full + s, pol_stream);
-                        }
+                        bulk_g2s_hint(b + L.vel, P.vel + t * kTile, kTile * 16, full + s, pol_stream);
+                        bulk_g2s_hint(b + L.grp, P.grp + t * kTile, kTile, full + s, pol_stream);
+                        bulk_g2s_hint(b + L.hdr, h, 64, full + s, pol_stream);
                     } else {
-                        bulk_g2s(b + L.nbr, P.nbr + e, ns * (kSlice * 4), full + s);
-                        if (kHasThr) bulk_g2s(b + L.thr, P.sp.thr + e, ns * (kSlice * 4), full + s);
-                        if (kHasTyp) bulk_g2s(b + L.typ, P.sp.typ + e, ns * kSlice, full + s);
-                        if (kHasKR) {
-                            bulk_g2s(b + L.kF, P.sp.kF + e, ns * (kSlice * 8), full + s);
-                            bulk_g2s(b + L.r0F, P.sp.r0F + e, ns * (kSlice * 8), full + s);
+                        bulk_g2s(b + L.vel, P.vel + t * kTile, kTile * 16, full + s);
+                        bulk_g2s(b + L.grp, P.grp + t * kTile, kTile, full + s);
+                        bulk_g2s(b + L.hdr, h, 64, full + s);
+                    }
+                    if (ns) {
+                        const size_t e = (size_t)o0 * kSlice;
+                        if (P.l2 & 2) {
+                            bulk_g2s_hint(b + L.nbr, P.nbr + e, ns * (kSlice * 4), full + s, pol_stream);
+                            if (kHasThr) bulk_g2s_hint(b + L.thr, P.sp.thr + e, ns * (kSlice * 4), full + s, pol_stream);
+                            if (kHasTyp) bulk_g2s_hint(b + L.typ, P.sp.typ + e, ns * kSlice, full + s, pol_stream);
+                            if (kHasKR) {
+                                bulk_g2s_hint(b + L.kF, P.sp.kF + e, ns * (kSlice * 8), full + s, pol_stream);
+                                bulk_g2s_hint(b + L.r0F, P.sp.r0F + e, ns * (kSlice * 8), full + s, pol_stream);
+                            }
+                        } else {
+                            bulk_g2s(b + L.nbr, P.nbr + e, ns * (kSlice * 4), full + s);
+                            if (kHasThr) bulk_g2s(b + L.thr, P.sp.thr + e, ns * (kSlice * 4), full + s);
+                            if (kHasTyp) bulk_g2s(b + L.typ, P.sp.typ + e, ns * kSlice, full + s);
+                            if (kHasKR) {
+                                bulk_g2s(b + L.kF, P.sp.kF + e, ns * (kSlice * 8), full + s);
+                                bulk_g2s(b + L.r0F, P.sp.r0F + e, ns * (kSlice * 8), full + s);
+                            }
                         }
                     }
+                    if (++s == L.stages) { s = 0; ++u; }
                 }
-                if (++s == L.stages) { s = 0; ++u; }
             }
         }
         return;
     }
     // ---------------- consumer warps: thread = particle ----------------
     int s = 0; unsigned u = 0;
-    for (long long t = blockIdx.x; t < P.T; t += gridDim.x) {
-        mbar_wait(full + s, u & 1);
-        const unsigned char *b = stage0 + (size_t)s * L.bytes;
-        const TileHdr *h = reinterpret_cast<const TileHdr *>(b + L.hdr);
-        const long long p = t * kTile + tid;
-        if (p < P.N) {
-            const unsigned w = h->w[wi];
-            const unsigned rel = (h->off[wi] - h->off[0]) * kSlice + lane;
-            const double2 xp = reinterpret_cast<const double2 *>(b + L.pos)[tid];
-            RowSrc R;
-            R.nbr = reinterpret_cast<const int32_t *>(b + L.nbr) + rel;
-            R.thr = reinterpret_cast<const uint32_t *>(b + L.thr) + rel;
-            R.typ = (b + L.typ) + rel;
-            R.kF = reinterpret_cast<const double *>(b + L.kF) + rel;
-            R.r0F = reinterpret_cast<const double *>(b + L.r0F) + rel;
-            R.tile_pos_s = smem_u32(b + L.pos);
-            R.p0 = (int)(t * kTile);
-            R.e0 = (size_t)h->off[wi] * kSlice + lane;
-            double fx = 0.0, fy = 0.0, uu = 0.0;
-            row_forces<PM, EXACT, SAMPLE, true>(P, R, s_tab, (int)p, w, xp, fx, fy, uu);
-            const double2 vh = reinterpret_cast<const double2 *>(b + L.vel)[tid];
-            const uint8_t g = (b + L.grp)[tid];
-            particle_update<EXACT, KICK2, ADVANCE, SAMPLE>(P, p, xp, vh, g, fx, fy, uu);
+    for (int it = 0; it < nsteps; ++it) {
+        StepVar V;
+        V.pos_cur = MULTI ? ((it & 1) ? M.pos_b : M.pos_a) : P.pos_cur;
+        V.pos_next = MULTI ? ((it & 1) ? M.pos_a : M.pos_b) : P.pos_next;
+        V.step = P.step + it;
+        for (long long t = blockIdx.x; t < P.T; t += gridDim.x) {
+            mbar_wait(full + s, u & 1);
+            const unsigned char *b = stage0 + (size_t)s * L.bytes;
+            const TileHdr *h = reinterpret_cast<const TileHdr *>(b + L.hdr);
+            const long long p = t * kTile + tid;
+            if (p < P.N) {
+                const unsigned w = h->w[wi];
+                const unsigned rel = (h->off[wi] - h->off[0]) * kSlice + lane;
+                const double2 xp = reinterpret_cast<const double2 *>(b + L.pos)[tid];
+                RowSrc R;
+                R.nbr = reinterpret_cast<const int32_t *>(b + L.nbr) + rel;
+                R.thr = reinterpret_cast<const uint32_t *>(b + L.thr) + rel;
+                R.typ = (b + L.typ) + rel;
+                R.kF = reinterpret_cast<const double *>(b + L.kF) + rel;
+                R.r0F = reinterpret_cast<const double *>(b + L.r0F) + rel;
+                R.e0 = (size_t)h->off[wi] * kSlice + lane;
+                double fx = 0.0, fy = 0.0, uu = 0.0;
+                row_forces<PM, EXACT, SAMPLE, MULTI>(P, V, R, s_tab, (int)p, w, xp, fx, fy, uu);
+                const double2 vh = reinterpret_cast<const double2 *>(b + L.vel)[tid];
+                const uint8_t g = (b + L.grp)[tid];
+                particle_update<EXACT, KICK2, ADVANCE, SAMPLE>(P, V, p, xp, vh, g, fx, fy, uu);
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty + s);
+            if (++s == L.stages) { s = 0; ++u; }
         }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(empty + s);
-        if (++s == L.stages) { s = 0; ++u; }
+        if (MULTI && it + 1 < nsteps) {  // publish this step's stores, then tell the producer this warp is done
+            __threadfence();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(stepdone);
+        }
     }
 }
 
@@ -621,7 +652,7 @@ __global__ void __launch_bounds__(kBlock) k_integrate(const StepParams P) {
     const uint8_t g = P.grp[p];
     const double2 f = P.f[p];
     // in-place variant: pos_next == pos_cur for this path
-    particle_update<false, KICK2, ADVANCE, SAMPLE>(P, p, xp, vh, g, f.x, f.y, 0.0);
+    particle_update<false, KICK2, ADVANCE, SAMPLE>(P, StepVar{P.pos_cur, P.pos_next, P.step}, p, xp, vh, g, f.x, f.y, 0.0);
     if (ADVANCE && !SAMPLE) P.f[p] = make_double2(0.0, 0.0);
 }
 
