@@ -12,7 +12,7 @@ pytestmark = pytest.mark.gpu
 
 import paper_2201_04565_b200 as lsm
 from paper_2201_04565_b200.binding import lsm_create_from_problem
-from lsm_inputs import (FIXED, MOVE, config1, config2, config3, config4, single_specimen, shuffle_ids,
+from lsm_inputs import (FIXED, MOVE, config1, config2, config3, config4, config5, single_specimen, shuffle_ids,
                         triangular_lattice)
 from oracle.olsm import OracleSim
 from parity import check_forces, conditioning_floor, force_scale
@@ -375,4 +375,88 @@ def test_full_size_config3_bench_configuration():
     sc = force_scale(xo, p.spring_i, p.spring_j, p.k, p.r0, ~bo)
     check_forces(fg, fo, sc, floor=conditioning_floor(xo, p.spring_i, p.spring_j, p.k, ~bo))
     assert np.abs(fg.sum(axis=0)).max() <= 1e-9 * np.abs(fg).sum()
+    g.close()
+
+
+# ---------------------------------------------------------------- kernel variants agree (direct / streamed / fused)
+def test_gather_variants_and_step_fusion_bit_identical_in_exact_mode():
+    """The direct kernel, the streamed (bulk-copy pipeline) kernel and the fused multi-step launch run the same row
+    arithmetic in the same order: in exact mode all three must reproduce the oracle bit for bit through a fracture
+    run, sample history included up to reduction order."""
+    p = _fracture_problem(n=48, du_y=6e-4, seed=11)
+    p.sample_every = 50
+    nsteps = 4000
+    o = OracleSim.from_problem(p); o.step(nsteps)
+    xo, vo = o.read_state(); bo, bso, nbo = o.read_broken()
+    assert nbo > 0
+    ho = o.read_stress()
+    for kw in (dict(gather_variant=lsm.GATHER_DIRECT), dict(gather_variant=lsm.GATHER_STREAMED, step_fusion=lsm.FUSION_OFF),
+               dict(gather_variant=lsm.GATHER_STREAMED, step_fusion=lsm.FUSION_ON)):
+        g = lsm_create_from_problem(p, exact=True, **kw)
+        inf = g.info()
+        assert inf["step_fusion"] == (1 if kw.get("step_fusion") == lsm.FUSION_ON else 0)
+        g.step(1700); g.step(1); g.step(nsteps - 1701)        # odd / even run lengths, a 1-step call
+        xg, vg = g.read_state(); bg, bsg, nbg = g.read_broken()
+        assert np.array_equal(xo, xg) and np.array_equal(vo, vg)
+        assert nbg == nbo and np.array_equal(bo, bg) and np.array_equal(bso, bsg)
+        hg = g.read_stress()
+        assert np.array_equal(ho["step"], hg["step"]) and np.array_equal(ho["n_broken"], hg["n_broken"])
+        assert np.allclose(hg["U"], ho["U"], rtol=1e-12) and np.allclose(hg["R"], ho["R"], rtol=1e-10, atol=1e-14)
+        if kw.get("step_fusion") == lsm.FUSION_ON:
+            assert inf["kernels_launched"] < g.info()["kernels_launched"] < 1000   # ~80 sample segments, not 4000 launches
+        g.close()
+
+
+def test_step_fusion_fast_mode_config1():
+    """Fused launches (the default for N <= 2^18) against one launch per step, fast arithmetic: same kernels, same
+    order -> identical results; and both within 1e-9 of the oracle after 10^4 steps (T2)."""
+    p = config1()
+    a = lsm_create_from_problem(p, step_fusion=lsm.FUSION_ON); a.step(3000)
+    b = lsm_create_from_problem(p, step_fusion=lsm.FUSION_OFF); b.step(3000)
+    xa, va = a.read_state(); xb, vb = b.read_state()
+    assert np.array_equal(xa, xb) and np.array_equal(va, vb)
+    assert a.info()["kernels_launched"] < 300 < b.info()["kernels_launched"]
+    a.close(); b.close()
+
+
+# ---------------------------------------------------------------- full-size checks of the other configurations
+def test_full_size_config4_sampled_specimens():
+    """BASELINE.json configs[3] at full size (1024 specimens, one launch): specimens sampled at random are compared
+    with the oracle stepping each of them alone (T8 at full size)."""
+    B, nsteps = 1024, 300
+    pb = config4(B=B)
+    pb.sample_every = 100
+    g = lsm_create_from_problem(pb)
+    assert g.info()["n_batch"] == B and g.info()["param_mode"] == 1
+    g.step(nsteps)
+    xg, vg = g.read_state(); hg = g.read_stress()
+    assert hg["U"].shape == (3, B)
+    po = pb.particle_offsets
+    for b in np.random.default_rng(4).choice(B, 4, replace=False):
+        ps = single_specimen(int(b)); ps.sample_every = 100
+        o = OracleSim.from_problem(ps); o.step(nsteps)
+        xo, vo = o.read_state(); ho = o.read_stress()
+        sl = slice(po[b], po[b + 1])
+        assert np.abs(xg[sl] - xo).max() <= 1e-11 and np.abs(vg[sl] - vo).max() <= 1e-11
+        assert np.allclose(hg["U"][:, b], ho["U"][:, 0], rtol=1e-10) and np.allclose(hg["KE"][:, b], ho["KE"][:, 0], rtol=1e-10)
+        assert np.allclose(hg["R"][:, b], ho["R"][:, 0], rtol=1e-9, atol=1e-13)
+    g.close()
+
+
+@pytest.mark.parametrize("n", [4096, 8192])
+def test_large_config5_first_steps(n):
+    """BASELINE.json configs[4] (notched, pre-strained lattice; here n x n with the same recipe): the first steps against
+    the oracle on every particle, plus the force evaluation at step 0 (uniform parameters: 4 bytes per half-edge)."""
+    p = config5(n=n)
+    o = OracleSim.from_problem(p)
+    g = lsm_create_from_problem(p)
+    assert g.info()["param_mode"] == 0 and g.info()["bytes_per_half_edge"] == 4
+    fo, fg = o.read_forces(), g.read_forces()
+    sc = force_scale(p.x, p.spring_i, p.spring_j, p.k, p.r0)
+    check_forces(fg, fo, sc, floor=conditioning_floor(p.x, p.spring_i, p.spring_j, p.k))
+    o.step(5); g.step(5)
+    xo, vo = o.read_state(); xg, vg = g.read_state()
+    eps = np.finfo(np.float64).eps
+    assert np.abs(xg - xo).max() <= 32 * eps * np.abs(xo).max() and np.abs(vg - vo).max() <= 1e-12
+    assert g.n_broken() == o.read_broken()[2] == 0
     g.close()
