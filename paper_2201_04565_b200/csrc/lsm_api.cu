@@ -354,7 +354,7 @@ void launch_reduce(lsm_sim *s, long long step, long long slot) {
         R.out_U = s->cur_U; R.out_KE = s->cur_KE;
     }
     k_reduce_chunks<<<(unsigned)s->nchunks, kBlock, 0, s->stream>>>(R);
-    k_finalize_sample<<<(unsigned)((s->B + 3) / 4), 128, 0, s->stream>>>(R);
+    k_finalize_sample<<<(unsigned)s->B, kBlock, 0, s->stream>>>(R);
     s->kernels_launched += 2;
 }
 

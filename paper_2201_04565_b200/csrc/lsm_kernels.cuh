@@ -708,15 +708,27 @@ __device__ __forceinline__ double warp_sum(double v) {
     return v;
 }
 
-__global__ void __launch_bounds__(128) k_finalize_sample(const ReduceParams R) {
-    const int b = blockIdx.x * 4 + (threadIdx.x >> 5);
-    const int lane = threadIdx.x & 31;
-    if (b >= R.B) return;
+// Fixed-order block sum (256 threads): shuffle tree inside each warp, then the 8 warp sums in warp order.
+__device__ __forceinline__ double block_sum(double v, double *sh8) {
+    v = warp_sum(v);
+    __syncthreads();
+    if ((threadIdx.x & 31) == 0) sh8[threadIdx.x >> 5] = v;
+    __syncthreads();
+    double t = 0.0;
+#pragma unroll
+    for (int w = 0; w < kBlock / 32; ++w) t += sh8[w];
+    return t;
+}
+
+// One block per specimen: sums its chunk partials and its boundary groups' spring forces in a fixed order.
+__global__ void __launch_bounds__(kBlock) k_finalize_sample(const ReduceParams R) {
+    __shared__ double sh8[kBlock / 32];
+    const int b = blockIdx.x;
     double u = 0.0, ke = 0.0;
-    for (int c = R.spec_chunk_off[b] + lane; c < R.spec_chunk_off[b + 1]; c += 32) { u += R.part[2 * c]; ke += R.part[2 * c + 1]; }
-    if (R.sUs) for (long long e = R.soff_list[b] + lane; e < R.soff_list[b + 1]; e += 32) u += R.sUs[e];
-    u = warp_sum(u); ke = warp_sum(ke);
-    if (lane == 0) {
+    for (int c = R.spec_chunk_off[b] + threadIdx.x; c < R.spec_chunk_off[b + 1]; c += kBlock) { u += R.part[2 * c]; ke += R.part[2 * c + 1]; }
+    if (R.sUs) for (long long e = R.soff_list[b] + threadIdx.x; e < R.soff_list[b + 1]; e += kBlock) u += R.sUs[e];
+    u = block_sum(u, sh8); ke = block_sum(ke, sh8);
+    if (threadIdx.x == 0) {
         R.out_U[b] = u; R.out_KE[b] = ke;
         if (R.out_nb) R.out_nb[b] = (long long)R.nbroken[b];
         if (!isfinite(u + ke)) atomicOr(R.flags, 1);
@@ -725,14 +737,14 @@ __global__ void __launch_bounds__(128) k_finalize_sample(const ReduceParams R) {
     if (R.out_R) {
         for (int g = 0; g < kMaxGroups; ++g) {
             double rx = 0.0, ry = 0.0;
-            if (R.gids[g]) {
-                for (long long q = R.gseg[g][b] + lane; q < R.gseg[g][b + 1]; q += 32) {
+            if (R.gids[g]) {   // block-uniform
+                for (long long q = R.gseg[g][b] + threadIdx.x; q < R.gseg[g][b + 1]; q += kBlock) {
                     const double2 f = R.f[R.gids[g][q]];
                     rx += f.x; ry += f.y;
                 }
+                rx = block_sum(rx, sh8); ry = block_sum(ry, sh8);
             }
-            rx = warp_sum(rx); ry = warp_sum(ry);
-            if (lane == 0) { R.out_R[((size_t)b * kMaxGroups + g) * 2] = rx; R.out_R[((size_t)b * kMaxGroups + g) * 2 + 1] = ry; }
+            if (threadIdx.x == 0) { R.out_R[((size_t)b * kMaxGroups + g) * 2] = rx; R.out_R[((size_t)b * kMaxGroups + g) * 2 + 1] = ry; }
         }
     }
 }
