@@ -639,7 +639,9 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
         for (long long t = 0; t < T; ++t) s->max_tile_slots = std::max(s->max_tile_slots, hh[t].off[kTileSlices] - hh[t].off[0]);
         const size_t E = (size_t)off[T * kTileSlices] * kSlice;
         s->E = (long long)E;
-        std::vector<int32_t> hn(E, kPad), hs(E, -1);
+        std::vector<int32_t> hn(E), hs(E, -1);
+        for (long long sl = 0; sl < T * kTileSlices; ++sl)       // padding slots point at their own particle
+            for (size_t e = (size_t)off[sl] * kSlice; e < (size_t)off[sl + 1] * kSlice; ++e) hn[e] = (int32_t)(sl * kSlice + (e & 31));
         std::vector<uint8_t> cnt(N, 0);
         auto slot = [&](int32_t p) { const size_t e = ((size_t)off[p >> 5] + cnt[p]) * kSlice + (p & 31); cnt[p]++; return e; };
         for (long long e = 0; e < M; ++e) {  // caller order -> every row is ascending in caller spring id
@@ -890,6 +892,7 @@ lsm_status lsm_step(lsm_sim *s, int64_t n_steps) {
                     MultiParams Mp;
                     Mp.nsteps = (int)run; Mp.gbar = s->gbar; Mp.gbar_base = s->gbar_base;
                     Mp.pos_a = s->pos[s->cur]; Mp.pos_b = s->pos[s->cur ^ 1];
+                    Mp.resident = (s->T + s->stream_grid - 1) / s->stream_grid <= s->L.stages;
                     CUDA_TRY(s, s->exact ? launch_stream_multi_pm<true>(s, P, Mp) : launch_stream_multi_pm<false>(s, P, Mp));
                     s->gbar_base += (unsigned long long)(run - 1) * (unsigned long long)s->stream_grid;
                     s->kernels_launched += 1;

@@ -8,7 +8,8 @@
 //   gather layout (particle-centric, sliced ELL, slice = one warp = 32 consecutive particles, tile = 8 slices = 256
 //   particles = one CTA's unit of work):
 //     hdr[T] (64 B per tile: slot offset of each of its 8 slices + end, live width of each slice),
-//     nbr[E] int32 neighbour id (bitwise-NOT of the id once the spring is dead, INT32_MIN = padding),
+//     nbr[E] int32 neighbour id; a padding slot or a dead spring holds the particle's OWN id (a spring never joins a
+//     particle to itself): its gather is legal, gives r = 0 and therefore contributes nothing, with no validity test,
 //     sid[E] caller spring id (cold: read only when a spring breaks or sits within one fp32 ulp of rc),
 //     per-slot parameters by ParamMode: typ[E] uint8, thr[E] uint32 = (high word of rc*rc) - 1 (a conservative integer
 //     filter on r^2; anything above it is decided by the exact fp64 rcS[sid], so the decision is the fp64 one), kF/r0F[E].
@@ -184,7 +185,7 @@ template <bool EXACT> __device__ __forceinline__ bool spring_eval(double dx, dou
 // completed state (v, f, fd).  SAMPLE: write per-particle energy terms and f for the reductions.
 template <bool EXACT, bool KICK2, bool ADVANCE, bool SAMPLE>
 __device__ __forceinline__ void particle_update(const StepParams &P, const StepVar &V, long long p, double2 xp, double2 vh, uint8_t g,
-                                                double fx, double fy, double u) {
+                                                double fx, double fy, double u, double2 *own_pos = nullptr, double2 *own_vel = nullptr) {
     if (g == kFree) {
         const double fdx = sub<EXACT>(fx, mul<EXACT>(P.gamma, vh.x));  // damping with the held velocity (Q7)
         const double fdy = sub<EXACT>(fy, mul<EXACT>(P.gamma, vh.y));
@@ -201,10 +202,15 @@ __device__ __forceinline__ void particle_update(const StepParams &P, const StepV
         if (SAMPLE || !ADVANCE) P.f[p] = make_double2(fx, fy);
         if (ADVANCE) {
             double2 w, xn;
-            w.x = mad<EXACT>(P.hdt, ax, v.x); w.y = mad<EXACT>(P.hdt, ay, v.y);          // Eq. 5, first half
+            if (!EXACT && KICK2 && !SAMPLE) {   // fast mode: the two half kicks of consecutive steps in one FMA (2 hdt = dt)
+                w.x = fma(P.dt, ax, vh.x); w.y = fma(P.dt, ay, vh.y);
+            } else {
+                w.x = mad<EXACT>(P.hdt, ax, v.x); w.y = mad<EXACT>(P.hdt, ay, v.y);      // Eq. 5, first half
+            }
             xn.x = mad<EXACT>(P.dt, w.x, xp.x); xn.y = mad<EXACT>(P.dt, w.y, xp.y);      // Eq. 3
             store_pos(V.pos_next + p, xn, P.l2);
             store_stream(P.vel + p, w, P.l2);
+            if (own_pos) { *own_pos = xn; *own_vel = w; }   // resident tiles: the staged copy is the next step's input
         } else {
             P.vel[p] = v;
             P.fd[p] = make_double2(fdx, fdy);
@@ -214,7 +220,9 @@ __device__ __forceinline__ void particle_update(const StepParams &P, const StepV
         if (SAMPLE || !ADVANCE) P.f[p] = make_double2(fx, fy);
         if (ADVANCE) {
             const double ns = (double)(V.step + 1 - P.g.n0[g]);
-            store_pos(V.pos_next + p, make_double2(mad<EXACT>(ns, P.g.dux[g], vh.x), mad<EXACT>(ns, P.g.duy[g], vh.y)), P.l2);
+            const double2 xn = make_double2(mad<EXACT>(ns, P.g.dux[g], vh.x), mad<EXACT>(ns, P.g.duy[g], vh.y));
+            store_pos(V.pos_next + p, xn, P.l2);
+            if (own_pos) *own_pos = xn;
         } else {
             P.fd[p] = make_double2(fx, fy);
         }
@@ -266,10 +274,11 @@ template <bool COHERENT> __device__ __forceinline__ double2 gather_pos(const Ste
 }
 
 // One spring seen from one endpoint (Eq. 2): d = x_other - x_self, g = k (r - r0) / r.
-// live: the slot holds a spring with a direction (valid and r2 > 0; coincident endpoints give no force, Q4);
+// live: the slot holds a spring with a direction (r2 > 0: padding / dead slots gather the own position and coincident
+// endpoints give no force, Q4);
 // near: r2 reaches the breakage filter (see above).  Both endpoints compute bit-identical r2 ((-dx)^2 == dx^2).
 template <bool EXACT, bool SAMPLE>
-__device__ __forceinline__ void slot_eval(double2 xq, double2 xp, bool valid, bool lower, double k, double r0, double kr0, uint32_t thr,
+__device__ __forceinline__ void slot_eval(double2 xq, double2 xp, bool lower, double k, double r0, double kr0, uint32_t thr,
                                           double &dx, double &dy, double &r2, double &g, double &ue, bool &near) {
     dx = sub<EXACT>(xq.x, xp.x); dy = sub<EXACT>(xq.y, xp.y);
     r2 = EXACT ? add<true>(mul<true>(dx, dx), mul<true>(dy, dy)) : fma(dy, dy, dx * dx);
@@ -281,12 +290,12 @@ __device__ __forceinline__ void slot_eval(double2 xq, double2 xp, bool valid, bo
         const double ext = sub<true>(r, r0);
         g = __ddiv_rn(mul<true>(k, ext), r);
         if (SAMPLE) ue = mul<true>(mul<true>(mul<true>(0.5, k), ext), ext);
-        live = valid && r2 > 0.0;
+        live = r2 > 0.0;
     } else {
         const double rinv = rsqrt_fast(r2);
         g = fma(-kr0, rinv, k);              // k (r - r0) / r = k - k r0 / r
         if (SAMPLE) { const double ext = fma(r2, rinv, -r0); ue = (0.5 * k) * ext * ext; }
-        live = valid && hi >= 0x00100000u;   // r2 zero (or denormal: treated as coincident)
+        live = hi >= 0x00100000u;            // r2 zero (or denormal: treated as coincident)
     }
     g = live ? g : 0.0;
     if (SAMPLE) ue = (live && lower) ? ue : 0.0;  // energy counted once, by the lower endpoint (Eq. 1)
@@ -302,14 +311,14 @@ __device__ __forceinline__ bool row_chunk(const StepParams &P, const StepVar &V,
 #pragma unroll
     for (int c = 0; c < CH; ++c) nb[c] = R.nbr[(s0 + c) * kSlice];
 #pragma unroll
-    for (int c = 0; c < CH; ++c) xq[c] = gather_pos<COHERENT>(V, nb[c] >= 0 ? nb[c] : p);  // padding / dead: own position
+    for (int c = 0; c < CH; ++c) xq[c] = gather_pos<COHERENT>(V, nb[c]);
 #pragma unroll
     for (int c = 0; c < CH; ++c) {
         double k, r0, kr0, dx, dy, r2, g, ue;
         uint32_t thr;
         bool near;
         slot_params<PM>(P, R, s_tab, (s0 + c) * kSlice, k, r0, kr0, thr);
-        slot_eval<EXACT, SAMPLE>(xq[c], xp, nb[c] >= 0, p < nb[c], k, r0, kr0, thr, dx, dy, r2, g, ue, near);
+        slot_eval<EXACT, SAMPLE>(xq[c], xp, p < nb[c], k, r0, kr0, thr, dx, dy, r2, g, ue, near);
         fx = mad<EXACT>(g, dx, fx);
         fy = mad<EXACT>(g, dy, fy);
         if (SAMPLE) u = add<EXACT>(u, ue);
@@ -326,12 +335,12 @@ __device__ __forceinline__ void row_careful(const StepParams &P, const StepVar &
     for (unsigned s = 0; s < w; ++s) {
         const unsigned so = s * kSlice;
         const int nb = R.nbr[so];
-        const double2 xq = gather_pos<COHERENT>(V, nb >= 0 ? nb : p);
+        const double2 xq = gather_pos<COHERENT>(V, nb);
         double k, r0, kr0, dx, dy, r2, g, ue;
         uint32_t thr;
         bool near;
         slot_params<PM>(P, R, s_tab, so, k, r0, kr0, thr);
-        slot_eval<EXACT, SAMPLE>(xq, xp, nb >= 0, p < nb, k, r0, kr0, thr, dx, dy, r2, g, ue, near);
+        slot_eval<EXACT, SAMPLE>(xq, xp, p < nb, k, r0, kr0, thr, dx, dy, r2, g, ue, near);
         if (near) {
             const size_t e = R.e0 + so;
             double rc;
@@ -339,7 +348,8 @@ __device__ __forceinline__ void row_careful(const StepParams &P, const StepVar &
             else if (PM == PM_TYPED) rc = s_tab[4 * R.typ[so] + 2];
             else rc = __ldg(P.sp.rcS + __ldg(P.sid + e));
             if (__dsqrt_rn(r2) > rc) {   // strict '>' (Q1)
-                P.nbr[e] = ~nb;
+                P.nbr[e] = p;                             // dead from now on: the slot points at its own particle
+                const_cast<int32_t *>(R.nbr)[so] = p;     // and the staged copy (resident tiles are not reloaded)
                 if (p < nb) {
                     P.break_step[P.sid[e]] = V.step;
                     atomicAdd(P.nbroken + spec_of(P.poff, P.B, p), 1ULL);
@@ -441,6 +451,8 @@ struct MultiParams {
     int nsteps;                       // time steps in this launch (1 when !MULTI)
     unsigned long long *gbar;         // global arrival counter (monotonic across launches)
     unsigned long long gbar_base;     // its value before this launch
+    int resident;                     // 1: every CTA's tiles fit in its pipeline stages -> loaded once, kept in shared
+                                      //    memory for the whole launch (rows, own x and v); later steps copy nothing
     double2 *pos_a, *pos_b;           // step i reads pos_a / writes pos_b when i is even, the reverse when odd
 };
 
@@ -454,12 +466,13 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
     uint64_t *full = reinterpret_cast<uint64_t *>(smem);          // [kMaxStages]
     uint64_t *empty = full + kMaxStages;                            // [kMaxStages]
     uint64_t *stepdone = empty + kMaxStages;                        // MULTI: all consumer warps of this CTA finished the step
+    uint64_t *go = stepdone + 1;                                    // MULTI resident: the grid barrier has been passed
     double *s_tab = reinterpret_cast<double *>(smem + kStreamHdrBytes);         // [4*kMaxTypes] when kTab
     unsigned char *stage0 = smem + L.first;
     const int tid = threadIdx.x, wi = tid >> 5, lane = tid & 31;
     if (tid == 0) {
         for (int s = 0; s < L.stages; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, kTileSlices); }
-        if (MULTI) mbar_init(stepdone, kTileSlices);
+        if (MULTI) { mbar_init(stepdone, kTileSlices); mbar_init(go, 1); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (kTab) for (int i = tid; i < 4 * P.sp.ntypes; i += kTile + 32) s_tab[i] = P.sp.tab[i];
@@ -480,6 +493,7 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
                     while (*reinterpret_cast<volatile unsigned long long *>(M.gbar) < target) { }
                     __threadfence();
                     asm volatile("fence.proxy.async;" ::: "memory");
+                    if (M.resident) { mbar_arrive(go); continue; }   // nothing to copy: the consumers own the staged tiles
                 }
                 uint32_t o0n = 0, o8n = 0;
                 if ((long long)blockIdx.x < P.T) { o0n = __ldg(&P.hdr[blockIdx.x].off[0]); o8n = __ldg(&P.hdr[blockIdx.x].off[kTileSlices]); }
@@ -538,9 +552,11 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
         V.pos_cur = MULTI ? ((it & 1) ? M.pos_b : M.pos_a) : P.pos_cur;
         V.pos_next = MULTI ? ((it & 1) ? M.pos_a : M.pos_b) : P.pos_next;
         V.step = P.step + it;
+        const bool kept = MULTI && M.resident && it > 0;   // tiles already in shared memory (stage i = i-th tile of this CTA)
+        if (kept) { mbar_wait(go, (it - 1) & 1); s = 0; }
         for (long long t = blockIdx.x; t < P.T; t += gridDim.x) {
-            mbar_wait(full + s, u & 1);
-            const unsigned char *b = stage0 + (size_t)s * L.bytes;
+            if (!kept) mbar_wait(full + s, u & 1);
+            unsigned char *b = stage0 + (size_t)s * L.bytes;
             const TileHdr *h = reinterpret_cast<const TileHdr *>(b + L.hdr);
             const long long p = t * kTile + tid;
             if (p < P.N) {
@@ -558,10 +574,14 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
                 row_forces<PM, EXACT, SAMPLE, MULTI>(P, V, R, s_tab, (int)p, w, xp, fx, fy, uu);
                 const double2 vh = reinterpret_cast<const double2 *>(b + L.vel)[tid];
                 const uint8_t g = (b + L.grp)[tid];
-                particle_update<EXACT, KICK2, ADVANCE, SAMPLE>(P, V, p, xp, vh, g, fx, fy, uu);
+                if (MULTI && M.resident)
+                    particle_update<EXACT, KICK2, ADVANCE, SAMPLE>(P, V, p, xp, vh, g, fx, fy, uu, reinterpret_cast<double2 *>(b + L.pos) + tid,
+                                                                   reinterpret_cast<double2 *>(b + L.vel) + tid);
+                else
+                    particle_update<EXACT, KICK2, ADVANCE, SAMPLE>(P, V, p, xp, vh, g, fx, fy, uu);
             }
             __syncwarp();
-            if (lane == 0) mbar_arrive(empty + s);
+            if (lane == 0 && !(MULTI && M.resident)) mbar_arrive(empty + s);
             if (++s == L.stages) { s = 0; ++u; }
         }
         if (MULTI && it + 1 < nsteps) {  // publish this step's stores, then tell the producer this warp is done
@@ -771,11 +791,12 @@ __global__ void __launch_bounds__(kBlock) k_compact_ell(const CompactParams C) {
     const int wi = (int)(sl % kTileSlices);
     const unsigned w = h->w[wi];
     const size_t e0 = (size_t)h->off[wi] * kSlice + lane;
+    const int self = (int)(sl * kSlice + lane);
     unsigned j = 0;
     for (unsigned s = 0; s < w; ++s) {
         const size_t e = e0 + (size_t)s * kSlice;
         const int nb = C.nbr[e];
-        if (nb >= 0) {
+        if (nb != self) {
             if (j != s) {
                 const size_t d = e0 + (size_t)j * kSlice;
                 C.nbr[d] = nb; C.sid[d] = C.sid[e];
@@ -787,7 +808,7 @@ __global__ void __launch_bounds__(kBlock) k_compact_ell(const CompactParams C) {
             ++j;
         }
     }
-    for (unsigned s = j; s < w; ++s) C.nbr[e0 + (size_t)s * kSlice] = kPad;
+    for (unsigned s = j; s < w; ++s) C.nbr[e0 + (size_t)s * kSlice] = self;
     unsigned wmax = j;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) wmax = max(wmax, __shfl_xor_sync(0xffffffffu, wmax, o));
