@@ -687,7 +687,7 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
             L.kF = o; if (need_krF) o += up(cap * kSlice * 8);
             L.r0F = o; if (need_krF) o += up(cap * kSlice * 8);
             L.bytes = up(o);
-            L.first = kStreamHdrBytes + (need_typ ? 4 * kMaxTypes * 8 : 0);
+            L.first = kStreamHdrBytes + (need_typ ? ((s->ntypes * kTabStride * 8 + 127) & ~127) : 0);
             int dev_smem = 0, n_sm = 0;
             CUDA_TRY(s, cudaDeviceGetAttribute(&dev_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, d->device));
             CUDA_TRY(s, cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, d->device));
@@ -746,12 +746,14 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
         return fail(s, LSM_E_INVALID, "bad force_mode");
     }
     if (!tab.empty()) {
-        if (s->force_mode == LSM_FORCE_GATHER) {   // gather kernels: 4 doubles per type, the 4th carries the filter word
-            std::vector<double> t4(tab.size() / 3 * 4, 0.0);
+        if (s->force_mode == LSM_FORCE_GATHER) {   // gather kernels: kTabStride doubles per type (k, k*r0, filter word, r0, rc)
+            std::vector<double> t4(tab.size() / 3 * kTabStride, 0.0);
             for (size_t t = 0; t < tab.size() / 3; ++t) {
-                t4[4 * t] = tab[3 * t]; t4[4 * t + 1] = tab[3 * t + 1]; t4[4 * t + 2] = tab[3 * t + 2];
-                const uint64_t w = thr_of(tab[3 * t + 2]);
-                std::memcpy(&t4[4 * t + 3], &w, 8);
+                const double k = tab[3 * t], r0 = tab[3 * t + 1], rc = tab[3 * t + 2];
+                double *q = &t4[kTabStride * t];
+                q[0] = k; q[1] = k * r0; q[3] = r0; q[4] = rc;
+                const uint64_t w = thr_of(rc);
+                std::memcpy(&q[2], &w, 8);
             }
             tab.swap(t4);
         }

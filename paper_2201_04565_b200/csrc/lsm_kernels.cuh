@@ -42,6 +42,7 @@ constexpr uint8_t kFree = 0xFF;
 constexpr int kMaxGroups = 8;
 constexpr int kChunk = 2048;  // particles per reduction chunk
 constexpr int kMaxTypes = 256;
+constexpr int kTabStride = 6;   // gather type table, doubles per type: k, k*r0, filter word (low 32 bits), r0, rc, pad
 
 enum ParamMode { PM_UNIFORM = 0, PM_TYPED = 1, PM_RCF = 2, PM_KRT_RCF = 3, PM_FULL = 4 };
 
@@ -62,7 +63,7 @@ struct SpringParams {  // parameter encoding shared by the gather (per half-edge
     const double *kF, *r0F, *rcF;      // rcF: scatter layout only
     const uint32_t *thr;               // gather layout: breakage filter per half-edge, (high word of rc*rc) - 1
     const double *rcS;                 // gather layout: exact rc per spring, caller numbering
-    const double *tab;  // scatter: [ntypes][3] = k, r0, rc;  gather: [ntypes][4] = k, r0, rc, (thr in the low word)
+    const double *tab;  // scatter: [ntypes][3] = k, r0, rc;  gather: [ntypes][kTabStride] (see kTabStride)
     int ntypes;
     double k_u, r0_u, rc_u, kr0_u;
     uint32_t thr_u;
@@ -259,9 +260,18 @@ struct RowSrc {            // where one particle's row lives: pointers already o
 template <int PM> __device__ __forceinline__ void slot_params(const StepParams &P, const RowSrc &R, const double *s_tab, unsigned so,
                                                               double &k, double &r0, double &kr0, uint32_t &thr) {
     if (PM == PM_UNIFORM) { k = P.sp.k_u; r0 = P.sp.r0_u; kr0 = P.sp.kr0_u; thr = P.sp.thr_u; }
-    else if (PM == PM_TYPED) { const int t = R.typ[so]; k = s_tab[4 * t]; r0 = s_tab[4 * t + 1]; kr0 = k * r0; thr = reinterpret_cast<const uint32_t *>(s_tab)[8 * t + 6]; }
+    else if (PM == PM_TYPED) {
+        const int t = R.typ[so];
+        const double2 kk = *reinterpret_cast<const double2 *>(s_tab + kTabStride * t);   // one 16-byte load: k, k*r0
+        k = kk.x; kr0 = kk.y; r0 = s_tab[kTabStride * t + 3];
+        thr = reinterpret_cast<const uint32_t *>(s_tab)[2 * (kTabStride * t + 2)];
+    }
     else if (PM == PM_RCF) { k = P.sp.k_u; r0 = P.sp.r0_u; kr0 = P.sp.kr0_u; thr = R.thr[so]; }
-    else if (PM == PM_KRT_RCF) { const int t = R.typ[so]; k = s_tab[4 * t]; r0 = s_tab[4 * t + 1]; kr0 = k * r0; thr = R.thr[so]; }
+    else if (PM == PM_KRT_RCF) {
+        const int t = R.typ[so];
+        const double2 kk = *reinterpret_cast<const double2 *>(s_tab + kTabStride * t);
+        k = kk.x; kr0 = kk.y; r0 = s_tab[kTabStride * t + 3]; thr = R.thr[so];
+    }
     else { k = R.kF[so]; r0 = R.r0F[so]; kr0 = k * r0; thr = R.thr[so]; }
 }
 
@@ -345,7 +355,7 @@ __device__ __forceinline__ void row_careful(const StepParams &P, const StepVar &
             const size_t e = R.e0 + so;
             double rc;
             if (PM == PM_UNIFORM) rc = P.sp.rc_u;
-            else if (PM == PM_TYPED) rc = s_tab[4 * R.typ[so] + 2];
+            else if (PM == PM_TYPED) rc = s_tab[kTabStride * R.typ[so] + 4];
             else rc = __ldg(P.sp.rcS + __ldg(P.sid + e));
             if (__dsqrt_rn(r2) > rc) {   // strict '>' (Q1)
                 P.nbr[e] = p;                             // dead from now on: the slot points at its own particle
@@ -378,9 +388,9 @@ __device__ __forceinline__ void row_forces(const StepParams &P, const StepVar &V
 template <int PM, bool EXACT, bool KICK2, bool ADVANCE, bool SAMPLE>
 __global__ void __launch_bounds__(kBlock) k_gather_step(const StepParams P) {
     constexpr bool kTab = (PM == PM_TYPED || PM == PM_KRT_RCF);
-    __shared__ double s_tab[kTab ? 4 * kMaxTypes : 1];
+    __shared__ __align__(16) double s_tab[kTab ? kTabStride * kMaxTypes : 1];
     if (kTab) {
-        for (int i = threadIdx.x; i < 4 * P.sp.ntypes; i += kBlock) s_tab[i] = P.sp.tab[i];
+        for (int i = threadIdx.x; i < kTabStride * P.sp.ntypes; i += kBlock) s_tab[i] = P.sp.tab[i];
         __syncthreads();
     }
     const long long p = (long long)blockIdx.x * kBlock + threadIdx.x;
@@ -467,7 +477,7 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
     uint64_t *empty = full + kMaxStages;                            // [kMaxStages]
     uint64_t *stepdone = empty + kMaxStages;                        // MULTI: all consumer warps of this CTA finished the step
     uint64_t *go = stepdone + 1;                                    // MULTI resident: the grid barrier has been passed
-    double *s_tab = reinterpret_cast<double *>(smem + kStreamHdrBytes);         // [4*kMaxTypes] when kTab
+    double *s_tab = reinterpret_cast<double *>(smem + kStreamHdrBytes);         // [kTabStride * ntypes] when kTab
     unsigned char *stage0 = smem + L.first;
     const int tid = threadIdx.x, wi = tid >> 5, lane = tid & 31;
     if (tid == 0) {
@@ -475,7 +485,7 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
         if (MULTI) { mbar_init(stepdone, kTileSlices); mbar_init(go, 1); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    if (kTab) for (int i = tid; i < 4 * P.sp.ntypes; i += kTile + 32) s_tab[i] = P.sp.tab[i];
+    if (kTab) for (int i = tid; i < kTabStride * P.sp.ntypes; i += kTile + 32) s_tab[i] = P.sp.tab[i];
     __syncthreads();
     const int nsteps = MULTI ? M.nsteps : 1;
 
