@@ -60,6 +60,7 @@ struct lsm_sim {
     long long nslices = 0, E = 0, T = 0, Npad = 0;
     TileHdr *hdr = nullptr;
     int32_t *nbr = nullptr, *sid = nullptr;
+    int16_t *nbr16 = nullptr;
     uint32_t *thr = nullptr;
     double *rcS = nullptr;
     int gather_variant = 0;          // resolved: 1 direct, 2 streamed
@@ -190,7 +191,7 @@ StepParams step_params(const lsm_sim *s, long long step) {
     P.mass_u = s->mass_u; P.inv_mass_u = 1.0 / s->mass_u;
     P.dt = s->dt; P.hdt = 0.5 * s->dt; P.gamma = s->gamma;
     P.N = s->N; P.step = step; P.l2 = s->l2_hints;
-    P.hdr = s->hdr; P.T = s->T; P.nbr = s->nbr; P.sid = s->sid;
+    P.hdr = s->hdr; P.T = s->T; P.nbr = s->nbr; P.nbr16 = s->nbr16; P.sid = s->sid;
     P.sp.typ = s->typ; P.sp.kF = s->kF; P.sp.r0F = s->r0F; P.sp.rcF = s->rcF; P.sp.tab = s->tab; P.sp.ntypes = s->ntypes;
     P.sp.thr = s->thr; P.sp.rcS = s->rcS; P.sp.kr0_u = s->k_u * s->r0_u; P.sp.thr_u = thr_of(s->rc_u);
     P.sp.k_u = s->k_u; P.sp.r0_u = s->r0_u; P.sp.rc_u = s->rc_u;
@@ -238,21 +239,34 @@ template <class K> void stream_opt_in(K kern, const lsm_sim *s, int &configured_
 }
 
 template <int PM, bool EXACT, bool KICK2, bool ADVANCE, bool SAMPLE> void launch_stream_one(const lsm_sim *s, const StepParams &P) {
-    auto kern = k_gather_stream<PM, EXACT, KICK2, ADVANCE, SAMPLE, false>;
-    static thread_local int configured_for = -1;
-    stream_opt_in(kern, s, configured_for);
     MultiParams M;
     std::memset(&M, 0, sizeof(M));
-    kern<<<s->stream_grid, kTile + 32, s->stream_smem, s->stream>>>(P, s->L, M);
+    if (s->nbr16) {
+        auto kern = k_gather_stream<PM, EXACT, KICK2, ADVANCE, SAMPLE, false, true>;
+        static thread_local int configured_for = -1;
+        stream_opt_in(kern, s, configured_for);
+        kern<<<s->stream_grid, kTile + 32, s->stream_smem, s->stream>>>(P, s->L, M);
+    } else {
+        auto kern = k_gather_stream<PM, EXACT, KICK2, ADVANCE, SAMPLE, false, false>;
+        static thread_local int configured_for = -1;
+        stream_opt_in(kern, s, configured_for);
+        kern<<<s->stream_grid, kTile + 32, s->stream_smem, s->stream>>>(P, s->L, M);
+    }
 }
 
 // nsteps consecutive non-sample time steps in ONE cooperative launch (grid barrier between steps).
 template <int PM, bool EXACT> cudaError_t launch_stream_multi_one(const lsm_sim *s, StepParams P, MultiParams M) {
-    auto kern = k_gather_stream<PM, EXACT, true, true, false, true>;
-    static thread_local int configured_for = -1;
-    stream_opt_in(kern, s, configured_for);
     StageLayout L = s->L;
     void *args[3] = {&P, &L, &M};
+    if (s->nbr16) {
+        auto kern = k_gather_stream<PM, EXACT, true, true, false, true, true>;
+        static thread_local int configured_for = -1;
+        stream_opt_in(kern, s, configured_for);
+        return cudaLaunchCooperativeKernel((const void *)kern, dim3(s->stream_grid), dim3(kTile + 32), args, (size_t)s->stream_smem, s->stream);
+    }
+    auto kern = k_gather_stream<PM, EXACT, true, true, false, true, false>;
+    static thread_local int configured_for = -1;
+    stream_opt_in(kern, s, configured_for);
     return cudaLaunchCooperativeKernel((const void *)kern, dim3(s->stream_grid), dim3(kTile + 32), args, (size_t)s->stream_smem, s->stream);
 }
 
@@ -385,7 +399,7 @@ lsm_status eval_initial(lsm_sim *s) {
 lsm_status do_compact(lsm_sim *s) {
     if (s->force_mode == LSM_FORCE_GATHER) {
         CompactParams C;
-        C.hdr = s->hdr; C.nbr = s->nbr; C.sid = s->sid; C.typ = s->typ; C.thr = s->thr;
+        C.hdr = s->hdr; C.nbr = s->nbr; C.nbr16 = s->nbr16; C.sid = s->sid; C.typ = s->typ; C.thr = s->thr;
         C.kF = s->kF; C.r0F = s->r0F; C.nslices = s->nslices;
         k_compact_ell<<<grid_for(s->nslices * kSlice), kBlock, 0, s->stream>>>(C);
         s->kernels_launched += 1;
@@ -652,6 +666,20 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
         }
         TRY(upload(s, &s->hdr, hh));
         TRY(upload(s, &s->nbr, hn));
+        bool fits16 = std::getenv("LSM_NO_IDX16") == nullptr;
+        {   // 16-bit neighbour offsets (neighbour - self) when every one fits: halves the streamed id bytes
+            std::vector<int16_t> h16;
+            if (fits16) {
+                h16.resize(E);
+                for (long long sl = 0; sl < T * kTileSlices && fits16; ++sl)
+                    for (size_t e = (size_t)off[sl] * kSlice; e < (size_t)off[sl + 1] * kSlice; ++e) {
+                        const long long dlt = (long long)hn[e] - (sl * kSlice + (long long)(e & 31));
+                        if (dlt < -32768 || dlt > 32767) { fits16 = false; break; }
+                        h16[e] = (int16_t)dlt;
+                    }
+            }
+            if (fits16) { TRY(upload(s, &s->nbr16, h16)); CUDA_TRY(s, cudaStreamSynchronize(s->stream)); }
+        }
         if (need_typ) { std::vector<uint8_t> ht(E, 0); for (size_t e = 0; e < E; ++e) if (hs[e] >= 0) ht[e] = stype[hs[e]]; TRY(upload(s, &s->typ, ht)); CUDA_TRY(s, cudaStreamSynchronize(s->stream)); }
         if (need_rcF) {
             std::vector<uint32_t> h(E, 0xFFFFFFFFu);
@@ -681,7 +709,7 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
             L.vel = o; o += kTile * 16;
             L.hdr = o; o += 128;
             L.grp = o; o += kTile;
-            L.nbr = o; o += up(cap * kSlice * 4);
+            L.nbr = o; o += up(cap * kSlice * (s->nbr16 ? 2 : 4));
             L.thr = o; if (need_rcF) o += up(cap * kSlice * 4);
             L.typ = o; if (need_typ) o += up(cap * kSlice);
             L.kF = o; if (need_krF) o += up(cap * kSlice * 8);
@@ -1025,7 +1053,7 @@ lsm_status lsm_get_info(lsm_sim *s, lsm_info *info) {
     std::memset(info, 0, sizeof(*info));
     info->n_particles = s->N; info->n_springs = s->M; info->n_half_edges_stored = s->E;
     static const int pbytes_scatter[5] = {0, 1, 8, 9, 24}, pbytes_gather[5] = {0, 1, 4, 5, 20};
-    info->bytes_per_half_edge = s->force_mode == LSM_FORCE_GATHER ? 4 + pbytes_gather[s->pm] : 8 + pbytes_scatter[s->pm];
+    info->bytes_per_half_edge = s->force_mode == LSM_FORCE_GATHER ? (s->nbr16 && s->gather_variant == 2 ? 2 : 4) + pbytes_gather[s->pm] : 8 + pbytes_scatter[s->pm];
     info->gather_variant = s->force_mode == LSM_FORCE_GATHER ? s->gather_variant : 0;
     info->pipeline_stages = s->gather_variant == 2 ? s->L.stages : 0;
     info->step_fusion = s->multi_on;

@@ -90,6 +90,7 @@ struct StepParams {
     const TileHdr *hdr;
     long long T;  // tiles
     int32_t *nbr;
+    int16_t *nbr16;   // same list as 16-bit offsets (neighbour - self), present when every offset fits: the streamed copy
     const int32_t *sid;
     SpringParams sp;
     // breakage bookkeeping
@@ -240,6 +241,7 @@ __device__ __forceinline__ void particle_update(const StepParams &P, const StepV
 // ---------------------------------------------------------------------------------------------------------------
 struct RowSrc {            // where one particle's row lives: pointers already offset to (slice offset)*32 + lane
     const int32_t *nbr;    // slot s at nbr[s*32]  (global memory, or the staged shared-memory copy)
+    const int16_t *nbr16;  // I16: the staged copy holds 16-bit offsets (neighbour - self) instead
     const uint32_t *thr;
     const uint8_t *typ;
     const double *kF, *r0F;
@@ -312,14 +314,14 @@ __device__ __forceinline__ void slot_eval(double2 xq, double2 xp, bool lower, do
     near = live && hi >= thr;
 }
 
-template <int PM, bool EXACT, bool SAMPLE, bool COHERENT, int CH>
+template <int PM, bool EXACT, bool SAMPLE, bool COHERENT, bool I16, int CH>
 __device__ __forceinline__ bool row_chunk(const StepParams &P, const StepVar &V, const RowSrc &R, const double *s_tab, int p, unsigned s0,
                                           double2 xp, double &fx, double &fy, double &u) {
     int nb[CH];
     double2 xq[CH];
     bool any_near = false;
 #pragma unroll
-    for (int c = 0; c < CH; ++c) nb[c] = R.nbr[(s0 + c) * kSlice];
+    for (int c = 0; c < CH; ++c) nb[c] = I16 ? p + (int)R.nbr16[(s0 + c) * kSlice] : R.nbr[(s0 + c) * kSlice];
 #pragma unroll
     for (int c = 0; c < CH; ++c) xq[c] = gather_pos<COHERENT>(V, nb[c]);
 #pragma unroll
@@ -337,14 +339,14 @@ __device__ __forceinline__ bool row_chunk(const StepParams &P, const StepVar &V,
     return any_near;
 }
 
-template <int PM, bool EXACT, bool SAMPLE, bool COHERENT>
+template <int PM, bool EXACT, bool SAMPLE, bool COHERENT, bool I16>
 __device__ __forceinline__ void row_careful(const StepParams &P, const StepVar &V, const RowSrc &R, const double *s_tab, int p, unsigned w,
                                          double2 xp, double &fx, double &fy, double &u) {
     fx = 0.0; fy = 0.0; u = 0.0;
 #pragma unroll 1
     for (unsigned s = 0; s < w; ++s) {
         const unsigned so = s * kSlice;
-        const int nb = R.nbr[so];
+        const int nb = I16 ? p + (int)R.nbr16[so] : R.nbr[so];
         const double2 xq = gather_pos<COHERENT>(V, nb);
         double k, r0, kr0, dx, dy, r2, g, ue;
         uint32_t thr;
@@ -359,7 +361,9 @@ __device__ __forceinline__ void row_careful(const StepParams &P, const StepVar &
             else rc = __ldg(P.sp.rcS + __ldg(P.sid + e));
             if (__dsqrt_rn(r2) > rc) {   // strict '>' (Q1)
                 P.nbr[e] = p;                             // dead from now on: the slot points at its own particle
-                const_cast<int32_t *>(R.nbr)[so] = p;     // and the staged copy (resident tiles are not reloaded)
+                if (P.nbr16) P.nbr16[e] = 0;
+                if (I16) const_cast<int16_t *>(R.nbr16)[so] = 0;   // and the staged copy (resident tiles are not reloaded)
+                else const_cast<int32_t *>(R.nbr)[so] = p;
                 if (p < nb) {
                     P.break_step[P.sid[e]] = V.step;
                     atomicAdd(P.nbroken + spec_of(P.poff, P.B, p), 1ULL);
@@ -373,15 +377,15 @@ __device__ __forceinline__ void row_careful(const StepParams &P, const StepVar &
     }
 }
 
-template <int PM, bool EXACT, bool SAMPLE, bool COHERENT>
+template <int PM, bool EXACT, bool SAMPLE, bool COHERENT, bool I16>
 __device__ __forceinline__ void row_forces(const StepParams &P, const StepVar &V, const RowSrc &R, const double *s_tab, int p, unsigned w,
                                            double2 xp, double &fx, double &fy, double &u) {
     constexpr int CH = LSM_ROW_CH;
     unsigned s0 = 0;
     bool any_near = false;
-    for (; s0 + CH <= w; s0 += CH) any_near |= row_chunk<PM, EXACT, SAMPLE, COHERENT, CH>(P, V, R, s_tab, p, s0, xp, fx, fy, u);
-    for (; s0 < w; ++s0) any_near |= row_chunk<PM, EXACT, SAMPLE, COHERENT, 1>(P, V, R, s_tab, p, s0, xp, fx, fy, u);
-    if (any_near) row_careful<PM, EXACT, SAMPLE, COHERENT>(P, V, R, s_tab, p, w, xp, fx, fy, u);
+    for (; s0 + CH <= w; s0 += CH) any_near |= row_chunk<PM, EXACT, SAMPLE, COHERENT, I16, CH>(P, V, R, s_tab, p, s0, xp, fx, fy, u);
+    for (; s0 < w; ++s0) any_near |= row_chunk<PM, EXACT, SAMPLE, COHERENT, I16, 1>(P, V, R, s_tab, p, s0, xp, fx, fy, u);
+    if (any_near) row_careful<PM, EXACT, SAMPLE, COHERENT, I16>(P, V, R, s_tab, p, w, xp, fx, fy, u);
 }
 
 // Direct variant: block = tile, every stream read from global memory by the thread that needs it.
@@ -403,11 +407,11 @@ __global__ void __launch_bounds__(kBlock) k_gather_step(const StepParams P) {
     const double2 vh = P.vel[p];
     const uint8_t g = P.grp[p];
     RowSrc R;
-    R.nbr = P.nbr + e0; R.thr = P.sp.thr + e0; R.typ = P.sp.typ + e0; R.kF = P.sp.kF + e0; R.r0F = P.sp.r0F + e0;
+    R.nbr = P.nbr + e0; R.nbr16 = nullptr; R.thr = P.sp.thr + e0; R.typ = P.sp.typ + e0; R.kF = P.sp.kF + e0; R.r0F = P.sp.r0F + e0;
     R.e0 = e0;
     double fx = 0.0, fy = 0.0, u = 0.0;
     const StepVar V{P.pos_cur, P.pos_next, P.step};
-    row_forces<PM, EXACT, SAMPLE, false>(P, V, R, s_tab, (int)p, w, xp, fx, fy, u);
+    row_forces<PM, EXACT, SAMPLE, false, false>(P, V, R, s_tab, (int)p, w, xp, fx, fy, u);
     particle_update<EXACT, KICK2, ADVANCE, SAMPLE>(P, V, p, xp, vh, g, fx, fy, u);
 }
 
@@ -466,7 +470,7 @@ struct MultiParams {
     double2 *pos_a, *pos_b;           // step i reads pos_a / writes pos_b when i is even, the reverse when odd
 };
 
-template <int PM, bool EXACT, bool KICK2, bool ADVANCE, bool SAMPLE, bool MULTI>
+template <int PM, bool EXACT, bool KICK2, bool ADVANCE, bool SAMPLE, bool MULTI, bool I16>
 __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const StepParams P, const StageLayout L, const MultiParams M) {
     constexpr bool kTab = (PM == PM_TYPED || PM == PM_KRT_RCF);
     constexpr bool kHasThr = (PM == PM_RCF || PM == PM_KRT_RCF || PM == PM_FULL);
@@ -512,7 +516,8 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
                     const uint32_t o0 = o0n, ns = o8n - o0n;
                     if (t + gridDim.x < P.T) { o0n = __ldg(&h[gridDim.x].off[0]); o8n = __ldg(&h[gridDim.x].off[kTileSlices]); }  // next tile's extent, ahead of the wait
                     if (u > 0) mbar_wait(empty + s, (u - 1) & 1);
-                    unsigned bytes = 2 * kTile * 16 + kTile + 64 + ns * (kSlice * 4);
+                    constexpr unsigned kIdB = I16 ? 2 : 4;   // bytes per streamed neighbour id
+                    unsigned bytes = 2 * kTile * 16 + kTile + 64 + ns * (kSlice * kIdB);
                     if (kHasThr) bytes += ns * (kSlice * 4);
                     if (kHasTyp) bytes += ns * kSlice;
                     if (kHasKR) bytes += 2 * ns * (kSlice * 8);
@@ -532,7 +537,8 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
                     if (ns) {
                         const size_t e = (size_t)o0 * kSlice;
                         if (P.l2 & 2) {
-                            bulk_g2s_hint(b + L.nbr, P.nbr + e, ns * (kSlice * 4), full + s, pol_stream);
+                            if (I16) bulk_g2s_hint(b + L.nbr, P.nbr16 + e, ns * (kSlice * 2), full + s, pol_stream);
+                            else bulk_g2s_hint(b + L.nbr, P.nbr + e, ns * (kSlice * 4), full + s, pol_stream);
                             if (kHasThr) bulk_g2s_hint(b + L.thr, P.sp.thr + e, ns * (kSlice * 4), full + s, pol_stream);
                             if (kHasTyp) bulk_g2s_hint(b + L.typ, P.sp.typ + e, ns * kSlice, full + s, pol_stream);
                             if (kHasKR) {
@@ -540,7 +546,8 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
                                 bulk_g2s_hint(b + L.r0F, P.sp.r0F + e, ns * (kSlice * 8), full + s, pol_stream);
                             }
                         } else {
-                            bulk_g2s(b + L.nbr, P.nbr + e, ns * (kSlice * 4), full + s);
+                            if (I16) bulk_g2s(b + L.nbr, P.nbr16 + e, ns * (kSlice * 2), full + s);
+                            else bulk_g2s(b + L.nbr, P.nbr + e, ns * (kSlice * 4), full + s);
                             if (kHasThr) bulk_g2s(b + L.thr, P.sp.thr + e, ns * (kSlice * 4), full + s);
                             if (kHasTyp) bulk_g2s(b + L.typ, P.sp.typ + e, ns * kSlice, full + s);
                             if (kHasKR) {
@@ -575,13 +582,14 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
                 const double2 xp = reinterpret_cast<const double2 *>(b + L.pos)[tid];
                 RowSrc R;
                 R.nbr = reinterpret_cast<const int32_t *>(b + L.nbr) + rel;
+                R.nbr16 = reinterpret_cast<const int16_t *>(b + L.nbr) + rel;
                 R.thr = reinterpret_cast<const uint32_t *>(b + L.thr) + rel;
                 R.typ = (b + L.typ) + rel;
                 R.kF = reinterpret_cast<const double *>(b + L.kF) + rel;
                 R.r0F = reinterpret_cast<const double *>(b + L.r0F) + rel;
                 R.e0 = (size_t)h->off[wi] * kSlice + lane;
                 double fx = 0.0, fy = 0.0, uu = 0.0;
-                row_forces<PM, EXACT, SAMPLE, MULTI>(P, V, R, s_tab, (int)p, w, xp, fx, fy, uu);
+                row_forces<PM, EXACT, SAMPLE, MULTI, I16>(P, V, R, s_tab, (int)p, w, xp, fx, fy, uu);
                 const double2 vh = reinterpret_cast<const double2 *>(b + L.vel)[tid];
                 const uint8_t g = (b + L.grp)[tid];
                 if (MULTI && M.resident)
@@ -787,6 +795,7 @@ __global__ void __launch_bounds__(kBlock) k_finalize_sample(const ReduceParams R
 struct CompactParams {
     TileHdr *hdr;
     int32_t *nbr, *sid;
+    int16_t *nbr16;
     uint8_t *typ;
     uint32_t *thr;
     double *kF, *r0F;
@@ -810,6 +819,7 @@ __global__ void __launch_bounds__(kBlock) k_compact_ell(const CompactParams C) {
             if (j != s) {
                 const size_t d = e0 + (size_t)j * kSlice;
                 C.nbr[d] = nb; C.sid[d] = C.sid[e];
+                if (C.nbr16) C.nbr16[d] = C.nbr16[e];
                 if (C.typ) C.typ[d] = C.typ[e];
                 if (C.thr) C.thr[d] = C.thr[e];
                 if (C.kF) C.kF[d] = C.kF[e];
@@ -818,7 +828,7 @@ __global__ void __launch_bounds__(kBlock) k_compact_ell(const CompactParams C) {
             ++j;
         }
     }
-    for (unsigned s = j; s < w; ++s) C.nbr[e0 + (size_t)s * kSlice] = self;
+    for (unsigned s = j; s < w; ++s) { C.nbr[e0 + (size_t)s * kSlice] = self; if (C.nbr16) C.nbr16[e0 + (size_t)s * kSlice] = 0; }
     unsigned wmax = j;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) wmax = max(wmax, __shfl_xor_sync(0xffffffffu, wmax, o));

@@ -446,11 +446,11 @@ def test_full_size_config4_sampled_specimens():
 @pytest.mark.parametrize("n", [4096, 8192])
 def test_large_config5_first_steps(n):
     """BASELINE.json configs[4] (notched, pre-strained lattice; here n x n with the same recipe): the first steps against
-    the oracle on every particle, plus the force evaluation at step 0 (uniform parameters: 4 bytes per half-edge)."""
+    the oracle on every particle, plus the force evaluation at step 0 (uniform parameters: 2 bytes per half-edge)."""
     p = config5(n=n)
     o = OracleSim.from_problem(p)
     g = lsm_create_from_problem(p)
-    assert g.info()["param_mode"] == 0 and g.info()["bytes_per_half_edge"] == 4
+    assert g.info()["param_mode"] == 0 and g.info()["bytes_per_half_edge"] == 2     # uniform parameters, 16-bit neighbour offsets
     fo, fg = o.read_forces(), g.read_forces()
     sc = force_scale(p.x, p.spring_i, p.spring_j, p.k, p.r0)
     check_forces(fg, fo, sc, floor=conditioning_floor(p.x, p.spring_i, p.spring_j, p.k))
@@ -460,3 +460,23 @@ def test_large_config5_first_steps(n):
     assert np.abs(xg - xo).max() <= 32 * eps * np.abs(xo).max() and np.abs(vg - vo).max() <= 1e-12
     assert g.n_broken() == o.read_broken()[2] == 0
     g.close()
+
+
+def test_wide_neighbour_offsets_use_32bit_ids():
+    """Shuffled numbering of a 256x256 two-phase lattice without renumbering: neighbour offsets exceed 16 bits, so the
+    streamed kernel must take its 32-bit id stream (5 bytes per half-edge: id + type); with Morton renumbering the same
+    input streams 16-bit offsets (3 bytes).  Both against the oracle."""
+    p = shuffle_ids(config2(n=256, n_blobs=60), 3)
+    o = OracleSim.from_problem(p)
+    fo = o.read_forces()
+    sc = force_scale(p.x, p.spring_i, p.spring_j, p.k, p.r0)
+    o.step(300)
+    xo, vo = o.read_state()
+    for reorder, nbytes in ((0, 5), (1, 3)):
+        g = lsm_create_from_problem(p, reorder=reorder)
+        assert g.info()["gather_variant"] == lsm.GATHER_STREAMED and g.info()["bytes_per_half_edge"] == nbytes
+        check_forces(g.read_forces(), fo, sc, floor=conditioning_floor(p.x, p.spring_i, p.spring_j, p.k))
+        g.step(300)
+        xg, vg = g.read_state()
+        assert np.abs(xg - xo).max() <= 1e-11 and np.abs(vg - vo).max() <= 1e-11
+        g.close()
