@@ -291,7 +291,9 @@ def main():
             "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 2 * xh.numel() * 8, "d2h_bytes_per_step": 2 * xh.numel() * 8 + d2h_hist,
                     "ms_per_step": te_ms_max / K},
             "gpu_launches": int(launches),
-            "roofline": {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": None,
+            # achieved = COUNTED (algorithmic) bytes / time.  The kernel streams fewer bytes than the counted model (16-bit
+            # neighbour offsets and filter words instead of int32 ids and fp64 rc), so this can pass the copy peak: capped.
+            "roofline": {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": min(1.0, ach / peak), "frac_uncapped": ach / peak, "traffic": None,
                          "peak_source": peak_src, "frac_of_nominal_8TBs": ach / 8000.0, "counted_bytes_per_time_step": bc,
                          "p_var": pv, "kernel": "fused step kernel (one launch per time step)",
                          "duration_us": t_launch * 1e6},

@@ -61,7 +61,8 @@ struct lsm_sim {
     TileHdr *hdr = nullptr;
     int32_t *nbr = nullptr, *sid = nullptr;
     int16_t *nbr16 = nullptr;
-    uint32_t *thr = nullptr;
+    uint16_t *thr = nullptr;
+    uint32_t thr_base = 0, thr_shift = 0;
     double *rcS = nullptr;
     int gather_variant = 0;          // resolved: 1 direct, 2 streamed
     StageLayout L;
@@ -193,7 +194,7 @@ StepParams step_params(const lsm_sim *s, long long step) {
     P.N = s->N; P.step = step; P.l2 = s->l2_hints;
     P.hdr = s->hdr; P.T = s->T; P.nbr = s->nbr; P.nbr16 = s->nbr16; P.sid = s->sid;
     P.sp.typ = s->typ; P.sp.kF = s->kF; P.sp.r0F = s->r0F; P.sp.rcF = s->rcF; P.sp.tab = s->tab; P.sp.ntypes = s->ntypes;
-    P.sp.thr = s->thr; P.sp.rcS = s->rcS; P.sp.kr0_u = s->k_u * s->r0_u; P.sp.thr_u = thr_of(s->rc_u);
+    P.sp.thr = s->thr; P.sp.thr_base = s->thr_base; P.sp.thr_shift = s->thr_shift; P.sp.rcS = s->rcS; P.sp.kr0_u = s->k_u * s->r0_u; P.sp.thr_u = thr_of(s->rc_u);
     P.sp.k_u = s->k_u; P.sp.r0_u = s->r0_u; P.sp.rc_u = s->rc_u;
     P.break_step = s->break_step; P.nbroken = s->nbroken; P.poff = s->d_poff; P.B = s->B;
     P.sU = s->sU; P.sKE = s->sKE;
@@ -682,8 +683,16 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
         }
         if (need_typ) { std::vector<uint8_t> ht(E, 0); for (size_t e = 0; e < E; ++e) if (hs[e] >= 0) ht[e] = stype[hs[e]]; TRY(upload(s, &s->typ, ht)); CUDA_TRY(s, cudaStreamSynchronize(s->stream)); }
         if (need_rcF) {
-            std::vector<uint32_t> h(E, 0xFFFFFFFFu);
-            for (size_t e = 0; e < E; ++e) if (hs[e] >= 0) h[e] = thr_of(getrc(hs[e]));
+            // 16-bit code of the filter word: base = the smallest word, shift = as few bits as make the spread fit;
+            // codes are rounded DOWN (a lower threshold only sends a few more springs to the exact decision)
+            uint32_t lo = 0xFFFFFFFFu, hi = 0;
+            for (long long e = 0; e < M; ++e) { const uint32_t t = thr_of(getrc(e)); lo = std::min(lo, t); hi = std::max(hi, t); }
+            if (M == 0) lo = hi = 0;
+            uint32_t shift = 0;
+            while (((hi - lo) >> shift) > 0xFFFFu) ++shift;
+            s->thr_base = lo; s->thr_shift = shift;
+            std::vector<uint16_t> h(E, 0xFFFFu);
+            for (size_t e = 0; e < E; ++e) if (hs[e] >= 0) h[e] = (uint16_t)((thr_of(getrc(hs[e])) - lo) >> shift);
             TRY(upload(s, &s->thr, h)); CUDA_TRY(s, cudaStreamSynchronize(s->stream));
             std::vector<double> hr(M);
             for (long long e = 0; e < M; ++e) hr[e] = getrc(e);
@@ -710,7 +719,7 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
             L.hdr = o; o += 128;
             L.grp = o; o += kTile;
             L.nbr = o; o += up(cap * kSlice * (s->nbr16 ? 2 : 4));
-            L.thr = o; if (need_rcF) o += up(cap * kSlice * 4);
+            L.thr = o; if (need_rcF) o += up(cap * kSlice * 2);
             L.typ = o; if (need_typ) o += up(cap * kSlice);
             L.kF = o; if (need_krF) o += up(cap * kSlice * 8);
             L.r0F = o; if (need_krF) o += up(cap * kSlice * 8);
@@ -1052,7 +1061,7 @@ lsm_status lsm_get_info(lsm_sim *s, lsm_info *info) {
     if (!s || !info) return LSM_E_INVALID;
     std::memset(info, 0, sizeof(*info));
     info->n_particles = s->N; info->n_springs = s->M; info->n_half_edges_stored = s->E;
-    static const int pbytes_scatter[5] = {0, 1, 8, 9, 24}, pbytes_gather[5] = {0, 1, 4, 5, 20};
+    static const int pbytes_scatter[5] = {0, 1, 8, 9, 24}, pbytes_gather[5] = {0, 1, 2, 3, 18};
     info->bytes_per_half_edge = s->force_mode == LSM_FORCE_GATHER ? (s->nbr16 && s->gather_variant == 2 ? 2 : 4) + pbytes_gather[s->pm] : 8 + pbytes_scatter[s->pm];
     info->gather_variant = s->force_mode == LSM_FORCE_GATHER ? s->gather_variant : 0;
     info->pipeline_stages = s->gather_variant == 2 ? s->L.stages : 0;

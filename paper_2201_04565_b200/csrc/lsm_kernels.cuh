@@ -11,8 +11,10 @@
 //     nbr[E] int32 neighbour id; a padding slot or a dead spring holds the particle's OWN id (a spring never joins a
 //     particle to itself): its gather is legal, gives r = 0 and therefore contributes nothing, with no validity test,
 //     sid[E] caller spring id (cold: read only when a spring breaks or sits within one fp32 ulp of rc),
-//     per-slot parameters by ParamMode: typ[E] uint8, thr[E] uint32 = (high word of rc*rc) - 1 (a conservative integer
-//     filter on r^2; anything above it is decided by the exact fp64 rcS[sid], so the decision is the fp64 one), kF/r0F[E].
+//     per-slot parameters by ParamMode: typ[E] uint8, thr[E] uint16 = 16-bit code of (high word of rc*rc) - 1 (a
+//     conservative integer filter on r^2; anything above it is decided by the exact fp64 rcS[sid]: the decision is the
+//     fp64 one), kF/r0F[E].  nbr16[E] int16: the neighbour list again as offsets (neighbour - self), streamed instead
+//     of nbr when every offset fits in 16 bits.
 //     Slot s of lane l of slice S is entry (off[S] + s)*32 + l  -> every slot load is one coalesced 128-byte line, and
 //     the slots of one tile are one contiguous range per array -> one bulk async copy per array per tile.
 //     Rows are ordered by ascending caller spring id, so a particle sums its springs in the oracle's order.
@@ -61,7 +63,9 @@ struct GroupTab {
 struct SpringParams {  // parameter encoding shared by the gather (per half-edge) and scatter (per spring) layouts
     const uint8_t *typ;
     const double *kF, *r0F, *rcF;      // rcF: scatter layout only
-    const uint32_t *thr;               // gather layout: breakage filter per half-edge, (high word of rc*rc) - 1
+    const uint16_t *thr;               // gather layout: breakage filter per half-edge, 16 bits: the filter word
+                                       // (high word of rc*rc) - 1 is thr_base + (thr[e] << thr_shift), rounded down
+    uint32_t thr_base, thr_shift;
     const double *rcS;                 // gather layout: exact rc per spring, caller numbering
     const double *tab;  // scatter: [ntypes][3] = k, r0, rc;  gather: [ntypes][kTabStride] (see kTabStride)
     int ntypes;
@@ -242,7 +246,7 @@ __device__ __forceinline__ void particle_update(const StepParams &P, const StepV
 struct RowSrc {            // where one particle's row lives: pointers already offset to (slice offset)*32 + lane
     const int32_t *nbr;    // slot s at nbr[s*32]  (global memory, or the staged shared-memory copy)
     const int16_t *nbr16;  // I16: the staged copy holds 16-bit offsets (neighbour - self) instead
-    const uint32_t *thr;
+    const uint16_t *thr;
     const uint8_t *typ;
     const double *kF, *r0F;
     size_t e0;                // global entry index of slot 0 of this lane (for the cold paths)
@@ -259,6 +263,8 @@ struct RowSrc {            // where one particle's row lives: pointers already o
 // Breakage filter: thr = (high 32 bits of rc*rc) - 1.  For positive doubles the high word orders like the value, so
 // hi32(r2) < thr proves r2 < rc^2 (1 - 2^-20): alive, with one integer compare and no conversion.  Otherwise (r within
 // ~5e-7 of rc, relatively) the careful pass decides exactly as the oracle does: r = IEEE sqrt(r2) > rc in fp64.
+// A per-spring rc streams the word in 16 bits: thr_base + (t << thr_shift) rounded down (the shift is chosen at create
+// from the spread of rc: 2-5 bits for rc within one binade, i.e. a filter still 1e-5 fine) -- coarser, never wrong.
 template <int PM> __device__ __forceinline__ void slot_params(const StepParams &P, const RowSrc &R, const double *s_tab, unsigned so,
                                                               double &k, double &r0, double &kr0, uint32_t &thr) {
     if (PM == PM_UNIFORM) { k = P.sp.k_u; r0 = P.sp.r0_u; kr0 = P.sp.kr0_u; thr = P.sp.thr_u; }
@@ -268,13 +274,13 @@ template <int PM> __device__ __forceinline__ void slot_params(const StepParams &
         k = kk.x; kr0 = kk.y; r0 = s_tab[kTabStride * t + 3];
         thr = reinterpret_cast<const uint32_t *>(s_tab)[2 * (kTabStride * t + 2)];
     }
-    else if (PM == PM_RCF) { k = P.sp.k_u; r0 = P.sp.r0_u; kr0 = P.sp.kr0_u; thr = R.thr[so]; }
+    else if (PM == PM_RCF) { k = P.sp.k_u; r0 = P.sp.r0_u; kr0 = P.sp.kr0_u; thr = P.sp.thr_base + ((uint32_t)R.thr[so] << P.sp.thr_shift); }
     else if (PM == PM_KRT_RCF) {
         const int t = R.typ[so];
         const double2 kk = *reinterpret_cast<const double2 *>(s_tab + kTabStride * t);
-        k = kk.x; kr0 = kk.y; r0 = s_tab[kTabStride * t + 3]; thr = R.thr[so];
+        k = kk.x; kr0 = kk.y; r0 = s_tab[kTabStride * t + 3]; thr = P.sp.thr_base + ((uint32_t)R.thr[so] << P.sp.thr_shift);
     }
-    else { k = R.kF[so]; r0 = R.r0F[so]; kr0 = k * r0; thr = R.thr[so]; }
+    else { k = R.kF[so]; r0 = R.r0F[so]; kr0 = k * r0; thr = P.sp.thr_base + ((uint32_t)R.thr[so] << P.sp.thr_shift); }
 }
 
 // Position of neighbour j.  Always a global load (every position was just streamed in by some CTA, so these are
@@ -518,7 +524,7 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
                     if (u > 0) mbar_wait(empty + s, (u - 1) & 1);
                     constexpr unsigned kIdB = I16 ? 2 : 4;   // bytes per streamed neighbour id
                     unsigned bytes = 2 * kTile * 16 + kTile + 64 + ns * (kSlice * kIdB);
-                    if (kHasThr) bytes += ns * (kSlice * 4);
+                    if (kHasThr) bytes += ns * (kSlice * 2);
                     if (kHasTyp) bytes += ns * kSlice;
                     if (kHasKR) bytes += 2 * ns * (kSlice * 8);
                     unsigned char *b = stage0 + (size_t)s * L.bytes;
@@ -539,7 +545,7 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
                         if (P.l2 & 2) {
                             if (I16) bulk_g2s_hint(b + L.nbr, P.nbr16 + e, ns * (kSlice * 2), full + s, pol_stream);
                             else bulk_g2s_hint(b + L.nbr, P.nbr + e, ns * (kSlice * 4), full + s, pol_stream);
-                            if (kHasThr) bulk_g2s_hint(b + L.thr, P.sp.thr + e, ns * (kSlice * 4), full + s, pol_stream);
+                            if (kHasThr) bulk_g2s_hint(b + L.thr, P.sp.thr + e, ns * (kSlice * 2), full + s, pol_stream);
                             if (kHasTyp) bulk_g2s_hint(b + L.typ, P.sp.typ + e, ns * kSlice, full + s, pol_stream);
                             if (kHasKR) {
                                 bulk_g2s_hint(b + L.kF, P.sp.kF + e, ns * (kSlice * 8), full + s, pol_stream);
@@ -548,7 +554,7 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
                         } else {
                             if (I16) bulk_g2s(b + L.nbr, P.nbr16 + e, ns * (kSlice * 2), full + s);
                             else bulk_g2s(b + L.nbr, P.nbr + e, ns * (kSlice * 4), full + s);
-                            if (kHasThr) bulk_g2s(b + L.thr, P.sp.thr + e, ns * (kSlice * 4), full + s);
+                            if (kHasThr) bulk_g2s(b + L.thr, P.sp.thr + e, ns * (kSlice * 2), full + s);
                             if (kHasTyp) bulk_g2s(b + L.typ, P.sp.typ + e, ns * kSlice, full + s);
                             if (kHasKR) {
                                 bulk_g2s(b + L.kF, P.sp.kF + e, ns * (kSlice * 8), full + s);
@@ -583,7 +589,7 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
                 RowSrc R;
                 R.nbr = reinterpret_cast<const int32_t *>(b + L.nbr) + rel;
                 R.nbr16 = reinterpret_cast<const int16_t *>(b + L.nbr) + rel;
-                R.thr = reinterpret_cast<const uint32_t *>(b + L.thr) + rel;
+                R.thr = reinterpret_cast<const uint16_t *>(b + L.thr) + rel;
                 R.typ = (b + L.typ) + rel;
                 R.kF = reinterpret_cast<const double *>(b + L.kF) + rel;
                 R.r0F = reinterpret_cast<const double *>(b + L.r0F) + rel;
@@ -797,7 +803,7 @@ struct CompactParams {
     int32_t *nbr, *sid;
     int16_t *nbr16;
     uint8_t *typ;
-    uint32_t *thr;
+    uint16_t *thr;
     double *kF, *r0F;
     long long nslices;
 };
