@@ -595,7 +595,9 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
                 R.r0F = reinterpret_cast<const double *>(b + L.r0F) + rel;
                 R.e0 = (size_t)h->off[wi] * kSlice + lane;
                 double fx = 0.0, fy = 0.0, uu = 0.0;
+#ifndef LSM_DEBUG_NOFORCE   // tuning probe only: skip the spring evaluation to expose the copy pipeline's own ceiling
                 row_forces<PM, EXACT, SAMPLE, MULTI, I16>(P, V, R, s_tab, (int)p, w, xp, fx, fy, uu);
+#endif
                 const double2 vh = reinterpret_cast<const double2 *>(b + L.vel)[tid];
                 const uint8_t g = (b + L.grp)[tid];
                 if (MULTI && M.resident)
