@@ -310,14 +310,16 @@ __device__ __forceinline__ void slot_eval(double2 xq, double2 xp, bool lower, do
         if (SAMPLE) ue = mul<true>(mul<true>(mul<true>(0.5, k), ext), ext);
         live = r2 > 0.0;
     } else {
-        const double rinv = rsqrt_fast(r2);
+        // r2 + 1e-300 is r2 itself for every r2 above 1e-284; at r2 = 0 (padding / dead slot or coincident endpoints)
+        // it makes 1/r a finite 1e150, so g is finite and g * dx = g * 0 = 0: no select needed on the hot path.
+        const double rinv = rsqrt_fast(r2 + 1e-300);
         g = fma(-kr0, rinv, k);              // k (r - r0) / r = k - k r0 / r
         if (SAMPLE) { const double ext = fma(r2, rinv, -r0); ue = (0.5 * k) * ext * ext; }
-        live = hi >= 0x00100000u;            // r2 zero (or denormal: treated as coincident)
+        live = hi >= 0x00100000u;            // r2 zero (or denormal: treated as coincident); SAMPLE and the filter only
     }
-    g = live ? g : 0.0;
+    if (EXACT) g = live ? g : 0.0;
     if (SAMPLE) ue = (live && lower) ? ue : 0.0;  // energy counted once, by the lower endpoint (Eq. 1)
-    near = live && hi >= thr;
+    near = EXACT ? (live && hi >= thr) : (hi >= thr);   // fast: thr is far above the high word of a zero r2
 }
 
 template <int PM, bool EXACT, bool SAMPLE, bool COHERENT, bool I16, int CH>
