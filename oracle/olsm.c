@@ -13,6 +13,8 @@
  *   olsm_step()   velocity Verlet, Eq. 3-5 (L64-L74), in the half-step-velocity form the paper says it uses (L76):
  *                 kick - drift - force - kick; boundary displacement applied first (L88).
  *   samples       U and KE (L113), boundary reaction sums and broken count (BASELINE.json north_star item 4).
+ *   olsm_read_virial()  per-particle virial stress, Eq. 7 (L147), pinned by P13 (virial = Cauchy stress in a homogeneous
+ *                 static state; kinetic term; sum over particles = sum over springs of g d (x) d).
  * Readings where the paper is silent are those of SURVEY.md 8(c) / DESIGN.md "Readings" (Q1..Q20), named inline.
  *
  * Pins (tests/test_oracle_pins.py, all run without a GPU): P1 paper's worked oscillator example (L123-L127) against
@@ -319,6 +321,32 @@ int32_t olsm_read_energy(const olsm_sim *s, double *U, double *KE)
             }
             KE[b] = ke;
         }
+    }
+    return 0;
+}
+
+/* Per-particle virial, Eq. 7 without the 1/Omega factor (the caller divides by a volume):
+ *   S^k_ij = 1/2 sum_l (x^l_i - x^k_i) f^kl_j  -  m^k v^k_i v^k_j ,   f^kl = force on k from its spring to l (Eq. 2).
+ * Serial loop over the alive springs in caller order; out[k] = {S_xx, S_yy, S_xy} (2-D, symmetric: central forces).
+ * Tension is positive.  Broken springs and coincident endpoints contribute nothing (Q3, Q4). */
+int32_t olsm_read_virial(const olsm_sim *s, double *out)
+{
+    if (!s || !out || s->D != 2) return -1;
+    for (int64_t q = 0; q < 3 * s->N; ++q) out[q] = 0.0;
+    for (int64_t e = 0; e < s->M; ++e) {
+        if (!s->alive[e]) continue;
+        const int64_t i = s->si[e], j = s->sj[e];
+        const double dx = s->x[2 * j] - s->x[2 * i], dy = s->x[2 * j + 1] - s->x[2 * i + 1];
+        const double r = sqrt(dx * dx + dy * dy);
+        if (r == 0.0) continue;
+        const double g = s->k[e] * (r - s->r0[e]) / r;      /* f^ij = g d,  f^ji = -g (-d): same dyad on both ends */
+        const double h = 0.5 * g;
+        out[3 * i] += h * dx * dx; out[3 * i + 1] += h * dy * dy; out[3 * i + 2] += h * dx * dy;
+        out[3 * j] += h * dx * dx; out[3 * j + 1] += h * dy * dy; out[3 * j + 2] += h * dx * dy;
+    }
+    for (int64_t p = 0; p < s->N; ++p) {
+        const double vx = s->v[2 * p], vy = s->v[2 * p + 1];
+        out[3 * p] -= s->m[p] * vx * vx; out[3 * p + 1] -= s->m[p] * vy * vy; out[3 * p + 2] -= s->m[p] * vx * vy;
     }
     return 0;
 }

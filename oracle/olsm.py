@@ -45,6 +45,7 @@ def lib():
         L.olsm_read_forces.argtypes = [C.c_void_p, d]
         L.olsm_read_broken.argtypes = [C.c_void_p, u8, i64, i64]
         L.olsm_read_energy.argtypes = [C.c_void_p, d, d]
+        L.olsm_read_virial.argtypes = [C.c_void_p, d]
         L.olsm_read_stress.argtypes = [C.c_void_p, C.c_int64, i64, i64, d, d, d, i64]
         L.olsm_n_samples.restype = C.c_int64
         L.olsm_n_samples.argtypes = [C.c_void_p]
@@ -129,6 +130,13 @@ class OracleSim:
         U = np.empty(self.B); KE = np.empty(self.B)
         lib().olsm_read_energy(self._h, _p(U, C.c_double), _p(KE, C.c_double))
         return U, KE
+
+    def read_virial(self):
+        """Per-particle virial (Eq. 7 without 1/Omega): [N,3] = S_xx, S_yy, S_xy."""
+        S = np.empty((self.N, 3))
+        if lib().olsm_read_virial(self._h, _p(S, C.c_double)) != 0:
+            raise ValueError("olsm_read_virial failed")
+        return S
 
     @property
     def current_step(self):

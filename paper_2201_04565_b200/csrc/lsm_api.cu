@@ -66,7 +66,7 @@ struct lsm_sim {
     double *rcS = nullptr;
     int gather_variant = 0;          // resolved: 1 direct, 2 streamed
     StageLayout L;
-    int stream_smem = 0, stream_grid = 0;
+    int stream_smem = 0, stream_grid = 0, stream_ctas_per_sm = 0;
     uint32_t max_tile_slots = 0;
     int l2_hints = 0;
     int multi_on = 0;                // fuse runs of plain time steps into one cooperative launch
@@ -232,11 +232,14 @@ template <bool EXACT> void launch_gather_pm(int pm, const StepParams &P, Variant
     }
 }
 
-template <class K> void stream_opt_in(K kern, const lsm_sim *s, int &configured_for) {
-    if (configured_for < s->stream_smem) {   // opt in to > 48 KB of dynamic shared memory once per kernel
-        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, s->stream_smem);
-        configured_for = s->stream_smem;
-    }
+// Opt a kernel in to > 48 KB of dynamic shared memory.  The attribute is per device: remembered per device ordinal.
+constexpr int kMaxDevices = 64;
+struct OptIn { int bytes[kMaxDevices]; OptIn() { for (int &b : bytes) b = -1; } };
+template <class K> void stream_opt_in(K kern, const lsm_sim *s, OptIn &done) {
+    int &have = done.bytes[s->device < kMaxDevices ? s->device : kMaxDevices - 1];
+    if (have < s->stream_smem || s->device >= kMaxDevices - 1) {
+        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, s->stream_smem) == cudaSuccess) have = s->stream_smem;
+    }   // a failure shows up as a launch error, which the callers check
 }
 
 template <int PM, bool EXACT, bool KICK2, bool ADVANCE, bool SAMPLE> void launch_stream_one(const lsm_sim *s, const StepParams &P) {
@@ -244,12 +247,12 @@ template <int PM, bool EXACT, bool KICK2, bool ADVANCE, bool SAMPLE> void launch
     std::memset(&M, 0, sizeof(M));
     if (s->nbr16) {
         auto kern = k_gather_stream<PM, EXACT, KICK2, ADVANCE, SAMPLE, false, true>;
-        static thread_local int configured_for = -1;
+        static thread_local OptIn configured_for;
         stream_opt_in(kern, s, configured_for);
         kern<<<s->stream_grid, kTile + 32, s->stream_smem, s->stream>>>(P, s->L, M);
     } else {
         auto kern = k_gather_stream<PM, EXACT, KICK2, ADVANCE, SAMPLE, false, false>;
-        static thread_local int configured_for = -1;
+        static thread_local OptIn configured_for;
         stream_opt_in(kern, s, configured_for);
         kern<<<s->stream_grid, kTile + 32, s->stream_smem, s->stream>>>(P, s->L, M);
     }
@@ -259,14 +262,16 @@ template <int PM, bool EXACT, bool KICK2, bool ADVANCE, bool SAMPLE> void launch
 template <int PM, bool EXACT> cudaError_t launch_stream_multi_one(const lsm_sim *s, StepParams P, MultiParams M) {
     StageLayout L = s->L;
     void *args[3] = {&P, &L, &M};
+    // (a grid the device cannot keep resident makes cudaLaunchCooperativeKernel fail with
+    //  cudaErrorCooperativeLaunchTooLarge instead of deadlocking at the grid barrier; lsm_step reports it)
     if (s->nbr16) {
         auto kern = k_gather_stream<PM, EXACT, true, true, false, true, true>;
-        static thread_local int configured_for = -1;
+        static thread_local OptIn configured_for;
         stream_opt_in(kern, s, configured_for);
         return cudaLaunchCooperativeKernel((const void *)kern, dim3(s->stream_grid), dim3(kTile + 32), args, (size_t)s->stream_smem, s->stream);
     }
     auto kern = k_gather_stream<PM, EXACT, true, true, false, true, false>;
-    static thread_local int configured_for = -1;
+    static thread_local OptIn configured_for;
     stream_opt_in(kern, s, configured_for);
     return cudaLaunchCooperativeKernel((const void *)kern, dim3(s->stream_grid), dim3(kTile + 32), args, (size_t)s->stream_smem, s->stream);
 }
@@ -739,6 +744,7 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
             if (s->gather_variant == 2 && !can_stream) return fail(s, LSM_E_UNSUPPORTED, "gather_variant = streamed: a tile's rows do not fit in shared memory (degree too high); use the direct variant");
             s->stream_smem = L.first + L.stages * L.bytes;
             s->stream_grid = (int)std::min<long long>(T, (long long)ctas_per_sm * n_sm);
+            s->stream_ctas_per_sm = ctas_per_sm;
             // step fusion (several time steps per cooperative launch): pays when a step is launch-bound, i.e. the
             // problem is L2-resident; above that the per-step grid barrier costs more than the launch gap it removes.
             int coop = 0;

@@ -336,3 +336,58 @@ def test_generators_match_paper_shapes():
     assert np.abs(d - 1.0).max() < 1e-14
     # Table 1: rc/r0 between 1.01 and 1.10; the synthetic configs stay in a comparable range
     assert 1.0 < g["t1_stiff_rc"] / g["t1_stiff_r0"] < p.rc[0] / p.r0[0] + 1e-12 <= g["t1_soft_rc"] / g["t1_soft_r0"] + 1e-12
+
+
+# ---------------------------------------------------------------- P13: per-particle virial stress (Eq. 7)
+@pytest.mark.parametrize("eps", [1e-3, 2e-2])
+def test_P13_virial_equals_cauchy_stress_in_affine_state(eps):
+    """In a homogeneous static state the virial stress of an interior particle, divided by its (deformed) cell area,
+    is the Cauchy stress: sigma_yy = the top row's reaction per unit deformed width (P3's closed form), sigma_xx = 0
+    (Poisson's ratio 1/3: the lateral contraction eps/3 is exactly the stress-free one to first order; the residual is
+    the second-order term given below), sigma_xy = 0 by symmetry."""
+    nx = ny = 32
+    kk = 1.7
+    x, si, sj, site, kind = triangular_lattice(nx, ny)
+    xa = x * np.array([1.0 - eps / 3.0, 1.0 + eps])
+    M = si.size
+    s = OracleSim(xa, si, sj, np.full(M, kk), np.ones(M), np.full(M, 2.0), 0.01)
+    S = s.read_virial()
+    row, col = site // nx, site % nx
+    interior = (row > 0) & (row < ny - 1) & (col > 0) & (col < nx - 1)
+    ax, ay = 1.0 - eps / 3.0, 1.0 + eps
+    L = np.sqrt(ax ** 2 / 4 + 3 * ay ** 2 / 4)
+    g_d, g_h = kk * (L - 1.0) / L, kk * (ax - 1.0) / ax          # k (r - r0)/r of a diagonal / a horizontal spring
+    cell = ax * SQ3_2 * ay                                        # deformed area per particle
+    # closed forms: 4 diagonal springs with d = (+-ax/2, +-sqrt3/2 ay), 2 horizontal springs with d = (+-ax, 0)
+    syy = 0.5 * 4 * g_d * (SQ3_2 * ay) ** 2
+    sxx = 0.5 * (4 * g_d * (ax / 2) ** 2 + 2 * g_h * ax ** 2)
+    assert np.allclose(S[interior, 1], syy, rtol=1e-11)
+    # sxx is a cancellation of terms of size syy; coordinates up to 32 carry ulp 7e-15, so each bond length does too
+    noise = 8 * np.finfo(float).eps * np.abs(xa).max() * kk
+    assert np.abs(S[interior, 0] - sxx).max() <= noise < 1e-9 * syy
+    assert np.abs(S[interior, 2]).max() <= noise
+    # sigma_yy = reaction of the top row per unit deformed width (the force f_y of P3 over the spacing ax)
+    f = s.read_forces()
+    top_int = (row == ny - 1) & (col > 0) & (col < nx - 1)
+    assert np.allclose(S[interior, 1] / cell, -f[top_int, 1].mean() / ax, rtol=1e-11)
+    # Poisson's ratio 1/3: sigma_xx vanishes to first order in eps (it is O(eps^2) of sigma_yy's O(eps))
+    assert abs(sxx) <= 2.0 * eps * syy
+
+
+def test_P13_virial_kinetic_term_and_sum_rule():
+    """Kinetic term -m v(x)v on a free particle without springs; and sum over particles of the static virial = sum
+    over springs of g d(x)d (each spring gives half to either end): trace = sum_s k (r - r0) r, brute force."""
+    x = np.array([[0.0, 0.0], [3.0, 0.0]])
+    v = np.array([[0.5, -2.0], [0.0, 0.0]])
+    s = OracleSim(x, [0], [1], 0.0, 1.0, 10.0, 0.01, v=v, mass=np.array([3.0, 1.0]))
+    S = s.read_virial()
+    assert np.allclose(S[0], [-3.0 * 0.25, -3.0 * 4.0, -3.0 * 0.5 * -2.0]) and np.all(S[1] == 0.0)
+    xs, si, sj, k, r0 = _random_state(7, 6, seed=5)
+    s = OracleSim(xs, si, sj, k, r0, np.full(si.size, 9.0), 0.01)
+    S = s.read_virial()
+    d = xs[sj] - xs[si]
+    r = np.sqrt((d ** 2).sum(axis=1))
+    g = k * (r - r0) / r
+    assert np.allclose(S[:, 0].sum(), (g * d[:, 0] ** 2).sum(), rtol=1e-12)
+    assert np.allclose(S[:, 2].sum(), (g * d[:, 0] * d[:, 1]).sum(), rtol=1e-11, atol=1e-14)
+    assert np.allclose((S[:, 0] + S[:, 1]).sum(), (k * (r - r0) * r).sum(), rtol=1e-12)
