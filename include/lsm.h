@@ -144,6 +144,10 @@ lsm_status lsm_write_state(lsm_sim *sim, const double *x, const double *v);
 lsm_status lsm_read_state(lsm_sim *sim, double *x /* [N*dim] or NULL */, double *v /* [N*dim] or NULL */);
 /* Spring force on every particle at the current positions (no damping term). */
 lsm_status lsm_read_forces(lsm_sim *sim, double *f /* [N*dim] */);
+/* Per-particle virial stress of the current state, Eq. 7 without the 1/Omega factor (the caller divides
+ * by a volume): S[p] = {S_xx, S_yy, S_xy} = 1/2 sum_l (x^l - x^p) (x) f^pl - m v (x) v, tension positive; broken
+ * springs contribute nothing.  Gather layout only (LSM_E_UNSUPPORTED with force_mode = SCATTER). */
+lsm_status lsm_read_virial(lsm_sim *sim, double *S /* [N*3] */);
 /* broken[s] = 1 if spring s is dead; break_step[s] = step of the force evaluation that broke it, -1 if alive. */
 lsm_status lsm_read_broken(lsm_sim *sim, uint8_t *broken /* [M] or NULL */, int64_t *break_step /* [M] or NULL */,
                            int64_t *n_broken /* scalar or NULL */);

@@ -21,7 +21,7 @@ FUSION_AUTO, FUSION_ON, FUSION_OFF = 0, 1, 2
 MAX_GROUPS = 8
 
 EXPORTS = ["lsm_create", "lsm_set_boundary", "lsm_step", "lsm_write_state", "lsm_read_state", "lsm_read_forces",
-           "lsm_read_broken", "lsm_read_energy", "lsm_read_stress", "lsm_compact", "lsm_sync", "lsm_get_info",
+           "lsm_read_broken", "lsm_read_energy", "lsm_read_virial", "lsm_read_stress", "lsm_compact", "lsm_sync", "lsm_get_info",
            "lsm_device_state", "lsm_last_error", "lsm_destroy", "lsm_abi_version"]
 
 _ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
@@ -85,6 +85,7 @@ def library():
         L.lsm_write_state.argtypes = [C.c_void_p, d, d]
         L.lsm_read_state.argtypes = [C.c_void_p, d, d]
         L.lsm_read_forces.argtypes = [C.c_void_p, d]
+        L.lsm_read_virial.argtypes = [C.c_void_p, d]
         L.lsm_read_broken.argtypes = [C.c_void_p, u8, i64, i64]
         L.lsm_read_energy.argtypes = [C.c_void_p, d, d]
         L.lsm_read_stress.argtypes = [C.c_void_p, C.c_int64, i64, i64, d, d, d, i64]
@@ -185,6 +186,11 @@ class LsmSim:
         f = np.empty((self.N, 2))
         self._check(library().lsm_read_forces(self._h, _ptr(f, C.c_double)))
         return f
+
+    def read_virial(self):
+        S = np.empty((self.N, 3))
+        self._check(library().lsm_read_virial(self._h, _ptr(S, C.c_double)))
+        return S
 
     def read_broken(self):
         b = np.empty(self.M, dtype=np.uint8); bs = np.empty(self.M, dtype=np.int64); n = C.c_int64(0)
@@ -316,6 +322,7 @@ def lsm_step(sim, n=1): return sim.step(n)
 def lsm_write_state(sim, x, v=None): return sim.write_state(x, v)
 def lsm_read_state(sim, out_x=None, out_v=None): return sim.read_state(out_x, out_v)
 def lsm_read_forces(sim): return sim.read_forces()
+def lsm_read_virial(sim): return sim.read_virial()
 def lsm_read_broken(sim): return sim.read_broken()
 def lsm_read_energy(sim): return sim.read_energy()
 def lsm_read_stress(sim, capacity=None): return sim.read_stress(capacity)

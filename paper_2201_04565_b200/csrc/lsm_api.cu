@@ -69,6 +69,7 @@ struct lsm_sim {
     int stream_smem = 0, stream_grid = 0, stream_ctas_per_sm = 0;
     uint32_t max_tile_slots = 0;
     int l2_hints = 0;
+    double *virial = nullptr;        // [N][3] output buffer of lsm_read_virial (allocated on first use)
     int multi_on = 0;                // fuse runs of plain time steps into one cooperative launch
     long long multi_max = 4096;
     unsigned long long *gbar = nullptr, gbar_base = 0;
@@ -1018,6 +1019,23 @@ lsm_status lsm_read_forces(lsm_sim *s, double *f) {
     k_to_caller<<<grid_for(s->N), kBlock, 0, s->stream>>>(s->f, s->stage[0], s->d_inv, s->N, s->grp, group_tab(s), s->dt, 0);
     s->kernels_launched += 1;
     CUDA_TRY(s, cudaMemcpyAsync(f, s->stage[0], sizeof(double2) * s->N, cudaMemcpyDeviceToHost, s->stream));
+    return check_flags(s);
+}
+
+lsm_status lsm_read_virial(lsm_sim *s, double *S) {
+    CHECK_SIM(s);
+    if (!S) { s->err = "S is NULL"; return LSM_E_INVALID; }
+    if (s->force_mode != LSM_FORCE_GATHER) { s->err = "lsm_read_virial needs the gather layout"; return LSM_E_UNSUPPORTED; }
+    if (!s->virial) TRY(dev_alloc(s, &s->virial, (size_t)s->N * 3));
+    VirialParams V;
+    std::memset(&V, 0, sizeof(V));
+    const StepParams P = step_params(s, s->step);
+    V.pos = s->pos[s->cur]; V.vel = s->vel; V.grp = s->grp; V.mass = s->mass; V.mass_u = s->mass_u; V.dt = s->dt;
+    V.hdr = s->hdr; V.nbr = s->nbr; V.sp = P.sp; V.pm = s->pm; V.inv = s->d_inv; V.N = s->N; V.g = P.g; V.out = s->virial;
+    k_virial<<<grid_for(s->N), kBlock, 0, s->stream>>>(V);
+    s->kernels_launched += 1;
+    CUDA_TRY(s, cudaGetLastError());
+    CUDA_TRY(s, cudaMemcpyAsync(S, s->virial, sizeof(double) * 3 * s->N, cudaMemcpyDeviceToHost, s->stream));
     return check_flags(s);
 }
 

@@ -845,6 +845,61 @@ __global__ void __launch_bounds__(kBlock) k_compact_ell(const CompactParams C) {
     if (lane == 0) h->w[wi] = (uint8_t)wmax;
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// Per-particle virial stress, Eq. 7 without 1/Omega:  S^k = 1/2 sum_l (x^l - x^k) (x) f^kl - m v (x) v,
+// f^kl = g d (Eq. 2).  One thread per particle in CALLER numbering, reading its row of the gather layout (master
+// 32-bit ids; a slot holding the own id is padding or a dead spring).  IEEE sqrt / divide: this is an output pass,
+// not the step.  out[c] = {S_xx, S_yy, S_xy}.
+// ---------------------------------------------------------------------------------------------------------------
+struct VirialParams {
+    const double2 *pos, *vel;
+    const uint8_t *grp;
+    const double *mass;
+    double mass_u, dt;
+    const TileHdr *hdr;
+    const int32_t *nbr;
+    SpringParams sp;
+    int pm;
+    const int32_t *inv;   // caller id -> internal id, or NULL
+    long long N;
+    GroupTab g;
+    double *out;          // [N][3]
+};
+
+__global__ void __launch_bounds__(kBlock) k_virial(const VirialParams V) {
+    const long long c = (long long)blockIdx.x * kBlock + threadIdx.x;
+    if (c >= V.N) return;
+    const int p = V.inv ? V.inv[c] : (int)c;
+    const TileHdr *h = V.hdr + (p >> 8);
+    const int wi = (p >> 5) & 7, lane = p & 31;
+    const unsigned w = h->w[wi];
+    const size_t e0 = (size_t)h->off[wi] * kSlice + lane;
+    const double2 xp = V.pos[p];
+    double sxx = 0.0, syy = 0.0, sxy = 0.0;
+    for (unsigned s = 0; s < w; ++s) {
+        const size_t e = e0 + (size_t)s * kSlice;
+        const int nb = V.nbr[e];
+        if (nb == p) continue;
+        double k, r0;
+        if (V.pm == PM_UNIFORM || V.pm == PM_RCF) { k = V.sp.k_u; r0 = V.sp.r0_u; }
+        else if (V.pm == PM_TYPED || V.pm == PM_KRT_RCF) { const int t = V.sp.typ[e]; k = V.sp.tab[kTabStride * t]; r0 = V.sp.tab[kTabStride * t + 3]; }
+        else { k = V.sp.kF[e]; r0 = V.sp.r0F[e]; }
+        const double2 xq = V.pos[nb];
+        const double dx = xq.x - xp.x, dy = xq.y - xp.y;
+        const double r = sqrt(dx * dx + dy * dy);
+        if (r == 0.0) continue;
+        const double hg = 0.5 * (k * (r - r0) / r);
+        sxx += hg * dx * dx; syy += hg * dy * dy; sxy += hg * dx * dy;
+    }
+    double2 v = V.vel[p];
+    const uint8_t gg = V.grp[p];
+    if (gg != kFree) v = make_double2(V.g.dux[gg] / V.dt, V.g.duy[gg] / V.dt);   // kinematic: the slot holds the origin
+    const double m = V.mass ? V.mass[p] : V.mass_u;
+    V.out[3 * c] = sxx - m * v.x * v.x;
+    V.out[3 * c + 1] = syy - m * v.y * v.y;
+    V.out[3 * c + 2] = sxy - m * v.x * v.y;
+}
+
 // ---- small utility kernels (numbering translation at the API boundary, boundary-group bookkeeping) ----
 // dst[perm_dst[q]] <- src[q] style copies.  inv: caller id -> internal id.
 __global__ void __launch_bounds__(kBlock) k_to_caller(const double2 *src, double2 *dst, const int32_t *inv, long long N,

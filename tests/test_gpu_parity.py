@@ -480,3 +480,31 @@ def test_wide_neighbour_offsets_use_32bit_ids():
         xg, vg = g.read_state()
         assert np.abs(xg - xo).max() <= 1e-11 and np.abs(vg - vo).max() <= 1e-11
         g.close()
+
+
+# ---------------------------------------------------------------- per-particle virial stress (Eq. 7)
+@pytest.mark.parametrize("reorder", [0, 1, 2])
+def test_virial_stress_matches_oracle(reorder):
+    """lsm_read_virial against the oracle's Eq. 7 on a moving, partly fractured two-phase specimen (typed parameters,
+    broken springs, kinematic grips) and on a batch with per-spring rc; per-particle error relative to the particle's
+    own sum of |contributions| (the Q11 norm)."""
+    p = _fracture_problem(n=48, du_y=6e-4, seed=11)
+    o = OracleSim.from_problem(p); o.step(3700)
+    g = lsm_create_from_problem(p, reorder=reorder, exact=True); g.step(3700)
+    assert o.read_broken()[2] > 0 and np.array_equal(o.read_broken()[0], g.read_broken()[0])
+    So, Sg = o.read_virial(), g.read_virial()
+    x, _ = o.read_state()
+    alive = ~o.read_broken()[0]
+    d = x[p.spring_j] - x[p.spring_i]
+    r = np.sqrt((d ** 2).sum(axis=1))
+    contrib = np.where(alive, 0.5 * np.abs(p.k * (r - p.r0) / r) * r * r, 0.0)
+    scale = np.zeros(p.N); np.add.at(scale, p.spring_i, contrib); np.add.at(scale, p.spring_j, contrib)
+    floor = 8 * np.finfo(float).eps * np.abs(x).max() * p.k.max()     # bond lengths carry the coordinates' ulp
+    assert np.all(np.abs(Sg - So).max(axis=1) <= 1e-12 * scale + floor + 1e-12 * np.abs(So).max(axis=1))
+    g.close()
+    q = _perturbed(config3(n=96), 0.02, 8)
+    q.v = np.random.default_rng(2).normal(0.0, 1e-3, q.x.shape)
+    o = OracleSim.from_problem(q); g = lsm_create_from_problem(q, reorder=reorder)
+    So, Sg = o.read_virial(), g.read_virial()
+    assert np.abs(Sg - So).max() <= 1e-12 * np.abs(So).max()
+    g.close()
