@@ -68,7 +68,6 @@ struct lsm_sim {
     StageLayout L;
     int stream_smem = 0, stream_grid = 0, stream_ctas_per_sm = 0;
     uint32_t max_tile_slots = 0;
-    int l2_hints = 0;
     double *virial = nullptr;        // [N][3] output buffer of lsm_read_virial (allocated on first use)
     int multi_on = 0;                // fuse runs of plain time steps into one cooperative launch
     long long multi_max = 4096;
@@ -192,7 +191,7 @@ StepParams step_params(const lsm_sim *s, long long step) {
     P.vel = s->vel; P.f = s->f; P.fd = s->fd; P.grp = s->grp; P.mass = s->mass;
     P.mass_u = s->mass_u; P.inv_mass_u = 1.0 / s->mass_u;
     P.dt = s->dt; P.hdt = 0.5 * s->dt; P.gamma = s->gamma;
-    P.N = s->N; P.step = step; P.l2 = s->l2_hints;
+    P.N = s->N; P.step = step;
     P.hdr = s->hdr; P.T = s->T; P.nbr = s->nbr; P.nbr16 = s->nbr16; P.sid = s->sid;
     P.sp.typ = s->typ; P.sp.kF = s->kF; P.sp.r0F = s->r0F; P.sp.rcF = s->rcF; P.sp.tab = s->tab; P.sp.ntypes = s->ntypes;
     P.sp.thr = s->thr; P.sp.thr_base = s->thr_base; P.sp.thr_shift = s->thr_shift; P.sp.rcS = s->rcS; P.sp.kr0_u = s->k_u * s->r0_u; P.sp.thr_u = thr_of(s->rc_u);
@@ -736,7 +735,6 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
             CUDA_TRY(s, cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, d->device));
             int ctas_per_sm = kStreamMinB, max_stages = 4;
             if (const char *e = std::getenv("LSM_STREAM_CTAS_PER_SM")) ctas_per_sm = std::max(1, std::min(4, std::atoi(e)));   // tuning overrides
-            if (const char *e = std::getenv("LSM_L2_HINTS")) s->l2_hints = std::atoi(e) & 3;
             if (const char *e = std::getenv("LSM_STREAM_STAGES")) max_stages = std::max(2, std::min<int>(kMaxStages, std::atoi(e)));
             const int budget = std::min(dev_smem, (dev_smem + 1024) / ctas_per_sm - 1024) - L.first;   // 1 KB reserved per CTA
             L.stages = std::min<int>(max_stages, budget / std::max(L.bytes, 1));

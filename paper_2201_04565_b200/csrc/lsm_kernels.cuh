@@ -89,7 +89,6 @@ struct StepParams {
     double dt, hdt, gamma;
     long long N;
     long long step;  // step number of THIS force evaluation (stamped on springs that break in it)
-    int l2;          // L2 residency hint bits (see l2_policy_*)
     // gather layout
     const TileHdr *hdr;
     long long T;  // tiles
@@ -106,29 +105,6 @@ struct StepParams {
     double *sU, *sKE;
     GroupTab g;
 };
-
-// ---- L2 residency hints (sm_80+ createpolicy): positions are re-read by the next step and gathered ~6x, the other
-// streams are touched once per step.  P.l2 bit 0: positions evict_last; bit 1: one-pass streams evict_first.
-__device__ __forceinline__ uint64_t l2_policy_evict_last() {
-    uint64_t pol; asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol)); return pol;
-}
-__device__ __forceinline__ uint64_t l2_policy_evict_first() {
-    uint64_t pol; asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol)); return pol;
-}
-__device__ __forceinline__ void st_hint(double2 *p, double2 v, uint64_t pol) {
-    asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1, %2}, %3;" ::"l"(p), "d"(v.x), "d"(v.y), "l"(pol) : "memory");
-}
-__device__ __forceinline__ double2 ldg_hint(const double2 *p, uint64_t pol) {
-    double2 v;
-    asm volatile("ld.global.nc.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(pol));
-    return v;
-}
-__device__ __forceinline__ void store_pos(double2 *p, double2 v, int l2) {
-    if (l2 & 1) st_hint(p, v, l2_policy_evict_last()); else *p = v;
-}
-__device__ __forceinline__ void store_stream(double2 *p, double2 v, int l2) {
-    if (l2 & 2) st_hint(p, v, l2_policy_evict_first()); else *p = v;
-}
 
 // ---- arithmetic: EXACT = IEEE sqrt / divide and never-contracted multiply-add (mirrors gcc -ffp-contract=off) ----
 template <bool E> __device__ __forceinline__ double mul(double a, double b) { return E ? __dmul_rn(a, b) : a * b; }
@@ -214,8 +190,8 @@ __device__ __forceinline__ void particle_update(const StepParams &P, const StepV
                 w.x = mad<EXACT>(P.hdt, ax, v.x); w.y = mad<EXACT>(P.hdt, ay, v.y);      // Eq. 5, first half
             }
             xn.x = mad<EXACT>(P.dt, w.x, xp.x); xn.y = mad<EXACT>(P.dt, w.y, xp.y);      // Eq. 3
-            store_pos(V.pos_next + p, xn, P.l2);
-            store_stream(P.vel + p, w, P.l2);
+            V.pos_next[p] = xn;
+            P.vel[p] = w;
             if (own_pos) { *own_pos = xn; *own_vel = w; }   // resident tiles: the staged copy is the next step's input
         } else {
             P.vel[p] = v;
@@ -227,7 +203,7 @@ __device__ __forceinline__ void particle_update(const StepParams &P, const StepV
         if (ADVANCE) {
             const double ns = (double)(V.step + 1 - P.g.n0[g]);
             const double2 xn = make_double2(mad<EXACT>(ns, P.g.dux[g], vh.x), mad<EXACT>(ns, P.g.duy[g], vh.y));
-            store_pos(V.pos_next + p, xn, P.l2);
+            V.pos_next[p] = xn;
             if (own_pos) *own_pos = xn;
         } else {
             P.fd[p] = make_double2(fx, fy);
@@ -438,8 +414,9 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity) {
     const uint32_t a = smem_u32(bar);
     uint32_t ok;
     do {
-        asm volatile("{\n\t.reg .pred q;\n\tmbarrier.try_wait.parity.shared::cta.b64 q, [%1], %2;\n\tselp.u32 %0, 1, 0, q;\n\t}"
-                     : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+        // the suspend-time hint (ns) lets the hardware park the thread until the phase completes instead of re-polling
+        asm volatile("{\n\t.reg .pred q;\n\tmbarrier.try_wait.parity.shared::cta.b64 q, [%1], %2, %3;\n\tselp.u32 %0, 1, 0, q;\n\t}"
+                     : "=r"(ok) : "r"(a), "r"(parity), "r"(0x989680u) : "memory");
     } while (!ok);
 }
 __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned bytes, uint64_t *bar) {
@@ -447,10 +424,6 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned by
                  ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
-__device__ __forceinline__ void bulk_g2s_hint(void *dst, const void *src, unsigned bytes, uint64_t *bar, uint64_t pol) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
-                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(pol) : "memory");
-}
 struct StageLayout {      // byte offsets of the staged arrays inside one pipeline stage (all multiples of 128)
     int pos, vel, hdr, grp, nbr, thr, typ, kF, r0F;
     int bytes;            // stage size
@@ -504,7 +477,6 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
     if (wi == kTileSlices) {  // ---------------- producer warp ----------------
         if (lane == 0) {
             int s = 0; unsigned u = 0;
-            const uint64_t pol_keep = l2_policy_evict_last(), pol_stream = l2_policy_evict_first();
             for (int it = 0; it < nsteps; ++it) {
                 const double2 *pos_cur = MULTI ? ((it & 1) ? M.pos_b : M.pos_a) : P.pos_cur;
                 if (MULTI && it > 0) {  // grid barrier: every CTA has finished (and published) step it-1
@@ -531,37 +503,19 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
                     if (kHasKR) bytes += 2 * ns * (kSlice * 8);
                     unsigned char *b = stage0 + (size_t)s * L.bytes;
                     mbar_expect_tx(full + s, bytes);
-                    if (P.l2 & 1) bulk_g2s_hint(b + L.pos, pos_cur + t * kTile, kTile * 16, full + s, pol_keep);
-                    else bulk_g2s(b + L.pos, pos_cur + t * kTile, kTile * 16, full + s);
-                    if (P.l2 & 2) {
-                        bulk_g2s_hint(b + L.vel, P.vel + t * kTile, kTile * 16, full + s, pol_stream);
-                        bulk_g2s_hint(b + L.grp, P.grp + t * kTile, kTile, full + s, pol_stream);
-                        bulk_g2s_hint(b + L.hdr, h, 64, full + s, pol_stream);
-                    } else {
-                        bulk_g2s(b + L.vel, P.vel + t * kTile, kTile * 16, full + s);
-                        bulk_g2s(b + L.grp, P.grp + t * kTile, kTile, full + s);
-                        bulk_g2s(b + L.hdr, h, 64, full + s);
-                    }
+                    bulk_g2s(b + L.pos, pos_cur + t * kTile, kTile * 16, full + s);
+                    bulk_g2s(b + L.vel, P.vel + t * kTile, kTile * 16, full + s);
+                    bulk_g2s(b + L.grp, P.grp + t * kTile, kTile, full + s);
+                    bulk_g2s(b + L.hdr, h, 64, full + s);
                     if (ns) {
                         const size_t e = (size_t)o0 * kSlice;
-                        if (P.l2 & 2) {
-                            if (I16) bulk_g2s_hint(b + L.nbr, P.nbr16 + e, ns * (kSlice * 2), full + s, pol_stream);
-                            else bulk_g2s_hint(b + L.nbr, P.nbr + e, ns * (kSlice * 4), full + s, pol_stream);
-                            if (kHasThr) bulk_g2s_hint(b + L.thr, P.sp.thr + e, ns * (kSlice * 2), full + s, pol_stream);
-                            if (kHasTyp) bulk_g2s_hint(b + L.typ, P.sp.typ + e, ns * kSlice, full + s, pol_stream);
-                            if (kHasKR) {
-                                bulk_g2s_hint(b + L.kF, P.sp.kF + e, ns * (kSlice * 8), full + s, pol_stream);
-                                bulk_g2s_hint(b + L.r0F, P.sp.r0F + e, ns * (kSlice * 8), full + s, pol_stream);
-                            }
-                        } else {
-                            if (I16) bulk_g2s(b + L.nbr, P.nbr16 + e, ns * (kSlice * 2), full + s);
-                            else bulk_g2s(b + L.nbr, P.nbr + e, ns * (kSlice * 4), full + s);
-                            if (kHasThr) bulk_g2s(b + L.thr, P.sp.thr + e, ns * (kSlice * 2), full + s);
-                            if (kHasTyp) bulk_g2s(b + L.typ, P.sp.typ + e, ns * kSlice, full + s);
-                            if (kHasKR) {
-                                bulk_g2s(b + L.kF, P.sp.kF + e, ns * (kSlice * 8), full + s);
-                                bulk_g2s(b + L.r0F, P.sp.r0F + e, ns * (kSlice * 8), full + s);
-                            }
+                        if (I16) bulk_g2s(b + L.nbr, P.nbr16 + e, ns * (kSlice * 2), full + s);
+                        else bulk_g2s(b + L.nbr, P.nbr + e, ns * (kSlice * 4), full + s);
+                        if (kHasThr) bulk_g2s(b + L.thr, P.sp.thr + e, ns * (kSlice * 2), full + s);
+                        if (kHasTyp) bulk_g2s(b + L.typ, P.sp.typ + e, ns * kSlice, full + s);
+                        if (kHasKR) {
+                            bulk_g2s(b + L.kF, P.sp.kF + e, ns * (kSlice * 8), full + s);
+                            bulk_g2s(b + L.r0F, P.sp.r0F + e, ns * (kSlice * 8), full + s);
                         }
                     }
                     if (++s == L.stages) { s = 0; ++u; }
