@@ -159,6 +159,15 @@ lsm_status lsm_read_energy(lsm_sim *sim, double *U /* [B] or NULL */, double *KE
 lsm_status lsm_read_stress(lsm_sim *sim, int64_t capacity, int64_t *n_samples, int64_t *step, double *reaction,
                            double *U, double *KE, int64_t *n_broken);
 
+/* Quasi-static driver for the paper's fracture protocol ("termination check each step", L143 grips
+ * displaced apart): advance in chunks that end on sample steps until, for EVERY specimen, the reaction |R[group][axis]|
+ * has fallen below stop_fraction (in [0,1)) of that specimen's own running peak (Q20), or max_steps have been
+ * taken.  Needs sample_every > 0.  steps_done: steps taken by this call; failed: 1 if the criterion fired;
+ * peak[B], peak_step[B]: the peak reaction magnitude seen during this call and its step (any may be NULL).  The samples
+ * stay in the history ring for lsm_read_stress (the ring keeps the newest history_capacity of them). */
+lsm_status lsm_run_to_failure(lsm_sim *sim, int64_t max_steps, int32_t group, int32_t axis, double stop_fraction,
+                              int64_t *steps_done, int32_t *failed, double *peak, int64_t *peak_step);
+
 /* Drop dead springs from the device lists now (also done every compact_every steps). Results never change. */
 lsm_status lsm_compact(lsm_sim *sim);
 lsm_status lsm_sync(lsm_sim *sim);

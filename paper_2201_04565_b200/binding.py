@@ -21,7 +21,7 @@ FUSION_AUTO, FUSION_ON, FUSION_OFF = 0, 1, 2
 MAX_GROUPS = 8
 
 EXPORTS = ["lsm_create", "lsm_set_boundary", "lsm_step", "lsm_write_state", "lsm_read_state", "lsm_read_forces",
-           "lsm_read_broken", "lsm_read_energy", "lsm_read_virial", "lsm_read_stress", "lsm_compact", "lsm_sync", "lsm_get_info",
+           "lsm_read_broken", "lsm_read_energy", "lsm_read_virial", "lsm_read_stress", "lsm_run_to_failure", "lsm_compact", "lsm_sync", "lsm_get_info",
            "lsm_device_state", "lsm_last_error", "lsm_destroy", "lsm_abi_version"]
 
 _ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
@@ -89,6 +89,7 @@ def library():
         L.lsm_read_broken.argtypes = [C.c_void_p, u8, i64, i64]
         L.lsm_read_energy.argtypes = [C.c_void_p, d, d]
         L.lsm_read_stress.argtypes = [C.c_void_p, C.c_int64, i64, i64, d, d, d, i64]
+        L.lsm_run_to_failure.argtypes = [C.c_void_p, C.c_int64, C.c_int32, C.c_int32, C.c_double, i64, i32, d, i64]
         L.lsm_compact.argtypes = [C.c_void_p]
         L.lsm_sync.argtypes = [C.c_void_p]
         L.lsm_get_info.argtypes = [C.c_void_p, C.POINTER(LsmInfo)]
@@ -217,6 +218,14 @@ class LsmSim:
         n = int(n.value)
         return dict(step=step[:n], R=R[:n], U=U[:n], KE=KE[:n], n_broken=nb[:n])
 
+    def run_to_failure(self, max_steps, group=1, axis=1, stop_fraction=0.1):
+        """Returns (steps_done, failed, peak[B], peak_step[B])."""
+        n = C.c_int64(0); failed = C.c_int32(0)
+        peak = np.zeros(self.B); pstep = np.zeros(self.B, dtype=np.int64)
+        self._check(library().lsm_run_to_failure(self._h, int(max_steps), int(group), int(axis), float(stop_fraction),
+                                                 C.byref(n), C.byref(failed), _ptr(peak, C.c_double), _ptr(pstep, C.c_int64)))
+        return int(n.value), bool(failed.value), peak, pstep
+
     def info(self):
         inf = LsmInfo()
         self._check(library().lsm_get_info(self._h, C.byref(inf)))
@@ -326,6 +335,7 @@ def lsm_read_virial(sim): return sim.read_virial()
 def lsm_read_broken(sim): return sim.read_broken()
 def lsm_read_energy(sim): return sim.read_energy()
 def lsm_read_stress(sim, capacity=None): return sim.read_stress(capacity)
+def lsm_run_to_failure(sim, max_steps, group=1, axis=1, stop_fraction=0.1): return sim.run_to_failure(max_steps, group, axis, stop_fraction)
 def lsm_compact(sim): return sim.compact()
 def lsm_sync(sim): return sim.sync()
 def lsm_get_info(sim): return sim.info()

@@ -1079,6 +1079,41 @@ lsm_status lsm_read_stress(lsm_sim *s, int64_t capacity, int64_t *n_samples, int
     return check_flags(s);
 }
 
+// Quasi-static driver: step in chunks that end on sample steps, look at the newest sample of the history ring (a few
+// hundred bytes device -> host per chunk) and stop once every specimen's reaction has fallen below stop_fraction of its
+// own running peak.  Host logic only: the steps themselves are lsm_step's.
+lsm_status lsm_run_to_failure(lsm_sim *s, int64_t max_steps, int32_t group, int32_t axis, double stop_fraction, int64_t *steps_done,
+                              int32_t *failed, double *peak, int64_t *peak_step) {
+    CHECK_SIM(s);
+    if (max_steps < 0 || group < 0 || group >= kMaxGroups || axis < 0 || axis > 1 || !(stop_fraction >= 0.0) || !(stop_fraction < 1.0)) { s->err = "bad arguments"; return LSM_E_INVALID; }
+    if (s->sample_every <= 0) { s->err = "lsm_run_to_failure needs sample_every > 0"; return LSM_E_INVALID; }
+    const long long B = s->B;
+    std::vector<double> pk(B, 0.0), R((size_t)B * kMaxGroups * 2);
+    std::vector<long long> pks(B, -1);
+    std::vector<char> done(B, 0);
+    long long run = 0, ndone = 0;
+    while (run < max_steps && ndone < B) {
+        const long long to_sample = s->sample_every - (s->step % s->sample_every);
+        const long long n = std::min<long long>(to_sample, max_steps - run);
+        TRY(lsm_step(s, n));
+        run += n;
+        if (s->step % s->sample_every != 0) break;   // max_steps ended between two samples
+        const long long slot = (s->hist_head - 1 + s->hist_cap) % s->hist_cap;   // the sample lsm_step just recorded
+        CUDA_TRY(s, cudaMemcpyAsync(R.data(), s->hist_R + slot * B * kMaxGroups * 2, sizeof(double) * R.size(), cudaMemcpyDeviceToHost, s->stream));
+        TRY(check_flags(s));                          // synchronises the stream
+        for (long long b = 0; b < B; ++b) {
+            if (done[b]) continue;
+            const double r = std::fabs(R[((size_t)b * kMaxGroups + group) * 2 + axis]);
+            if (r > pk[b]) { pk[b] = r; pks[b] = s->step; }
+            else if (pk[b] > 0.0 && r < stop_fraction * pk[b]) { done[b] = 1; ++ndone; }
+        }
+    }
+    if (steps_done) *steps_done = run;
+    if (failed) *failed = ndone == B;
+    for (long long b = 0; b < B; ++b) { if (peak) peak[b] = pk[b]; if (peak_step) peak_step[b] = pks[b]; }
+    return LSM_OK;
+}
+
 lsm_status lsm_get_info(lsm_sim *s, lsm_info *info) {
     if (!s || !info) return LSM_E_INVALID;
     std::memset(info, 0, sizeof(*info));

@@ -508,3 +508,38 @@ def test_virial_stress_matches_oracle(reorder):
     So, Sg = o.read_virial(), g.read_virial()
     assert np.abs(Sg - So).max() <= 1e-12 * np.abs(So).max()
     g.close()
+
+
+# ---------------------------------------------------------------- the paper's protocol: both grips displaced apart, run to failure
+def test_symmetric_grips_run_to_failure_matches_oracle():
+    """PAPER.md:L143 "boundary particles were displaced apart": bottom row MOVE -du, top row MOVE +du, and the driver
+    lsm_run_to_failure (stop when the top reaction falls below 10 % of its running peak, Q20) against the same
+    loop written over the oracle.  Exact mode: identical stop step, peak step, broken set; peak within 1e-12."""
+    p = _fracture_problem(n=48, du_y=3e-4, seed=11)
+    p.sample_every = 100
+    p.groups[0].mode = MOVE; p.groups[0].du = np.array([0.0, -3e-4])
+    o = OracleSim.from_problem(p)
+    peak, peak_step, steps, failed = 0.0, -1, 0, False
+    while steps < 20000 and not failed:
+        o.step(100); steps += 100
+        r = abs(o.read_stress()["R"][-1, 0, 1, 1])
+        if r > peak:
+            peak, peak_step = r, steps
+        elif peak > 0 and r < 0.1 * peak:
+            failed = True
+    assert failed and 1000 < steps < 20000
+    g = lsm_create_from_problem(p, exact=True, history_capacity=256)
+    n, gf, gpeak, gstep = g.run_to_failure(20000, group=1, axis=1, stop_fraction=0.1)
+    assert gf and n == steps and gstep[0] == peak_step and abs(gpeak[0] / peak - 1) <= 1e-12
+    assert g.current_step == steps
+    bo, bso, nbo = o.read_broken(); bg, bsg, nbg = g.read_broken()
+    assert nbo == nbg > 0 and np.array_equal(bso, bsg)
+    h = g.read_stress()
+    assert len(h["step"]) == steps // 100 and h["step"][-1] == steps
+    # bottom and top reactions are equal and opposite up to the waves in flight: same sign convention for both grips
+    assert h["R"][-1, 0, 0, 1] * h["R"][-1, 0, 1, 1] <= 0
+    # fast mode: same protocol within the statistical tier (T5)
+    f = lsm_create_from_problem(p, history_capacity=256)
+    nf, ff, fpeak, _ = f.run_to_failure(20000, group=1, axis=1, stop_fraction=0.1)
+    assert ff and abs(nf - steps) <= 0.01 * steps + 100 and abs(fpeak[0] / peak - 1) <= 0.01
+    g.close(); f.close()
