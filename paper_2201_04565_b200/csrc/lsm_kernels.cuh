@@ -275,7 +275,9 @@ template <bool EXACT, bool SAMPLE>
 __device__ __forceinline__ void slot_eval(double2 xq, double2 xp, bool lower, double k, double r0, double kr0, uint32_t thr,
                                           double &dx, double &dy, double &r2, double &g, double &ue, bool &near) {
     dx = sub<EXACT>(xq.x, xp.x); dy = sub<EXACT>(xq.y, xp.y);
-    r2 = EXACT ? add<true>(mul<true>(dx, dx), mul<true>(dy, dy)) : fma(dy, dy, dx * dx);
+    // fast: the 1e-300 rides in the first FMA.  r2 is unchanged by it for every r2 above 1e-284; at r2 = 0 (padding /
+    // dead slot or coincident endpoints) it makes 1/r a finite 1e150, so g is finite and g * dx = g * 0 = 0: no select.
+    r2 = EXACT ? add<true>(mul<true>(dx, dx), mul<true>(dy, dy)) : fma(dy, dy, fma(dx, dx, 1e-300));
     const uint32_t hi = (uint32_t)__double2hiint(r2);
     bool live;
     ue = 0.0;
@@ -286,12 +288,10 @@ __device__ __forceinline__ void slot_eval(double2 xq, double2 xp, bool lower, do
         if (SAMPLE) ue = mul<true>(mul<true>(mul<true>(0.5, k), ext), ext);
         live = r2 > 0.0;
     } else {
-        // r2 + 1e-300 is r2 itself for every r2 above 1e-284; at r2 = 0 (padding / dead slot or coincident endpoints)
-        // it makes 1/r a finite 1e150, so g is finite and g * dx = g * 0 = 0: no select needed on the hot path.
-        const double rinv = rsqrt_fast(r2 + 1e-300);
+        const double rinv = rsqrt_fast(r2);
         g = fma(-kr0, rinv, k);              // k (r - r0) / r = k - k r0 / r
         if (SAMPLE) { const double ext = fma(r2, rinv, -r0); ue = (0.5 * k) * ext * ext; }
-        live = hi >= 0x00100000u;            // r2 zero (or denormal: treated as coincident); SAMPLE and the filter only
+        live = r2 > 1e-290;                  // false for r2 = 0 + 1e-300 (coincident / padding); used by SAMPLE only
     }
     if (EXACT) g = live ? g : 0.0;
     if (SAMPLE) ue = (live && lower) ? ue : 0.0;  // energy counted once, by the lower endpoint (Eq. 1)
