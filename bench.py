@@ -307,7 +307,7 @@ def main():
                 pass
         if not args.no_cpu_baseline:
             import lsm_inputs as gen
-            n_cpu = args.cpu_steps or max(2, int(15.0 * 4.0e7 / max(p.M, 1)))
+            n_cpu = args.cpu_steps or max(2, int(15.0 * 1.1e8 / max(p.M, 1)))   # ~15 s of the serial oracle (1.1e8 spring-updates/s)
             dt_o, _ = time_oracle(p, n_cpu)
             line["cpu_baseline"] = {"value": p.M * n_cpu / dt_o, "unit": UNIT, "cores": 1, "kind": "oracle",
                                     "sample": "first %d time steps of the same workload (after 1 warm-up step), serial oracle" % n_cpu,

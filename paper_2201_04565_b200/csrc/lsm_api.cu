@@ -194,7 +194,7 @@ StepParams step_params(const lsm_sim *s, long long step) {
     P.N = s->N; P.step = step;
     P.hdr = s->hdr; P.T = s->T; P.nbr = s->nbr; P.nbr16 = s->nbr16; P.sid = s->sid;
     P.sp.typ = s->typ; P.sp.kF = s->kF; P.sp.r0F = s->r0F; P.sp.rcF = s->rcF; P.sp.tab = s->tab; P.sp.ntypes = s->ntypes;
-    P.sp.thr = s->thr; P.sp.thr_base = s->thr_base; P.sp.thr_shift = s->thr_shift; P.sp.rcS = s->rcS; P.sp.kr0_u = s->k_u * s->r0_u; P.sp.thr_u = thr_of(s->rc_u);
+    P.sp.thr = s->thr; P.sp.thr_base = s->thr_base; P.sp.thr_mul = 1u << s->thr_shift; P.sp.rcS = s->rcS; P.sp.kr0_u = s->k_u * s->r0_u; P.sp.thr_u = thr_of(s->rc_u);
     P.sp.k_u = s->k_u; P.sp.r0_u = s->r0_u; P.sp.rc_u = s->rc_u;
     P.break_step = s->break_step; P.nbroken = s->nbroken; P.poff = s->d_poff; P.B = s->B;
     P.sU = s->sU; P.sKE = s->sKE;

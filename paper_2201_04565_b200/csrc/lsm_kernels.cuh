@@ -64,8 +64,8 @@ struct SpringParams {  // parameter encoding shared by the gather (per half-edge
     const uint8_t *typ;
     const double *kF, *r0F, *rcF;      // rcF: scatter layout only
     const uint16_t *thr;               // gather layout: breakage filter per half-edge, 16 bits: the filter word
-                                       // (high word of rc*rc) - 1 is thr_base + (thr[e] << thr_shift), rounded down
-    uint32_t thr_base, thr_shift;
+                                       // (high word of rc*rc) - 1 is thr_base + thr[e] * thr_mul, rounded down
+    uint32_t thr_base, thr_mul;       // thr_mul = 1 << shift (decode = one multiply-add)
     const double *rcS;                 // gather layout: exact rc per spring, caller numbering
     const double *tab;  // scatter: [ntypes][3] = k, r0, rc;  gather: [ntypes][kTabStride] (see kTabStride)
     int ntypes;
@@ -250,13 +250,13 @@ template <int PM> __device__ __forceinline__ void slot_params(const StepParams &
         k = kk.x; kr0 = kk.y; r0 = s_tab[kTabStride * t + 3];
         thr = reinterpret_cast<const uint32_t *>(s_tab)[2 * (kTabStride * t + 2)];
     }
-    else if (PM == PM_RCF) { k = P.sp.k_u; r0 = P.sp.r0_u; kr0 = P.sp.kr0_u; thr = P.sp.thr_base + ((uint32_t)R.thr[so] << P.sp.thr_shift); }
+    else if (PM == PM_RCF) { k = P.sp.k_u; r0 = P.sp.r0_u; kr0 = P.sp.kr0_u; thr = P.sp.thr_base + (uint32_t)R.thr[so] * P.sp.thr_mul; }
     else if (PM == PM_KRT_RCF) {
         const int t = R.typ[so];
         const double2 kk = *reinterpret_cast<const double2 *>(s_tab + kTabStride * t);
-        k = kk.x; kr0 = kk.y; r0 = s_tab[kTabStride * t + 3]; thr = P.sp.thr_base + ((uint32_t)R.thr[so] << P.sp.thr_shift);
+        k = kk.x; kr0 = kk.y; r0 = s_tab[kTabStride * t + 3]; thr = P.sp.thr_base + (uint32_t)R.thr[so] * P.sp.thr_mul;
     }
-    else { k = R.kF[so]; r0 = R.r0F[so]; kr0 = k * r0; thr = P.sp.thr_base + ((uint32_t)R.thr[so] << P.sp.thr_shift); }
+    else { k = R.kF[so]; r0 = R.r0F[so]; kr0 = k * r0; thr = P.sp.thr_base + (uint32_t)R.thr[so] * P.sp.thr_mul; }
 }
 
 // Position of neighbour j.  Always a global load (every position was just streamed in by some CTA, so these are
@@ -304,10 +304,14 @@ __device__ __forceinline__ bool row_chunk(const StepParams &P, const StepVar &V,
     int nb[CH];
     double2 xq[CH];
     bool any_near = false;
+    const double2 *own = V.pos_cur + p;
 #pragma unroll
-    for (int c = 0; c < CH; ++c) nb[c] = I16 ? p + (int)R.nbr16[(s0 + c) * kSlice] : R.nbr[(s0 + c) * kSlice];
+    for (int c = 0; c < CH; ++c) nb[c] = I16 ? (int)R.nbr16[(s0 + c) * kSlice] : R.nbr[(s0 + c) * kSlice];   // I16: offset
 #pragma unroll
-    for (int c = 0; c < CH; ++c) xq[c] = gather_pos<COHERENT>(V, nb[c]);
+    for (int c = 0; c < CH; ++c) {   // I16: address = own address + offset (one wide multiply-add per gather)
+        xq[c] = I16 ? (COHERENT ? __ldcg(own + nb[c]) : __ldg(own + nb[c])) : gather_pos<COHERENT>(V, nb[c]);
+        if (I16) nb[c] += p;
+    }
 #pragma unroll
     for (int c = 0; c < CH; ++c) {
         double k, r0, kr0, dx, dy, r2, g, ue;
