@@ -570,8 +570,10 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
             if (lane == 0 && !(MULTI && M.resident)) mbar_arrive(empty + s);
             if (++s == L.stages) { s = 0; ++u; }
         }
-        if (MULTI && it + 1 < nsteps) {  // publish this step's stores, then tell the producer this warp is done
-            __threadfence();
+        if (MULTI && it + 1 < nsteps) {  // tell the producer this warp is done with the step.  No fence here: the warp's
+            // stores are ordered before lane 0's arrive (release.cta) by __syncwarp, the producer's wait acquires them,
+            // and ITS __threadfence before the global arrival is cumulative -- the pattern of a cooperative grid sync
+            // (one fencing thread per CTA).  A fence per warp cost 0.3-0.6 us per step.
             __syncwarp();
             if (lane == 0) mbar_arrive(stepdone);
         }
