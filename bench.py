@@ -286,7 +286,8 @@ def main():
                        "compact_every": args.compact_every, "force_mode": inf0["force_mode"], "param_mode": inf0["param_mode"],
                        "exact": inf0["exact"], "reorder": inf0["reorder"], "gather_variant": inf0["gather_variant"], "step_fusion": inf0["step_fusion"], "pipeline_stages": inf0["pipeline_stages"], "stage_bytes": inf0["stage_bytes"], "bytes_per_half_edge": inf0["bytes_per_half_edge"],
                        "half_edges_stored": inf0["n_half_edges_stored"], "device_bytes": inf0["device_bytes"],
-                       "l2": "inputs larger than L2 (%.0f MB touched per time step vs 126 MB L2)" % (bc / 1e6),
+                       "l2": "inputs larger than L2 (%.0f MB streamed per time step vs 126 MB L2)"
+                             % ((64.0 * p.N + inf0["n_half_edges_stored"] * inf0["bytes_per_half_edge"] + 1.25 * p.N) / 1e6),
                        "parallelism": "replicas x%d" % world if world > 1 else "1 GPU"},
             "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 2 * xh.numel() * 8, "d2h_bytes_per_step": 2 * xh.numel() * 8 + d2h_hist,
                     "ms_per_step": te_ms_max / K},
