@@ -10,7 +10,7 @@
 //     hdr[T] (64 B per tile: slot offset of each of its 8 slices + end, live width of each slice),
 //     nbr[E] int32 neighbour id; a padding slot or a dead spring holds the particle's OWN id (a spring never joins a
 //     particle to itself): its gather is legal, gives r = 0 and therefore contributes nothing, with no validity test,
-//     sid[E] caller spring id (cold: read only when a spring breaks or sits within one fp32 ulp of rc),
+//     sid[E] caller spring id (cold: read only when a spring breaks or comes within the filter margin of rc),
 //     per-slot parameters by ParamMode: typ[E] uint8, thr[E] uint16 = 16-bit code of (high word of rc*rc) - 1 (a
 //     conservative integer filter on r^2; anything above it is decided by the exact fp64 rcS[sid]: the decision is the
 //     fp64 one), kF/r0F[E].  nbr16[E] int16: the neighbour list again as offsets (neighbour - self), streamed instead
@@ -39,7 +39,6 @@ constexpr int kMaxStages = 8;
 #endif
 constexpr int kStreamMinB = LSM_STREAM_MINB;
 constexpr int kStreamHdrBytes = 256;   // mbarriers at the front of the streamed kernel's dynamic shared memory
-constexpr int32_t kPad = INT32_MIN;
 constexpr uint8_t kFree = 0xFF;
 constexpr int kMaxGroups = 8;
 constexpr int kChunk = 2048;  // particles per reduction chunk
@@ -215,7 +214,7 @@ __device__ __forceinline__ void particle_update(const StepParams &P, const StepV
 // Fused gather step: one thread per particle.  Gathers the positions of its (<= slice width) neighbours, evaluates
 // every incident spring (each spring is evaluated from both of its endpoints: twice the arithmetic, no atomics, no
 // force array round trip, deterministic), applies the breakage test, then integrates.  Reads x (double-buffered),
-// v, ids, parameters; writes x_next, v.  HBM bytes per step: 64 N + (4 + parameter bytes) * 2M.
+// v, ids, parameters; writes x_next, v.  HBM bytes per step: 64 N + (2 or 4 id bytes + parameter bytes) * 2M.
 // Two kernels share the row evaluation below: k_gather_step reads the slot streams straight from global memory;
 // k_gather_stream (the product path) stages them tile by tile through shared memory with bulk async copies.
 // ---------------------------------------------------------------------------------------------------------------
