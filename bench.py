@@ -55,6 +55,8 @@ def make_problem(name):
         return gen.config4(B=128), "BASELINE.json configs[3] reduced to 128 specimens"
     if name == "cfg5":
         return gen.config5(), "BASELINE.json configs[4]: 8192x8192 notched lattice"
+    if name == "table2":
+        return gen.config2(n=216), "two-phase composite of the size of the paper's largest model (Table 2, PAPER.md:L176-L186: 46,836 particles, 137,759 springs): 216x216"
     if name == "cfg5s":
         return gen.config5(n=4096), "BASELINE.json configs[4] reduced to 4096x4096"
     raise SystemExit("unknown workload " + name)
