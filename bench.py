@@ -55,6 +55,8 @@ def make_problem(name):
         return gen.config4(B=128), "BASELINE.json configs[3] reduced to 128 specimens"
     if name == "cfg5":
         return gen.config5(), "BASELINE.json configs[4]: 8192x8192 notched lattice"
+    if name == "cube3d":
+        return gen.config3d(), "3-D cubic network with face diagonals, 128^3 particles (D = 3 path; not a BASELINE.json config)"
     if name == "table2":
         return gen.config2(n=216), "two-phase composite of the size of the paper's largest model (Table 2, PAPER.md:L176-L186: 46,836 particles, 137,759 springs): 216x216"
     if name == "cfg5s":
@@ -62,10 +64,10 @@ def make_problem(name):
     raise SystemExit("unknown workload " + name)
 
 
-def counted_bytes(N, M_alive, p_var):
+def counted_bytes(N, M_alive, p_var, dim=2):
     """SURVEY.md 8(d) / DESIGN.md "Counted bytes": x and v read and written once, two int32 ids per live spring, fp64
     parameters that truly vary per spring, one alive bit."""
-    return 64.0 * N + M_alive * (8.0 + 8.0 * p_var) + M_alive / 8.0
+    return 32.0 * dim * N + M_alive * (8.0 + 8.0 * p_var) + M_alive / 8.0
 
 
 def p_var_of(p):
@@ -237,10 +239,10 @@ def main():
     nb_after = sim.n_broken()
 
     # ---------------- end to end through the C ABI with host buffers ----------------
-    xh = torch.empty((p.N, 2), dtype=torch.float64, pin_memory=True)
-    vh = torch.empty((p.N, 2), dtype=torch.float64, pin_memory=True)
-    xo = torch.empty((p.N, 2), dtype=torch.float64, pin_memory=True)
-    vo = torch.empty((p.N, 2), dtype=torch.float64, pin_memory=True)
+    xh = torch.empty((p.N, p.x.shape[1]), dtype=torch.float64, pin_memory=True)
+    vh = torch.empty((p.N, p.x.shape[1]), dtype=torch.float64, pin_memory=True)
+    xo = torch.empty((p.N, p.x.shape[1]), dtype=torch.float64, pin_memory=True)
+    vo = torch.empty((p.N, p.x.shape[1]), dtype=torch.float64, pin_memory=True)
     sim.read_state(xh.numpy(), vh.numpy())
     d2h_hist = 0
     for it in range(2 + K):                    # 2 untimed warm-up rounds
@@ -274,7 +276,7 @@ def main():
         peak = float(peaks.get("hbm_gbs", 6650.0))
         peak_src = "measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
         pv = p_var_of(p)
-        bc = counted_bytes(p.N, M_alive0, pv)
+        bc = counted_bytes(p.N, M_alive0, pv, p.x.shape[1])
         t_launch = ms_max * 1e-3 / (K * S)     # upper bound of the step kernel's mean duration: every other launch in
         ach = bc / t_launch / 1e9              # the region (start/end, reductions, compaction) is charged to it
         value = world * M_alive0 * S * K / (ms_max * 1e-3)

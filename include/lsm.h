@@ -14,8 +14,9 @@
  *
  * Conventions
  *   - plain C; no exceptions or C++ types cross the boundary; every function returns lsm_status unless noted.
- *   - dim = 2 only (all configurations of the paper and of BASELINE.json are 2-D; the paper's listing is 3-D AoS,
- *     PAPER.md:L93-L97 -> LSM_E_UNSUPPORTED for dim = 3 in this round).
+ *   - dim = 2 is the tuned path (all configurations of the paper and of BASELINE.json are 2-D).  dim = 3 (the layout of
+ *     the paper's kernel listing) runs on a plain one-thread-per-particle gather kernel: same
+ *     semantics, same entry points, vectors [N*3]; no scatter path, streaming, step fusion or virial there yet.
  *   - HOST pointers unless a parameter says DEVICE.  Vector arrays are interleaved [N*dim] (x0 y0 x1 y1 ...) as in the
  *     paper's flattened 1-D arrays.  Inputs are borrowed for the duration of the call and copied;
  *     outputs are caller-allocated buffers of the documented size.  The handle owns all device memory.
@@ -48,7 +49,8 @@ typedef enum {
     LSM_E_CUDA = -4,        /* CUDA runtime error, or no CUDA device                                               */
     LSM_E_NOMEM = -5,       /* host or device allocation failed                                                    */
     LSM_E_STATE = -6,       /* the simulation failed earlier (e.g. non-finite energy detected on the device)       */
-    LSM_E_UNSUPPORTED = -7  /* dim = 3, exact arithmetic with the scatter kernel, degree > 255 in the gather layout  */
+    LSM_E_UNSUPPORTED = -7  /* exact arithmetic with the scatter kernel, degree > 255 in the gather layout, a dim = 3
+                               request for the scatter / streamed / fused / virial paths                            */
 } lsm_status;
 
 enum { LSM_FIXED = 0, LSM_MOVE = 1 };                      /* boundary group modes */
@@ -65,7 +67,7 @@ typedef void (*lsm_free_fn)(void *dptr, void *user);
 
 typedef struct lsm_desc {
     uint32_t struct_size;             /* = sizeof(lsm_desc): ABI check                                           */
-    int32_t dim;                      /* 2                                                                        */
+    int32_t dim;                      /* 2 or 3                                                                   */
     int64_t n_particles, n_springs;   /* N >= 1, M >= 0, both < 2^31 - 1                                          */
     int32_t n_batch;                  /* B >= 1 independent specimens stored as one disjoint union                */
     int32_t _pad0;

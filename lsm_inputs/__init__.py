@@ -6,5 +6,5 @@ and the CUDA path (`paper_2201_04565_b200/`) each implement that on their own an
 """
 from .generators import (  # noqa: F401
     Problem, BoundaryGroup, triangular_lattice, blob_image, two_phase_spring_params, porous_keep_mask,
-    config1, config2, config3, config4, config5, shuffle_ids, velocity_ramp, single_specimen, FIXED, MOVE,
+    config1, config2, config3, config4, config5, shuffle_ids, velocity_ramp, single_specimen, cubic_lattice_3d, config3d, FIXED, MOVE,
 )

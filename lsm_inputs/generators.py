@@ -296,3 +296,43 @@ def shuffle_ids(p: Problem, seed: int) -> Problem:
     q.meta["perm"] = perm          # new particle id -> old particle id
     q.meta["spring_perm"] = sp     # new spring id -> old spring id
     return q
+
+
+def cubic_lattice_3d(nx: int, ny: int, nz: int, r0: float = 1.0, diagonals: bool = True):
+    """3-D test network (the paper's kernel listing is 3-D): simple cubic sites with springs to the
+    +x, +y, +z neighbours (rest length r0) and, optionally, the face diagonals in the xy, yz and zx planes (rest length
+    sqrt(2) r0) that make the network rigid.  Returns x [N,3], spring_i, spring_j, r0_s."""
+    ix, iy, iz = np.meshgrid(np.arange(nx), np.arange(ny), np.arange(nz), indexing="ij")
+    idx = (ix * ny + iy) * nz + iz
+    x = np.stack([ix, iy, iz], axis=-1).reshape(-1, 3).astype(np.float64) * r0
+    si, sj, rr = [], [], []
+
+    def link(a, b, length):
+        si.append(a.ravel()); sj.append(b.ravel()); rr.append(np.full(a.size, length))
+
+    link(idx[:-1], idx[1:], r0); link(idx[:, :-1], idx[:, 1:], r0); link(idx[:, :, :-1], idx[:, :, 1:], r0)
+    if diagonals:
+        s2 = np.sqrt(2.0) * r0
+        link(idx[:-1, :-1], idx[1:, 1:], s2); link(idx[:-1, 1:], idx[1:, :-1], s2)
+        link(idx[:, :-1, :-1], idx[:, 1:, 1:], s2); link(idx[:, :-1, 1:], idx[:, 1:, :-1], s2)
+        link(idx[:-1, :, :-1], idx[1:, :, 1:], s2); link(idx[1:, :, :-1], idx[:-1, :, 1:], s2)
+    return x, np.concatenate(si).astype(np.int32), np.concatenate(sj).astype(np.int32), np.concatenate(rr)
+
+
+def config3d(n: int = 128, strain_per_step: float = 1e-6) -> Problem:
+    """A 3-D workload for the D = 3 path (not a BASELINE.json config: those are all 2-D): n^3 cubic network with face
+    diagonals, k = 1, rc = 1.1 x rest length, bottom face (z = 0) fixed, top face pulled in +z, velocity ramp."""
+    x, si, sj, r0 = cubic_lattice_3d(n, n, n)
+    M = si.size
+    dt = 0.02
+    H0 = float(n - 1)
+    du = np.array([0.0, 0.0, strain_per_step * H0])
+    iz = np.round(x[:, 2]).astype(int)
+    bot = np.flatnonzero(iz == 0).astype(np.int32)
+    top = np.flatnonzero(iz == n - 1).astype(np.int32)
+    v = np.zeros_like(x)
+    v[:, 2] = (x[:, 2] / H0) * (du[2] / dt)
+    v[bot] = 0.0
+    g = [BoundaryGroup(bot, FIXED, np.zeros(3)), BoundaryGroup(top, MOVE, du)]
+    return Problem("cube3d_%d" % n, x, v, si, sj, np.ones(M), r0, 1.1 * r0, dt, 0.01, g, steps=2000,
+                   meta=dict(nx=n, ny=n, nz=n, r0=1.0, W0=float(n * n), H0=H0))

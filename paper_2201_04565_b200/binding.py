@@ -145,9 +145,9 @@ class _TorchAllocator:
 class LsmSim:
     """Handle returned by lsm_create.  Methods mirror the C entry points one to one."""
 
-    def __init__(self, handle, N, M, B, allocator, keep):
+    def __init__(self, handle, N, M, B, allocator, keep, D=2):
         self._h = handle
-        self.N, self.M, self.B, self.D = N, M, B, 2
+        self.N, self.M, self.B, self.D = N, M, B, D
         self._allocator = allocator
         self._keep = keep
 
@@ -157,7 +157,9 @@ class LsmSim:
 
     def set_boundary(self, group, ids, mode, du=None):
         ids = np.ascontiguousarray(ids, dtype=np.int32)
-        du = np.zeros(2) if du is None else np.ascontiguousarray(du, dtype=np.float64)
+        du = np.zeros(self.D) if du is None else np.ascontiguousarray(du, dtype=np.float64)
+        if du.size != self.D:
+            raise LsmError(-1, "disp_per_step must have dim entries")
         self._check(library().lsm_set_boundary(self._h, int(group), _ptr(ids, C.c_int32), ids.size, int(mode), _ptr(du, C.c_double)))
 
     def step(self, n=1):
@@ -178,13 +180,13 @@ class LsmSim:
         self._check(library().lsm_write_state(self._h, _host_ptr(x, C.c_double), _host_ptr(v, C.c_double)))
 
     def read_state(self, out_x=None, out_v=None):
-        x = np.empty((self.N, 2)) if out_x is None else out_x
-        v = np.empty((self.N, 2)) if out_v is None else out_v
+        x = np.empty((self.N, self.D)) if out_x is None else out_x
+        v = np.empty((self.N, self.D)) if out_v is None else out_v
         self._check(library().lsm_read_state(self._h, _host_ptr(x, C.c_double), _host_ptr(v, C.c_double)))
         return x, v
 
     def read_forces(self):
-        f = np.empty((self.N, 2))
+        f = np.empty((self.N, self.D))
         self._check(library().lsm_read_forces(self._h, _ptr(f, C.c_double)))
         return f
 
@@ -210,7 +212,7 @@ class LsmSim:
 
     def read_stress(self, capacity=None):
         cap = int(self.history_capacity if capacity is None else capacity)
-        step = np.empty(cap, dtype=np.int64); R = np.empty((cap, self.B, MAX_GROUPS, 2))
+        step = np.empty(cap, dtype=np.int64); R = np.empty((cap, self.B, MAX_GROUPS, self.D))
         U = np.empty((cap, self.B)); KE = np.empty((cap, self.B)); nb = np.empty((cap, self.B), dtype=np.int64)
         n = C.c_int64(0)
         self._check(library().lsm_read_stress(self._h, cap, C.byref(n), _ptr(step, C.c_int64), _ptr(R, C.c_double),
@@ -307,7 +309,7 @@ def lsm_create(x, spring_i, spring_j, k, r0, rc, dt, gamma=0.0, v=None, mass=1.0
     st = L.lsm_create(C.byref(d), C.byref(h))
     if st != 0:
         raise LsmError(st, (L.lsm_last_error(None) or b"").decode())
-    sim = LsmSim(h, N, M, int(n_batch), allocator, keep=None)
+    sim = LsmSim(h, N, M, int(n_batch), allocator, keep=None, D=int(x.shape[1]))
     sim.history_capacity = int(history_capacity) if history_capacity else 1024
     return sim
 

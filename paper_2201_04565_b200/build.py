@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "liblsm_b200.so")
 SOURCES = [os.path.join(CSRC, "lsm_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "lsm_kernels.cuh"), os.path.join(os.path.dirname(HERE), "include", "lsm.h")]
+DEPS = SOURCES + [os.path.join(CSRC, "lsm_kernels.cuh"), os.path.join(CSRC, "lsm_kernels3.cuh"), os.path.join(os.path.dirname(HERE), "include", "lsm.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "--fmad=true",
               "-Xcompiler", "-fPIC", "-shared"]
 

@@ -14,6 +14,7 @@
 
 #include "../../include/lsm.h"
 #include "lsm_kernels.cuh"
+#include "lsm_kernels3.cuh"
 
 using namespace lsmk;
 
@@ -24,7 +25,7 @@ namespace {
 struct Group {
     bool set = false;
     int mode = 0;
-    double du[2] = {0, 0};
+    double du[3] = {0, 0, 0};
     long long n0 = 0;
     std::vector<int32_t> ids;  // internal ids, sorted
     int32_t *d_ids = nullptr;
@@ -36,7 +37,7 @@ struct Group {
 struct lsm_sim {
     // configuration
     long long N = 0, M = 0;
-    int B = 1;
+    int B = 1, dim = 2;
     double dt = 0, gamma = 0, mass_u = 1;
     int sample_every = 0, hist_cap = 1024, compact_every = 0, reorder = 0, force_mode = LSM_FORCE_GATHER, exact = 0, step_fusion = 0;
     int device = 0;
@@ -53,6 +54,8 @@ struct lsm_sim {
     int32_t *d_inv = nullptr;
     // device state
     double2 *pos[2] = {nullptr, nullptr}, *vel = nullptr, *f = nullptr, *fd = nullptr, *stage[2] = {nullptr, nullptr};
+    double4 *pos3[2] = {nullptr, nullptr}, *vel3 = nullptr, *f3 = nullptr, *fd3 = nullptr;   // dim = 3 (lsm_kernels3.cuh)
+    double *stage3[2] = {nullptr, nullptr};                                                  // packed [N*3] staging
     uint8_t *grp = nullptr;
     double *mass = nullptr;
     int cur = 0;
@@ -213,6 +216,36 @@ ScatterParams scatter_params(const lsm_sim *s) {
 
 enum Variant { V_MID = 0, V_MID_SAMPLE = 1, V_END = 2, V_INIT = 3 };
 
+GroupTab3 group_tab3(const lsm_sim *s) {
+    GroupTab3 g;
+    for (int i = 0; i < kMaxGroups; ++i) {
+        for (int c = 0; c < 3; ++c) g.du[c][i] = s->groups[i].set ? s->groups[i].du[c] : 0.0;
+        g.n0[i] = s->groups[i].n0;
+    }
+    return g;
+}
+
+Step3Params step_params3(const lsm_sim *s, long long step, Variant v) {
+    Step3Params P;
+    std::memset(&P, 0, sizeof(P));
+    const StepParams P2 = step_params(s, step);   // spring layout, parameters and bookkeeping are shared with the 2-D path
+    P.pos_cur = s->pos3[s->cur]; P.pos_next = s->pos3[s->cur ^ 1];
+    P.vel = s->vel3; P.f = s->f3; P.fd = s->fd3; P.grp = s->grp; P.mass = s->mass; P.mass_u = s->mass_u;
+    P.dt = s->dt; P.hdt = 0.5 * s->dt; P.gamma = s->gamma; P.N = s->N; P.step = step;
+    P.hdr = s->hdr; P.nbr = s->nbr; P.nbr16 = s->nbr16; P.sid = s->sid; P.sp = P2.sp; P.pm = s->pm;
+    P.break_step = s->break_step; P.nbroken = s->nbroken; P.poff = s->d_poff; P.B = s->B; P.sU = s->sU; P.sKE = s->sKE;
+    P.kick2 = v != V_INIT; P.advance = v == V_MID || v == V_MID_SAMPLE; P.sample = v != V_MID;
+    P.g = group_tab3(s);
+    return P;
+}
+
+void launch_gather3(lsm_sim *s, long long step, Variant v) {
+    const Step3Params P = step_params3(s, step, v);
+    if (s->exact) k3_step<true><<<grid_for(s->N), kBlock, 0, s->stream>>>(P);
+    else k3_step<false><<<grid_for(s->N), kBlock, 0, s->stream>>>(P);
+    s->kernels_launched += 1;
+}
+
 template <int PM, bool EXACT> void launch_gather_v(const StepParams &P, Variant v, unsigned grid, cudaStream_t st) {
     switch (v) {
         case V_MID: k_gather_step<PM, EXACT, true, true, false><<<grid, kBlock, 0, st>>>(P); break;
@@ -306,6 +339,7 @@ template <bool EXACT> void launch_stream_pm(const lsm_sim *s, const StepParams &
 }
 
 void launch_gather(lsm_sim *s, const StepParams &P, Variant v) {
+    if (s->dim == 3) { launch_gather3(s, P.step, v); return; }
     if (s->gather_variant == 2) {
         if (s->exact) launch_stream_pm<true>(s, P, v);
         else launch_stream_pm<false>(s, P, v);
@@ -366,7 +400,7 @@ void launch_reduce(lsm_sim *s, long long step, long long slot) {
     ReduceParams R = reduce_params(s, step);
     if (slot >= 0) {
         R.out_step = s->hist_step + slot;
-        R.out_R = s->hist_R + (size_t)slot * s->B * kMaxGroups * 2;
+        R.out_R = s->hist_R + (size_t)slot * s->B * kMaxGroups * s->dim;
         R.out_U = s->hist_U + (size_t)slot * s->B;
         R.out_KE = s->hist_KE + (size_t)slot * s->B;
         R.out_nb = s->hist_nb + (size_t)slot * s->B;
@@ -374,7 +408,13 @@ void launch_reduce(lsm_sim *s, long long step, long long slot) {
         R.out_U = s->cur_U; R.out_KE = s->cur_KE;
     }
     k_reduce_chunks<<<(unsigned)s->nchunks, kBlock, 0, s->stream>>>(R);
-    k_finalize_sample<<<(unsigned)s->B, kBlock, 0, s->stream>>>(R);
+    if (s->dim == 3) {
+        Reduce3Params Q;
+        Q.R = R; Q.f3 = s->f3; Q.out_R3 = R.out_R; Q.R.out_R = nullptr;
+        k3_finalize_sample<<<(unsigned)s->B, kBlock, 0, s->stream>>>(Q);
+    } else {
+        k_finalize_sample<<<(unsigned)s->B, kBlock, 0, s->stream>>>(R);
+    }
     s->kernels_launched += 2;
 }
 
@@ -438,7 +478,8 @@ void lsm_destroy(lsm_sim *s) {
 static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
     const long long N = d->n_particles, M = d->n_springs;
     const int B = d->n_batch;
-    s->N = N; s->M = M; s->B = B; s->dt = d->dt; s->gamma = d->gamma;
+    s->N = N; s->M = M; s->B = B; s->dim = d->dim; s->dt = d->dt; s->gamma = d->gamma;
+    const int D = d->dim;
     s->mass_u = d->mass ? 1.0 : d->mass_uniform;
     s->sample_every = d->sample_every; s->hist_cap = d->history_capacity > 0 ? d->history_capacity : 1024;
     s->compact_every = d->compact_every; s->reorder = d->reorder;
@@ -463,7 +504,7 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
         if (s->poff[b + 1] < s->poff[b] || soff[b + 1] < soff[b]) return fail(s, LSM_E_INVALID, "offsets must ascend");
 
     // ---- validation of values ----
-    for (long long q = 0; q < 2 * N; ++q) {
+    for (long long q = 0; q < D * N; ++q) {
         if (!std::isfinite(d->x[q])) return fail(s, LSM_E_NONFINITE, "non-finite position");
         if (d->v && !std::isfinite(d->v[q])) return fail(s, LSM_E_NONFINITE, "non-finite velocity");
     }
@@ -488,16 +529,23 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
         s->perm.resize(N); s->inv.resize(N);
         std::vector<std::pair<uint64_t, int32_t>> keys(N);
         for (int b = 0; b < B; ++b) {
-            double lox = 1e300, loy = 1e300, hix = -1e300, hiy = -1e300;
-            for (long long p = s->poff[b]; p < s->poff[b + 1]; ++p) {
-                lox = std::min(lox, d->x[2 * p]); hix = std::max(hix, d->x[2 * p]);
-                loy = std::min(loy, d->x[2 * p + 1]); hiy = std::max(hiy, d->x[2 * p + 1]);
-            }
-            const double ext = std::max(std::max(hix - lox, hiy - loy), 1e-300);
+            double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
+            for (long long p = s->poff[b]; p < s->poff[b + 1]; ++p)
+                for (int c = 0; c < D; ++c) { lo[c] = std::min(lo[c], d->x[D * p + c]); hi[c] = std::max(hi[c], d->x[D * p + c]); }
+            double ext = 1e-300;
+            for (int c = 0; c < D; ++c) ext = std::max(ext, hi[c] - lo[c]);
             const double sc = 1048575.0 / ext;  // 20 bits per axis
             for (long long p = s->poff[b]; p < s->poff[b + 1]; ++p) {
-                const uint64_t qx = (uint64_t)((d->x[2 * p] - lox) * sc), qy = (uint64_t)((d->x[2 * p + 1] - loy) * sc);
-                keys[p] = {part1by1(qx) | (part1by1(qy) << 1), (int32_t)p};
+                uint64_t key = 0;
+                if (D == 2) {
+                    key = part1by1((uint64_t)((d->x[2 * p] - lo[0]) * sc)) | (part1by1((uint64_t)((d->x[2 * p + 1] - lo[1]) * sc)) << 1);
+                } else {   // 3-way bit interleave
+                    uint64_t q[3];
+                    for (int c = 0; c < 3; ++c) q[c] = (uint64_t)((d->x[3 * p + c] - lo[c]) * sc);
+                    for (int bit = 0; bit < 20; ++bit)
+                        for (int c = 0; c < 3; ++c) key |= ((q[c] >> bit) & 1ull) << (3 * bit + c);
+                }
+                keys[p] = {key, (int32_t)p};
             }
             std::sort(keys.begin() + s->poff[b], keys.begin() + s->poff[b + 1]);
         }
@@ -597,6 +645,26 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
         s->T = (N + kTile - 1) / kTile;
         s->Npad = s->T * kTile;                       // the streamed kernel copies whole tiles: pad the tail tile
         const long long Np = s->Npad;
+        if (D == 3) {
+            const double4 z4 = make_double4(0.0, 0.0, 0.0, 0.0);
+            std::vector<double4> hx(Np, z4), hv(Np, z4);
+            for (long long c = 0; c < N; ++c) {
+                const int32_t p = to_int(c);
+                hx[p] = make_double4(d->x[3 * c], d->x[3 * c + 1], d->x[3 * c + 2], 0.0);
+                if (d->v) hv[p] = make_double4(d->v[3 * c], d->v[3 * c + 1], d->v[3 * c + 2], 0.0);
+            }
+            TRY(upload(s, &s->pos3[0], hx));
+            TRY(dev_alloc(s, &s->pos3[1], (size_t)Np));
+            CUDA_TRY(s, cudaMemcpyAsync(s->pos3[1], s->pos3[0], sizeof(double4) * Np, cudaMemcpyDeviceToDevice, s->stream));
+            TRY(upload(s, &s->vel3, hv));
+            TRY(dev_alloc(s, &s->f3, (size_t)N));
+            TRY(dev_alloc(s, &s->fd3, (size_t)N));
+            TRY(dev_alloc(s, &s->stage3[0], (size_t)N * 3));
+            TRY(dev_alloc(s, &s->stage3[1], (size_t)N * 3));
+            CUDA_TRY(s, cudaMemsetAsync(s->f3, 0, sizeof(double4) * N, s->stream));
+            CUDA_TRY(s, cudaMemsetAsync(s->fd3, 0, sizeof(double4) * N, s->stream));
+            CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+        } else {
         std::vector<double2> hx(Np, make_double2(0.0, 0.0)), hv(Np, make_double2(0.0, 0.0));
         for (long long c = 0; c < N; ++c) {
             const int32_t p = to_int(c);
@@ -613,6 +681,7 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
         TRY(dev_alloc(s, &s->stage[1], (size_t)N));
         CUDA_TRY(s, cudaMemsetAsync(s->f, 0, sizeof(double2) * N, s->stream));
         CUDA_TRY(s, cudaMemsetAsync(s->fd, 0, sizeof(double2) * N, s->stream));
+        }
         s->h_grp.assign(Np, kFree);
         TRY(upload(s, &s->grp, s->h_grp));
         s->h_grp.resize(N);
@@ -739,6 +808,7 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
             const int budget = std::min(dev_smem, (dev_smem + 1024) / ctas_per_sm - 1024) - L.first;   // 1 KB reserved per CTA
             L.stages = std::min<int>(max_stages, budget / std::max(L.bytes, 1));
             const bool can_stream = L.stages >= 2;
+            if (D == 3) s->gather_variant = 1;
             if (s->gather_variant == 0) s->gather_variant = can_stream ? 2 : 1;
             if (s->gather_variant == 2 && !can_stream) return fail(s, LSM_E_UNSUPPORTED, "gather_variant = streamed: a tile's rows do not fit in shared memory (degree too high); use the direct variant");
             s->stream_smem = L.first + L.stages * L.bytes;
@@ -751,7 +821,7 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
             long long fuse_below = 1 << 18;   // measured: 64^2 5.8 -> 3.6 us per step, 512^2 8.4 -> 8.3, 2.1 M particles 39.1 -> 40.4
             if (const char *e = std::getenv("LSM_FUSE_BELOW")) fuse_below = std::atoll(e);
             if (s->step_fusion == LSM_FUSION_ON && !(coop && s->gather_variant == 2)) return fail(s, LSM_E_UNSUPPORTED, "step_fusion = ON needs the streamed gather kernel and cooperative launch support");
-            s->multi_on = coop && s->gather_variant == 2 && (s->step_fusion == LSM_FUSION_ON || (s->step_fusion == LSM_FUSION_AUTO && N <= fuse_below));
+            s->multi_on = D == 2 && coop && s->gather_variant == 2 && (s->step_fusion == LSM_FUSION_ON || (s->step_fusion == LSM_FUSION_AUTO && N <= fuse_below));
             if (s->multi_on) {
                 TRY(dev_alloc(s, &s->gbar, 1));
                 CUDA_TRY(s, cudaMemsetAsync(s->gbar, 0, sizeof(unsigned long long), s->stream));
@@ -820,7 +890,7 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
         TRY(dev_alloc(s, &s->cur_U, (size_t)B)); TRY(dev_alloc(s, &s->cur_KE, (size_t)B));
         const size_t cap = (size_t)s->hist_cap;
         TRY(dev_alloc(s, &s->hist_step, cap)); TRY(dev_alloc(s, &s->hist_nb, cap * B));
-        TRY(dev_alloc(s, &s->hist_R, cap * B * kMaxGroups * 2));
+        TRY(dev_alloc(s, &s->hist_R, cap * B * kMaxGroups * D));
         TRY(dev_alloc(s, &s->hist_U, cap * B)); TRY(dev_alloc(s, &s->hist_KE, cap * B));
     }
     s->step = 0;
@@ -833,8 +903,9 @@ lsm_status lsm_create(const lsm_desc *d, lsm_sim **out) {
     if (out) *out = nullptr;
     if (!d || !out) return fail(nullptr, LSM_E_INVALID, "desc / out is NULL");
     if (d->struct_size != sizeof(lsm_desc)) return fail(nullptr, LSM_E_INVALID, "lsm_desc.struct_size does not match this library (ABI mismatch)");
-    if (d->dim == 3) return fail(nullptr, LSM_E_UNSUPPORTED, "dim = 3 is not built in this round (hot path is 2-D)");
-    if (d->dim != 2) return fail(nullptr, LSM_E_INVALID, "dim must be 2");
+    if (d->dim != 2 && d->dim != 3) return fail(nullptr, LSM_E_INVALID, "dim must be 2 or 3");
+    if (d->dim == 3 && (d->force_mode == LSM_FORCE_SCATTER || d->gather_variant == LSM_GATHER_STREAMED || d->step_fusion == LSM_FUSION_ON))
+        return fail(nullptr, LSM_E_UNSUPPORTED, "dim = 3 runs on the direct gather kernel only (no scatter path, streaming or step fusion yet)");
     if (d->n_particles < 1 || d->n_springs < 0 || d->n_particles >= 2147483647LL || d->n_springs >= 2147483647LL) return fail(nullptr, LSM_E_INVALID, "need 1 <= N < 2^31-1 and 0 <= M < 2^31-1");
     if (d->n_batch < 1 || !d->x) return fail(nullptr, LSM_E_INVALID, "n_batch < 1 or x is NULL");
     if (!(d->dt > 0.0) || !(d->gamma >= 0.0) || !std::isfinite(d->dt) || !std::isfinite(d->gamma)) return fail(nullptr, LSM_E_INVALID, "need dt > 0 and gamma >= 0");
@@ -865,7 +936,7 @@ lsm_status lsm_set_boundary(lsm_sim *s, int32_t gi, const int32_t *ids, int64_t 
     CHECK_SIM(s);
     if (gi < 0 || gi >= kMaxGroups) { s->err = "group id out of range"; return LSM_E_RANGE; }
     if (n < 0 || (n > 0 && !ids) || (mode != LSM_FIXED && mode != LSM_MOVE)) { s->err = "bad arguments"; return LSM_E_INVALID; }
-    if (mode == LSM_MOVE && (!du || !std::isfinite(du[0]) || !std::isfinite(du[1]))) { s->err = "MOVE needs a finite disp_per_step"; return LSM_E_INVALID; }
+    if (mode == LSM_MOVE && (!du || !std::isfinite(du[0]) || !std::isfinite(du[1]) || (s->dim == 3 && !std::isfinite(du[2])))) { s->err = "MOVE needs a finite disp_per_step"; return LSM_E_INVALID; }
     Group &g = s->groups[gi];
     std::vector<int32_t> nid((size_t)n);
     for (long long q = 0; q < n; ++q) {
@@ -878,12 +949,14 @@ lsm_status lsm_set_boundary(lsm_sim *s, int32_t gi, const int32_t *ids, int64_t 
     if (std::adjacent_find(nid.begin(), nid.end()) != nid.end()) { s->err = "duplicate particle id in the group"; return LSM_E_RANGE; }
     // release the old members (they keep the kinematic velocity du/dt, like the oracle's stored v)
     if (g.set && !g.ids.empty()) {
-        k_group_release<<<grid_for((long long)g.ids.size()), kBlock, 0, s->stream>>>(g.d_ids, (long long)g.ids.size(), s->grp, s->vel, g.du[0] / s->dt, g.du[1] / s->dt);
+        if (s->dim == 3) k3_group_release<<<grid_for((long long)g.ids.size()), kBlock, 0, s->stream>>>(g.d_ids, (long long)g.ids.size(), s->grp, s->vel3, g.du[0] / s->dt, g.du[1] / s->dt, g.du[2] / s->dt);
+        else k_group_release<<<grid_for((long long)g.ids.size()), kBlock, 0, s->stream>>>(g.d_ids, (long long)g.ids.size(), s->grp, s->vel, g.du[0] / s->dt, g.du[1] / s->dt);
         s->kernels_launched += 1;
         for (int32_t p : g.ids) s->h_grp[p] = kFree;
     }
     g.set = true; g.mode = mode; g.n0 = s->step;
     g.du[0] = mode == LSM_MOVE ? du[0] : 0.0; g.du[1] = mode == LSM_MOVE ? du[1] : 0.0;
+    g.du[2] = (mode == LSM_MOVE && s->dim == 3) ? du[2] : 0.0;
     g.ids = nid;
     for (int32_t p : nid) s->h_grp[p] = (uint8_t)gi;
     std::vector<long long> seg(s->B + 1, 0);
@@ -892,7 +965,8 @@ lsm_status lsm_set_boundary(lsm_sim *s, int32_t gi, const int32_t *ids, int64_t 
     TRY(upload(s, &g.d_ids, nid));
     TRY(upload(s, &g.d_seg, seg));
     if (n > 0) {
-        k_group_assign<<<grid_for(n), kBlock, 0, s->stream>>>(g.d_ids, n, s->grp, s->vel, s->pos[s->cur], (uint8_t)gi);
+        if (s->dim == 3) k3_group_assign<<<grid_for(n), kBlock, 0, s->stream>>>(g.d_ids, n, s->grp, s->vel3, s->pos3[s->cur], (uint8_t)gi);
+        else k_group_assign<<<grid_for(n), kBlock, 0, s->stream>>>(g.d_ids, n, s->grp, s->vel, s->pos[s->cur], (uint8_t)gi);
         s->kernels_launched += 1;
     }
     CUDA_TRY(s, cudaGetLastError());
@@ -916,9 +990,15 @@ lsm_status lsm_step(lsm_sim *s, int64_t n_steps) {
         if (s->compact_every > 0) seg = std::min<long long>(seg, s->compact_every - (s->step - s->last_compact_step) > 0 ? s->compact_every - (s->step - s->last_compact_step) : 1);
         // START: first half kick + drift from the completed state
         {
-            StepParams P = step_params(s, s->step);
-            if (s->exact) k_start<true><<<grid_for(s->N), kBlock, 0, s->stream>>>(P);
-            else k_start<false><<<grid_for(s->N), kBlock, 0, s->stream>>>(P);
+            if (s->dim == 3) {
+                const Step3Params P3 = step_params3(s, s->step, V_MID);
+                if (s->exact) k3_start<true><<<grid_for(s->N), kBlock, 0, s->stream>>>(P3);
+                else k3_start<false><<<grid_for(s->N), kBlock, 0, s->stream>>>(P3);
+            } else {
+                StepParams P = step_params(s, s->step);
+                if (s->exact) k_start<true><<<grid_for(s->N), kBlock, 0, s->stream>>>(P);
+                else k_start<false><<<grid_for(s->N), kBlock, 0, s->stream>>>(P);
+            }
             s->kernels_launched += 1;
             if (gather) s->cur ^= 1;
             else { k_zero_f<<<grid_for(s->N), kBlock, 0, s->stream>>>(s->f, s->N); s->kernels_launched += 1; }
@@ -986,9 +1066,15 @@ lsm_status lsm_sync(lsm_sim *s) {
 lsm_status lsm_write_state(lsm_sim *s, const double *x, const double *v) {
     CHECK_SIM(s);
     if (!x) { s->err = "x is NULL"; return LSM_E_INVALID; }
-    CUDA_TRY(s, cudaMemcpyAsync(s->stage[0], x, sizeof(double2) * s->N, cudaMemcpyHostToDevice, s->stream));
-    if (v) CUDA_TRY(s, cudaMemcpyAsync(s->stage[1], v, sizeof(double2) * s->N, cudaMemcpyHostToDevice, s->stream));
-    k_from_caller<<<grid_for(s->N), kBlock, 0, s->stream>>>(s->stage[0], v ? s->stage[1] : nullptr, s->pos[s->cur], s->vel, s->d_inv, s->N, s->grp);
+    if (s->dim == 3) {
+        CUDA_TRY(s, cudaMemcpyAsync(s->stage3[0], x, sizeof(double) * 3 * s->N, cudaMemcpyHostToDevice, s->stream));
+        if (v) CUDA_TRY(s, cudaMemcpyAsync(s->stage3[1], v, sizeof(double) * 3 * s->N, cudaMemcpyHostToDevice, s->stream));
+        k3_from_caller<<<grid_for(s->N), kBlock, 0, s->stream>>>(s->stage3[0], v ? s->stage3[1] : nullptr, s->pos3[s->cur], s->vel3, s->d_inv, s->N, s->grp);
+    } else {
+        CUDA_TRY(s, cudaMemcpyAsync(s->stage[0], x, sizeof(double2) * s->N, cudaMemcpyHostToDevice, s->stream));
+        if (v) CUDA_TRY(s, cudaMemcpyAsync(s->stage[1], v, sizeof(double2) * s->N, cudaMemcpyHostToDevice, s->stream));
+        k_from_caller<<<grid_for(s->N), kBlock, 0, s->stream>>>(s->stage[0], v ? s->stage[1] : nullptr, s->pos[s->cur], s->vel, s->d_inv, s->N, s->grp);
+    }
     s->kernels_launched += 1;
     for (int g = 0; g < kMaxGroups; ++g) s->groups[g].n0 = s->step;
     TRY(eval_initial(s));
@@ -997,6 +1083,20 @@ lsm_status lsm_write_state(lsm_sim *s, const double *x, const double *v) {
 
 lsm_status lsm_read_state(lsm_sim *s, double *x, double *v) {
     CHECK_SIM(s);
+    if (s->dim == 3) {
+        const GroupTab3 g3 = group_tab3(s);
+        if (x) {
+            k3_to_caller<<<grid_for(s->N), kBlock, 0, s->stream>>>(s->pos3[s->cur], s->stage3[0], s->d_inv, s->N, s->grp, g3, s->dt, 0);
+            CUDA_TRY(s, cudaMemcpyAsync(x, s->stage3[0], sizeof(double) * 3 * s->N, cudaMemcpyDeviceToHost, s->stream));
+            s->kernels_launched += 1;
+        }
+        if (v) {
+            k3_to_caller<<<grid_for(s->N), kBlock, 0, s->stream>>>(s->vel3, s->stage3[1], s->d_inv, s->N, s->grp, g3, s->dt, 1);
+            CUDA_TRY(s, cudaMemcpyAsync(v, s->stage3[1], sizeof(double) * 3 * s->N, cudaMemcpyDeviceToHost, s->stream));
+            s->kernels_launched += 1;
+        }
+        return check_flags(s);
+    }
     const GroupTab g = group_tab(s);
     if (x) {
         k_to_caller<<<grid_for(s->N), kBlock, 0, s->stream>>>(s->pos[s->cur], s->stage[0], s->d_inv, s->N, s->grp, g, s->dt, 0);
@@ -1014,6 +1114,12 @@ lsm_status lsm_read_state(lsm_sim *s, double *x, double *v) {
 lsm_status lsm_read_forces(lsm_sim *s, double *f) {
     CHECK_SIM(s);
     if (!f) { s->err = "f is NULL"; return LSM_E_INVALID; }
+    if (s->dim == 3) {
+        k3_to_caller<<<grid_for(s->N), kBlock, 0, s->stream>>>(s->f3, s->stage3[0], s->d_inv, s->N, s->grp, group_tab3(s), s->dt, 0);
+        s->kernels_launched += 1;
+        CUDA_TRY(s, cudaMemcpyAsync(f, s->stage3[0], sizeof(double) * 3 * s->N, cudaMemcpyDeviceToHost, s->stream));
+        return check_flags(s);
+    }
     k_to_caller<<<grid_for(s->N), kBlock, 0, s->stream>>>(s->f, s->stage[0], s->d_inv, s->N, s->grp, group_tab(s), s->dt, 0);
     s->kernels_launched += 1;
     CUDA_TRY(s, cudaMemcpyAsync(f, s->stage[0], sizeof(double2) * s->N, cudaMemcpyDeviceToHost, s->stream));
@@ -1023,7 +1129,7 @@ lsm_status lsm_read_forces(lsm_sim *s, double *f) {
 lsm_status lsm_read_virial(lsm_sim *s, double *S) {
     CHECK_SIM(s);
     if (!S) { s->err = "S is NULL"; return LSM_E_INVALID; }
-    if (s->force_mode != LSM_FORCE_GATHER) { s->err = "lsm_read_virial needs the gather layout"; return LSM_E_UNSUPPORTED; }
+    if (s->force_mode != LSM_FORCE_GATHER || s->dim != 2) { s->err = "lsm_read_virial needs the 2-D gather layout"; return LSM_E_UNSUPPORTED; }
     if (!s->virial) TRY(dev_alloc(s, &s->virial, (size_t)s->N * 3));
     VirialParams V;
     std::memset(&V, 0, sizeof(V));
@@ -1069,7 +1175,7 @@ lsm_status lsm_read_stress(lsm_sim *s, int64_t capacity, int64_t *n_samples, int
     for (long long t = 0; t < n; ++t) {  // oldest of the last n first
         const long long slot = ((s->hist_head - n + t) % s->hist_cap + s->hist_cap) % s->hist_cap;
         if (step) CUDA_TRY(s, cudaMemcpyAsync(step + t, s->hist_step + slot, sizeof(long long), cudaMemcpyDeviceToHost, s->stream));
-        if (R) CUDA_TRY(s, cudaMemcpyAsync(R + t * B * kMaxGroups * 2, s->hist_R + slot * B * kMaxGroups * 2, sizeof(double) * B * kMaxGroups * 2, cudaMemcpyDeviceToHost, s->stream));
+        if (R) CUDA_TRY(s, cudaMemcpyAsync(R + t * B * kMaxGroups * s->dim, s->hist_R + slot * B * kMaxGroups * s->dim, sizeof(double) * B * kMaxGroups * s->dim, cudaMemcpyDeviceToHost, s->stream));
         if (U) CUDA_TRY(s, cudaMemcpyAsync(U + t * B, s->hist_U + slot * B, sizeof(double) * B, cudaMemcpyDeviceToHost, s->stream));
         if (KE) CUDA_TRY(s, cudaMemcpyAsync(KE + t * B, s->hist_KE + slot * B, sizeof(double) * B, cudaMemcpyDeviceToHost, s->stream));
         if (nb) CUDA_TRY(s, cudaMemcpyAsync(nb + t * B, s->hist_nb + slot * B, sizeof(long long) * B, cudaMemcpyDeviceToHost, s->stream));
@@ -1085,10 +1191,10 @@ lsm_status lsm_read_stress(lsm_sim *s, int64_t capacity, int64_t *n_samples, int
 lsm_status lsm_run_to_failure(lsm_sim *s, int64_t max_steps, int32_t group, int32_t axis, double stop_fraction, int64_t *steps_done,
                               int32_t *failed, double *peak, int64_t *peak_step) {
     CHECK_SIM(s);
-    if (max_steps < 0 || group < 0 || group >= kMaxGroups || axis < 0 || axis > 1 || !(stop_fraction >= 0.0) || !(stop_fraction < 1.0)) { s->err = "bad arguments"; return LSM_E_INVALID; }
+    if (max_steps < 0 || group < 0 || group >= kMaxGroups || axis < 0 || axis >= s->dim || !(stop_fraction >= 0.0) || !(stop_fraction < 1.0)) { s->err = "bad arguments"; return LSM_E_INVALID; }
     if (s->sample_every <= 0) { s->err = "lsm_run_to_failure needs sample_every > 0"; return LSM_E_INVALID; }
     const long long B = s->B;
-    std::vector<double> pk(B, 0.0), R((size_t)B * kMaxGroups * 2);
+    std::vector<double> pk(B, 0.0), R((size_t)B * kMaxGroups * s->dim);
     std::vector<long long> pks(B, -1);
     std::vector<char> done(B, 0);
     long long run = 0, ndone = 0;
@@ -1099,11 +1205,11 @@ lsm_status lsm_run_to_failure(lsm_sim *s, int64_t max_steps, int32_t group, int3
         run += n;
         if (s->step % s->sample_every != 0) break;   // max_steps ended between two samples
         const long long slot = (s->hist_head - 1 + s->hist_cap) % s->hist_cap;   // the sample lsm_step just recorded
-        CUDA_TRY(s, cudaMemcpyAsync(R.data(), s->hist_R + slot * B * kMaxGroups * 2, sizeof(double) * R.size(), cudaMemcpyDeviceToHost, s->stream));
+        CUDA_TRY(s, cudaMemcpyAsync(R.data(), s->hist_R + slot * B * kMaxGroups * s->dim, sizeof(double) * R.size(), cudaMemcpyDeviceToHost, s->stream));
         TRY(check_flags(s));                          // synchronises the stream
         for (long long b = 0; b < B; ++b) {
             if (done[b]) continue;
-            const double r = std::fabs(R[((size_t)b * kMaxGroups + group) * 2 + axis]);
+            const double r = std::fabs(R[((size_t)b * kMaxGroups + group) * s->dim + axis]);
             if (r > pk[b]) { pk[b] = r; pks[b] = s->step; }
             else if (pk[b] > 0.0 && r < stop_fraction * pk[b]) { done[b] = 1; ++ndone; }
         }
@@ -1132,8 +1238,8 @@ lsm_status lsm_get_info(lsm_sim *s, lsm_info *info) {
 
 lsm_status lsm_device_state(lsm_sim *s, const double **pos_xy, const double **vel_xy) {
     CHECK_SIM(s);
-    if (pos_xy) *pos_xy = reinterpret_cast<const double *>(s->pos[s->cur]);
-    if (vel_xy) *vel_xy = reinterpret_cast<const double *>(s->vel);
+    if (pos_xy) *pos_xy = s->dim == 3 ? reinterpret_cast<const double *>(s->pos3[s->cur]) : reinterpret_cast<const double *>(s->pos[s->cur]);
+    if (vel_xy) *vel_xy = s->dim == 3 ? reinterpret_cast<const double *>(s->vel3) : reinterpret_cast<const double *>(s->vel);
     return LSM_OK;
 }
 

@@ -51,8 +51,12 @@ def test_create_validation_before_cuda():
     assert L.lsm_create(C.byref(d), C.byref(h)) == -1 and not h.value
     assert b"ABI" in L.lsm_last_error(None)
     d.struct_size = C.sizeof(LsmDesc)
+    d.dim = 4
+    assert L.lsm_create(C.byref(d), C.byref(h)) == -1            # dim must be 2 or 3
     d.dim = 3
-    assert L.lsm_create(C.byref(d), C.byref(h)) == -7            # LSM_E_UNSUPPORTED
+    d.force_mode = lsm.FORCE_SCATTER
+    assert L.lsm_create(C.byref(d), C.byref(h)) == -7            # LSM_E_UNSUPPORTED: 3-D has no scatter path
+    d.force_mode = lsm.FORCE_AUTO
     d.dim = 2
     d.n_particles = 0
     assert L.lsm_create(C.byref(d), C.byref(h)) == -1

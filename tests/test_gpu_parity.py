@@ -543,3 +543,77 @@ def test_symmetric_grips_run_to_failure_matches_oracle():
     nf, ff, fpeak, _ = f.run_to_failure(20000, group=1, axis=1, stop_fraction=0.1)
     assert ff and abs(nf - steps) <= 0.01 * steps + 100 and abs(fpeak[0] / peak - 1) <= 0.01
     g.close(); f.close()
+
+
+# ---------------------------------------------------------------- D = 3 (the layout of the paper's kernel listing, L93-L97)
+def _problem_3d(n=(9, 8, 7), seed=5, rc_spread=True):
+    from lsm_inputs import cubic_lattice_3d
+    x, si, sj, r0 = cubic_lattice_3d(*n)
+    rng = np.random.default_rng(seed)
+    x = x + rng.uniform(-0.01, 0.01, x.shape)
+    k = rng.choice([1.0, 3.0], si.size)
+    rc = r0 * (rng.uniform(1.05, 1.10, si.size) if rc_spread else 1.06)
+    g = np.round(x).astype(int)
+    bot = np.flatnonzero(g[:, 2] == 0).astype(np.int32)
+    top = np.flatnonzero(g[:, 2] == n[2] - 1).astype(np.int32)
+    return x, si, sj, k, r0, rc, bot, top
+
+
+@pytest.mark.parametrize("exact", [True, False])
+@pytest.mark.parametrize("reorder", [0, 1, 2])
+def test_3d_path_matches_oracle(exact, reorder):
+    """Pulling a perturbed 3-D network apart until springs break: forces at step 0, then 2500 steps with samples and
+    compaction.  Exact mode: x, v, broken set and break steps bit-identical to the oracle; fast mode: the 2-D tolerances."""
+    x, si, sj, k, r0, rc, bot, top = _problem_3d()
+    du = np.array([0.0, 1e-4, 4e-4])
+    o = OracleSim(x, si, sj, k, r0, rc, 0.02, gamma=0.02, sample_every=100)
+    o.set_boundary(0, bot, FIXED); o.set_boundary(1, top, MOVE, du)
+    g = lsm.lsm_create(x, si, sj, k, r0, rc, 0.02, gamma=0.02, sample_every=100, exact=exact, reorder=reorder, compact_every=300)
+    g.set_boundary(0, bot, FIXED); g.set_boundary(1, top, MOVE, du)
+    assert g.D == 3 and g.info()["gather_variant"] == lsm.GATHER_DIRECT and g.info()["step_fusion"] == 0
+    fo, fg = o.read_forces(), g.read_forces()
+    assert fg.shape == (x.shape[0], 3)
+    if exact:
+        assert np.array_equal(fo, fg)
+    else:
+        assert np.abs(fg - fo).max() <= 1e-12 * np.abs(fo).max()
+    o.step(2500); g.step(1200); g.step(1); g.step(1299)
+    xo, vo = o.read_state(); xg, vg = g.read_state()
+    bo, bso, nbo = o.read_broken(); bg, bsg, nbg = g.read_broken()
+    assert nbo > 5
+    ho, hg = o.read_stress(), g.read_stress()
+    assert hg["R"].shape == ho["R"].shape == (25, 1, 8, 3) and np.array_equal(ho["step"], hg["step"])
+    if exact:
+        assert np.array_equal(xo, xg) and np.array_equal(vo, vg) and np.array_equal(bso, bsg)
+        assert np.array_equal(ho["n_broken"], hg["n_broken"])
+        for key in ("R", "U", "KE"):
+            assert np.abs(hg[key] - ho[key]).max() <= 1e-12 * np.abs(ho[key]).max(), key
+    else:
+        first = bso[bso >= 0].min()
+        assert first > 200 and bsg[bsg >= 0].min() == first
+        pre = ho["step"] < first
+        for key in ("R", "U", "KE"):
+            assert np.abs(hg[key][pre] - ho[key][pre]).max() <= 1e-6 * np.abs(ho[key][pre]).max(), key
+    # restart through write_state, and the energies of the current state
+    g.write_state(xo, vo)
+    Uo, KEo = o.read_energy(); Ug, KEg = g.read_energy()
+    assert np.allclose(Ug, Uo, rtol=1e-12) and np.allclose(KEg, KEo, rtol=1e-12)
+    g.close()
+
+
+def test_3d_oscillator_and_unsupported_combinations():
+    """PAPER.md:L123-L127 rotated onto a skew axis, through the CUDA 3-D path; and the combinations the 3-D path does not
+    have yet are refused, not silently downgraded."""
+    n = np.array([1.0, 2.0, 2.0]) / 3.0
+    x = np.array([[0.0, 0.0, 0.0], 15.0 * n])
+    g = lsm.lsm_create(x, [0], [1], 1e-4, 10.0, 100.0, 1.0)
+    g.set_boundary(0, [0], FIXED)
+    g.step(1000)
+    xs, _ = g.read_state()
+    theta = np.arccos(1.0 - 1e-4 / 2)
+    assert np.abs(xs[1] - (10.0 + 5.0 * np.cos(1000 * theta)) * n).max() <= 1e-11
+    g.close()
+    for kw in (dict(force_mode=lsm.FORCE_SCATTER), dict(gather_variant=lsm.GATHER_STREAMED), dict(step_fusion=lsm.FUSION_ON)):
+        with pytest.raises(lsm.LsmError) as ei:
+            lsm.lsm_create(x, [0], [1], 1e-4, 10.0, 100.0, 1.0, **kw)
+        assert ei.value.status == -7

@@ -391,3 +391,52 @@ def test_P13_virial_kinetic_term_and_sum_rule():
     assert np.allclose(S[:, 0].sum(), (g * d[:, 0] ** 2).sum(), rtol=1e-12)
     assert np.allclose(S[:, 2].sum(), (g * d[:, 0] * d[:, 1]).sum(), rtol=1e-11, atol=1e-14)
     assert np.allclose((S[:, 0] + S[:, 1]).sum(), (k * (r - r0) * r).sum(), rtol=1e-12)
+
+
+# ---------------------------------------------------------------- P14: the oracle's D = 3 branch (the paper's listing is 3-D, L93-L97)
+def test_P14_3d_oscillator_along_a_skew_axis_and_invariants():
+    """(a) P1's worked example rotated onto the axis (1,2,2)/3: the 3-D trajectory must be the 1-D closed form along
+    that axis (velocity Verlet commutes with rotations); (b) zero net force and torque, F = -grad U by central
+    differences, on a perturbed cubic network with face diagonals; (c) uniform stretch of a plain cubic network:
+    every interior particle force-free, each face particle pulled back by k (stretch - 1) r0 per bond."""
+    from lsm_inputs import cubic_lattice_3d
+    n = np.array([1.0, 2.0, 2.0]) / 3.0
+    k, r0, dt, m = 1e-4, 10.0, 1.0, 1.0
+    x = np.array([[0.0, 0.0, 0.0], 15.0 * n])
+    s = OracleSim(x, [0], [1], k, r0, 100.0, dt)
+    s.set_boundary(0, [0], FIXED)
+    theta = np.arccos(1.0 - k * dt * dt / (2 * m))
+    for nstep in (1, 10, 250, 1000):
+        s.step(nstep - s.current_step)
+        xs, _ = s.read_state()
+        assert np.abs(xs[1] - (r0 + 5.0 * np.cos(nstep * theta)) * n).max() <= 1e-11
+    # (b)
+    xs, si, sj, r0s = cubic_lattice_3d(4, 3, 5)
+    rng = np.random.default_rng(3)
+    xs = xs + rng.uniform(-0.05, 0.05, xs.shape)
+    ks = rng.uniform(0.5, 2.0, si.size)
+    s = OracleSim(xs, si, sj, ks, r0s, np.full(si.size, 9.0), 0.01)
+    f = s.read_forces()
+    scale = np.abs(f).sum()
+    assert np.abs(f.sum(axis=0)).max() <= 1e-13 * scale and np.abs(np.cross(xs, f).sum(axis=0)).max() <= 1e-12 * scale
+    U0 = s.read_energy()[0][0]
+    d = xs[sj] - xs[si]
+    assert np.isclose(U0, (0.5 * ks * (np.sqrt((d ** 2).sum(axis=1)) - r0s) ** 2).sum(), rtol=1e-13)
+    h = 1e-6
+    for p, c in ((7, 0), (20, 1), (33, 2)):
+        up = []
+        for sgn in (+1, -1):
+            xq = xs.copy(); xq[p, c] += sgn * h
+            up.append(OracleSim(xq, si, sj, ks, r0s, np.full(si.size, 9.0), 0.01).read_energy()[0][0])
+        assert abs(-(up[0] - up[1]) / (2 * h) - f[p, c]) <= 1e-7 * np.abs(f).max()
+    # (c)
+    nx = 5
+    xs, si, sj, r0s = cubic_lattice_3d(nx, nx, nx, diagonals=False)
+    lam, kk = 1.01, 1.7
+    s = OracleSim(xs * lam, si, sj, kk, r0s, np.full(si.size, 9.0), 0.01)
+    f = s.read_forces()
+    g = np.round(xs).astype(int)
+    interior = np.all((g > 0) & (g < nx - 1), axis=1)
+    assert np.abs(f[interior]).max() <= 1e-14
+    face = (g[:, 0] == nx - 1) & np.all((g[:, 1:] > 0) & (g[:, 1:] < nx - 1), axis=1)
+    assert np.allclose(f[face, 0], -kk * (lam - 1.0), rtol=1e-12) and np.abs(f[face, 1:]).max() <= 1e-14
