@@ -180,6 +180,7 @@ GroupTab group_tab(const lsm_sim *s) {
     for (int i = 0; i < kMaxGroups; ++i) {
         g.dux[i] = s->groups[i].set ? s->groups[i].du[0] : 0.0;
         g.duy[i] = s->groups[i].set ? s->groups[i].du[1] : 0.0;
+        g.duz[i] = s->groups[i].set ? s->groups[i].du[2] : 0.0;
         g.n0[i] = s->groups[i].n0;
     }
     return g;
@@ -189,9 +190,16 @@ StepParams step_params(const lsm_sim *s, long long step) {
     StepParams P;
     std::memset(&P, 0, sizeof(P));
     const bool gather = s->force_mode == LSM_FORCE_GATHER;
-    P.pos_cur = s->pos[s->cur];
-    P.pos_next = gather ? s->pos[s->cur ^ 1] : s->pos[s->cur];
-    P.vel = s->vel; P.f = s->f; P.fd = s->fd; P.grp = s->grp; P.mass = s->mass;
+    if (s->dim == 3) {   // the streamed D = 3 instantiation reads these as double4 records (lsm_rows3.cuh)
+        P.pos_cur = reinterpret_cast<const double2 *>(s->pos3[s->cur]);
+        P.pos_next = reinterpret_cast<double2 *>(s->pos3[s->cur ^ 1]);
+        P.vel = reinterpret_cast<double2 *>(s->vel3); P.f = reinterpret_cast<double2 *>(s->f3); P.fd = reinterpret_cast<double2 *>(s->fd3);
+    } else {
+        P.pos_cur = s->pos[s->cur];
+        P.pos_next = gather ? s->pos[s->cur ^ 1] : s->pos[s->cur];
+        P.vel = s->vel; P.f = s->f; P.fd = s->fd;
+    }
+    P.grp = s->grp; P.mass = s->mass;
     P.mass_u = s->mass_u; P.inv_mass_u = 1.0 / s->mass_u;
     P.dt = s->dt; P.hdt = 0.5 * s->dt; P.gamma = s->gamma;
     P.N = s->N; P.step = step;
@@ -278,7 +286,19 @@ template <class K> void stream_opt_in(K kern, const lsm_sim *s, OptIn &done) {
 template <int PM, bool EXACT, bool KICK2, bool ADVANCE, bool SAMPLE> void launch_stream_one(const lsm_sim *s, const StepParams &P) {
     MultiParams M;
     std::memset(&M, 0, sizeof(M));
-    if (s->nbr16) {
+    if (s->dim == 3) {
+        if (s->nbr16) {
+            auto kern = k_gather_stream<PM, EXACT, KICK2, ADVANCE, SAMPLE, false, true, 3>;
+            static thread_local OptIn configured_for;
+            stream_opt_in(kern, s, configured_for);
+            kern<<<s->stream_grid, kTile + 32, s->stream_smem, s->stream>>>(P, s->L, M);
+        } else {
+            auto kern = k_gather_stream<PM, EXACT, KICK2, ADVANCE, SAMPLE, false, false, 3>;
+            static thread_local OptIn configured_for;
+            stream_opt_in(kern, s, configured_for);
+            kern<<<s->stream_grid, kTile + 32, s->stream_smem, s->stream>>>(P, s->L, M);
+        }
+    } else if (s->nbr16) {
         auto kern = k_gather_stream<PM, EXACT, KICK2, ADVANCE, SAMPLE, false, true>;
         static thread_local OptIn configured_for;
         stream_opt_in(kern, s, configured_for);
@@ -339,7 +359,7 @@ template <bool EXACT> void launch_stream_pm(const lsm_sim *s, const StepParams &
 }
 
 void launch_gather(lsm_sim *s, const StepParams &P, Variant v) {
-    if (s->dim == 3) { launch_gather3(s, P.step, v); return; }
+    if (s->dim == 3 && s->gather_variant != 2) { launch_gather3(s, P.step, v); return; }
     if (s->gather_variant == 2) {
         if (s->exact) launch_stream_pm<true>(s, P, v);
         else launch_stream_pm<false>(s, P, v);
@@ -788,8 +808,9 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
             auto up = [](int x) { return (x + 127) & ~127; };
             const int cap = (int)s->max_tile_slots;
             int o = 0;
-            L.pos = o; o += kTile * 16;
-            L.vel = o; o += kTile * 16;
+            const int vb = D == 3 ? 32 : 16;   // bytes per position / velocity record
+            L.pos = o; o += kTile * vb;
+            L.vel = o; o += kTile * vb;
             L.hdr = o; o += 128;
             L.grp = o; o += kTile;
             L.nbr = o; o += up(cap * kSlice * (s->nbr16 ? 2 : 4));
@@ -805,10 +826,13 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
             int ctas_per_sm = kStreamMinB, max_stages = 4;
             if (const char *e = std::getenv("LSM_STREAM_CTAS_PER_SM")) ctas_per_sm = std::max(1, std::min(4, std::atoi(e)));   // tuning overrides
             if (const char *e = std::getenv("LSM_STREAM_STAGES")) max_stages = std::max(2, std::min<int>(kMaxStages, std::atoi(e)));
-            const int budget = std::min(dev_smem, (dev_smem + 1024) / ctas_per_sm - 1024) - L.first;   // 1 KB reserved per CTA
-            L.stages = std::min<int>(max_stages, budget / std::max(L.bytes, 1));
+            // big tiles (high degree, 3-D records): fewer resident CTAs per SM until at least two stages fit
+            for (;; --ctas_per_sm) {
+                const int budget = std::min(dev_smem, (dev_smem + 1024) / ctas_per_sm - 1024) - L.first;   // 1 KB reserved per CTA
+                L.stages = std::min<int>(max_stages, budget / std::max(L.bytes, 1));
+                if (L.stages >= 2 || ctas_per_sm == 1) break;
+            }
             const bool can_stream = L.stages >= 2;
-            if (D == 3) s->gather_variant = 1;
             if (s->gather_variant == 0) s->gather_variant = can_stream ? 2 : 1;
             if (s->gather_variant == 2 && !can_stream) return fail(s, LSM_E_UNSUPPORTED, "gather_variant = streamed: a tile's rows do not fit in shared memory (degree too high); use the direct variant");
             s->stream_smem = L.first + L.stages * L.bytes;
@@ -904,8 +928,8 @@ lsm_status lsm_create(const lsm_desc *d, lsm_sim **out) {
     if (!d || !out) return fail(nullptr, LSM_E_INVALID, "desc / out is NULL");
     if (d->struct_size != sizeof(lsm_desc)) return fail(nullptr, LSM_E_INVALID, "lsm_desc.struct_size does not match this library (ABI mismatch)");
     if (d->dim != 2 && d->dim != 3) return fail(nullptr, LSM_E_INVALID, "dim must be 2 or 3");
-    if (d->dim == 3 && (d->force_mode == LSM_FORCE_SCATTER || d->gather_variant == LSM_GATHER_STREAMED || d->step_fusion == LSM_FUSION_ON))
-        return fail(nullptr, LSM_E_UNSUPPORTED, "dim = 3 runs on the direct gather kernel only (no scatter path, streaming or step fusion yet)");
+    if (d->dim == 3 && (d->force_mode == LSM_FORCE_SCATTER || d->step_fusion == LSM_FUSION_ON))
+        return fail(nullptr, LSM_E_UNSUPPORTED, "dim = 3 has no scatter path and no step fusion yet");
     if (d->n_particles < 1 || d->n_springs < 0 || d->n_particles >= 2147483647LL || d->n_springs >= 2147483647LL) return fail(nullptr, LSM_E_INVALID, "need 1 <= N < 2^31-1 and 0 <= M < 2^31-1");
     if (d->n_batch < 1 || !d->x) return fail(nullptr, LSM_E_INVALID, "n_batch < 1 or x is NULL");
     if (!(d->dt > 0.0) || !(d->gamma >= 0.0) || !std::isfinite(d->dt) || !std::isfinite(d->gamma)) return fail(nullptr, LSM_E_INVALID, "need dt > 0 and gamma >= 0");

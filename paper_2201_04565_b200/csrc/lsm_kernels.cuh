@@ -55,7 +55,7 @@ struct __align__(16) TileHdr {          // 64 bytes per tile of 256 particles
 static_assert(sizeof(TileHdr) == 64, "TileHdr must be 64 bytes");
 
 struct GroupTab {
-    double dux[kMaxGroups], duy[kMaxGroups];
+    double dux[kMaxGroups], duy[kMaxGroups], duz[kMaxGroups];   // duz: D = 3 only
     long long n0[kMaxGroups];
 };
 
@@ -454,7 +454,13 @@ struct MultiParams {
     double2 *pos_a, *pos_b;           // step i reads pos_a / writes pos_b when i is even, the reverse when odd
 };
 
-template <int PM, bool EXACT, bool KICK2, bool ADVANCE, bool SAMPLE, bool MULTI, bool I16>
+}  // namespace lsmk
+#include "lsm_rows3.cuh"
+namespace lsmk {
+
+// D = 3: the same pipeline with 32-byte {x, y, z, 0} position / velocity records (the pointers of StepParams / StepVar /
+// MultiParams then address double4) and the row functions of lsm_rows3.cuh; D = 3 is not instantiated with MULTI.
+template <int PM, bool EXACT, bool KICK2, bool ADVANCE, bool SAMPLE, bool MULTI, bool I16, int D = 2>
 __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const StepParams P, const StageLayout L, const MultiParams M) {
     constexpr bool kTab = (PM == PM_TYPED || PM == PM_KRT_RCF);
     constexpr bool kHasThr = (PM == PM_RCF || PM == PM_KRT_RCF || PM == PM_FULL);
@@ -476,6 +482,7 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
     if (kTab) for (int i = tid; i < kTabStride * P.sp.ntypes; i += kTile + 32) s_tab[i] = P.sp.tab[i];
     __syncthreads();
     const int nsteps = MULTI ? M.nsteps : 1;
+    constexpr int kVB = D == 3 ? 32 : 16;   // bytes of one position / velocity record
 
     if (wi == kTileSlices) {  // ---------------- producer warp ----------------
         if (lane == 0) {
@@ -500,14 +507,14 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
                     if (t + gridDim.x < P.T) { o0n = __ldg(&h[gridDim.x].off[0]); o8n = __ldg(&h[gridDim.x].off[kTileSlices]); }  // next tile's extent, ahead of the wait
                     if (u > 0) mbar_wait(empty + s, (u - 1) & 1);
                     constexpr unsigned kIdB = I16 ? 2 : 4;   // bytes per streamed neighbour id
-                    unsigned bytes = 2 * kTile * 16 + kTile + 64 + ns * (kSlice * kIdB);
+                    unsigned bytes = 2 * kTile * kVB + kTile + 64 + ns * (kSlice * kIdB);
                     if (kHasThr) bytes += ns * (kSlice * 2);
                     if (kHasTyp) bytes += ns * kSlice;
                     if (kHasKR) bytes += 2 * ns * (kSlice * 8);
                     unsigned char *b = stage0 + (size_t)s * L.bytes;
                     mbar_expect_tx(full + s, bytes);
-                    bulk_g2s(b + L.pos, pos_cur + t * kTile, kTile * 16, full + s);
-                    bulk_g2s(b + L.vel, P.vel + t * kTile, kTile * 16, full + s);
+                    bulk_g2s(b + L.pos, reinterpret_cast<const char *>(pos_cur) + t * (kTile * kVB), kTile * kVB, full + s);
+                    bulk_g2s(b + L.vel, reinterpret_cast<const char *>(P.vel) + t * (kTile * kVB), kTile * kVB, full + s);
                     bulk_g2s(b + L.grp, P.grp + t * kTile, kTile, full + s);
                     bulk_g2s(b + L.hdr, h, 64, full + s);
                     if (ns) {
@@ -544,7 +551,6 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
             if (p < P.N) {
                 const unsigned w = h->w[wi];
                 const unsigned rel = (h->off[wi] - h->off[0]) * kSlice + lane;
-                const double2 xp = reinterpret_cast<const double2 *>(b + L.pos)[tid];
                 RowSrc R;
                 R.nbr = reinterpret_cast<const int32_t *>(b + L.nbr) + rel;
                 R.nbr16 = reinterpret_cast<const int16_t *>(b + L.nbr) + rel;
@@ -553,17 +559,29 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
                 R.kF = reinterpret_cast<const double *>(b + L.kF) + rel;
                 R.r0F = reinterpret_cast<const double *>(b + L.r0F) + rel;
                 R.e0 = (size_t)h->off[wi] * kSlice + lane;
-                double fx = 0.0, fy = 0.0, uu = 0.0;
-#ifndef LSM_DEBUG_NOFORCE   // tuning probe only: skip the spring evaluation to expose the copy pipeline's own ceiling
-                row_forces<PM, EXACT, SAMPLE, MULTI, I16>(P, V, R, s_tab, (int)p, w, xp, fx, fy, uu);
+                if constexpr (D == 3) {
+                    const double4 xp = reinterpret_cast<const double4 *>(b + L.pos)[tid];
+                    double fx = 0.0, fy = 0.0, fz = 0.0, uu = 0.0;
+#ifndef LSM_DEBUG_NOFORCE
+                    row_forces3<PM, EXACT, SAMPLE, MULTI, I16>(P, V, R, s_tab, (int)p, w, xp, fx, fy, fz, uu);
 #endif
-                const double2 vh = reinterpret_cast<const double2 *>(b + L.vel)[tid];
-                const uint8_t g = (b + L.grp)[tid];
-                if (MULTI && M.resident)
-                    particle_update<EXACT, KICK2, ADVANCE, SAMPLE>(P, V, p, xp, vh, g, fx, fy, uu, reinterpret_cast<double2 *>(b + L.pos) + tid,
-                                                                   reinterpret_cast<double2 *>(b + L.vel) + tid);
-                else
-                    particle_update<EXACT, KICK2, ADVANCE, SAMPLE>(P, V, p, xp, vh, g, fx, fy, uu);
+                    const double4 vh = reinterpret_cast<const double4 *>(b + L.vel)[tid];
+                    const uint8_t g = (b + L.grp)[tid];
+                    particle_update3<EXACT, KICK2, ADVANCE, SAMPLE>(P, V, p, xp, vh, g, fx, fy, fz, uu);
+                } else {
+                    const double2 xp = reinterpret_cast<const double2 *>(b + L.pos)[tid];
+                    double fx = 0.0, fy = 0.0, uu = 0.0;
+#ifndef LSM_DEBUG_NOFORCE   // tuning probe only: skip the spring evaluation to expose the copy pipeline's own ceiling
+                    row_forces<PM, EXACT, SAMPLE, MULTI, I16>(P, V, R, s_tab, (int)p, w, xp, fx, fy, uu);
+#endif
+                    const double2 vh = reinterpret_cast<const double2 *>(b + L.vel)[tid];
+                    const uint8_t g = (b + L.grp)[tid];
+                    if (MULTI && M.resident)
+                        particle_update<EXACT, KICK2, ADVANCE, SAMPLE>(P, V, p, xp, vh, g, fx, fy, uu, reinterpret_cast<double2 *>(b + L.pos) + tid,
+                                                                       reinterpret_cast<double2 *>(b + L.vel) + tid);
+                    else
+                        particle_update<EXACT, KICK2, ADVANCE, SAMPLE>(P, V, p, xp, vh, g, fx, fy, uu);
+                }
             }
             __syncwarp();
             if (lane == 0 && !(MULTI && M.resident)) mbar_arrive(empty + s);

@@ -560,17 +560,18 @@ def _problem_3d(n=(9, 8, 7), seed=5, rc_spread=True):
 
 
 @pytest.mark.parametrize("exact", [True, False])
-@pytest.mark.parametrize("reorder", [0, 1, 2])
-def test_3d_path_matches_oracle(exact, reorder):
-    """Pulling a perturbed 3-D network apart until springs break: forces at step 0, then 2500 steps with samples and
-    compaction.  Exact mode: x, v, broken set and break steps bit-identical to the oracle; fast mode: the 2-D tolerances."""
+@pytest.mark.parametrize("reorder,variant", [(0, 2), (1, 2), (2, 2), (0, 1), (2, 1)])
+def test_3d_path_matches_oracle(exact, reorder, variant):
+    """Pulling a perturbed 3-D network apart until springs break (streamed kernel = variant 2, plain direct kernel =
+    variant 1): forces at step 0, then 2500 steps with samples and compaction.  Exact mode: x, v, broken set and break steps bit-identical to the oracle; fast mode: the 2-D tolerances."""
     x, si, sj, k, r0, rc, bot, top = _problem_3d()
     du = np.array([0.0, 1e-4, 4e-4])
     o = OracleSim(x, si, sj, k, r0, rc, 0.02, gamma=0.02, sample_every=100)
     o.set_boundary(0, bot, FIXED); o.set_boundary(1, top, MOVE, du)
-    g = lsm.lsm_create(x, si, sj, k, r0, rc, 0.02, gamma=0.02, sample_every=100, exact=exact, reorder=reorder, compact_every=300)
+    g = lsm.lsm_create(x, si, sj, k, r0, rc, 0.02, gamma=0.02, sample_every=100, exact=exact, reorder=reorder, compact_every=300,
+                       gather_variant=variant)
     g.set_boundary(0, bot, FIXED); g.set_boundary(1, top, MOVE, du)
-    assert g.D == 3 and g.info()["gather_variant"] == lsm.GATHER_DIRECT and g.info()["step_fusion"] == 0
+    assert g.D == 3 and g.info()["gather_variant"] == variant and g.info()["step_fusion"] == 0
     fo, fg = o.read_forces(), g.read_forces()
     assert fg.shape == (x.shape[0], 3)
     if exact:
@@ -613,7 +614,7 @@ def test_3d_oscillator_and_unsupported_combinations():
     theta = np.arccos(1.0 - 1e-4 / 2)
     assert np.abs(xs[1] - (10.0 + 5.0 * np.cos(1000 * theta)) * n).max() <= 1e-11
     g.close()
-    for kw in (dict(force_mode=lsm.FORCE_SCATTER), dict(gather_variant=lsm.GATHER_STREAMED), dict(step_fusion=lsm.FUSION_ON)):
+    for kw in (dict(force_mode=lsm.FORCE_SCATTER), dict(step_fusion=lsm.FUSION_ON)):
         with pytest.raises(lsm.LsmError) as ei:
             lsm.lsm_create(x, [0], [1], 1e-4, 10.0, 100.0, 1.0, **kw)
         assert ei.value.status == -7
