@@ -618,3 +618,20 @@ def test_3d_oscillator_and_unsupported_combinations():
         with pytest.raises(lsm.LsmError) as ei:
             lsm.lsm_create(x, [0], [1], 1e-4, 10.0, 100.0, 1.0, **kw)
         assert ei.value.status == -7
+
+
+def test_step_fusion_non_resident_pipeline_large_lattice():
+    """Forced step fusion on a lattice too large for its tiles to stay resident in shared memory (T > CTAs x stages):
+    the fused launch then refills its pipeline from global memory after every grid barrier (generic-proxy stores ->
+    fence.proxy.async -> bulk copies).  Exact mode, 250 steps: bit-identical to the oracle."""
+    p = config2(n=720, n_blobs=80)
+    p.sample_every = 100
+    o = OracleSim.from_problem(p); o.step(250)
+    g = lsm_create_from_problem(p, exact=True, step_fusion=lsm.FUSION_ON)
+    inf = g.info()
+    assert inf["step_fusion"] == 1 and (p.N + 255) // 256 > 3 * 148 * inf["pipeline_stages"]
+    g.step(250)
+    xo, vo = o.read_state(); xg, vg = g.read_state()
+    assert np.array_equal(xo, xg) and np.array_equal(vo, vg)
+    assert g.info()["kernels_launched"] - inf["kernels_launched"] < 40
+    g.close()
