@@ -635,3 +635,38 @@ def test_step_fusion_non_resident_pipeline_large_lattice():
     assert np.array_equal(xo, xg) and np.array_equal(vo, vg)
     assert g.info()["kernels_launched"] - inf["kernels_launched"] < 40
     g.close()
+
+
+@pytest.mark.parametrize("pm", [3, 4])
+@pytest.mark.parametrize("variant", [1, 2])
+def test_all_parameter_encodings(pm, variant):
+    """Parameter modes 3 (k, r0 from a type table + rc per spring) and 4 (k, r0, rc all per spring, > 256 distinct
+    values each) on both gather kernels: forces at step 0 (1e-12) and a 1500-step pull with breakage, bit-identical in
+    exact mode."""
+    x, si, sj, site, _ = triangular_lattice(40, 36)
+    rng = np.random.default_rng(17)
+    M = si.size
+    if pm == 3:
+        k = rng.choice([0.7, 1.0, 2.5], M); r0 = rng.choice([0.98, 1.0, 1.02], M)
+    else:
+        k = rng.uniform(0.5, 2.0, M); r0 = rng.uniform(0.97, 1.03, M)
+    rc = r0 * rng.uniform(1.04, 1.12, M)
+    row = site // 40
+    bot = np.flatnonzero(row == 0).astype(np.int32); top = np.flatnonzero(row == 35).astype(np.int32)
+    du = np.array([1e-4, 6e-4])
+    o = OracleSim(x, si, sj, k, r0, rc, 0.03, gamma=0.02, sample_every=100)
+    o.set_boundary(0, bot, FIXED); o.set_boundary(1, top, MOVE, du)
+    fo = o.read_forces()
+    for exact in (False, True):
+        g = lsm.lsm_create(x, si, sj, k, r0, rc, 0.03, gamma=0.02, sample_every=100, exact=exact, gather_variant=variant,
+                           compact_every=400)
+        g.set_boundary(0, bot, FIXED); g.set_boundary(1, top, MOVE, du)
+        assert g.info()["param_mode"] == pm
+        fg = g.read_forces()
+        assert np.abs(fg - fo).max() <= 1e-12 * np.abs(fo).max() and (not exact or np.array_equal(fg, fo))
+        if exact:
+            o.step(1500); g.step(1500)
+            xo, vo = o.read_state(); xg, vg = g.read_state()
+            bo, bso, nbo = o.read_broken(); bg, bsg, nbg = g.read_broken()
+            assert nbo > 0 and np.array_equal(bso, bsg) and np.array_equal(xo, xg) and np.array_equal(vo, vg)
+        g.close()
