@@ -16,7 +16,7 @@
  *   - plain C; no exceptions or C++ types cross the boundary; every function returns lsm_status unless noted.
  *   - dim = 2 is the tuned path (all configurations of the paper and of BASELINE.json are 2-D).  dim = 3 (the layout of
  *     the paper's kernel listing) has the same semantics and entry points, vectors [N*3], on the
- *     streamed kernel with 32-byte records (or the plain direct kernel); no scatter path, step fusion or virial there.
+ *     streamed kernel with 32-byte records (or the plain direct kernel); no scatter path and no virial there.
  *   - HOST pointers unless a parameter says DEVICE.  Vector arrays are interleaved [N*dim] (x0 y0 x1 y1 ...) as in the
  *     paper's flattened 1-D arrays.  Inputs are borrowed for the duration of the call and copied;
  *     outputs are caller-allocated buffers of the documented size.  The handle owns all device memory.
@@ -50,7 +50,7 @@ typedef enum {
     LSM_E_NOMEM = -5,       /* host or device allocation failed                                                    */
     LSM_E_STATE = -6,       /* the simulation failed earlier (e.g. non-finite energy detected on the device)       */
     LSM_E_UNSUPPORTED = -7  /* exact arithmetic with the scatter kernel, degree > 255 in the gather layout, a dim = 3
-                               request for the scatter / fused / virial paths                            */
+                               request for the scatter / virial paths                            */
 } lsm_status;
 
 enum { LSM_FIXED = 0, LSM_MOVE = 1 };                      /* boundary group modes */

@@ -317,6 +317,18 @@ template <int PM, bool EXACT> cudaError_t launch_stream_multi_one(const lsm_sim 
     void *args[3] = {&P, &L, &M};
     // (a grid the device cannot keep resident makes cudaLaunchCooperativeKernel fail with
     //  cudaErrorCooperativeLaunchTooLarge instead of deadlocking at the grid barrier; lsm_step reports it)
+    if (s->dim == 3) {
+        if (s->nbr16) {
+            auto kern = k_gather_stream<PM, EXACT, true, true, false, true, true, 3>;
+            static thread_local OptIn configured_for;
+            stream_opt_in(kern, s, configured_for);
+            return cudaLaunchCooperativeKernel((const void *)kern, dim3(s->stream_grid), dim3(kTile + 32), args, (size_t)s->stream_smem, s->stream);
+        }
+        auto kern = k_gather_stream<PM, EXACT, true, true, false, true, false, 3>;
+        static thread_local OptIn configured_for;
+        stream_opt_in(kern, s, configured_for);
+        return cudaLaunchCooperativeKernel((const void *)kern, dim3(s->stream_grid), dim3(kTile + 32), args, (size_t)s->stream_smem, s->stream);
+    }
     if (s->nbr16) {
         auto kern = k_gather_stream<PM, EXACT, true, true, false, true, true>;
         static thread_local OptIn configured_for;
@@ -845,7 +857,7 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
             long long fuse_below = 1 << 18;   // measured: 64^2 5.8 -> 3.6 us per step, 512^2 8.4 -> 8.3, 2.1 M particles 39.1 -> 40.4
             if (const char *e = std::getenv("LSM_FUSE_BELOW")) fuse_below = std::atoll(e);
             if (s->step_fusion == LSM_FUSION_ON && !(coop && s->gather_variant == 2)) return fail(s, LSM_E_UNSUPPORTED, "step_fusion = ON needs the streamed gather kernel and cooperative launch support");
-            s->multi_on = D == 2 && coop && s->gather_variant == 2 && (s->step_fusion == LSM_FUSION_ON || (s->step_fusion == LSM_FUSION_AUTO && N <= fuse_below));
+            s->multi_on = coop && s->gather_variant == 2 && (s->step_fusion == LSM_FUSION_ON || (s->step_fusion == LSM_FUSION_AUTO && N <= fuse_below));
             if (s->multi_on) {
                 TRY(dev_alloc(s, &s->gbar, 1));
                 CUDA_TRY(s, cudaMemsetAsync(s->gbar, 0, sizeof(unsigned long long), s->stream));
@@ -928,8 +940,7 @@ lsm_status lsm_create(const lsm_desc *d, lsm_sim **out) {
     if (!d || !out) return fail(nullptr, LSM_E_INVALID, "desc / out is NULL");
     if (d->struct_size != sizeof(lsm_desc)) return fail(nullptr, LSM_E_INVALID, "lsm_desc.struct_size does not match this library (ABI mismatch)");
     if (d->dim != 2 && d->dim != 3) return fail(nullptr, LSM_E_INVALID, "dim must be 2 or 3");
-    if (d->dim == 3 && (d->force_mode == LSM_FORCE_SCATTER || d->step_fusion == LSM_FUSION_ON))
-        return fail(nullptr, LSM_E_UNSUPPORTED, "dim = 3 has no scatter path and no step fusion yet");
+    if (d->dim == 3 && d->force_mode == LSM_FORCE_SCATTER) return fail(nullptr, LSM_E_UNSUPPORTED, "dim = 3 has no scatter path");
     if (d->n_particles < 1 || d->n_springs < 0 || d->n_particles >= 2147483647LL || d->n_springs >= 2147483647LL) return fail(nullptr, LSM_E_INVALID, "need 1 <= N < 2^31-1 and 0 <= M < 2^31-1");
     if (d->n_batch < 1 || !d->x) return fail(nullptr, LSM_E_INVALID, "n_batch < 1 or x is NULL");
     if (!(d->dt > 0.0) || !(d->gamma >= 0.0) || !std::isfinite(d->dt) || !std::isfinite(d->gamma)) return fail(nullptr, LSM_E_INVALID, "need dt > 0 and gamma >= 0");
@@ -1039,7 +1050,8 @@ lsm_status lsm_step(lsm_sim *s, int64_t n_steps) {
                     StepParams P = step_params(s, m);
                     MultiParams Mp;
                     Mp.nsteps = (int)run; Mp.gbar = s->gbar; Mp.gbar_base = s->gbar_base;
-                    Mp.pos_a = s->pos[s->cur]; Mp.pos_b = s->pos[s->cur ^ 1];
+                    if (s->dim == 3) { Mp.pos_a = reinterpret_cast<double2 *>(s->pos3[s->cur]); Mp.pos_b = reinterpret_cast<double2 *>(s->pos3[s->cur ^ 1]); }
+                    else { Mp.pos_a = s->pos[s->cur]; Mp.pos_b = s->pos[s->cur ^ 1]; }
                     Mp.resident = (s->T + s->stream_grid - 1) / s->stream_grid <= s->L.stages;
                     CUDA_TRY(s, s->exact ? launch_stream_multi_pm<true>(s, P, Mp) : launch_stream_multi_pm<false>(s, P, Mp));
                     s->gbar_base += (unsigned long long)(run - 1) * (unsigned long long)s->stream_grid;

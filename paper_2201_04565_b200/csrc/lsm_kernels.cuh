@@ -459,7 +459,7 @@ struct MultiParams {
 namespace lsmk {
 
 // D = 3: the same pipeline with 32-byte {x, y, z, 0} position / velocity records (the pointers of StepParams / StepVar /
-// MultiParams then address double4) and the row functions of lsm_rows3.cuh; D = 3 is not instantiated with MULTI.
+// MultiParams then address double4) and the row functions of lsm_rows3.cuh.
 template <int PM, bool EXACT, bool KICK2, bool ADVANCE, bool SAMPLE, bool MULTI, bool I16, int D = 2>
 __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const StepParams P, const StageLayout L, const MultiParams M) {
     constexpr bool kTab = (PM == PM_TYPED || PM == PM_KRT_RCF);
@@ -567,7 +567,11 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
 #endif
                     const double4 vh = reinterpret_cast<const double4 *>(b + L.vel)[tid];
                     const uint8_t g = (b + L.grp)[tid];
-                    particle_update3<EXACT, KICK2, ADVANCE, SAMPLE>(P, V, p, xp, vh, g, fx, fy, fz, uu);
+                    if (MULTI && M.resident)
+                        particle_update3<EXACT, KICK2, ADVANCE, SAMPLE>(P, V, p, xp, vh, g, fx, fy, fz, uu, reinterpret_cast<double4 *>(b + L.pos) + tid,
+                                                                        reinterpret_cast<double4 *>(b + L.vel) + tid);
+                    else
+                        particle_update3<EXACT, KICK2, ADVANCE, SAMPLE>(P, V, p, xp, vh, g, fx, fy, fz, uu);
                 } else {
                     const double2 xp = reinterpret_cast<const double2 *>(b + L.pos)[tid];
                     double fx = 0.0, fy = 0.0, uu = 0.0;

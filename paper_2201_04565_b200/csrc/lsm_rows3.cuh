@@ -123,7 +123,7 @@ __device__ __forceinline__ void row_forces3(const StepParams &P, const StepVar &
 // Velocity-Verlet particle update in 3-D (see particle_update): same order, same rounding sequence.
 template <bool EXACT, bool KICK2, bool ADVANCE, bool SAMPLE>
 __device__ __forceinline__ void particle_update3(const StepParams &P, const StepVar &V, long long p, double4 xp, double4 vh, uint8_t g,
-                                                 double fx, double fy, double fz, double u) {
+                                                 double fx, double fy, double fz, double u, double4 *own_pos = nullptr, double4 *own_vel = nullptr) {
     double4 *pos_next = as4(V.pos_next), *vel = as4(P.vel), *f = as4(P.f), *fd = as4(P.fd);
     if (g == kFree) {
         const double fdx = sub<EXACT>(fx, mul<EXACT>(P.gamma, vh.x)), fdy = sub<EXACT>(fy, mul<EXACT>(P.gamma, vh.y)),
@@ -148,6 +148,7 @@ __device__ __forceinline__ void particle_update3(const StepParams &P, const Step
             xn.x = mad<EXACT>(P.dt, w.x, xp.x); xn.y = mad<EXACT>(P.dt, w.y, xp.y); xn.z = mad<EXACT>(P.dt, w.z, xp.z); xn.w = 0.0;
             pos_next[p] = xn;
             vel[p] = w;
+            if (own_pos) { *own_pos = xn; *own_vel = w; }   // resident tiles: the staged copy is the next step's input
         } else {
             vel[p] = v;
             fd[p] = make_double4(fdx, fdy, fdz, 0.0);
@@ -157,7 +158,9 @@ __device__ __forceinline__ void particle_update3(const StepParams &P, const Step
         if (SAMPLE || !ADVANCE) f[p] = make_double4(fx, fy, fz, 0.0);
         if (ADVANCE) {
             const double ns = (double)(V.step + 1 - P.g.n0[g]);
-            pos_next[p] = make_double4(mad<EXACT>(ns, P.g.dux[g], vh.x), mad<EXACT>(ns, P.g.duy[g], vh.y), mad<EXACT>(ns, P.g.duz[g], vh.z), 0.0);
+            const double4 xn = make_double4(mad<EXACT>(ns, P.g.dux[g], vh.x), mad<EXACT>(ns, P.g.duy[g], vh.y), mad<EXACT>(ns, P.g.duz[g], vh.z), 0.0);
+            pos_next[p] = xn;
+            if (own_pos) *own_pos = xn;
         } else {
             fd[p] = make_double4(fx, fy, fz, 0.0);
         }

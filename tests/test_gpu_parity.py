@@ -571,7 +571,7 @@ def test_3d_path_matches_oracle(exact, reorder, variant):
     g = lsm.lsm_create(x, si, sj, k, r0, rc, 0.02, gamma=0.02, sample_every=100, exact=exact, reorder=reorder, compact_every=300,
                        gather_variant=variant)
     g.set_boundary(0, bot, FIXED); g.set_boundary(1, top, MOVE, du)
-    assert g.D == 3 and g.info()["gather_variant"] == variant and g.info()["step_fusion"] == 0
+    assert g.D == 3 and g.info()["gather_variant"] == variant and g.info()["step_fusion"] == (1 if variant == 2 else 0)
     fo, fg = o.read_forces(), g.read_forces()
     assert fg.shape == (x.shape[0], 3)
     if exact:
@@ -614,7 +614,7 @@ def test_3d_oscillator_and_unsupported_combinations():
     theta = np.arccos(1.0 - 1e-4 / 2)
     assert np.abs(xs[1] - (10.0 + 5.0 * np.cos(1000 * theta)) * n).max() <= 1e-11
     g.close()
-    for kw in (dict(force_mode=lsm.FORCE_SCATTER), dict(step_fusion=lsm.FUSION_ON)):
+    for kw in (dict(force_mode=lsm.FORCE_SCATTER), dict(step_fusion=lsm.FUSION_ON, gather_variant=lsm.GATHER_DIRECT)):
         with pytest.raises(lsm.LsmError) as ei:
             lsm.lsm_create(x, [0], [1], 1e-4, 10.0, 100.0, 1.0, **kw)
         assert ei.value.status == -7
