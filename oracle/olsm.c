@@ -327,26 +327,36 @@ int32_t olsm_read_energy(const olsm_sim *s, double *U, double *KE)
 
 /* Per-particle virial, Eq. 7 without the 1/Omega factor (the caller divides by a volume):
  *   S^k_ij = 1/2 sum_l (x^l_i - x^k_i) f^kl_j  -  m^k v^k_i v^k_j ,   f^kl = force on k from its spring to l (Eq. 2).
- * Serial loop over the alive springs in caller order; out[k] = {S_xx, S_yy, S_xy} (2-D, symmetric: central forces).
+ * Serial loop over the alive springs in caller order; out[k] = {S_xx, S_yy, S_xy} in 2-D, {S_xx, S_yy, S_zz, S_xy, S_yz,
+ * S_zx} in 3-D (symmetric: central forces).
  * Tension is positive.  Broken springs and coincident endpoints contribute nothing (Q3, Q4). */
 int32_t olsm_read_virial(const olsm_sim *s, double *out)
 {
-    if (!s || !out || s->D != 2) return -1;
-    for (int64_t q = 0; q < 3 * s->N; ++q) out[q] = 0.0;
+    if (!s || !out) return -1;
+    const int D = s->D, C = D == 2 ? 3 : 6;   /* D = 3: out[k] = {S_xx, S_yy, S_zz, S_xy, S_yz, S_zx} */
+    for (int64_t q = 0; q < C * s->N; ++q) out[q] = 0.0;
     for (int64_t e = 0; e < s->M; ++e) {
         if (!s->alive[e]) continue;
         const int64_t i = s->si[e], j = s->sj[e];
-        const double dx = s->x[2 * j] - s->x[2 * i], dy = s->x[2 * j + 1] - s->x[2 * i + 1];
-        const double r = sqrt(dx * dx + dy * dy);
+        double d[3] = {0.0, 0.0, 0.0}, r2 = 0.0;
+        for (int c = 0; c < D; ++c) { d[c] = s->x[D * j + c] - s->x[D * i + c]; r2 = r2 + d[c] * d[c]; }
+        const double r = sqrt(r2);
         if (r == 0.0) continue;
         const double g = s->k[e] * (r - s->r0[e]) / r;      /* f^ij = g d,  f^ji = -g (-d): same dyad on both ends */
         const double h = 0.5 * g;
-        out[3 * i] += h * dx * dx; out[3 * i + 1] += h * dy * dy; out[3 * i + 2] += h * dx * dy;
-        out[3 * j] += h * dx * dx; out[3 * j + 1] += h * dy * dy; out[3 * j + 2] += h * dx * dy;
+        double t[6];
+        if (D == 2) { t[0] = h * d[0] * d[0]; t[1] = h * d[1] * d[1]; t[2] = h * d[0] * d[1]; }
+        else { t[0] = h * d[0] * d[0]; t[1] = h * d[1] * d[1]; t[2] = h * d[2] * d[2]; t[3] = h * d[0] * d[1]; t[4] = h * d[1] * d[2]; t[5] = h * d[2] * d[0]; }
+        for (int c = 0; c < C; ++c) { out[C * i + c] += t[c]; out[C * j + c] += t[c]; }
     }
     for (int64_t p = 0; p < s->N; ++p) {
-        const double vx = s->v[2 * p], vy = s->v[2 * p + 1];
-        out[3 * p] -= s->m[p] * vx * vx; out[3 * p + 1] -= s->m[p] * vy * vy; out[3 * p + 2] -= s->m[p] * vx * vy;
+        const double *v = s->v + D * p;
+        const double m = s->m[p];
+        if (D == 2) { out[3 * p] -= m * v[0] * v[0]; out[3 * p + 1] -= m * v[1] * v[1]; out[3 * p + 2] -= m * v[0] * v[1]; }
+        else {
+            out[6 * p] -= m * v[0] * v[0]; out[6 * p + 1] -= m * v[1] * v[1]; out[6 * p + 2] -= m * v[2] * v[2];
+            out[6 * p + 3] -= m * v[0] * v[1]; out[6 * p + 4] -= m * v[1] * v[2]; out[6 * p + 5] -= m * v[2] * v[0];
+        }
     }
     return 0;
 }

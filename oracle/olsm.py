@@ -132,8 +132,8 @@ class OracleSim:
         return U, KE
 
     def read_virial(self):
-        """Per-particle virial (Eq. 7 without 1/Omega): [N,3] = S_xx, S_yy, S_xy."""
-        S = np.empty((self.N, 3))
+        """Per-particle virial (Eq. 7 without 1/Omega): [N,3] = S_xx, S_yy, S_xy; 3-D: [N,6] = xx, yy, zz, xy, yz, zx."""
+        S = np.empty((self.N, 3 if self.D == 2 else 6))
         if lib().olsm_read_virial(self._h, _p(S, C.c_double)) != 0:
             raise ValueError("olsm_read_virial failed")
         return S

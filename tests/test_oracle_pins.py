@@ -440,3 +440,29 @@ def test_P14_3d_oscillator_along_a_skew_axis_and_invariants():
     assert np.abs(f[interior]).max() <= 1e-14
     face = (g[:, 0] == nx - 1) & np.all((g[:, 1:] > 0) & (g[:, 1:] < nx - 1), axis=1)
     assert np.allclose(f[face, 0], -kk * (lam - 1.0), rtol=1e-12) and np.abs(f[face, 1:]).max() <= 1e-14
+
+
+def test_P13_virial_3d_uniform_stretch_and_sum_rule():
+    """3-D virial: a plain cubic network stretched uniformly by lam has, at every interior particle, the diagonal virial
+    S_cc = 1/2 * 2 bonds * k (lam - 1) r0 * lam r0 per axis = the Cauchy stress k (lam-1)/(lam r0) x the cell volume
+    lam^3; off-diagonals 0.  Sum rule on a perturbed network with diagonals: sum_p tr S_p = sum_s k (r - r0) r."""
+    from lsm_inputs import cubic_lattice_3d
+    nx, lam, kk = 5, 1.02, 1.7
+    xs, si, sj, r0s = cubic_lattice_3d(nx, nx, nx, diagonals=False)
+    s = OracleSim(xs * lam, si, sj, kk, r0s, np.full(si.size, 9.0), 0.01)
+    S = s.read_virial()
+    g = np.round(xs).astype(int)
+    interior = np.all((g > 0) & (g < nx - 1), axis=1)
+    assert S.shape == (xs.shape[0], 6)
+    assert np.allclose(S[interior, :3], kk * (lam - 1.0) * lam, rtol=1e-12) and np.abs(S[interior, 3:]).max() <= 1e-14
+    sigma = S[interior, 0] / lam ** 3                       # virial / deformed cell volume
+    assert np.allclose(sigma, kk * (lam - 1.0) / lam ** 2, rtol=1e-12)   # = bond force k (lam-1) over the face area lam^2
+    xs, si, sj, r0s = cubic_lattice_3d(4, 5, 3)
+    rng = np.random.default_rng(9)
+    xs = xs + rng.uniform(-0.05, 0.05, xs.shape)
+    ks = rng.uniform(0.5, 2.0, si.size)
+    v = rng.normal(0, 0.1, xs.shape)
+    S = OracleSim(xs, si, sj, ks, r0s, np.full(si.size, 9.0), 0.01, v=v, mass=2.0).read_virial()
+    d = xs[sj] - xs[si]; r = np.sqrt((d ** 2).sum(axis=1))
+    assert np.isclose(S[:, :3].sum(), (ks * (r - r0s) * r).sum() - 2.0 * (v ** 2).sum(), rtol=1e-12)
+    assert np.isclose(S[:, 4].sum(), (ks * (r - r0s) / r * d[:, 1] * d[:, 2]).sum() - 2.0 * (v[:, 1] * v[:, 2]).sum(), rtol=1e-11)
