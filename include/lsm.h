@@ -16,7 +16,7 @@
  *   - plain C; no exceptions or C++ types cross the boundary; every function returns lsm_status unless noted.
  *   - dim = 2 is the tuned path (all configurations of the paper and of BASELINE.json are 2-D).  dim = 3 (the layout of
  *     the paper's kernel listing) has the same semantics and entry points, vectors [N*3], on the
- *     streamed kernel with 32-byte records (or the plain direct kernel); no scatter path and no virial there.
+ *     streamed kernel with 32-byte records (or the plain direct kernel); no scatter path there.
  *   - HOST pointers unless a parameter says DEVICE.  Vector arrays are interleaved [N*dim] (x0 y0 x1 y1 ...) as in the
  *     paper's flattened 1-D arrays.  Inputs are borrowed for the duration of the call and copied;
  *     outputs are caller-allocated buffers of the documented size.  The handle owns all device memory.
@@ -50,7 +50,7 @@ typedef enum {
     LSM_E_NOMEM = -5,       /* host or device allocation failed                                                    */
     LSM_E_STATE = -6,       /* the simulation failed earlier (e.g. non-finite energy detected on the device)       */
     LSM_E_UNSUPPORTED = -7  /* exact arithmetic with the scatter kernel, degree > 255 in the gather layout, a dim = 3
-                               request for the scatter / virial paths                            */
+                               request for the scatter path                            */
 } lsm_status;
 
 enum { LSM_FIXED = 0, LSM_MOVE = 1 };                      /* boundary group modes */
@@ -148,8 +148,9 @@ lsm_status lsm_read_state(lsm_sim *sim, double *x /* [N*dim] or NULL */, double 
 lsm_status lsm_read_forces(lsm_sim *sim, double *f /* [N*dim] */);
 /* Per-particle virial stress of the current state, Eq. 7 without the 1/Omega factor (the caller divides
  * by a volume): S[p] = {S_xx, S_yy, S_xy} = 1/2 sum_l (x^l - x^p) (x) f^pl - m v (x) v, tension positive; broken
- * springs contribute nothing.  Gather layout only (LSM_E_UNSUPPORTED with force_mode = SCATTER). */
-lsm_status lsm_read_virial(lsm_sim *sim, double *S /* [N*3] */);
+ * springs contribute nothing.  dim = 3: S[p] = {S_xx, S_yy, S_zz, S_xy, S_yz, S_zx}.  Gather layout only
+ * (LSM_E_UNSUPPORTED with force_mode = SCATTER). */
+lsm_status lsm_read_virial(lsm_sim *sim, double *S /* [N*3], dim = 3: [N*6] */);
 /* broken[s] = 1 if spring s is dead; break_step[s] = step of the force evaluation that broke it, -1 if alive. */
 lsm_status lsm_read_broken(lsm_sim *sim, uint8_t *broken /* [M] or NULL */, int64_t *break_step /* [M] or NULL */,
                            int64_t *n_broken /* scalar or NULL */);

@@ -191,7 +191,7 @@ class LsmSim:
         return f
 
     def read_virial(self):
-        S = np.empty((self.N, 3))
+        S = np.empty((self.N, 3 if self.D == 2 else 6))
         self._check(library().lsm_read_virial(self._h, _ptr(S, C.c_double)))
         return S
 

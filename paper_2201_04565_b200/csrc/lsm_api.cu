@@ -1165,8 +1165,20 @@ lsm_status lsm_read_forces(lsm_sim *s, double *f) {
 lsm_status lsm_read_virial(lsm_sim *s, double *S) {
     CHECK_SIM(s);
     if (!S) { s->err = "S is NULL"; return LSM_E_INVALID; }
-    if (s->force_mode != LSM_FORCE_GATHER || s->dim != 2) { s->err = "lsm_read_virial needs the 2-D gather layout"; return LSM_E_UNSUPPORTED; }
-    if (!s->virial) TRY(dev_alloc(s, &s->virial, (size_t)s->N * 3));
+    if (s->force_mode != LSM_FORCE_GATHER) { s->err = "lsm_read_virial needs the gather layout"; return LSM_E_UNSUPPORTED; }
+    if (!s->virial) TRY(dev_alloc(s, &s->virial, (size_t)s->N * (s->dim == 3 ? 6 : 3)));
+    if (s->dim == 3) {
+        Virial3Params V;
+        std::memset(&V, 0, sizeof(V));
+        const StepParams P = step_params(s, s->step);
+        V.pos = s->pos3[s->cur]; V.vel = s->vel3; V.grp = s->grp; V.mass = s->mass; V.mass_u = s->mass_u; V.dt = s->dt;
+        V.hdr = s->hdr; V.nbr = s->nbr; V.sp = P.sp; V.pm = s->pm; V.inv = s->d_inv; V.N = s->N; V.g = group_tab3(s); V.out = s->virial;
+        k3_virial<<<grid_for(s->N), kBlock, 0, s->stream>>>(V);
+        s->kernels_launched += 1;
+        CUDA_TRY(s, cudaGetLastError());
+        CUDA_TRY(s, cudaMemcpyAsync(S, s->virial, sizeof(double) * 6 * s->N, cudaMemcpyDeviceToHost, s->stream));
+        return check_flags(s);
+    }
     VirialParams V;
     std::memset(&V, 0, sizeof(V));
     const StepParams P = step_params(s, s->step);

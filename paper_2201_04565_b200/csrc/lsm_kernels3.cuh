@@ -181,6 +181,58 @@ __global__ void __launch_bounds__(kBlock) k3_finalize_sample(const Reduce3Params
     }
 }
 
+// Per-particle virial stress in 3-D (Eq. 7, without 1/Omega): out[c] = {S_xx, S_yy, S_zz, S_xy, S_yz, S_zx}.
+// Same structure as k_virial (one thread per particle in caller numbering, master 32-bit ids, IEEE sqrt / divide).
+struct Virial3Params {
+    const double4 *pos, *vel;
+    const uint8_t *grp;
+    const double *mass;
+    double mass_u, dt;
+    const TileHdr *hdr;
+    const int32_t *nbr;
+    SpringParams sp;
+    int pm;
+    const int32_t *inv;
+    long long N;
+    GroupTab3 g;
+    double *out;          // [N][6]
+};
+
+__global__ void __launch_bounds__(kBlock) k3_virial(const Virial3Params V) {
+    const long long c = (long long)blockIdx.x * kBlock + threadIdx.x;
+    if (c >= V.N) return;
+    const int p = V.inv ? V.inv[c] : (int)c;
+    const TileHdr *h = V.hdr + (p >> 8);
+    const int wi = (p >> 5) & 7, lane = p & 31;
+    const unsigned w = h->w[wi];
+    const size_t e0 = (size_t)h->off[wi] * kSlice + lane;
+    const double4 xp = V.pos[p];
+    double s[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    for (unsigned q = 0; q < w; ++q) {
+        const size_t e = e0 + (size_t)q * kSlice;
+        const int nb = V.nbr[e];
+        if (nb == p) continue;
+        double k, r0;
+        if (V.pm == PM_UNIFORM || V.pm == PM_RCF) { k = V.sp.k_u; r0 = V.sp.r0_u; }
+        else if (V.pm == PM_TYPED || V.pm == PM_KRT_RCF) { const int t = V.sp.typ[e]; k = V.sp.tab[kTabStride * t]; r0 = V.sp.tab[kTabStride * t + 3]; }
+        else { k = V.sp.kF[e]; r0 = V.sp.r0F[e]; }
+        const double4 xq = V.pos[nb];
+        const double dx = xq.x - xp.x, dy = xq.y - xp.y, dz = xq.z - xp.z;
+        const double r = sqrt(dx * dx + dy * dy + dz * dz);
+        if (r == 0.0) continue;
+        const double hg = 0.5 * (k * (r - r0) / r);
+        s[0] += hg * dx * dx; s[1] += hg * dy * dy; s[2] += hg * dz * dz;
+        s[3] += hg * dx * dy; s[4] += hg * dy * dz; s[5] += hg * dz * dx;
+    }
+    double4 v = V.vel[p];
+    const uint8_t gg = V.grp[p];
+    if (gg != kFree) v = make_double4(V.g.du[0][gg] / V.dt, V.g.du[1][gg] / V.dt, V.g.du[2][gg] / V.dt, 0.0);
+    const double m = V.mass ? V.mass[p] : V.mass_u;
+    double *o = V.out + 6 * c;
+    o[0] = s[0] - m * v.x * v.x; o[1] = s[1] - m * v.y * v.y; o[2] = s[2] - m * v.z * v.z;
+    o[3] = s[3] - m * v.x * v.y; o[4] = s[4] - m * v.y * v.z; o[5] = s[5] - m * v.z * v.x;
+}
+
 // Numbering translation at the boundary: packed [N*3] caller arrays <-> double4 internal arrays.
 __global__ void __launch_bounds__(kBlock) k3_to_caller(const double4 *src, double *dst, const int32_t *inv, long long N,
                                                        const uint8_t *grp, GroupTab3 g, double dt, int synth_vel) {

@@ -595,6 +595,9 @@ def test_3d_path_matches_oracle(exact, reorder, variant):
         pre = ho["step"] < first
         for key in ("R", "U", "KE"):
             assert np.abs(hg[key][pre] - ho[key][pre]).max() <= 1e-6 * np.abs(ho[key][pre]).max(), key
+    # virial stress of the fractured, moving state (six components)
+    So, Sg = o.read_virial(), g.read_virial()
+    assert Sg.shape == (x.shape[0], 6) and np.abs(Sg - So).max() <= (1e-12 if exact else 1e-6) * np.abs(So).max()
     # restart through write_state, and the energies of the current state
     g.write_state(xo, vo)
     Uo, KEo = o.read_energy(); Ug, KEg = g.read_energy()
