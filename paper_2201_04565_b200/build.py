@@ -13,7 +13,7 @@ CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "liblsm_b200.so")
 SOURCES = [os.path.join(CSRC, "lsm_api.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, "lsm_kernels.cuh"), os.path.join(CSRC, "lsm_kernels3.cuh"), os.path.join(os.path.dirname(HERE), "include", "lsm.h")]
-NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "--fmad=true",
+NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "--fmad=true", "-split-compile=0",
               "-Xcompiler", "-fPIC", "-shared"]
 
 
