@@ -304,6 +304,7 @@ __device__ __forceinline__ bool row_chunk(const StepParams &P, const StepVar &V,
     double2 xq[CH];
     bool any_near = false;
     const double2 *own = V.pos_cur + p;
+    asm("" : "+l"(own));   // keep the own address in a register pair: each gather address is then one wide multiply-add
 #pragma unroll
     for (int c = 0; c < CH; ++c) nb[c] = I16 ? (int)R.nbr16[(s0 + c) * kSlice] : R.nbr[(s0 + c) * kSlice];   // I16: offset
 #pragma unroll

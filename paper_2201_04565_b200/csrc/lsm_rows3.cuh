@@ -51,6 +51,7 @@ __device__ __forceinline__ bool row_chunk3(const StepParams &P, const StepVar &V
     double4 xq[CH];
     bool any_near = false;
     const double4 *own = as4(V.pos_cur) + p;
+    asm("" : "+l"(own));   // as in row_chunk: one wide multiply-add per gather address
 #pragma unroll
     for (int c = 0; c < CH; ++c) nb[c] = I16 ? (int)R.nbr16[(s0 + c) * kSlice] : R.nbr[(s0 + c) * kSlice];
 #pragma unroll
