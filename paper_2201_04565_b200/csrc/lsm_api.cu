@@ -835,7 +835,7 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
             int dev_smem = 0, n_sm = 0;
             CUDA_TRY(s, cudaDeviceGetAttribute(&dev_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, d->device));
             CUDA_TRY(s, cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, d->device));
-            int ctas_per_sm = kStreamMinB, max_stages = 4;
+            int ctas_per_sm = kStreamMinB, max_stages = 3;   // 3 stages: within noise of 4, leaves more of the SM for L1 (gathers)
             if (const char *e = std::getenv("LSM_STREAM_CTAS_PER_SM")) ctas_per_sm = std::max(1, std::min(4, std::atoi(e)));   // tuning overrides
             if (const char *e = std::getenv("LSM_STREAM_STAGES")) max_stages = std::max(2, std::min<int>(kMaxStages, std::atoi(e)));
             // big tiles (high degree, 3-D records): fewer resident CTAs per SM until at least two stages fit
