@@ -304,7 +304,7 @@ def main():
                          "duration_us": t_launch * 1e6},
             "clocks": sampler.summary(tw0, tw1) if sampler else None,
         }
-        tr = os.path.join(ROOT, "profiles", "traffic_%s.json" % args.workload)
+        tr = os.path.join(ROOT, "profiles", "traffic_%s.txt" % args.workload)
         if os.path.exists(tr):                 # per-launch DRAM bytes of the step kernel from the committed ncu --set full capture
             try:
                 line["roofline"]["traffic"] = json.load(open(tr)).get("dram_bytes_per_launch")
