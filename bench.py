@@ -17,7 +17,8 @@ e2e: the same K bench steps through the C ABI with HOST buffers inside the timed
 host memory (x, v) -> lsm_step(S) -> lsm_read_state into pinned host memory + lsm_read_stress.
 
 N > 1 (torchrun): the path runs on one GPU by construction (north_star; replicas only), so each
-rank steps an independent replica of the workload; no data-path collective; scaling = "weak".
+rank steps an independent replica of the workload; no data-path collective; scaling = "weak".  The batch workload
+(--workload cfg4) shards its 1024 specimens over the ranks instead (contiguous ranges, scaling = "strong").
 """
 from __future__ import annotations
 
@@ -198,7 +199,15 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
-    p, desc = make_problem(args.workload)
+    sharded = world > 1 and args.workload == "cfg4"
+    if sharded:       # a batch shards by contiguous specimen ranges (no data-path collective): strong scaling
+        import lsm_inputs as gen
+        from paper_2201_04565_b200.multi import shard_units
+        lo, hi = shard_units(1024, rank, world)
+        p = gen.config4(B=hi - lo, first=lo)
+        desc = "BASELINE.json configs[3]: 1024 x 128x128 two-phase specimens, batched; specimens [%d, %d) of 1024 on rank %d" % (lo, hi, rank)
+    else:
+        p, desc = make_problem(args.workload)
     if args.shuffle_ids:
         import lsm_inputs as gen
         p = gen.shuffle_ids(p, args.shuffle_ids)
@@ -260,10 +269,9 @@ def main():
     te = time.perf_counter() - te0
     assert np.isfinite(h["U"]).all()
 
-    t_all = torch.tensor([ms, te * 1e3], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(t_all, op=dist.ReduceOp.MAX)
-    ms_max, te_ms_max = float(t_all[0]), float(t_all[1])
+    from paper_2201_04565_b200.multi import reduce_over_ranks
+    ms_max, te_ms_max = reduce_over_ranks([ms, te * 1e3], "max", dist, device="cuda")          # device time: max over ranks
+    units, = reduce_over_ranks([float(M_alive0)], "sum", dist, device="cuda")                   # springs over all ranks
     if sampler:
         sampler.stop()
 
@@ -279,11 +287,11 @@ def main():
         bc = counted_bytes(p.N, M_alive0, pv, p.x.shape[1])
         t_launch = ms_max * 1e-3 / (K * S)     # upper bound of the step kernel's mean duration: every other launch in
         ach = bc / t_launch / 1e9              # the region (start/end, reductions, compaction) is charged to it
-        value = world * M_alive0 * S * K / (ms_max * 1e-3)
-        e2e = world * M_alive0 * S * K / (te_ms_max * 1e-3)
+        value = units * S * K / (ms_max * 1e-3)
+        e2e = units * S * K / (te_ms_max * 1e-3)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-            "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": desc, "N": p.N, "M": p.M, "M_alive_at_start": M_alive0, "broken_at_end": nb_after,
                        "time_steps_per_bench_step": S, "ns_per_time_step": 1e6 * ms_max / (K * S), "sample_every": SAMPLE_EVERY,
@@ -292,7 +300,7 @@ def main():
                        "half_edges_stored": inf0["n_half_edges_stored"], "device_bytes": inf0["device_bytes"],
                        "l2": "inputs larger than L2 (%.0f MB streamed per time step vs 126 MB L2)"
                              % ((64.0 * p.N + inf0["n_half_edges_stored"] * inf0["bytes_per_half_edge"] + 1.25 * p.N) / 1e6),
-                       "parallelism": "replicas x%d" % world if world > 1 else "1 GPU"},
+                       "parallelism": ("specimen shards x%d" % world if sharded else "replicas x%d" % world) if world > 1 else "1 GPU"},
             "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 2 * xh.numel() * 8, "d2h_bytes_per_step": 2 * xh.numel() * 8 + d2h_hist,
                     "ms_per_step": te_ms_max / K},
             "gpu_launches": int(launches),
