@@ -703,3 +703,39 @@ def test_per_particle_mass_array_and_nonunit_uniform_mass(dim):
                 assert np.abs(xg - xo).max() <= 1e-11 and np.abs(vg - vo).max() <= 1e-11
             assert np.allclose(KEg, KEo, rtol=1e-9) and np.allclose(Ug, Uo, rtol=1e-9)
             g.close()
+
+
+def test_T4_T5_config3_downscale_fracture_statistics():
+    """SURVEY 8(c) T3-T5 on the 256^2 down-scale of config 3 (porous lattice, per-spring rc), fast arithmetic, pulled
+    12x faster than the bench so that it fails within 4000 steps: same first broken spring and step as the oracle, curve
+    within 1e-6 up to the first breakage, then the statistics tier -- peak reaction and the step at which the reaction
+    has halved within 1 % (one sample), broken count within 10 %."""
+    p = config3(n=256, strain_per_step=1.2e-5)
+    p.sample_every = 100
+    o = OracleSim.from_problem(p)
+    peak, peak_step, steps, failed = 0.0, -1, 0, False
+    while steps < 8000 and not failed:
+        o.step(100); steps += 100
+        r = abs(o.read_stress()["R"][-1, 0, 1, 1])
+        if r > peak:
+            peak, peak_step = r, steps
+        elif peak > 0 and r < 0.5 * peak:
+            failed = True
+    assert failed
+    bo, bso, nbo = o.read_broken()
+    first = bso[bso >= 0].min()
+    o2 = OracleSim.from_problem(p); o2.step(steps); ho = o2.read_stress()
+    g = lsm_create_from_problem(p, history_capacity=256)
+    n, gf, gpeak, gstep = g.run_to_failure(8000, group=1, axis=1, stop_fraction=0.5)
+    bg, bsg, nbg = g.read_broken()
+    hg = g.read_stress()
+    assert gf and abs(n - steps) <= 100 and abs(gstep[0] - peak_step) <= 100 and abs(gpeak[0] / peak - 1) <= 0.01
+    assert bsg[bsg >= 0].min() == first and int(np.flatnonzero(bsg == first)[0]) == int(np.flatnonzero(bso == first)[0])
+    assert abs(nbg - nbo) <= 0.1 * nbo + 5
+    m = min(len(hg["step"]), len(ho["step"]))
+    pre = ho["step"][:m] < first
+    assert pre.sum() >= 3
+    for key in ("R", "U", "KE"):
+        a, r = hg[key][:m][pre], ho[key][:m][pre]
+        assert np.abs(a - r).max() <= 1e-6 * np.abs(r).max(), key
+    g.close()
