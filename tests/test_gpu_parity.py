@@ -739,3 +739,42 @@ def test_T4_T5_config3_downscale_fracture_statistics():
         a, r = hg[key][:m][pre], ho[key][:m][pre]
         assert np.abs(a - r).max() <= 1e-6 * np.abs(r).max(), key
     g.close()
+
+
+def test_T4_T5_config4_specimen_to_failure_inside_a_batch():
+    """One config-4 specimen (128^2 two-phase, BASELINE.json configs[3] recipe) run to failure -- alone through the
+    oracle, and as member 2 of a 4-specimen batch on the GPU (fast arithmetic, fused launches): curve within 1e-6 up
+    to the first breakage, then peak reaction and failure step within 1 %."""
+    b = 7
+    ps = single_specimen(b); ps.sample_every = 100
+    o = OracleSim.from_problem(ps)
+    peak, peak_step, steps, failed = 0.0, -1, 0, False
+    while steps < 20000 and not failed:
+        o.step(100); steps += 100
+        r = abs(o.read_stress()["R"][-1, 0, 1, 1])
+        if r > peak:
+            peak, peak_step = r, steps
+        elif peak > 0 and r < 0.5 * peak:
+            failed = True
+    assert failed
+    bo, bso, nbo = o.read_broken()
+    first = bso[bso >= 0].min()
+    o2 = OracleSim.from_problem(ps); o2.step(steps); ho = o2.read_stress()
+    pb = config4(B=4, first=b - 2); pb.sample_every = 100          # specimens 5, 6, 7, 8: ours is member 2
+    g = lsm_create_from_problem(pb, history_capacity=256)
+    g.step(steps)
+    hg = g.read_stress()
+    R = np.abs(hg["R"][:, 2, 1, 1])
+    assert abs(R.max() / peak - 1) <= 0.01 and abs(hg["step"][R.argmax()] - peak_step) <= 200
+    after = np.flatnonzero((hg["step"] > peak_step) & (R < 0.5 * R.max()))
+    assert after.size and abs(hg["step"][after[0]] - steps) <= 0.01 * steps + 100
+    pre = ho["step"] < first
+    assert pre.sum() > 50
+    for key in ("R", "U", "KE"):
+        a, r = hg[key][:, 2][pre], ho[key][:, 0][pre]
+        assert np.abs(a - r).max() <= 1e-6 * np.abs(r).max(), key
+    _, bsg, _ = g.read_broken()
+    so = pb.spring_offsets
+    mine = bsg[so[2]:so[3]]
+    assert mine[mine >= 0].min() == first and abs((mine >= 0).sum() - nbo) <= 0.1 * nbo + 5
+    g.close()
