@@ -466,3 +466,19 @@ def test_P13_virial_3d_uniform_stretch_and_sum_rule():
     d = xs[sj] - xs[si]; r = np.sqrt((d ** 2).sum(axis=1))
     assert np.isclose(S[:, :3].sum(), (ks * (r - r0s) * r).sum() - 2.0 * (v ** 2).sum(), rtol=1e-12)
     assert np.isclose(S[:, 4].sum(), (ks * (r - r0s) / r * d[:, 1] * d[:, 2]).sum() - 2.0 * (v[:, 1] * v[:, 2]).sum(), rtol=1e-11)
+
+
+def test_P11_summation_order_sensitivity_budget():
+    """P11: what the GPU tolerances rest on.  The same config-1 run with the spring list permuted, the
+    endpoints swapped at random and the particles renumbered differs from the original only by rounding: after 10^4
+    steps |dx|, |dv| stay below 1e-11 (survey scratch: 4e-13, 7e-13), three orders inside north_star's 1e-9."""
+    from lsm_inputs import config1, shuffle_ids
+    p = config1()
+    q = shuffle_ids(p, 12)
+    a = OracleSim.from_problem(p); a.step(10000)
+    b = OracleSim.from_problem(q); b.step(10000)
+    xa, va = a.read_state(); xb, vb = b.read_state()
+    perm = q.meta["perm"]                     # new particle id -> old particle id
+    assert a.read_broken()[2] == 0 and b.read_broken()[2] == 0
+    dx, dv = np.abs(xb - xa[perm]).max(), np.abs(vb - va[perm]).max()
+    assert 0 < dx <= 1e-11 and dv <= 1e-11
