@@ -55,7 +55,9 @@ typedef enum {
 
 enum { LSM_FIXED = 0, LSM_MOVE = 1 };                      /* boundary group modes */
 enum { LSM_FORCE_AUTO = 0, LSM_FORCE_SCATTER = 1, LSM_FORCE_GATHER = 2 };
-enum { LSM_REORDER_NONE = 0, LSM_REORDER_MORTON = 1, LSM_REORDER_RCM = 2 };
+enum { LSM_REORDER_NONE = 0, LSM_REORDER_MORTON = 1, LSM_REORDER_RCM = 2,
+       LSM_REORDER_BLOCKED = 3 /* 2-D only: bins of ~32 x 8 particles in row-major order, row-major inside a bin, so that a
+                                  tile of 256 consecutive ids is a compact patch and neighbour offsets stay small */ };
 /* kernels of the gather path: DIRECT = one thread per particle reading global memory; STREAMED = persistent CTAs,
  * bulk-async-copy (TMA engine) staging of the tile streams through a shared-memory mbarrier pipeline */
 enum { LSM_GATHER_AUTO = 0, LSM_GATHER_DIRECT = 1, LSM_GATHER_STREAMED = 2 };

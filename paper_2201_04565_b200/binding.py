@@ -15,7 +15,7 @@ from . import build as _build
 
 FIXED, MOVE = 0, 1
 FORCE_AUTO, FORCE_SCATTER, FORCE_GATHER = 0, 1, 2
-REORDER_NONE, REORDER_MORTON, REORDER_RCM = 0, 1, 2
+REORDER_NONE, REORDER_MORTON, REORDER_RCM, REORDER_BLOCKED = 0, 1, 2, 3
 GATHER_AUTO, GATHER_DIRECT, GATHER_STREAMED = 0, 1, 2
 FUSION_AUTO, FUSION_ON, FUSION_OFF = 0, 1, 2
 MAX_GROUPS = 8

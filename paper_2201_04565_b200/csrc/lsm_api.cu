@@ -583,6 +583,34 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
         }
         for (long long p = 0; p < N; ++p) { s->perm[p] = keys[p].second; s->inv[keys[p].second] = (int32_t)p; }
     }
+    // ---- (a8) renumbering: blocked -- bins of ~32 x 8 particles (x by y), bins in row-major order, row-major inside ----
+    if (s->reorder == LSM_REORDER_BLOCKED) {
+        s->perm.resize(N); s->inv.resize(N);
+        struct Key { uint32_t bin; float y, x; int32_t id; };
+        std::vector<Key> keys(N);
+        for (int b = 0; b < B; ++b) {
+            const long long lo_p = s->poff[b], hi_p = s->poff[b + 1];
+            if (hi_p == lo_p) continue;
+            double lo[2] = {1e300, 1e300}, hi[2] = {-1e300, -1e300};
+            for (long long p = lo_p; p < hi_p; ++p)
+                for (int c = 0; c < 2; ++c) { lo[c] = std::min(lo[c], d->x[2 * p + c]); hi[c] = std::max(hi[c], d->x[2 * p + c]); }
+            const double area = std::max((hi[0] - lo[0]) * (hi[1] - lo[1]), 1e-300);
+            const double sp = std::sqrt(area / (double)(hi_p - lo_p));           // mean spacing
+            const double wx = 32.0 * sp, wy = 8.0 * sp;
+            const uint32_t nbx = (uint32_t)std::min(65535.0, std::floor((hi[0] - lo[0]) / wx) + 1.0);
+            for (long long p = lo_p; p < hi_p; ++p) {
+                const uint32_t bx = (uint32_t)std::min(65535.0, (d->x[2 * p] - lo[0]) / wx), by = (uint32_t)std::min(65535.0, (d->x[2 * p + 1] - lo[1]) / wy);
+                keys[p] = {by * nbx + bx, (float)d->x[2 * p + 1], (float)d->x[2 * p], (int32_t)p};
+            }
+            std::sort(keys.begin() + lo_p, keys.begin() + hi_p, [](const Key &a, const Key &c) {
+                if (a.bin != c.bin) return a.bin < c.bin;
+                if (a.y != c.y) return a.y < c.y;
+                if (a.x != c.x) return a.x < c.x;
+                return a.id < c.id;
+            });
+        }
+        for (long long p = 0; p < N; ++p) { s->perm[p] = keys[p].id; s->inv[keys[p].id] = (int32_t)p; }
+    }
     // ---- (a8) renumbering: reverse Cuthill-McKee on the spring graph, per specimen (no coordinates needed) ----
     if (s->reorder == LSM_REORDER_RCM) {
         std::vector<int64_t> aoff(N + 1, 0);
@@ -945,7 +973,8 @@ lsm_status lsm_create(const lsm_desc *d, lsm_sim **out) {
     if (d->n_batch < 1 || !d->x) return fail(nullptr, LSM_E_INVALID, "n_batch < 1 or x is NULL");
     if (!(d->dt > 0.0) || !(d->gamma >= 0.0) || !std::isfinite(d->dt) || !std::isfinite(d->gamma)) return fail(nullptr, LSM_E_INVALID, "need dt > 0 and gamma >= 0");
     if (d->sample_every < 0 || d->compact_every < 0 || d->history_capacity < 0) return fail(nullptr, LSM_E_INVALID, "negative sample_every / compact_every / history_capacity");
-    if (d->reorder < LSM_REORDER_NONE || d->reorder > LSM_REORDER_RCM) return fail(nullptr, LSM_E_INVALID, "bad reorder");
+    if (d->reorder < LSM_REORDER_NONE || d->reorder > LSM_REORDER_BLOCKED) return fail(nullptr, LSM_E_INVALID, "bad reorder");
+    if (d->reorder == LSM_REORDER_BLOCKED && d->dim != 2) return fail(nullptr, LSM_E_UNSUPPORTED, "reorder = BLOCKED is 2-D only");
     if (d->force_mode < 0 || d->force_mode > 2) return fail(nullptr, LSM_E_INVALID, "bad force_mode");
     if (d->gather_variant < 0 || d->gather_variant > 2) return fail(nullptr, LSM_E_INVALID, "bad gather_variant");
     if (d->step_fusion < 0 || d->step_fusion > 2) return fail(nullptr, LSM_E_INVALID, "bad step_fusion");

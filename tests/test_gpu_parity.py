@@ -42,7 +42,7 @@ def _fracture_problem(n=64, du_y=4.4e-4, seed=7):
 
 # ---------------------------------------------------------------- T1: single force evaluation
 @pytest.mark.parametrize("mode", MODES, ids=MODE_IDS)
-@pytest.mark.parametrize("reorder", [0, 1, 2])
+@pytest.mark.parametrize("reorder", [0, 1, 2, 3])
 @pytest.mark.parametrize("make", [lambda: _perturbed(config1(), 0.03, 1), lambda: _perturbed(config2(n=96, n_blobs=20), 0.02, 2),
                                   lambda: _perturbed(config3(n=160), 0.02, 3), lambda: _perturbed(config4(B=3, n=24), 0.02, 4)],
                          ids=["cfg1", "cfg2-96", "cfg3-160", "cfg4-3x24"])
@@ -131,7 +131,7 @@ def test_T3_T4_T5_fracture_curve(mode):
 
 
 # ---------------------------------------------------------------- T6: exact mode is bit-identical through fracture
-@pytest.mark.parametrize("reorder,compact", [(0, 0), (1, 500), (2, 300)])
+@pytest.mark.parametrize("reorder,compact", [(0, 0), (1, 500), (2, 300), (3, 400)])
 def test_T6_exact_mode_bit_identical_fracture(reorder, compact):
     p = _fracture_problem()
     o = OracleSim.from_problem(p); o.step(9000)
@@ -160,7 +160,7 @@ def test_T7_reorder_compaction_shuffle_transparent(mode):
     xo, vo = o.read_state(); bo, bso, nbo = o.read_broken()
     assert nbo > 0
     first = bso[bso >= 0].min()
-    for prob, reorder, compact in [(p, 1, 0), (p, 0, 300), (q, 1, 300), (q, 0, 0), (q, 2, 300), (p, 2, 0)]:
+    for prob, reorder, compact in [(p, 1, 0), (p, 0, 300), (q, 1, 300), (q, 0, 0), (q, 2, 300), (p, 2, 0), (q, 3, 300), (p, 3, 0)]:
         g = lsm_create_from_problem(prob, reorder=reorder, compact_every=compact, **mode)
         g.step(nsteps)
         xg, vg = g.read_state(); bg, bsg, nbg = g.read_broken()
