@@ -138,25 +138,33 @@ lsm_status lsm_create(const lsm_desc *desc, lsm_sim **out);
 lsm_status lsm_set_boundary(lsm_sim *sim, int32_t group, const int32_t *particle_ids, int64_t n, int32_t mode,
                             const double *disp_per_step /* [dim] */);
 
-/* Advance n_steps velocity-Verlet steps (kick - drift - force+breakage - kick).  Asynchronous. */
+/* Advance n_steps time steps: velocity Verlet, Eq. 3-5 in half-step-velocity form (L76): boundary
+ * displacement first (L88), kick - drift - spring forces (Eq. 2) with the breakage test (L98) - damping - kick;
+ * samples every sample_every steps, compaction every compact_every.  Only enqueues work on `stream` (asynchronous);
+ * n_steps < 0 -> LSM_E_INVALID; a launch failure is sticky (LSM_E_CUDA). */
 lsm_status lsm_step(lsm_sim *sim, int64_t n_steps);
 
-/* Overwrite positions and velocities (restart / perturbation); forces are re-evaluated at the current step and
- * kinematic particles take the new position as their origin.  v NULL = zeros. */
+/* Overwrite positions and velocities (restart / perturbation) from HOST arrays [N*dim] in caller numbering; forces are
+ * re-evaluated at the current step and kinematic particles take the new position as their origin.  v NULL = zeros. */
 lsm_status lsm_write_state(lsm_sim *sim, const double *x, const double *v);
 
+/* Positions and velocities of the completed state (what Eq. 3-5 hold after the last step) into caller-allocated HOST
+ * arrays, caller numbering; a kinematic particle reports v = disp_per_step / dt.  Synchronises the stream; returns
+ * LSM_E_STATE (sticky) if a non-finite energy was detected on the device. */
 lsm_status lsm_read_state(lsm_sim *sim, double *x /* [N*dim] or NULL */, double *v /* [N*dim] or NULL */);
-/* Spring force on every particle at the current positions (no damping term). */
+/* Spring force on every particle at the current positions, Eq. 2 (no damping term). */
 lsm_status lsm_read_forces(lsm_sim *sim, double *f /* [N*dim] */);
 /* Per-particle virial stress of the current state, Eq. 7 without the 1/Omega factor (the caller divides
  * by a volume): S[p] = {S_xx, S_yy, S_xy} = 1/2 sum_l (x^l - x^p) (x) f^pl - m v (x) v, tension positive; broken
  * springs contribute nothing.  dim = 3: S[p] = {S_xx, S_yy, S_zz, S_xy, S_yz, S_zx}.  Gather layout only
  * (LSM_E_UNSUPPORTED with force_mode = SCATTER). */
 lsm_status lsm_read_virial(lsm_sim *sim, double *S /* [N*3], dim = 3: [N*6] */);
-/* broken[s] = 1 if spring s is dead; break_step[s] = step of the force evaluation that broke it, -1 if alive. */
+/* Irreversible breakage, caller spring numbering: broken[s] = 1 if spring s is dead;
+ * break_step[s] = step of the force evaluation that broke it, -1 if alive; *n_broken = total over all specimens. */
 lsm_status lsm_read_broken(lsm_sim *sim, uint8_t *broken /* [M] or NULL */, int64_t *break_step /* [M] or NULL */,
                            int64_t *n_broken /* scalar or NULL */);
-/* Per-specimen energies of the current state: U (Eq. 1) and KE of the free particles. */
+/* Per-specimen energies of the current state: U = sum over alive springs of k (r - r0)^2 / 2 (Eq. 1) and
+ * KE of the free particles (PAPER.md:L113 sums them on the CPU; here a deterministic device reduction). */
 lsm_status lsm_read_energy(lsm_sim *sim, double *U /* [B] or NULL */, double *KE /* [B] or NULL */);
 /* Copy out (and clear) the samples recorded since the last call, oldest first, at most `capacity`:
  * step[n], reaction[n][B][LSM_MAX_GROUPS][dim] (raw sums of spring forces over each group's particles; the caller
@@ -173,12 +181,14 @@ lsm_status lsm_read_stress(lsm_sim *sim, int64_t capacity, int64_t *n_samples, i
 lsm_status lsm_run_to_failure(lsm_sim *sim, int64_t max_steps, int32_t group, int32_t axis, double stop_fraction,
                               int64_t *steps_done, int32_t *failed, double *peak, int64_t *peak_step);
 
-/* Drop dead springs from the device lists now (also done every compact_every steps). Results never change. */
+/* Drop dead springs from the device lists now (also done every compact_every steps): stable, in-row, so every
+ * particle keeps its summation order and no result changes (the paper keeps dead springs with k = 0, L196). */
 lsm_status lsm_compact(lsm_sim *sim);
-lsm_status lsm_sync(lsm_sim *sim);
-lsm_status lsm_get_info(lsm_sim *sim, lsm_info *info);
-/* Device pointers of the current state in INTERNAL numbering, for zero-copy consumers (may change after lsm_step). */
-lsm_status lsm_device_state(lsm_sim *sim, const double **pos_xy /* DEVICE [N*2] */, const double **vel_xy);
+lsm_status lsm_sync(lsm_sim *sim);                                   /* cudaStreamSynchronize on the handle's stream */
+lsm_status lsm_get_info(lsm_sim *sim, lsm_info *info);               /* never fails on a valid handle, even after an error */
+/* Device pointers of the current state in INTERNAL numbering, for zero-copy consumers (may change after lsm_step):
+ * records of 2 doubles {x, y} per particle for dim = 2, of 4 doubles {x, y, z, 0} for dim = 3; owned by the handle. */
+lsm_status lsm_device_state(lsm_sim *sim, const double **pos_xy /* DEVICE */, const double **vel_xy /* DEVICE */);
 const char *lsm_last_error(const lsm_sim *sim); /* sim NULL: error of the last failed lsm_create on this thread */
 void lsm_destroy(lsm_sim *sim);
 int32_t lsm_abi_version(void);
