@@ -10,7 +10,7 @@ target ("the 4M-particle lattice", >= 60 % of HBM) is quoted on.  Synthetic and 
 A bench "step" is one lsm_step(S) call: S = --inner consecutive time steps of the whole hot path (boundary
 displacement, kick + drift, spring forces + breakage, damping + kick, the sample reductions every 100 time steps and
 the scheduled compaction), on state already resident in HBM.  value = live springs x time steps / second over all
-ranks.  The per-step traffic (~400 MB) is larger than the 126 MB L2, so consecutive time steps cannot serve each other
+ranks.  The per-step traffic (~262 MB streamed by the kernel) is larger than the 126 MB L2, so consecutive time steps cannot serve each other
 from cache (config.l2: "inputs larger than L2").
 
 e2e: the same K bench steps through the C ABI with HOST buffers inside the timed region: lsm_write_state from pinned
@@ -170,7 +170,7 @@ def main():
     ap.add_argument("--ref-inner", type=int, default=2, help="time steps per bench step of --impl reference")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--workload", default="cfg3")
-    ap.add_argument("--force-mode", default="auto", choices=["auto", "gather", "scatter", "tile"])
+    ap.add_argument("--force-mode", default="auto", choices=["auto", "gather", "scatter"])
     ap.add_argument("--reorder", type=int, default=0)
     ap.add_argument("--compact-every", type=int, default=1000)
     ap.add_argument("--exact", type=int, default=0)
@@ -213,7 +213,7 @@ def main():
         p = gen.shuffle_ids(p, args.shuffle_ids)
         desc += " (ids shuffled, seed %d)" % args.shuffle_ids
     p.sample_every = SAMPLE_EVERY
-    fm = {"auto": lsm.FORCE_AUTO, "gather": lsm.FORCE_GATHER, "scatter": lsm.FORCE_SCATTER, "tile": getattr(lsm, "FORCE_TILE", 3)}[args.force_mode]
+    fm = {"auto": lsm.FORCE_AUTO, "gather": lsm.FORCE_GATHER, "scatter": lsm.FORCE_SCATTER}[args.force_mode]
     sim = lsm_create_from_problem(p, device=local, force_mode=fm, reorder=args.reorder, compact_every=args.compact_every,
                                   exact=bool(args.exact), history_capacity=64, gather_variant=args.gather_variant, step_fusion=args.step_fusion)
     inf0 = sim.info()

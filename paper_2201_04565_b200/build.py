@@ -4,6 +4,7 @@
 """
 from __future__ import annotations
 
+import glob
 import os
 import subprocess
 import sys
@@ -12,7 +13,14 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "liblsm_b200.so")
 SOURCES = [os.path.join(CSRC, "lsm_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "lsm_kernels.cuh"), os.path.join(CSRC, "lsm_kernels3.cuh"), os.path.join(os.path.dirname(HERE), "include", "lsm.h")]
+INCLUDE = os.path.join(os.path.dirname(HERE), "include")
+
+
+def deps():
+    """Everything the library is compiled from: every file under csrc/ and include/."""
+    return sorted(glob.glob(os.path.join(CSRC, "*.cu*")) + glob.glob(os.path.join(INCLUDE, "*.h")))
+
+
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "--fmad=true", "-split-compile=0",
               "-Xcompiler", "-fPIC", "-shared"]
 
@@ -28,13 +36,12 @@ def stale() -> bool:
     if not os.path.exists(SO):
         return True
     t = os.path.getmtime(SO)
-    return any(os.path.getmtime(d) > t for d in DEPS)
+    return any(os.path.getmtime(d) > t for d in deps())
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or stale():
-        extra = os.environ.get("LSM_NVCC_FLAGS", "").split()          # e.g. -DLSM_STREAM_MINB=3 for tuning sweeps
-        cmd = [nvcc()] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", SO] + SOURCES
+        cmd = [nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", SO] + SOURCES
         subprocess.run(cmd, check=True)
     return SO
 

@@ -1,6 +1,6 @@
 // lsm_api.cu -- host side of liblsm_b200.so: the C ABI of include/lsm.h.
-// Validation, renumbering (a8), layout construction, the step loop (launch sequencing / CUDA graphs), sampling ring,
-// compaction scheduling, numbering translation at the boundary.  All arithmetic of the method runs in the kernels of
+// Validation, renumbering (a8), layout construction, the step loop (launch sequencing, fused cooperative launches),
+// sampling ring, compaction scheduling, numbering translation at the boundary.  All arithmetic of the method runs in the kernels of
 // lsm_kernels.cuh; nothing here computes a force or integrates.
 #include <algorithm>
 #include <cmath>
@@ -148,6 +148,23 @@ template <class T> lsm_status upload(lsm_sim *s, T **out, const std::vector<T> &
     if (!h.empty()) CUDA_TRY(s, cudaMemcpyAsync(*out, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice, s->stream));
     return LSM_OK;
 }
+
+// Return one allocation made through dev_alloc (the caller has made sure no enqueued work still uses it).
+void dev_free(lsm_sim *s, void *p) {
+    if (!p) return;
+    auto it = std::find(s->dev_allocs.begin(), s->dev_allocs.end(), p);
+    if (it == s->dev_allocs.end()) return;
+    s->dev_allocs.erase(it);
+    if (s->alloc) { if (s->free_) s->free_(p, s->alloc_user); }
+    else cudaFree(p);
+}
+
+// Makes the handle's device current for the duration of an entry point and restores the caller's device afterwards.
+struct DeviceScope {
+    int prev = -1;
+    explicit DeviceScope(int dev) { if (cudaGetDevice(&prev) != cudaSuccess) prev = -1; if (prev != dev) cudaSetDevice(dev); else prev = -1; }
+    ~DeviceScope() { if (prev >= 0) cudaSetDevice(prev); }
+};
 
 #define TRY(expr)                         \
     do {                                  \
@@ -801,7 +818,7 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
         }
         TRY(upload(s, &s->hdr, hh));
         TRY(upload(s, &s->nbr, hn));
-        bool fits16 = std::getenv("LSM_NO_IDX16") == nullptr;
+        bool fits16 = true;
         {   // 16-bit neighbour offsets (neighbour - self) when every one fits: halves the streamed id bytes
             std::vector<int16_t> h16;
             if (fits16) {
@@ -864,8 +881,6 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
             CUDA_TRY(s, cudaDeviceGetAttribute(&dev_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, d->device));
             CUDA_TRY(s, cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, d->device));
             int ctas_per_sm = kStreamMinB, max_stages = 3;   // 3 stages: within noise of 4, leaves more of the SM for L1 (gathers)
-            if (const char *e = std::getenv("LSM_STREAM_CTAS_PER_SM")) ctas_per_sm = std::max(1, std::min(4, std::atoi(e)));   // tuning overrides
-            if (const char *e = std::getenv("LSM_STREAM_STAGES")) max_stages = std::max(2, std::min<int>(kMaxStages, std::atoi(e)));
             // big tiles (high degree, 3-D records): fewer resident CTAs per SM until at least two stages fit
             for (;; --ctas_per_sm) {
                 const int budget = std::min(dev_smem, (dev_smem + 1024) / ctas_per_sm - 1024) - L.first;   // 1 KB reserved per CTA
@@ -882,8 +897,7 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
             // problem is L2-resident; above that the per-step grid barrier costs more than the launch gap it removes.
             int coop = 0;
             CUDA_TRY(s, cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, d->device));
-            long long fuse_below = 1 << 18;   // measured: 64^2 5.8 -> 3.6 us per step, 512^2 8.4 -> 8.3, 2.1 M particles 39.1 -> 40.4
-            if (const char *e = std::getenv("LSM_FUSE_BELOW")) fuse_below = std::atoll(e);
+            const long long fuse_below = 1 << 18;   // measured: 64^2 5.8 -> 3.6 us per step, 512^2 8.4 -> 8.3, 2.1 M particles 39.1 -> 40.4
             if (s->step_fusion == LSM_FUSION_ON && !(coop && s->gather_variant == 2)) return fail(s, LSM_E_UNSUPPORTED, "step_fusion = ON needs the streamed gather kernel and cooperative launch support");
             s->multi_on = coop && s->gather_variant == 2 && (s->step_fusion == LSM_FUSION_ON || (s->step_fusion == LSM_FUSION_AUTO && N <= fuse_below));
             if (s->multi_on) {
@@ -989,12 +1003,10 @@ lsm_status lsm_create(const lsm_desc *d, lsm_sim **out) {
     return LSM_OK;
 }
 
-#define CHECK_SIM(s)                                   \
-    do {                                               \
-        if (!(s)) return LSM_E_INVALID;                \
-        if ((s)->sticky != LSM_OK) return (s)->sticky; \
-        cudaSetDevice((s)->device);                    \
-    } while (0)
+#define CHECK_SIM(s)                               \
+    if (!(s)) return LSM_E_INVALID;                \
+    if ((s)->sticky != LSM_OK) return (s)->sticky; \
+    DeviceScope _device_scope((s)->device)
 
 lsm_status lsm_set_boundary(lsm_sim *s, int32_t gi, const int32_t *ids, int64_t n, int32_t mode, const double *du) {
     CHECK_SIM(s);
@@ -1011,12 +1023,17 @@ lsm_status lsm_set_boundary(lsm_sim *s, int32_t gi, const int32_t *ids, int64_t 
     }
     std::sort(nid.begin(), nid.end());
     if (std::adjacent_find(nid.begin(), nid.end()) != nid.end()) { s->err = "duplicate particle id in the group"; return LSM_E_RANGE; }
-    // release the old members (they keep the kinematic velocity du/dt, like the oracle's stored v)
+    // release the old members: free again, carrying the kinematic velocity du/dt (Q6)
     if (g.set && !g.ids.empty()) {
-        if (s->dim == 3) k3_group_release<<<grid_for((long long)g.ids.size()), kBlock, 0, s->stream>>>(g.d_ids, (long long)g.ids.size(), s->grp, s->vel3, g.du[0] / s->dt, g.du[1] / s->dt, g.du[2] / s->dt);
-        else k_group_release<<<grid_for((long long)g.ids.size()), kBlock, 0, s->stream>>>(g.d_ids, (long long)g.ids.size(), s->grp, s->vel, g.du[0] / s->dt, g.du[1] / s->dt);
+        if (s->dim == 3) k3_group_release<<<grid_for((long long)g.ids.size()), kBlock, 0, s->stream>>>(g.d_ids, (long long)g.ids.size(), s->grp, s->vel3, g.du[0] / s->dt, g.du[1] / s->dt, g.du[2] / s->dt, s->sKE, s->mass, s->mass_u);
+        else k_group_release<<<grid_for((long long)g.ids.size()), kBlock, 0, s->stream>>>(g.d_ids, (long long)g.ids.size(), s->grp, s->vel, g.du[0] / s->dt, g.du[1] / s->dt, s->sKE, s->mass, s->mass_u);
         s->kernels_launched += 1;
         for (int32_t p : g.ids) s->h_grp[p] = kFree;
+    }
+    if (g.d_ids || g.d_seg) {   // the group's previous device lists: nothing enqueued may still read them
+        CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+        dev_free(s, g.d_ids); dev_free(s, g.d_seg);
+        g.d_ids = nullptr; g.d_seg = nullptr;
     }
     g.set = true; g.mode = mode; g.n0 = s->step;
     g.du[0] = mode == LSM_MOVE ? du[0] : 0.0; g.du[1] = mode == LSM_MOVE ? du[1] : 0.0;
@@ -1025,19 +1042,18 @@ lsm_status lsm_set_boundary(lsm_sim *s, int32_t gi, const int32_t *ids, int64_t 
     for (int32_t p : nid) s->h_grp[p] = (uint8_t)gi;
     std::vector<long long> seg(s->B + 1, 0);
     { int b = 0; for (size_t q = 0; q < nid.size(); ++q) { while (nid[q] >= s->poff[b + 1]) { ++b; seg[b] = (long long)q; } } for (int bb = b + 1; bb <= s->B; ++bb) seg[bb] = (long long)nid.size(); }
-    // (old device lists stay owned by the handle until destroy; groups are set a handful of times)
     TRY(upload(s, &g.d_ids, nid));
     TRY(upload(s, &g.d_seg, seg));
     if (n > 0) {
-        if (s->dim == 3) k3_group_assign<<<grid_for(n), kBlock, 0, s->stream>>>(g.d_ids, n, s->grp, s->vel3, s->pos3[s->cur], (uint8_t)gi);
-        else k_group_assign<<<grid_for(n), kBlock, 0, s->stream>>>(g.d_ids, n, s->grp, s->vel, s->pos[s->cur], (uint8_t)gi);
+        if (s->dim == 3) k3_group_assign<<<grid_for(n), kBlock, 0, s->stream>>>(g.d_ids, n, s->grp, s->vel3, s->pos3[s->cur], (uint8_t)gi, s->sKE);
+        else k_group_assign<<<grid_for(n), kBlock, 0, s->stream>>>(g.d_ids, n, s->grp, s->vel, s->pos[s->cur], (uint8_t)gi, s->sKE);
         s->kernels_launched += 1;
     }
     CUDA_TRY(s, cudaGetLastError());
-    // membership changed: refresh fd (released particles are damped again) and the per-particle energy terms
-    // (kinematic particles carry no KE).  Positions are unchanged, so no spring can break here.
-    TRY(eval_initial(s));
-    CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    // Membership and origins change, nothing else (R3): positions are untouched, so the spring forces f and the
+    // held total force fd = f - gamma v of the last force evaluation stay what they were -- fd still feeds the next first
+    // half kick of every free particle (Q7) -- and only the members' kinetic-energy terms were adjusted above.
+    CUDA_TRY(s, cudaStreamSynchronize(s->stream));   // nid / seg go out of scope
     return LSM_OK;
 }
 
@@ -1131,6 +1147,8 @@ lsm_status lsm_sync(lsm_sim *s) {
 lsm_status lsm_write_state(lsm_sim *s, const double *x, const double *v) {
     CHECK_SIM(s);
     if (!x) { s->err = "x is NULL"; return LSM_E_INVALID; }
+    for (long long q = 0; q < s->dim * s->N; ++q)
+        if (!std::isfinite(x[q]) || (v && !std::isfinite(v[q]))) { s->err = "non-finite position / velocity"; return LSM_E_NONFINITE; }
     if (s->dim == 3) {
         CUDA_TRY(s, cudaMemcpyAsync(s->stage3[0], x, sizeof(double) * 3 * s->N, cudaMemcpyHostToDevice, s->stream));
         if (v) CUDA_TRY(s, cudaMemcpyAsync(s->stage3[1], v, sizeof(double) * 3 * s->N, cudaMemcpyHostToDevice, s->stream));
@@ -1143,6 +1161,7 @@ lsm_status lsm_write_state(lsm_sim *s, const double *x, const double *v) {
     s->kernels_launched += 1;
     for (int g = 0; g < kMaxGroups; ++g) s->groups[g].n0 = s->step;
     TRY(eval_initial(s));
+    CUDA_TRY(s, cudaStreamSynchronize(s->stream));   // x / v are borrowed for the duration of the call only (lsm.h)
     return LSM_OK;
 }
 
@@ -1247,16 +1266,22 @@ lsm_status lsm_read_energy(lsm_sim *s, double *U, double *KE) {
 lsm_status lsm_read_stress(lsm_sim *s, int64_t capacity, int64_t *n_samples, int64_t *step, double *R, double *U, double *KE, int64_t *nb) {
     CHECK_SIM(s);
     if (!n_samples || capacity < 0) { s->err = "n_samples is NULL or capacity < 0"; return LSM_E_INVALID; }
-    const long long n = std::min<long long>(s->hist_count, capacity);
+    const long long n = std::min<long long>(s->hist_count, capacity);   // the newest n (older unread samples are dropped)
     const long long B = s->B;
-    for (long long t = 0; t < n; ++t) {  // oldest of the last n first
-        const long long slot = ((s->hist_head - n + t) % s->hist_cap + s->hist_cap) % s->hist_cap;
-        if (step) CUDA_TRY(s, cudaMemcpyAsync(step + t, s->hist_step + slot, sizeof(long long), cudaMemcpyDeviceToHost, s->stream));
-        if (R) CUDA_TRY(s, cudaMemcpyAsync(R + t * B * kMaxGroups * s->dim, s->hist_R + slot * B * kMaxGroups * s->dim, sizeof(double) * B * kMaxGroups * s->dim, cudaMemcpyDeviceToHost, s->stream));
-        if (U) CUDA_TRY(s, cudaMemcpyAsync(U + t * B, s->hist_U + slot * B, sizeof(double) * B, cudaMemcpyDeviceToHost, s->stream));
-        if (KE) CUDA_TRY(s, cudaMemcpyAsync(KE + t * B, s->hist_KE + slot * B, sizeof(double) * B, cudaMemcpyDeviceToHost, s->stream));
-        if (nb) CUDA_TRY(s, cudaMemcpyAsync(nb + t * B, s->hist_nb + slot * B, sizeof(long long) * B, cudaMemcpyDeviceToHost, s->stream));
-    }
+    // the last n slots of the ring, oldest first: one contiguous run, or two when the run wraps past the end of the ring
+    const long long first = ((s->hist_head - n) % s->hist_cap + s->hist_cap) % s->hist_cap;
+    const long long n1 = std::min<long long>(n, s->hist_cap - first), n2 = n - n1;
+    auto copy_out = [&](void *dst, const void *src, size_t rec) -> cudaError_t {   // rec = bytes per sample
+        if (!dst || n == 0) return cudaSuccess;
+        cudaError_t e = cudaMemcpyAsync(dst, static_cast<const char *>(src) + (size_t)first * rec, (size_t)n1 * rec, cudaMemcpyDeviceToHost, s->stream);
+        if (e == cudaSuccess && n2 > 0) e = cudaMemcpyAsync(static_cast<char *>(dst) + (size_t)n1 * rec, src, (size_t)n2 * rec, cudaMemcpyDeviceToHost, s->stream);
+        return e;
+    };
+    CUDA_TRY(s, copy_out(step, s->hist_step, sizeof(long long)));
+    CUDA_TRY(s, copy_out(R, s->hist_R, sizeof(double) * B * kMaxGroups * s->dim));
+    CUDA_TRY(s, copy_out(U, s->hist_U, sizeof(double) * B));
+    CUDA_TRY(s, copy_out(KE, s->hist_KE, sizeof(double) * B));
+    CUDA_TRY(s, copy_out(nb, s->hist_nb, sizeof(long long) * B));
     *n_samples = n;
     s->hist_count = 0;
     return check_flags(s);

@@ -204,8 +204,10 @@ __device__ __forceinline__ void particle_update(const StepParams &P, const StepV
             const double2 xn = make_double2(mad<EXACT>(ns, P.g.dux[g], vh.x), mad<EXACT>(ns, P.g.duy[g], vh.y));
             V.pos_next[p] = xn;
             if (own_pos) *own_pos = xn;
-        } else {
-            P.fd[p] = make_double2(fx, fy);
+        } else {   // completed state: the held total force of a kinematic particle is f - gamma * (du/dt), its stored
+            // velocity being du/dt (Q6, Q7); it matters only if the particle is released later (lsm_set_boundary)
+            const double vkx = __ddiv_rn(P.g.dux[g], P.dt), vky = __ddiv_rn(P.g.duy[g], P.dt);
+            P.fd[p] = make_double2(sub<EXACT>(fx, mul<EXACT>(P.gamma, vkx)), sub<EXACT>(fy, mul<EXACT>(P.gamma, vky)));
         }
     }
 }
@@ -563,9 +565,7 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
                 if constexpr (D == 3) {
                     const double4 xp = reinterpret_cast<const double4 *>(b + L.pos)[tid];
                     double fx = 0.0, fy = 0.0, fz = 0.0, uu = 0.0;
-#ifndef LSM_DEBUG_NOFORCE
                     row_forces3<PM, EXACT, SAMPLE, MULTI, I16>(P, V, R, s_tab, (int)p, w, xp, fx, fy, fz, uu);
-#endif
                     const double4 vh = reinterpret_cast<const double4 *>(b + L.vel)[tid];
                     const uint8_t g = (b + L.grp)[tid];
                     if (MULTI && M.resident)
@@ -576,9 +576,7 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
                 } else {
                     const double2 xp = reinterpret_cast<const double2 *>(b + L.pos)[tid];
                     double fx = 0.0, fy = 0.0, uu = 0.0;
-#ifndef LSM_DEBUG_NOFORCE   // tuning probe only: skip the spring evaluation to expose the copy pipeline's own ceiling
                     row_forces<PM, EXACT, SAMPLE, MULTI, I16>(P, V, R, s_tab, (int)p, w, xp, fx, fy, uu);
-#endif
                     const double2 vh = reinterpret_cast<const double2 *>(b + L.vel)[tid];
                     const uint8_t g = (b + L.grp)[tid];
                     if (MULTI && M.resident)
@@ -904,18 +902,27 @@ __global__ void __launch_bounds__(kBlock) k_from_caller(const double2 *srcx, con
     vel[p] = (grp[p] != kFree) ? x : (srcv ? srcv[c] : make_double2(0.0, 0.0));  // kinematic: vel slot = origin
 }
 
-__global__ void __launch_bounds__(kBlock) k_group_release(const int32_t *ids, long long n, uint8_t *grp, double2 *vel, double vx, double vy) {
+// Released particles become free with the kinematic velocity (vx, vy) = du/dt they were carrying; their kinetic-energy
+// term (kept per particle for lsm_read_energy) follows.  Nothing else changes: f and the held fd stay (R3).
+__global__ void __launch_bounds__(kBlock) k_group_release(const int32_t *ids, long long n, uint8_t *grp, double2 *vel, double vx, double vy,
+                                                          double *sKE, const double *mass, double mass_u) {
     const long long q = (long long)blockIdx.x * kBlock + threadIdx.x;
     if (q >= n) return;
-    grp[ids[q]] = kFree;
-    vel[ids[q]] = make_double2(vx, vy);
+    const int p = ids[q];
+    grp[p] = kFree;
+    vel[p] = make_double2(vx, vy);
+    const double m = mass ? mass[p] : mass_u;
+    sKE[p] = __dmul_rn(__dmul_rn(0.5, m), __dadd_rn(__dmul_rn(vx, vx), __dmul_rn(vy, vy)));
 }
 
-__global__ void __launch_bounds__(kBlock) k_group_assign(const int32_t *ids, long long n, uint8_t *grp, double2 *vel, const double2 *pos, uint8_t g) {
+__global__ void __launch_bounds__(kBlock) k_group_assign(const int32_t *ids, long long n, uint8_t *grp, double2 *vel, const double2 *pos, uint8_t g,
+                                                         double *sKE) {
     const long long q = (long long)blockIdx.x * kBlock + threadIdx.x;
     if (q >= n) return;
-    grp[ids[q]] = g;
-    vel[ids[q]] = pos[ids[q]];
+    const int p = ids[q];
+    grp[p] = g;
+    vel[p] = pos[p];        // kinematic: the vel slot holds the origin
+    sKE[p] = 0.0;           // kinematic particles carry no KE (Q6)
 }
 
 __global__ void __launch_bounds__(kBlock) k_broken_from_steps(const long long *break_step, uint8_t *broken, long long M) {

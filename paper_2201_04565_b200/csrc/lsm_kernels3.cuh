@@ -114,8 +114,10 @@ __global__ void __launch_bounds__(kBlock) k3_step(const Step3Params P) {
             const double ns = (double)(P.step + 1 - P.g.n0[gg]);
             P.pos_next[p] = make_double4(mad<EXACT>(ns, P.g.du[0][gg], vh.x), mad<EXACT>(ns, P.g.du[1][gg], vh.y),
                                          mad<EXACT>(ns, P.g.du[2][gg], vh.z), 0.0);
-        } else {
-            P.fd[p] = make_double4(fx, fy, fz, 0.0);
+        } else {   // held total force of a kinematic particle: f - gamma * (du/dt) (see particle_update)
+            const double vkx = __ddiv_rn(P.g.du[0][gg], P.dt), vky = __ddiv_rn(P.g.du[1][gg], P.dt), vkz = __ddiv_rn(P.g.du[2][gg], P.dt);
+            P.fd[p] = make_double4(sub<EXACT>(fx, mul<EXACT>(P.gamma, vkx)), sub<EXACT>(fy, mul<EXACT>(P.gamma, vky)),
+                                   sub<EXACT>(fz, mul<EXACT>(P.gamma, vkz)), 0.0);
         }
     }
 }
@@ -254,18 +256,25 @@ __global__ void __launch_bounds__(kBlock) k3_from_caller(const double *srcx, con
     vel[p] = (grp[p] != kFree) ? x : (srcv ? make_double4(srcv[3 * c], srcv[3 * c + 1], srcv[3 * c + 2], 0.0) : make_double4(0.0, 0.0, 0.0, 0.0));
 }
 
-__global__ void __launch_bounds__(kBlock) k3_group_release(const int32_t *ids, long long n, uint8_t *grp, double4 *vel, double vx, double vy, double vz) {
+__global__ void __launch_bounds__(kBlock) k3_group_release(const int32_t *ids, long long n, uint8_t *grp, double4 *vel, double vx, double vy, double vz,
+                                                           double *sKE, const double *mass, double mass_u) {
     const long long q = (long long)blockIdx.x * kBlock + threadIdx.x;
     if (q >= n) return;
-    grp[ids[q]] = kFree;
-    vel[ids[q]] = make_double4(vx, vy, vz, 0.0);
+    const int p = ids[q];
+    grp[p] = kFree;
+    vel[p] = make_double4(vx, vy, vz, 0.0);
+    const double m = mass ? mass[p] : mass_u;
+    sKE[p] = __dmul_rn(__dmul_rn(0.5, m), __dadd_rn(__dadd_rn(__dmul_rn(vx, vx), __dmul_rn(vy, vy)), __dmul_rn(vz, vz)));
 }
 
-__global__ void __launch_bounds__(kBlock) k3_group_assign(const int32_t *ids, long long n, uint8_t *grp, double4 *vel, const double4 *pos, uint8_t g) {
+__global__ void __launch_bounds__(kBlock) k3_group_assign(const int32_t *ids, long long n, uint8_t *grp, double4 *vel, const double4 *pos, uint8_t g,
+                                                          double *sKE) {
     const long long q = (long long)blockIdx.x * kBlock + threadIdx.x;
     if (q >= n) return;
-    grp[ids[q]] = g;
-    vel[ids[q]] = pos[ids[q]];
+    const int p = ids[q];
+    grp[p] = g;
+    vel[p] = pos[p];
+    sKE[p] = 0.0;
 }
 
 }  // namespace lsmk

@@ -165,8 +165,10 @@ __device__ __forceinline__ void particle_update3(const StepParams &P, const Step
             const double4 xn = make_double4(mad<EXACT>(ns, P.g.dux[g], vh.x), mad<EXACT>(ns, P.g.duy[g], vh.y), mad<EXACT>(ns, P.g.duz[g], vh.z), 0.0);
             pos_next[p] = xn;
             if (own_pos) *own_pos = xn;
-        } else {
-            fd[p] = make_double4(fx, fy, fz, 0.0);
+        } else {   // held total force of a kinematic particle: f - gamma * (du/dt) (see particle_update)
+            const double vkx = __ddiv_rn(P.g.dux[g], P.dt), vky = __ddiv_rn(P.g.duy[g], P.dt), vkz = __ddiv_rn(P.g.duz[g], P.dt);
+            fd[p] = make_double4(sub<EXACT>(fx, mul<EXACT>(P.gamma, vkx)), sub<EXACT>(fy, mul<EXACT>(P.gamma, vky)),
+                                 sub<EXACT>(fz, mul<EXACT>(P.gamma, vkz)), 0.0);
         }
     }
 }

@@ -79,5 +79,7 @@ def test_product_does_not_import_oracle():
         for fn in fns:
             if fn.endswith((".py", ".cu", ".cuh", ".h", ".cpp")):
                 txt = open(os.path.join(dp, fn)).read()
-                assert "oracle" not in txt.lower().replace("the oracle's", "").replace("oracle's order", "") or fn.endswith((".cuh", ".cu")), fn
-                assert "import oracle" not in txt and "from oracle" not in txt and "olsm" not in txt, fn
+                # the word may appear in comments ("bit-identical to the oracle"); what must not appear is any way of
+                # reaching it: an import, an include, a path, a dlopen name, one of its symbols
+                for needle in ("import oracle", "from oracle", "olsm", "oracle/", "oracle\\", "liboracle", "oracle."):
+                    assert needle not in txt, (fn, needle)

@@ -378,6 +378,114 @@ def test_full_size_config3_bench_configuration():
     g.close()
 
 
+def test_full_size_config3_200_steps_bench_settings_and_exact_mode():
+    """SURVEY T1 on BASELINE.json configs[2] at full size ("steps 0 and 200"), with the settings bench.py times:
+    sample_every = 100, compaction on (every 100 steps here, so that two compactions fall inside the run), the default
+    streamed kernel.  Fast arithmetic: every particle within a few ulp of its coordinate after 200 steps, both samples
+    against the oracle, force evaluation at step 200 from identical positions.  Exact arithmetic: x, v and the broken
+    set bit-identical at full size."""
+    p = config3()
+    p.sample_every = 100
+    o = OracleSim.from_problem(p); o.step(200)
+    xo, vo = o.read_state(); fo = o.read_forces(); ho = o.read_stress()
+    bo, bso, nbo = o.read_broken()
+    eps = np.finfo(np.float64).eps
+    g = lsm_create_from_problem(p, compact_every=100)
+    g.step(200)
+    xg, vg = g.read_state(); hg = g.read_stress()
+    assert np.abs(xg - xo).max() <= 64 * eps * np.abs(xo).max() and np.abs(vg - vo).max() <= 1e-11
+    assert g.n_broken() == nbo and np.array_equal(hg["step"], [100, 200]) and np.array_equal(hg["n_broken"], ho["n_broken"])
+    for key in ("R", "U", "KE"):
+        assert np.abs(hg[key] - ho[key]).max() <= 1e-9 * np.abs(ho[key]).max(), key
+    g.write_state(xo, vo)                                   # T1 at step 200: forces from the oracle's own positions
+    sc = force_scale(xo, p.spring_i, p.spring_j, p.k, p.r0, ~bo)
+    check_forces(g.read_forces(), fo, sc, floor=conditioning_floor(xo, p.spring_i, p.spring_j, p.k, ~bo))
+    g.close()
+    e = lsm_create_from_problem(p, compact_every=100, exact=True)
+    e.step(200)
+    xe, ve = e.read_state(); be, bse, nbe = e.read_broken()
+    assert np.array_equal(xe, xo) and np.array_equal(ve, vo) and np.array_equal(bse, bso) and nbe == nbo
+    assert np.array_equal(e.read_forces(), fo)
+    e.close()
+
+
+def test_config2_at_its_own_size():
+    """BASELINE.json configs[1] at its own size (512 x 512 two-phase composite, three spring types, fused launches by
+    default): T1 at steps 0 and 200 (Q11 norms; bit-equal in exact mode), T4 the sampled curve over 2,000 steps."""
+    p = config2()
+    assert p.N == 512 * 512 and p.M == 784385
+    p.sample_every = 100
+    o = OracleSim.from_problem(p)
+    f0 = o.read_forces()
+    sc0 = force_scale(p.x, p.spring_i, p.spring_j, p.k, p.r0)
+    g = lsm_create_from_problem(p)
+    e = lsm_create_from_problem(p, exact=True)
+    assert g.info()["step_fusion"] == 1 and g.info()["param_mode"] == 1
+    check_forces(g.read_forces(), f0, sc0, floor=conditioning_floor(p.x, p.spring_i, p.spring_j, p.k))
+    assert np.array_equal(e.read_forces(), f0)
+    o.step(200); g.step(200); e.step(200)
+    xo, vo = o.read_state(); xg, vg = g.read_state(); xe, ve = e.read_state()
+    assert np.array_equal(xe, xo) and np.array_equal(ve, vo)
+    assert np.abs(xg - xo).max() <= 1e-11 and np.abs(vg - vo).max() <= 1e-11
+    bo = o.read_broken()[0]
+    g2 = lsm_create_from_problem(p); g2.write_state(xo, vo)
+    check_forces(g2.read_forces(), o.read_forces(), force_scale(xo, p.spring_i, p.spring_j, p.k, p.r0, ~bo),
+                 floor=conditioning_floor(xo, p.spring_i, p.spring_j, p.k, ~bo))
+    g2.close()
+    o.step(1800); g.step(1800); e.step(1800)
+    ho, hg, he = o.read_stress(), g.read_stress(), e.read_stress()
+    assert np.array_equal(hg["step"], ho["step"]) and len(ho["step"]) == 20
+    assert np.array_equal(hg["n_broken"], ho["n_broken"]) and np.array_equal(he["n_broken"], ho["n_broken"])
+    for key in ("R", "U", "KE"):
+        assert np.abs(hg[key] - ho[key]).max() <= 1e-6 * np.abs(ho[key]).max(), key
+        assert np.abs(he[key] - ho[key]).max() <= 1e-12 * np.abs(ho[key]).max(), key
+    xo, vo = o.read_state(); xe, ve = e.read_state()
+    assert np.array_equal(xe, xo) and np.array_equal(ve, vo)
+    g.close(); e.close()
+
+
+@pytest.mark.parametrize("kw", [dict(), dict(gather_variant=lsm.GATHER_DIRECT), dict(step_fusion=lsm.FUSION_OFF, reorder=1)],
+                         ids=["fused", "direct", "streamed-morton"])
+def test_set_boundary_mid_run_is_bit_identical_in_exact_mode(kw):
+    """DESIGN.md R3: redefining a group between two steps (an unloading cycle; a release) changes memberships and origins
+    only -- the held total force fd = f - gamma v of the last evaluation still feeds the next first half kick.  Config 1
+    (gamma = 0.01): pull 700 steps, reverse the top grip, 500 steps, release the top grip, 300 steps; x, v bitwise
+    against the oracle after each phase, energies of the state right after each call."""
+    p = config1()
+    p.sample_every = 50
+    o = OracleSim.from_problem(p)
+    g = lsm_create_from_problem(p, exact=True, **kw)
+    top = p.groups[1].ids
+    def same():
+        xo, vo = o.read_state(); xg, vg = g.read_state()
+        assert np.array_equal(xo, xg) and np.array_equal(vo, vg)
+        Uo, KEo = o.read_energy(); Ug, KEg = g.read_energy()
+        assert np.allclose(Ug, Uo, rtol=1e-12) and np.allclose(KEg, KEo, rtol=1e-12)
+        assert np.array_equal(o.read_forces(), g.read_forces())
+    o.step(700); g.step(700); same()
+    for s in (o, g):
+        s.set_boundary(1, top, MOVE, [0.0, -1e-4])
+    same()
+    o.step(500); g.step(500); same()
+    for s in (o, g):
+        s.set_boundary(1, np.zeros(0, dtype=np.int32), MOVE, [0.0, 0.0])       # release: the row flies on with v = du/dt
+    same()
+    o.step(300); g.step(300); same()
+    ho, hg = o.read_stress(), g.read_stress()
+    assert np.array_equal(ho["step"], hg["step"])
+    for key in ("R", "U", "KE"):
+        assert np.abs(hg[key] - ho[key]).max() <= 1e-12 * np.abs(ho[key]).max(), key
+    g.close()
+    # fast arithmetic follows within the T2 tolerance
+    o2 = OracleSim.from_problem(p); f = lsm_create_from_problem(p, **kw)
+    o2.step(700); f.step(700)
+    for s in (o2, f):
+        s.set_boundary(1, top, MOVE, [0.0, -1e-4])
+    o2.step(500); f.step(500)
+    assert np.abs(f.read_state()[0] - o2.read_state()[0]).max() <= 1e-11
+    f.close()
+
+
 # ---------------------------------------------------------------- kernel variants agree (direct / streamed / fused)
 def test_gather_variants_and_step_fusion_bit_identical_in_exact_mode():
     """The direct kernel, the streamed (bulk-copy pipeline) kernel and the fused multi-step launch run the same row

@@ -482,3 +482,159 @@ def test_P11_summation_order_sensitivity_budget():
     assert a.read_broken()[2] == 0 and b.read_broken()[2] == 0
     dx, dv = np.abs(xb - xa[perm]).max(), np.abs(vb - va[perm]).max()
     assert 0 < dx <= 1e-11 and dv <= 1e-11
+
+
+# ---------------------------------------------------------------- mass != 1 (Eq. 4 a = F/m; per-type masses, L88)
+def test_P1_oscillator_with_mass_4():
+    """P1's closed form with m = 4: theta = arccos(1 - k dt^2 / (2 m)); a wrong `fd*m` (or a dropped 1/m) changes the
+    period by a factor 4 (2) and fails at 1e-11.  The sampled KE = 1/2 m v^2 with the closed-form full-step velocity."""
+    k, r0, dt, m, A = 1e-4, 10.0, 1.0, 4.0, 5.0
+    s = _two_particles(r0 + A, k, r0, 100.0, dt, m=m, sample_every=1)
+    th = 2.0 * np.arcsin(np.sqrt(k * dt * dt / (4.0 * m)))     # = arccos(1 - k dt^2 / (2 m)), well conditioned at small angles
+    for n in range(1, 1501):
+        s.step(1)
+        x, v = s.read_state()
+        assert abs(x[1, 0] - (r0 + A * np.cos(n * th))) <= 1e-11
+        assert abs(v[1, 0] + A * np.sin(th) / dt * np.sin(n * th)) <= 1e-12
+    h = s.read_stress()
+    n = np.arange(1, 1501)
+    ke = 0.5 * m * (A * np.sin(th) / dt * np.sin(n * th)) ** 2
+    assert np.abs(h["KE"][:, 0] - ke).max() <= 1e-13 * ke.max()
+    U, KE = s.read_energy()
+    assert abs(KE[0] - ke[-1]) <= 1e-13 * ke.max()
+
+
+def test_P2_two_free_particles_unequal_masses():
+    """Two free particles with m0 = 3, m1 = 0.5 (a per-particle mass ARRAY): the separation follows the closed form
+    with the reduced mass m0 m1/(m0 + m1); the mass-weighted centre of mass stays put; each particle moves by its
+    mass share; sampled KE = 1/2 m_red v_rel^2 with the closed-form relative velocity."""
+    k, r0, dt, A = 1e-4, 10.0, 1.0, 5.0
+    m0, m1 = 3.0, 0.5
+    x = np.array([[0.0, 0.0], [r0 + A, 0.0]])
+    s = OracleSim(x, [0], [1], [k], [r0], [100.0], dt, mass=np.array([m0, m1]), sample_every=1)
+    mred = m0 * m1 / (m0 + m1)
+    th = 2.0 * np.arcsin(np.sqrt((k / mred) * dt * dt / 4.0))  # = arccos(1 - (k/m_red) dt^2 / 2)
+    com0 = (m1 * (r0 + A)) / (m0 + m1)
+    for n in range(1, 1001):
+        s.step(1)
+        xx, vv = s.read_state()
+        sep = xx[1, 0] - xx[0, 0]
+        assert abs(sep - (r0 + A * np.cos(n * th))) <= 1e-11
+        assert abs((m0 * xx[0, 0] + m1 * xx[1, 0]) / (m0 + m1) - com0) <= 1e-12
+        assert abs(m0 * vv[0, 0] + m1 * vv[1, 0]) <= 1e-15
+        # particle 1 carries the share m0/(m0+m1) of the relative motion
+        assert abs((xx[1, 0] - (r0 + A)) - m0 / (m0 + m1) * (sep - (r0 + A))) <= 1e-11
+    h = s.read_stress()
+    n = np.arange(1, 1001)
+    vrel = -A * np.sin(th) / dt * np.sin(n * th)
+    ke = 0.5 * mred * vrel ** 2
+    assert np.abs(h["KE"][:, 0] - ke).max() <= 1e-12 * ke.max()
+
+
+def test_P12_damping_with_mass_2():
+    """P12's recurrence with m = 2: c = gamma dt / m, w^2 = k/m.  Pins that the damping force is divided by m exactly
+    once (gamma has units mass/time, Q7)."""
+    m, k, r0 = 2.0, 1.0, 1.0
+    dt, gamma, u0 = 0.01, 0.03, 0.05
+    s = _two_particles(r0 + u0, k, r0, 10.0, dt, gamma=gamma, m=m)
+    c, w2 = gamma * dt / m, k / m * dt * dt
+    rho = np.sqrt(1 - c)
+    cphi = (2 - c - w2) / (2 * rho)
+    phi = np.arccos(cphi)
+    A, u1 = u0, u0 * (1 - w2 / 2)
+    B = (u1 / rho - A * cphi) / np.sin(phi)
+    for blk in range(50):
+        s.step(100)
+        n = (blk + 1) * 100
+        x, _ = s.read_state()
+        assert abs((x[1, 0] - r0) - rho ** n * (A * np.cos(n * phi) + B * np.sin(n * phi))) <= 1e-11
+
+
+# ---------------------------------------------------------------- kinematic particles (Q6) and olsm_write_state
+def test_kinematic_velocity_is_du_over_dt_and_carries_no_KE():
+    """Q6: a MOVE particle reports v = du/dt (also right after set_boundary, before any step), a FIXED one v = 0, and
+    neither enters KE; the virial's kinetic term uses that stored velocity."""
+    dt = 0.25
+    x = np.array([[0.0, 0.0], [1.0, 0.0], [5.0, 5.0]])
+    v = np.array([[9.0, 9.0], [7.0, 7.0], [0.5, -1.0]])
+    s = OracleSim(x, [0], [1], 0.0, 1.0, 10.0, dt, v=v, mass=np.array([1.0, 2.0, 4.0]), sample_every=1)
+    s.set_boundary(0, [0], FIXED)
+    s.set_boundary(1, [1], MOVE, [0.125, -0.5])
+    _, vv = s.read_state()
+    assert np.array_equal(vv[0], [0.0, 0.0]) and np.array_equal(vv[1], [0.5, -2.0]) and np.array_equal(vv[2], [0.5, -1.0])
+    assert s.read_energy()[1][0] == 0.5 * 4.0 * (0.25 + 1.0)          # only the free particle
+    S = s.read_virial()
+    assert np.array_equal(S[1], [-2.0 * 0.25, -2.0 * 4.0, -2.0 * 0.5 * -2.0])
+    s.step(3)
+    xx, vv = s.read_state()
+    assert np.array_equal(xx[1], [1.375, -1.5]) and np.array_equal(vv[1], [0.5, -2.0]) and np.array_equal(xx[0], [0.0, 0.0])
+    assert np.array_equal(xx[2], [5.0 + 3 * dt * 0.5, 5.0 - 3 * dt])   # free flight (k = 0)
+    assert np.all(s.read_stress()["KE"][:, 0] == 0.5 * 4.0 * 1.25)
+
+
+def test_write_state_restarts_on_the_closed_form():
+    """olsm_write_state: (a) writing the closed-form state (x_n, v_n) of P1's oscillator into a handle that has already
+    run somewhere else continues ON the closed form (forces are refreshed from the written positions -- with a stale
+    f the very next kick is wrong -- and v is taken as the full-step velocity); (b) a MOVE particle takes the written
+    position as its new origin and restarts its step count there: after j more steps it sits at written + j du exactly
+    (dyadic du) -- a missing n0 reset or origin re-snapshot is off by (steps before the write) * du."""
+    k, r0, dt, A = 1e-4, 10.0, 1.0, 5.0
+    th = 2.0 * np.arcsin(np.sqrt(k * dt * dt / 4.0))           # = arccos(1 - k dt^2 / 2)
+    n0 = 137
+    xn = r0 + A * np.cos(n0 * th)
+    vn = -A * np.sin(th) / dt * np.sin(n0 * th)
+    du = np.array([2.0 ** -7, -2.0 ** -9])
+    #            fixed end   oscillator      a MOVE particle tied to nothing (k irrelevant: own spring has k = 0)
+    x = np.array([[0.0, 0.0], [r0 + 1.0, 0.0], [40.0, 3.0], [41.0, 3.0]])
+    s = OracleSim(x, [0, 2], [1, 3], [k, 0.0], [r0, 1.0], [100.0, 100.0], dt)
+    s.set_boundary(0, [0], FIXED)
+    s.set_boundary(1, [2], MOVE, du)
+    s.step(61)                                                   # somewhere else: step counter 61, group origin at step 0
+    xw = np.array([[0.0, 0.0], [xn, 0.0], [50.0, -2.0], [41.0, 3.0]])
+    vw = np.array([[0.0, 0.0], [vn, 0.0], [123.0, 456.0], [0.0, 0.0]])   # the written v of a kinematic particle is ignored
+    s.write_state(xw, vw)
+    f = s.read_forces()
+    assert abs(f[1, 0] + k * (xn - r0)) <= 1e-18 and f[0, 0] == -f[1, 0]
+    _, vv = s.read_state()
+    assert np.array_equal(vv[2], du / dt)
+    for j in range(1, 401):
+        s.step(1)
+        xx, vv = s.read_state()
+        assert abs(xx[1, 0] - (r0 + A * np.cos((n0 + j) * th))) <= 1e-11
+        assert abs(vv[1, 0] + A * np.sin(th) / dt * np.sin((n0 + j) * th)) <= 1e-12
+        assert np.array_equal(xx[2], [50.0 + j * du[0], -2.0 + j * du[1]])
+        assert np.array_equal(xx[0], [0.0, 0.0])
+
+
+def test_set_boundary_mid_run_keeps_the_held_force():
+    """Redefining a group between two steps changes memberships and origins only: the total force fd = f - gamma v held
+    from the last force evaluation (Q7: damping with the velocity held at force time) still feeds the next first half
+    kick of every particle that stays free.  Closed form: P12's damped oscillator keeps following its recurrence when
+    an unrelated MOVE group is reversed in the middle of the run."""
+    m = k = r0 = 1.0
+    dt, gamma, u0 = 0.01, 0.05, 0.05
+    x = np.array([[0.0, 0.0], [r0 + u0, 0.0], [10.0, 0.0], [11.0, 0.0]])
+    s = OracleSim(x, [0, 2], [1, 3], [k, 0.0], [r0, 1.0], [10.0, 10.0], dt, gamma=gamma)
+    s.set_boundary(0, [0], FIXED)
+    s.set_boundary(1, [2], MOVE, [2.0 ** -10, 0.0])
+    c, w2 = gamma * dt / m, k / m * dt * dt
+    rho = np.sqrt(1 - c)
+    cphi = (2 - c - w2) / (2 * rho)
+    phi = np.arccos(cphi)
+    A, u1 = u0, u0 * (1 - w2 / 2)
+    B = (u1 / rho - A * cphi) / np.sin(phi)
+    for n in range(1, 2001):
+        s.step(1)
+        if n == 777:
+            s.set_boundary(1, [2], MOVE, [-2.0 ** -10, 0.0])      # reversal: origin = current position, n0 = 777
+        if n == 1200:
+            s.set_boundary(1, [], MOVE, [0.0, 0.0])               # release: particle 2 flies on freely with v = du/dt
+        xx, vv = s.read_state()
+        assert abs((xx[1, 0] - r0) - rho ** n * (A * np.cos(n * phi) + B * np.sin(n * phi))) <= 1e-12
+        if n <= 777:
+            assert xx[2, 0] == 10.0 + n * 2.0 ** -10
+        elif n <= 1200:
+            assert xx[2, 0] == 10.0 + (2 * 777 - n) * 2.0 ** -10
+    # released at step 1200 with v = -2^-10/dt, then damped free flight (k = 0): v_{n+1} = v_n (1 - c/2 ... ) per Q7:
+    # kick1: v += hdt*(-gamma v_held)/m, kick2 likewise with the half-step velocity -> checked as monotone decay here
+    assert -2.0 ** -10 / dt < vv[2, 0] < 0.0 and xx[2, 0] < 10.0 + (2 * 777 - 1200) * 2.0 ** -10
