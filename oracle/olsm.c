@@ -22,8 +22,15 @@
  * P3 affine uniaxial-stress state of a full triangular lattice (Young's modulus 2k/sqrt3, Poisson ratio 1/3, energy);
  * P4 zero net force / torque; P5 brute-force all-pairs; P6 energy conservation; P7 strict '>' with dyadic numbers;
  * P8 irreversibility; P9 time reversibility (L76); P10 F = -grad U by finite differences; P12 damping closed form.
+ * Mass != 1 (Eq. 4), olsm_write_state, the stored velocity of kinematic particles and olsm_set_boundary between steps
+ * have their own closed-form pins (P1 with m = 4, P2 with unequal masses, P12 with m = 2, restart on the closed form).
  * Unpinned: the fracture path AFTER the first breakage has no closed form (statistics only) -- "parity unpinned"
  * for that part; see DESIGN.md.
+ *
+ * olsm_set_threads(n > 1) switches the force evaluation to force_eval_threads(): the same arithmetic per spring, summed
+ * per particle in the same ascending spring order, run over OpenMP threads.  It exists only so that bench.py can time
+ * the oracle on all host cores; the serial loop stays the reference every parity test compares with,
+ * and tests/test_oracle_pins.py asserts the threaded variant is bit-equal to it through a fracture run.
  */
 #include <math.h>
 #include <stdint.h>
@@ -66,6 +73,13 @@ typedef struct olsm_sim {
     double *h_R;                    /* [cap][B][8][D] */
     double *h_U, *h_KE;             /* [cap][B] */
     int64_t *h_nb;                  /* [cap][B] */
+    /* all-cores variant (olsm_set_threads): per-particle incidence lists in ascending spring id, per-spring scratch */
+    int32_t threads;                /* 0 / 1 = the serial loop */
+    int64_t *adj_off;               /* [N+1] */
+    int32_t *adj_e;                 /* [2M] spring ids, ascending inside each particle's list */
+    double *gs, *ue;                /* [M] k (r - r0)/r and the energy of each spring in the last evaluation */
+    uint8_t *act;                   /* [M] 1 if the spring contributed to the last evaluation */
+    int32_t U_stale;                /* per-specimen U not yet summed from ue[] */
 } olsm_sim;
 
 /* Eq. 1 / Eq. 2 / listing L91-L107.  Serial loop, caller spring order. */
@@ -102,10 +116,69 @@ static void force_eval(olsm_sim *s)
     }
 }
 
+/* The same evaluation over OpenMP threads (all-cores timing leg only).  Pass 1, one iteration per spring: the same
+ * expressions as force_eval() for r, the breakage test, g and the energy, stored per spring.  Pass 2, one iteration per
+ * particle: add its springs' g*d in ascending spring id -- the order, and hence every rounding, of the serial loop
+ * (which does f[i] += gd, f[j] -= gd spring by spring).  U is summed serially in spring order when it is next read. */
+static void sum_U(olsm_sim *s)
+{
+    if (!s->U_stale) return;
+    for (int b = 0; b < s->B; ++b) s->U[b] = 0.0;
+    for (int64_t e = 0; e < s->M; ++e)
+        if (s->act[e]) s->U[s->spec_of_spring[e]] += s->ue[e];
+    s->U_stale = 0;
+}
+
+static void force_eval_threads(olsm_sim *s)
+{
+    const int D = s->D;
+    #pragma omp parallel for schedule(static) num_threads(s->threads)
+    for (int64_t e = 0; e < s->M; ++e) {
+        s->act[e] = 0;
+        if (!s->alive[e]) continue;
+        const int64_t i = s->si[e], j = s->sj[e];
+        double d[3] = {0.0, 0.0, 0.0};
+        double r2 = 0.0;
+        for (int c = 0; c < D; ++c) {
+            d[c] = s->x[j * D + c] - s->x[i * D + c];
+            r2 = r2 + d[c] * d[c];
+        }
+        const double r = sqrt(r2);
+        if (r > s->rc[e]) {
+            s->alive[e] = 0;
+            s->break_step[e] = s->step;
+            #pragma omp atomic
+            s->nbroken[s->spec_of_spring[e]] += 1;
+            continue;
+        }
+        if (r == 0.0) continue;
+        const double ext = r - s->r0[e];
+        s->gs[e] = s->k[e] * ext / r;
+        s->ue[e] = 0.5 * s->k[e] * ext * ext;
+        s->act[e] = 1;
+    }
+    #pragma omp parallel for schedule(static) num_threads(s->threads)
+    for (int64_t p = 0; p < s->N; ++p) {
+        double fp[3] = {0.0, 0.0, 0.0};
+        for (int64_t q = s->adj_off[p]; q < s->adj_off[p + 1]; ++q) {
+            const int64_t e = s->adj_e[q];
+            if (!s->act[e]) continue;
+            const int64_t i = s->si[e], j = s->sj[e];
+            for (int c = 0; c < D; ++c) {
+                const double gd = s->gs[e] * (s->x[j * D + c] - s->x[i * D + c]);
+                if (p == i) fp[c] += gd; else fp[c] -= gd;
+            }
+        }
+        for (int c = 0; c < D; ++c) s->f[p * D + c] = fp[c];
+    }
+    s->U_stale = 1;
+}
+
 static void damp(olsm_sim *s)
 {
     /* Q7: viscous force -gamma*v, v = the velocity held at force time. gamma = 0 reproduces the paper. */
     const int64_t n = s->N * s->D;
+    #pragma omp parallel for schedule(static) num_threads(s->threads) if (s->threads > 1)
     for (int64_t q = 0; q < n; ++q) s->fd[q] = s->f[q] - s->gamma * s->v[q];
 }
 
@@ -121,6 +194,7 @@ static void record_sample(olsm_sim *s)
         s->h_nb = realloc(s->h_nb, sizeof(int64_t) * (size_t)(nc * s->B));
         s->cap = nc;
     }
+    sum_U(s);
     const int64_t t = s->ns++;
     s->h_step[t] = s->step;
     double *R = s->h_R + t * s->B * OLSM_MAX_GROUPS * D;
@@ -218,6 +292,7 @@ int32_t olsm_step(olsm_sim *s, int64_t n_steps)
     const double dt = s->dt, hdt = 0.5 * s->dt;
     for (int64_t it = 0; it < n_steps; ++it) {
         /* 1-2. first half kick (Eq. 5, first half) and drift (Eq. 3) of the free particles */
+        #pragma omp parallel for schedule(static) num_threads(s->threads) if (s->threads > 1)
         for (int64_t p = 0; p < s->N; ++p) {
             if (s->group_of[p] >= 0) continue;
             for (int c = 0; c < D; ++c) {
@@ -238,10 +313,11 @@ int32_t olsm_step(olsm_sim *s, int64_t n_steps)
         }
         /* 3. forces at the new positions (Eq. 4) + breakage (L98) */
         s->step += 1;
-        force_eval(s);
+        if (s->threads > 1) force_eval_threads(s); else force_eval(s);
         /* 4. damping with the half-step velocity (Q7) */
         damp(s);
         /* 5. second half kick (Eq. 5, second half) */
+        #pragma omp parallel for schedule(static) num_threads(s->threads) if (s->threads > 1)
         for (int64_t p = 0; p < s->N; ++p) {
             if (s->group_of[p] >= 0) continue;
             for (int c = 0; c < D; ++c) {
@@ -272,8 +348,32 @@ int32_t olsm_write_state(olsm_sim *s, const double *x, const double *v)
                 s->v[g->ids[q] * s->D + c] = g->du[c] / s->dt;
             }
     }
-    force_eval(s);
+    if (s->threads > 1) force_eval_threads(s); else force_eval(s);
     damp(s);
+    return 0;
+}
+
+/* Run the following steps on n OpenMP threads (n <= 1: the serial loop).  Builds the per-particle incidence lists. */
+int32_t olsm_set_threads(olsm_sim *s, int32_t n)
+{
+    if (!s) return -1;
+    if (n > 1 && !s->adj_off) {
+        s->adj_off = calloc((size_t)(s->N + 1), sizeof(int64_t));
+        s->adj_e = malloc(sizeof(int32_t) * (size_t)(2 * s->M + 1));
+        s->gs = calloc((size_t)(s->M + 1), sizeof(double));
+        s->ue = calloc((size_t)(s->M + 1), sizeof(double));
+        s->act = calloc((size_t)(s->M + 1), 1);
+        for (int64_t e = 0; e < s->M; ++e) { s->adj_off[s->si[e] + 1]++; s->adj_off[s->sj[e] + 1]++; }
+        for (int64_t p = 0; p < s->N; ++p) s->adj_off[p + 1] += s->adj_off[p];
+        int64_t *fill = malloc(sizeof(int64_t) * (size_t)(s->N + 1));
+        memcpy(fill, s->adj_off, sizeof(int64_t) * (size_t)(s->N + 1));
+        for (int64_t e = 0; e < s->M; ++e) {               /* ascending e -> every list is ascending */
+            s->adj_e[fill[s->si[e]]++] = (int32_t)e;
+            s->adj_e[fill[s->sj[e]]++] = (int32_t)e;
+        }
+        free(fill);
+    }
+    s->threads = n > 1 ? n : 0;
     return 0;
 }
 
@@ -306,9 +406,10 @@ int32_t olsm_read_broken(const olsm_sim *s, uint8_t *broken, int64_t *break_step
 }
 
 /* Current per-specimen energies: U of the last force evaluation, KE of the current velocities. */
-int32_t olsm_read_energy(const olsm_sim *s, double *U, double *KE)
+int32_t olsm_read_energy(olsm_sim *s, double *U, double *KE)
 {
     if (!s) return -1;
+    sum_U(s);
     for (int b = 0; b < s->B; ++b) {
         if (U) U[b] = s->U[b];
         if (KE) {
@@ -390,5 +491,6 @@ void olsm_destroy(olsm_sim *s)
     free(s->si); free(s->sj); free(s->k); free(s->r0); free(s->rc); free(s->alive); free(s->break_step);
     free(s->nbroken); free(s->U); free(s->spec_of_spring); free(s->spec_of_particle); free(s->group_of);
     free(s->h_step); free(s->h_R); free(s->h_U); free(s->h_KE); free(s->h_nb);
+    free(s->adj_off); free(s->adj_e); free(s->gs); free(s->ue); free(s->act);
     free(s);
 }

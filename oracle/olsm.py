@@ -21,7 +21,7 @@ MAX_GROUPS = 8
 
 def build(force: bool = False) -> str:
     if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
-        cmd = ["gcc", "-std=c11", "-O2", "-ffp-contract=off", "-fPIC", "-shared", "-Wall", "-o", _SO, _SRC, "-lm"]
+        cmd = ["gcc", "-std=c11", "-O2", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared", "-Wall", "-o", _SO, _SRC, "-lm"]
         subprocess.run(cmd, check=True)
     return _SO
 
@@ -40,6 +40,7 @@ def lib():
                                   i32, i32, d, d, d, C.c_double, C.c_double, C.c_int32]
         L.olsm_set_boundary.argtypes = [C.c_void_p, C.c_int32, i32, C.c_int64, C.c_int32, d]
         L.olsm_step.argtypes = [C.c_void_p, C.c_int64]
+        L.olsm_set_threads.argtypes = [C.c_void_p, C.c_int32]
         L.olsm_write_state.argtypes = [C.c_void_p, d, d]
         L.olsm_read_state.argtypes = [C.c_void_p, d, d]
         L.olsm_read_forces.argtypes = [C.c_void_p, d]
@@ -105,6 +106,11 @@ class OracleSim:
     def step(self, n=1):
         if lib().olsm_step(self._h, int(n)) != 0:
             raise ValueError("olsm_step failed")
+
+    def set_threads(self, n):
+        """n > 1: the all-cores timing variant (bit-equal to the serial loop); n <= 1: the serial reference loop."""
+        if lib().olsm_set_threads(self._h, int(n)) != 0:
+            raise ValueError("olsm_set_threads failed")
 
     def write_state(self, x, v=None):
         x = np.ascontiguousarray(x, dtype=np.float64)

@@ -638,3 +638,34 @@ def test_set_boundary_mid_run_keeps_the_held_force():
     # released at step 1200 with v = -2^-10/dt, then damped free flight (k = 0): v_{n+1} = v_n (1 - c/2 ... ) per Q7:
     # kick1: v += hdt*(-gamma v_held)/m, kick2 likewise with the half-step velocity -> checked as monotone decay here
     assert -2.0 ** -10 / dt < vv[2, 0] < 0.0 and xx[2, 0] < 10.0 + (2 * 777 - 1200) * 2.0 ** -10
+
+
+def test_threaded_variant_is_bit_equal_to_the_serial_loop():
+    """olsm_set_threads (the all-cores timing leg of bench.py): same arithmetic per spring, same ascending-spring-id
+    summation per particle -> x, v, f, broken set, break steps and the sampled history must all be BIT-equal to the
+    serial reference loop through a fracture run; also in a batch, in 3-D, and when switching back and forth."""
+    from lsm_inputs import config2, config4, cubic_lattice_3d
+    p = config2(n=48, seed=11, n_blobs=24, du_y=6e-4)
+    p.sample_every = 50
+    a = OracleSim.from_problem(p); b = OracleSim.from_problem(p)
+    b.set_threads(4)
+    a.step(4000); b.step(1500); b.set_threads(1); b.step(500); b.set_threads(3); b.step(2000)
+    assert a.read_broken()[2] > 10
+    for u, w in zip(a.read_state() + (a.read_forces(),) + a.read_broken()[:2], b.read_state() + (b.read_forces(),) + b.read_broken()[:2]):
+        assert np.array_equal(u, w)
+    ha, hb = a.read_stress(), b.read_stress()
+    for key in ha:
+        assert np.array_equal(ha[key], hb[key]), key
+    assert np.array_equal(a.read_energy()[0], b.read_energy()[0]) and np.array_equal(a.read_virial(), b.read_virial())
+    pb = config4(B=3, n=16)
+    a = OracleSim.from_problem(pb, sample_every=50); b = OracleSim.from_problem(pb, sample_every=50)
+    b.set_threads(8)
+    a.step(300); b.step(300)
+    assert np.array_equal(a.read_state()[0], b.read_state()[0]) and np.array_equal(a.read_stress()["U"], b.read_stress()["U"])
+    x, si, sj, r0 = cubic_lattice_3d(5, 4, 6)
+    x = x + np.random.default_rng(1).uniform(-0.05, 0.05, x.shape)
+    a = OracleSim(x, si, sj, 1.0, r0, 1.04 * r0, 0.02); b = OracleSim(x, si, sj, 1.0, r0, 1.04 * r0, 0.02)
+    b.set_threads(4)
+    a.step(200); b.step(200)
+    assert a.read_broken()[2] > 0 and np.array_equal(a.read_broken()[1], b.read_broken()[1])
+    assert np.array_equal(a.read_state()[0], b.read_state()[0]) and np.array_equal(a.read_state()[1], b.read_state()[1])
