@@ -175,7 +175,8 @@ def main():
     ap.add_argument("--compact-every", type=int, default=1000)
     ap.add_argument("--exact", type=int, default=0)
     ap.add_argument("--gather-variant", type=int, default=0, help="0 auto, 1 direct, 2 streamed")
-    ap.add_argument("--step-fusion", type=int, default=0, help="0 auto, 1 on, 2 off")
+    ap.add_argument("--step-fusion", type=int, default=0, help="0 auto, 1 cooperative multi-step launches, 2 off, 3 cluster-resident")
+    ap.add_argument("--cluster-size", type=int, default=0, help="cluster-resident stepping: CTAs per cluster (0 = library's choice)")
     ap.add_argument("--shuffle-ids", type=int, default=0, help="seed > 0: renumber particles / springs at random first (an arbitrary input-file order)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-steps", type=int, default=0, help="oracle time steps for cpu_baseline (0 = sized to ~15 s)")
@@ -215,7 +216,8 @@ def main():
     p.sample_every = SAMPLE_EVERY
     fm = {"auto": lsm.FORCE_AUTO, "gather": lsm.FORCE_GATHER, "scatter": lsm.FORCE_SCATTER}[args.force_mode]
     sim = lsm_create_from_problem(p, device=local, force_mode=fm, reorder=args.reorder, compact_every=args.compact_every,
-                                  exact=bool(args.exact), history_capacity=64, gather_variant=args.gather_variant, step_fusion=args.step_fusion)
+                                  exact=bool(args.exact), history_capacity=64, gather_variant=args.gather_variant, step_fusion=args.step_fusion,
+                                  cluster_size=args.cluster_size)
     inf0 = sim.info()
     M_alive0 = p.M - sim.n_broken()
     S, K, W = args.inner, args.steps, args.warmup
@@ -296,7 +298,7 @@ def main():
             "config": {"workload": desc, "N": p.N, "M": p.M, "M_alive_at_start": M_alive0, "broken_at_end": nb_after,
                        "time_steps_per_bench_step": S, "ns_per_time_step": 1e6 * ms_max / (K * S), "sample_every": SAMPLE_EVERY,
                        "compact_every": args.compact_every, "force_mode": inf0["force_mode"], "param_mode": inf0["param_mode"],
-                       "exact": inf0["exact"], "reorder": inf0["reorder"], "gather_variant": inf0["gather_variant"], "step_fusion": inf0["step_fusion"], "pipeline_stages": inf0["pipeline_stages"], "stage_bytes": inf0["stage_bytes"], "bytes_per_half_edge": inf0["bytes_per_half_edge"],
+                       "exact": inf0["exact"], "reorder": inf0["reorder"], "gather_variant": inf0["gather_variant"], "step_fusion": inf0["step_fusion"], "cluster_size": inf0["cluster_size"], "pipeline_stages": inf0["pipeline_stages"], "stage_bytes": inf0["stage_bytes"], "bytes_per_half_edge": inf0["bytes_per_half_edge"],
                        "half_edges_stored": inf0["n_half_edges_stored"], "device_bytes": inf0["device_bytes"],
                        "l2": "inputs larger than L2 (%.0f MB streamed per time step vs 126 MB L2)"
                              % ((64.0 * p.N + inf0["n_half_edges_stored"] * inf0["bytes_per_half_edge"] + 1.25 * p.N) / 1e6),

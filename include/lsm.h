@@ -37,7 +37,7 @@ extern "C" {
 #endif
 
 #define LSM_MAX_GROUPS 8
-#define LSM_ABI_VERSION 3
+#define LSM_ABI_VERSION 4
 
 typedef struct lsm_sim lsm_sim; /* opaque */
 
@@ -61,7 +61,12 @@ enum { LSM_REORDER_NONE = 0, LSM_REORDER_MORTON = 1, LSM_REORDER_RCM = 2,
 /* kernels of the gather path: DIRECT = one thread per particle reading global memory; STREAMED = persistent CTAs,
  * bulk-async-copy (TMA engine) staging of the tile streams through a shared-memory mbarrier pipeline */
 enum { LSM_GATHER_AUTO = 0, LSM_GATHER_DIRECT = 1, LSM_GATHER_STREAMED = 2 };
-enum { LSM_FUSION_AUTO = 0, LSM_FUSION_ON = 1, LSM_FUSION_OFF = 2 };
+/* several time steps per launch: ON = one cooperative launch with a grid barrier between steps (state stays in L2 /
+ * the CTAs' pipeline stages); RESIDENT = one thread-block cluster per specimen keeps it in shared memory for the whole
+ * run of steps, ghosts exchanged through distributed shared memory, cluster barrier per step (needs dim = 2, 16-bit
+ * neighbour offsets, specimens starting on multiples of 32 particles and fitting one cluster; else LSM_E_UNSUPPORTED);
+ * AUTO = RESIDENT where it applies, else ON for L2-resident launch-bound problems, else one launch per step */
+enum { LSM_FUSION_AUTO = 0, LSM_FUSION_ON = 1, LSM_FUSION_OFF = 2, LSM_FUSION_RESIDENT = 3 };
 
 /* Optional device allocator (the Python binding passes PyTorch's caching allocator). */
 typedef void *(*lsm_alloc_fn)(size_t bytes, void *user);  /* returns a DEVICE pointer, NULL on failure */
@@ -94,11 +99,10 @@ typedef struct lsm_desc {
     int32_t exact;                    /* 1: IEEE sqrt/divide, no FMA contraction, each particle sums its springs in
                                          ascending caller spring id -> bit-identical to a serial loop over the
                                          spring list (GATHER only).  0: fast arithmetic (FMA, rsqrt)              */
-    int32_t step_fusion;              /* LSM_FUSION_*: run several time steps per (cooperative) launch with a grid
-                                         barrier between steps; AUTO = ON for L2-resident, launch-bound problems    */
+    int32_t step_fusion;              /* LSM_FUSION_* (above)                                                     */
     int32_t gather_variant;           /* LSM_GATHER_*: AUTO = STREAMED when a tile's rows fit in shared memory    */
     int32_t device;                   /* CUDA device ordinal                                                      */
-    int32_t _pad1;
+    int32_t cluster_size;             /* RESIDENT stepping: CTAs per cluster, 0 = chosen by the library, else 1, 2, 4, 8, 16 */
     void *stream;                     /* cudaStream_t, NULL = the default stream                                  */
     lsm_alloc_fn alloc;               /* NULL -> cudaMalloc / cudaFree                                            */
     lsm_free_fn free_;
@@ -122,8 +126,9 @@ typedef struct lsm_info {
     int32_t gather_variant;           /* resolved LSM_GATHER_* (0 for the scatter path)                           */
     int32_t pipeline_stages;          /* streamed variant: stages of the shared-memory pipeline                   */
     int64_t stage_bytes;              /* streamed variant: bytes per stage                                        */
-    int32_t step_fusion;              /* 1 if runs of plain time steps are fused into one launch                  */
-    int32_t _pad;
+    int32_t step_fusion;              /* 0: one launch per step; 1: cooperative multi-step launches; 2: cluster-resident */
+    int32_t cluster_size;             /* cluster-resident stepping: CTAs per cluster (0 otherwise)                */
+    int64_t resident_smem_bytes;      /* cluster-resident stepping: dynamic shared memory per CTA                 */
 } lsm_info;
 
 /* Build a simulation from particle / spring arrays.  Copies everything (the caller may free its inputs afterwards),

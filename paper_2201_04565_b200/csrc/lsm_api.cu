@@ -15,6 +15,7 @@
 #include "../../include/lsm.h"
 #include "lsm_kernels.cuh"
 #include "lsm_kernels3.cuh"
+#include "lsm_resident.cuh"
 
 using namespace lsmk;
 
@@ -39,7 +40,7 @@ struct lsm_sim {
     long long N = 0, M = 0;
     int B = 1, dim = 2;
     double dt = 0, gamma = 0, mass_u = 1;
-    int sample_every = 0, hist_cap = 1024, compact_every = 0, reorder = 0, force_mode = LSM_FORCE_GATHER, exact = 0, step_fusion = 0;
+    int sample_every = 0, hist_cap = 1024, compact_every = 0, reorder = 0, force_mode = LSM_FORCE_GATHER, exact = 0, step_fusion = 0, cluster_size = 0;
     int device = 0;
     cudaStream_t stream = nullptr;
     lsm_alloc_fn alloc = nullptr;
@@ -73,6 +74,11 @@ struct lsm_sim {
     uint32_t max_tile_slots = 0;
     double *virial = nullptr;        // [N][3] output buffer of lsm_read_virial (allocated on first use)
     int multi_on = 0;                // fuse runs of plain time steps into one cooperative launch
+    // cluster-resident stepping (lsm_resident.cuh): one thread-block cluster per unit (specimen / small lattice)
+    int res_on = 0, res_cluster = 0, res_grid = 0, res_active_clusters = 0;
+    ResLayout RL;
+    ResCta *res_desc = nullptr;
+    uint16_t *res_order = nullptr;
     long long multi_max = 4096;
     unsigned long long *gbar = nullptr, gbar_base = 0;
     // scatter layout
@@ -387,6 +393,134 @@ template <bool EXACT> void launch_stream_pm(const lsm_sim *s, const StepParams &
     }
 }
 
+// ---- cluster-resident stepping: plan (host, at create) and launch -------------------------------------------------------
+// Splits every unit (specimen) into C contiguous slice ranges, one per CTA of a cluster, and derives each CTA's window
+// (own particles + ghosts), the ghost ranges it pushes to the other CTAs, and its boundary-first slice order.
+// nbmin / nbmax: smallest / largest neighbour id of every particle (own id where it has none).
+struct ResPlan {
+    int C = 0;
+    std::vector<ResCta> desc;
+    std::vector<uint16_t> order;
+    ResLayout L;
+    bool ok = false;
+};
+
+ResPlan plan_resident(const lsm_sim *s, int C, const std::vector<int32_t> &nbmin, const std::vector<int32_t> &nbmax,
+                      const std::vector<uint32_t> &off, int smem_budget) {
+    ResPlan R;
+    R.C = C;
+    std::memset(&R.L, 0, sizeof(R.L));
+    const int B = s->B;
+    R.desc.assign((size_t)B * C, ResCta{});
+    std::vector<std::vector<uint16_t>> ord((size_t)B * C);
+    long long win_cap = 0, sl_cap = 0, slot_cap = 0;
+    for (int b = 0; b < B; ++b) {
+        const long long u0 = s->poff[b], u1 = s->poff[b + 1];
+        if (u0 % kSlice) return R;                                    // units must start on a slice boundary
+        const long long S0 = u0 / kSlice, S1 = (u1 + kSlice - 1) / kSlice, nsu = S1 - S0;
+        const long long base = nsu / C, rem = nsu % C;
+        ResCta *dd = &R.desc[(size_t)b * C];
+        for (int c = 0; c < C; ++c) {
+            const long long a = S0 + c * base + std::min<long long>(c, rem), e = a + base + (c < rem ? 1 : 0);
+            ResCta &q = dd[c];
+            q.sl0 = (int32_t)a; q.n_sl = (int32_t)(e - a);
+            q.own_lo = (int32_t)(a * kSlice);
+            q.n_own = (int32_t)std::max<long long>(0, std::min<long long>(u1, e * kSlice) - a * kSlice);
+            long long lo = q.own_lo, hi = (long long)q.own_lo + q.n_own;
+            for (long long p = q.own_lo; p < (long long)q.own_lo + q.n_own; ++p) { lo = std::min<long long>(lo, nbmin[p]); hi = std::max<long long>(hi, (long long)nbmax[p] + 1); }
+            q.wlo = (int32_t)lo; q.wlen = (int32_t)(hi - lo);
+            win_cap = std::max<long long>(win_cap, q.wlen);
+            sl_cap = std::max<long long>(sl_cap, q.n_sl);
+            slot_cap = std::max<long long>(slot_cap, (long long)off[e] - (long long)off[a]);
+        }
+        for (int c = 0; c < C; ++c) {   // ghost ranges: my own particles inside another CTA's window
+            ResCta &q = dd[c];
+            q.n_push = 0;
+            const long long o0 = q.own_lo, o1 = (long long)q.own_lo + q.n_own;
+            for (int r = 0; r < C; ++r) {
+                if (r == c || dd[r].wlen == 0) continue;
+                const long long lo = std::max<long long>(o0, dd[r].wlo), hi = std::min<long long>(o1, (long long)dd[r].wlo + dd[r].wlen);
+                if (lo >= hi) continue;
+                if (q.n_push == kResMaxPush) return R;               // numbering not banded enough for this cluster size
+                q.push[q.n_push++] = ResPush{r, (int32_t)lo, (int32_t)hi, dd[r].wlo};
+            }
+            std::vector<uint16_t> bnd, inner;   // boundary slices (exchange ghosts either way) first
+            for (int ls = 0; ls < q.n_sl; ++ls) {
+                const long long p0 = o0 + (long long)ls * kSlice, p1 = std::min<long long>(o1, p0 + kSlice);
+                bool bd = false;
+                for (int k = 0; k < q.n_push && !bd; ++k) bd = p0 < q.push[k].hi && q.push[k].lo < p1;
+                for (long long p = p0; p < p1 && !bd; ++p) bd = nbmin[p] < o0 || nbmax[p] >= o1;
+                (bd ? bnd : inner).push_back((uint16_t)ls);
+            }
+            q.n_boundary = (int32_t)bnd.size();
+            bnd.insert(bnd.end(), inner.begin(), inner.end());
+            ord[(size_t)b * C + c].swap(bnd);
+        }
+    }
+    if (sl_cap > 65535) return R;
+    const bool need_typ = s->pm == PM_TYPED || s->pm == PM_KRT_RCF, need_thr = s->pm == PM_RCF || s->pm == PM_KRT_RCF || s->pm == PM_FULL, need_kr = s->pm == PM_FULL;
+    ResLayout &L = R.L;
+    auto up = [](long long x) { return (x + 127) & ~127LL; };
+    long long o = 0;
+    L.tab = (int)o; if (need_typ) o += up((long long)s->ntypes * kTabStride * 8);
+    L.win_cap = (int)win_cap; L.sl_cap = (int)std::max<long long>(sl_cap, 1); L.own_cap = (int)(sl_cap * kSlice); L.slot_cap = (int)slot_cap;
+    L.pos0 = (int)o; o += up(win_cap * 16);
+    L.pos1 = (int)o; o += up(win_cap * 16);
+    L.vel = (int)o; o += up(sl_cap * kSlice * 16);
+    L.grp = (int)o; o += up(sl_cap * kSlice);
+    L.sl_off = (int)o; o += up(sl_cap * 8);        // {slice | width << 16, slot offset} per entry of the order list
+    L.nbr = (int)o; o += up(slot_cap * kSlice * 2);
+    L.thr = (int)o; if (need_thr) o += up(slot_cap * kSlice * 2);
+    L.typ = (int)o; if (need_typ) o += up(slot_cap * kSlice);
+    L.kF = (int)o; if (need_kr) o += up(slot_cap * kSlice * 8);
+    L.r0F = (int)o; if (need_kr) o += up(slot_cap * kSlice * 8);
+    if (o > smem_budget) return R;
+    L.bytes = (int)o;
+    R.order.assign((size_t)B * C * L.sl_cap, 0);
+    for (size_t i = 0; i < ord.size(); ++i) std::copy(ord[i].begin(), ord[i].end(), R.order.begin() + i * L.sl_cap);
+    R.ok = true;
+    return R;
+}
+
+template <int PM, bool EXACT> cudaError_t launch_resident_one(const lsm_sim *s, const StepParams &P, const ResParams &Q) {
+    auto kern = k_resident<PM, EXACT>;
+    static thread_local OptIn configured_for;
+    int &have = configured_for.bytes[s->device < kMaxDevices ? s->device : kMaxDevices - 1];
+    if (have < s->RL.bytes || s->device >= kMaxDevices - 1) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, s->RL.bytes);
+        if (e != cudaSuccess) return e;
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+        if (e != cudaSuccess) return e;
+        have = s->RL.bytes;
+    }
+    cudaLaunchConfig_t cfg;
+    std::memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = dim3((unsigned)s->res_grid); cfg.blockDim = dim3(kResThreads); cfg.dynamicSmemBytes = (size_t)s->RL.bytes; cfg.stream = s->stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = (unsigned)s->res_cluster; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, P, s->RL, Q);
+}
+
+template <bool EXACT> cudaError_t launch_resident_pm(const lsm_sim *s, const StepParams &P, const ResParams &Q) {
+    switch (s->pm) {
+        case PM_UNIFORM: return launch_resident_one<PM_UNIFORM, EXACT>(s, P, Q);
+        case PM_TYPED: return launch_resident_one<PM_TYPED, EXACT>(s, P, Q);
+        case PM_RCF: return launch_resident_one<PM_RCF, EXACT>(s, P, Q);
+        case PM_KRT_RCF: return launch_resident_one<PM_KRT_RCF, EXACT>(s, P, Q);
+        default: return launch_resident_one<PM_FULL, EXACT>(s, P, Q);
+    }
+}
+
+// nsteps plain time steps, first force evaluation = step `step`, state resident in the clusters' shared memory.
+cudaError_t launch_resident(lsm_sim *s, long long step, int nsteps) {
+    const StepParams P = step_params(s, step);
+    ResParams Q;
+    Q.desc = s->res_desc; Q.order = s->res_order; Q.pos_io = s->pos[s->cur]; Q.nsteps = nsteps;
+    return s->exact ? launch_resident_pm<true>(s, P, Q) : launch_resident_pm<false>(s, P, Q);
+}
+
 void launch_gather(lsm_sim *s, const StepParams &P, Variant v) {
     if (s->dim == 3 && s->gather_variant != 2) { launch_gather3(s, P.step, v); return; }
     if (s->gather_variant == 2) {
@@ -533,7 +667,7 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
     s->sample_every = d->sample_every; s->hist_cap = d->history_capacity > 0 ? d->history_capacity : 1024;
     s->compact_every = d->compact_every; s->reorder = d->reorder;
     s->force_mode = d->force_mode == LSM_FORCE_AUTO ? LSM_FORCE_GATHER : d->force_mode;
-    s->exact = d->exact; s->step_fusion = d->step_fusion; s->gather_variant = d->gather_variant; s->device = d->device; s->stream = (cudaStream_t)d->stream;
+    s->exact = d->exact; s->step_fusion = d->step_fusion; s->cluster_size = d->cluster_size; s->gather_variant = d->gather_variant; s->device = d->device; s->stream = (cudaStream_t)d->stream;
     s->alloc = d->alloc; s->free_ = d->free_; s->alloc_user = d->alloc_user;
 
     int ndev = 0;
@@ -899,7 +1033,39 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
             CUDA_TRY(s, cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, d->device));
             const long long fuse_below = 1 << 18;   // measured: 64^2 5.8 -> 3.6 us per step, 512^2 8.4 -> 8.3, 2.1 M particles 39.1 -> 40.4
             if (s->step_fusion == LSM_FUSION_ON && !(coop && s->gather_variant == 2)) return fail(s, LSM_E_UNSUPPORTED, "step_fusion = ON needs the streamed gather kernel and cooperative launch support");
-            s->multi_on = coop && s->gather_variant == 2 && (s->step_fusion == LSM_FUSION_ON || (s->step_fusion == LSM_FUSION_AUTO && N <= fuse_below));
+            s->multi_on = coop && s->gather_variant == 2 && (s->step_fusion == LSM_FUSION_ON || ((s->step_fusion == LSM_FUSION_AUTO || s->step_fusion == LSM_FUSION_RESIDENT) && N <= fuse_below));
+            // cluster-resident stepping: units (specimens) small enough for one thread-block cluster's shared memory
+            const bool want_res = s->step_fusion == LSM_FUSION_RESIDENT || s->step_fusion == LSM_FUSION_AUTO;
+            if (want_res && D == 2 && s->nbr16 && s->gather_variant == 2 && N <= 0x7FFFFFFF) {
+                std::vector<int32_t> nbmin(N), nbmax(N);
+                for (long long p = 0; p < N; ++p) {
+                    int32_t lo = (int32_t)p, hi = (int32_t)p;
+                    for (uint32_t q = off[p >> 5]; q < off[(p >> 5) + 1]; ++q) { const int32_t nb = hn[(size_t)q * kSlice + (p & 31)]; lo = std::min(lo, nb); hi = std::max(hi, nb); }
+                    nbmin[p] = lo; nbmax[p] = hi;
+                }
+                const int budget = dev_smem - 2048;            // static shared memory (the CTA descriptor) + reserve
+                ResPlan best;
+                for (int C = 1; C <= kResMaxCluster; C *= 2) {
+                    if (s->cluster_size > 0 && C != s->cluster_size) continue;
+                    ResPlan R = plan_resident(s, C, nbmin, nbmax, off, budget);
+                    if (!R.ok) continue;
+                    if (!best.ok) { best = std::move(R); if (s->cluster_size > 0) break; continue; }
+                    // a single (or a few) small units: more CTAs per unit while the GPU is not full and each keeps >= 8 slices
+                    if ((long long)B * C <= n_sm && R.L.sl_cap >= 8) best = std::move(R); else break;
+                }
+                // AUTO: a cluster uses at most 16 SMs, so one mid-size lattice is better off on the whole GPU with the
+                // cooperative multi-step launch (measured: 46k particles 3.3 us per step there, 6.0 us on one cluster);
+                // resident pays when the clusters fill the GPU, or when each warp has about one slice per step
+                if (best.ok && s->step_fusion == LSM_FUSION_AUTO && !((long long)B * best.C * 2 >= n_sm || best.L.sl_cap <= 16)) best.ok = false;
+                if (best.ok) {
+                    s->res_on = 1; s->res_cluster = best.C; s->res_grid = B * best.C; s->RL = best.L;
+                    TRY(upload(s, &s->res_desc, best.desc));
+                    TRY(upload(s, &s->res_order, best.order));
+                    CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+                    s->multi_on = 0;                               // the cluster barrier replaces the grid barrier
+                }
+            }
+            if (s->step_fusion == LSM_FUSION_RESIDENT && !s->res_on) return fail(s, LSM_E_UNSUPPORTED, "step_fusion = RESIDENT: needs dim = 2, the streamed gather kernel, 16-bit neighbour offsets (a banded numbering), specimens that start on multiples of 32 particles and fit one cluster's shared memory");
             if (s->multi_on) {
                 TRY(dev_alloc(s, &s->gbar, 1));
                 CUDA_TRY(s, cudaMemsetAsync(s->gbar, 0, sizeof(unsigned long long), s->stream));
@@ -991,7 +1157,8 @@ lsm_status lsm_create(const lsm_desc *d, lsm_sim **out) {
     if (d->reorder == LSM_REORDER_BLOCKED && d->dim != 2) return fail(nullptr, LSM_E_UNSUPPORTED, "reorder = BLOCKED is 2-D only");
     if (d->force_mode < 0 || d->force_mode > 2) return fail(nullptr, LSM_E_INVALID, "bad force_mode");
     if (d->gather_variant < 0 || d->gather_variant > 2) return fail(nullptr, LSM_E_INVALID, "bad gather_variant");
-    if (d->step_fusion < 0 || d->step_fusion > 2) return fail(nullptr, LSM_E_INVALID, "bad step_fusion");
+    if (d->step_fusion < 0 || d->step_fusion > 3) return fail(nullptr, LSM_E_INVALID, "bad step_fusion");
+    if (d->cluster_size != 0 && d->cluster_size != 1 && d->cluster_size != 2 && d->cluster_size != 4 && d->cluster_size != 8 && d->cluster_size != 16) return fail(nullptr, LSM_E_INVALID, "cluster_size must be 0 (auto), 1, 2, 4, 8 or 16");
     if ((d->alloc == nullptr) != (d->free_ == nullptr)) return fail(nullptr, LSM_E_INVALID, "alloc and free_ must be given together");
     lsm_sim *s = new (std::nothrow) lsm_sim();
     if (!s) return fail(nullptr, LSM_E_NOMEM, "out of host memory");
@@ -1088,6 +1255,16 @@ lsm_status lsm_step(lsm_sim *s, int64_t n_steps) {
             const bool last = i == seg;
             const bool samp = is_sample_step(s, m);
             const Variant v = last ? V_END : (samp ? V_MID_SAMPLE : V_MID);
+            if (gather && s->res_on && v == V_MID) {     // the run of plain MID steps that starts here, resident in the clusters
+                long long run = 1;
+                while (i + run < seg && !is_sample_step(s, m + run) && run < 65536) ++run;
+                if (run >= 2) {
+                    CUDA_TRY(s, launch_resident(s, m, (int)run));
+                    s->kernels_launched += 1;
+                    i += run - 1;
+                    continue;
+                }
+            }
             if (gather && s->multi_on && v == V_MID) {   // fuse the run of plain MID steps that starts here into one launch
                 long long run = 1;
                 while (i + run < seg && !is_sample_step(s, m + run) && run < s->multi_max) ++run;
@@ -1330,7 +1507,9 @@ lsm_status lsm_get_info(lsm_sim *s, lsm_info *info) {
     info->bytes_per_half_edge = s->force_mode == LSM_FORCE_GATHER ? (s->nbr16 && s->gather_variant == 2 ? 2 : 4) + pbytes_gather[s->pm] : 8 + pbytes_scatter[s->pm];
     info->gather_variant = s->force_mode == LSM_FORCE_GATHER ? s->gather_variant : 0;
     info->pipeline_stages = s->gather_variant == 2 ? s->L.stages : 0;
-    info->step_fusion = s->multi_on;
+    info->step_fusion = s->res_on ? 2 : s->multi_on;
+    info->cluster_size = s->res_on ? s->res_cluster : 0;
+    info->resident_smem_bytes = s->res_on ? s->RL.bytes : 0;
     info->stage_bytes = s->gather_variant == 2 ? s->L.bytes : 0;
     info->param_mode = s->pm; info->n_types = s->ntypes; info->force_mode = s->force_mode; info->exact = s->exact;
     info->reorder = s->reorder; info->n_batch = s->B; info->device_bytes = s->device_bytes;

@@ -76,7 +76,19 @@ struct StepVar {        // what changes from one time step to the next inside a 
     const double2 *pos_cur;
     double2 *pos_next;
     long long step;     // step number of THIS force evaluation (stamped on springs that break in it)
+    uint32_t pos_s;     // GM_SMEM only: shared-memory address of (hypothetical) particle 0 in the current position buffer
 };
+
+// Where a neighbour's position is gathered from.
+enum GatherMode { GM_GLOBAL_NC = 0,   // global memory through the read-only path (positions are constant during the launch)
+                  GM_GLOBAL_CG = 1,   // global memory, L2 only: positions written by other CTAs earlier in the same launch
+                  GM_SMEM = 2 };      // the CTA's shared-memory window (lsm_resident.cuh): own particles + ghosts
+
+__device__ __forceinline__ double2 lds_d2(uint32_t addr) {
+    double2 v;
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
+    return v;
+}
 
 struct StepParams {
     const double2 *pos_cur;
@@ -162,11 +174,21 @@ template <bool EXACT> __device__ __forceinline__ bool spring_eval(double dx, dou
 
 // Velocity-Verlet particle update (Eq. 3-5, half-step-velocity form L76), given the spring force
 // (fx,fy) at the current positions.  KICK2: second half kick completing the step; ADVANCE: first half kick + drift of
-// the next step fused behind it (the half-step velocity is what is stored between kernels); !ADVANCE: store the
-// completed state (v, f, fd).  SAMPLE: write per-particle energy terms and f for the reductions.
+// the next step fused behind it (the half-step velocity is what is stored between kernels); !ADVANCE: the completed
+// state (v, fd).  SAMPLE: the kinetic-energy term.  particle_math is the arithmetic (the one place it is written);
+// particle_update adds the stores of the direct / streamed kernels, lsm_resident.cuh its own.
+struct Upd {
+    double2 xn;      // ADVANCE: position after the next drift
+    double2 w;       // ADVANCE: half-step velocity carried to the next force evaluation (free particles)
+    double2 v;       // completed velocity of this step (free particles)
+    double2 fd;      // total force f - gamma v held at force time (Q7)
+    double ke;       // SAMPLE: 1/2 m |v|^2 (0 for kinematic particles, Q6)
+};
+
 template <bool EXACT, bool KICK2, bool ADVANCE, bool SAMPLE>
-__device__ __forceinline__ void particle_update(const StepParams &P, const StepVar &V, long long p, double2 xp, double2 vh, uint8_t g,
-                                                double fx, double fy, double u, double2 *own_pos = nullptr, double2 *own_vel = nullptr) {
+__device__ __forceinline__ Upd particle_math(const StepParams &P, long long step, long long p, double2 xp, double2 vh, uint8_t g, double fx, double fy) {
+    Upd o;
+    o.ke = 0.0;
     if (g == kFree) {
         const double fdx = sub<EXACT>(fx, mul<EXACT>(P.gamma, vh.x));  // damping with the held velocity (Q7)
         const double fdy = sub<EXACT>(fy, mul<EXACT>(P.gamma, vh.y));
@@ -177,38 +199,45 @@ __device__ __forceinline__ void particle_update(const StepParams &P, const StepV
         if (KICK2) { v.x = mad<EXACT>(P.hdt, ax, vh.x); v.y = mad<EXACT>(P.hdt, ay, vh.y); }  // Eq. 5, second half
         if (SAMPLE) {
             const double v2 = add<EXACT>(mul<EXACT>(v.x, v.x), mul<EXACT>(v.y, v.y));
-            P.sU[p] = u;
-            P.sKE[p] = mul<EXACT>(mul<EXACT>(0.5, m), v2);
+            o.ke = mul<EXACT>(mul<EXACT>(0.5, m), v2);
         }
-        if (SAMPLE || !ADVANCE) P.f[p] = make_double2(fx, fy);
+        o.v = v;
+        o.fd = make_double2(fdx, fdy);
         if (ADVANCE) {
-            double2 w, xn;
             if (!EXACT && KICK2 && !SAMPLE) {   // fast mode: the two half kicks of consecutive steps in one FMA (2 hdt = dt)
-                w.x = fma(P.dt, ax, vh.x); w.y = fma(P.dt, ay, vh.y);
+                o.w.x = fma(P.dt, ax, vh.x); o.w.y = fma(P.dt, ay, vh.y);
             } else {
-                w.x = mad<EXACT>(P.hdt, ax, v.x); w.y = mad<EXACT>(P.hdt, ay, v.y);      // Eq. 5, first half
+                o.w.x = mad<EXACT>(P.hdt, ax, v.x); o.w.y = mad<EXACT>(P.hdt, ay, v.y);      // Eq. 5, first half
             }
-            xn.x = mad<EXACT>(P.dt, w.x, xp.x); xn.y = mad<EXACT>(P.dt, w.y, xp.y);      // Eq. 3
-            V.pos_next[p] = xn;
-            P.vel[p] = w;
-            if (own_pos) { *own_pos = xn; *own_vel = w; }   // resident tiles: the staged copy is the next step's input
-        } else {
-            P.vel[p] = v;
-            P.fd[p] = make_double2(fdx, fdy);
+            o.xn.x = mad<EXACT>(P.dt, o.w.x, xp.x); o.xn.y = mad<EXACT>(P.dt, o.w.y, xp.y);  // Eq. 3
         }
     } else {  // kinematic particle: vh holds its origin x0 ("boundary displacements are first applied")
-        if (SAMPLE) { P.sU[p] = u; P.sKE[p] = 0.0; }
-        if (SAMPLE || !ADVANCE) P.f[p] = make_double2(fx, fy);
+        o.w = vh; o.v = vh;
         if (ADVANCE) {
-            const double ns = (double)(V.step + 1 - P.g.n0[g]);
-            const double2 xn = make_double2(mad<EXACT>(ns, P.g.dux[g], vh.x), mad<EXACT>(ns, P.g.duy[g], vh.y));
-            V.pos_next[p] = xn;
-            if (own_pos) *own_pos = xn;
+            const double ns = (double)(step + 1 - P.g.n0[g]);
+            o.xn = make_double2(mad<EXACT>(ns, P.g.dux[g], vh.x), mad<EXACT>(ns, P.g.duy[g], vh.y));
         } else {   // completed state: the held total force of a kinematic particle is f - gamma * (du/dt), its stored
             // velocity being du/dt (Q6, Q7); it matters only if the particle is released later (lsm_set_boundary)
             const double vkx = __ddiv_rn(P.g.dux[g], P.dt), vky = __ddiv_rn(P.g.duy[g], P.dt);
-            P.fd[p] = make_double2(sub<EXACT>(fx, mul<EXACT>(P.gamma, vkx)), sub<EXACT>(fy, mul<EXACT>(P.gamma, vky)));
+            o.fd = make_double2(sub<EXACT>(fx, mul<EXACT>(P.gamma, vkx)), sub<EXACT>(fy, mul<EXACT>(P.gamma, vky)));
         }
+    }
+    return o;
+}
+
+template <bool EXACT, bool KICK2, bool ADVANCE, bool SAMPLE>
+__device__ __forceinline__ void particle_update(const StepParams &P, const StepVar &V, long long p, double2 xp, double2 vh, uint8_t g,
+                                                double fx, double fy, double u, double2 *own_pos = nullptr, double2 *own_vel = nullptr) {
+    const Upd o = particle_math<EXACT, KICK2, ADVANCE, SAMPLE>(P, V.step, p, xp, vh, g, fx, fy);
+    if (SAMPLE) { P.sU[p] = u; P.sKE[p] = o.ke; }
+    if (SAMPLE || !ADVANCE) P.f[p] = make_double2(fx, fy);
+    if (ADVANCE) {
+        V.pos_next[p] = o.xn;
+        if (own_pos) *own_pos = o.xn;                    // resident tiles: the staged copy is the next step's input
+        if (g == kFree) { P.vel[p] = o.w; if (own_vel) *own_vel = o.w; }
+    } else {
+        if (g == kFree) P.vel[p] = o.v;
+        P.fd[p] = o.fd;
     }
 }
 
@@ -264,8 +293,9 @@ template <int PM> __device__ __forceinline__ void slot_params(const StepParams &
 // L1 / L2 hits); reading in-tile neighbours from the staged copy instead was measured equal on config 3 and 17 %
 // slower on full lattices (a per-slot branch).  COHERENT (multi-step launches): positions written by other CTAs
 // earlier in the same launch must not come from a stale L1 line -> ld.global.cg (L2 only).
-template <bool COHERENT> __device__ __forceinline__ double2 gather_pos(const StepVar &V, int j) {
-    return COHERENT ? __ldcg(V.pos_cur + j) : __ldg(V.pos_cur + j);
+template <int GM> __device__ __forceinline__ double2 gather_pos(const StepVar &V, int j) {
+    if (GM == GM_SMEM) return lds_d2(V.pos_s + (uint32_t)j * 16u);
+    return GM == GM_GLOBAL_CG ? __ldcg(V.pos_cur + j) : __ldg(V.pos_cur + j);
 }
 
 // One spring seen from one endpoint (Eq. 2): d = x_other - x_self, g = k (r - r0) / r.
@@ -299,7 +329,7 @@ __device__ __forceinline__ void slot_eval(double2 xq, double2 xp, bool lower, do
     near = EXACT ? (live && hi >= thr) : (hi >= thr);   // fast: thr is far above the high word of a zero r2
 }
 
-template <int PM, bool EXACT, bool SAMPLE, bool COHERENT, bool I16, int CH>
+template <int PM, bool EXACT, bool SAMPLE, int GM, bool I16, int CH>
 __device__ __forceinline__ bool row_chunk(const StepParams &P, const StepVar &V, const RowSrc &R, const double *s_tab, int p, unsigned s0,
                                           double2 xp, double &fx, double &fy, double &u) {
     int nb[CH];
@@ -311,7 +341,8 @@ __device__ __forceinline__ bool row_chunk(const StepParams &P, const StepVar &V,
     for (int c = 0; c < CH; ++c) nb[c] = I16 ? (int)R.nbr16[(s0 + c) * kSlice] : R.nbr[(s0 + c) * kSlice];   // I16: offset
 #pragma unroll
     for (int c = 0; c < CH; ++c) {   // I16: address = own address + offset (one wide multiply-add per gather)
-        xq[c] = I16 ? (COHERENT ? __ldcg(own + nb[c]) : __ldg(own + nb[c])) : gather_pos<COHERENT>(V, nb[c]);
+        if (I16 && GM == GM_SMEM) xq[c] = lds_d2(V.pos_s + (uint32_t)(p + nb[c]) * 16u);
+        else xq[c] = I16 ? (GM == GM_GLOBAL_CG ? __ldcg(own + nb[c]) : __ldg(own + nb[c])) : gather_pos<GM>(V, nb[c]);
         if (I16) nb[c] += p;
     }
 #pragma unroll
@@ -329,7 +360,7 @@ __device__ __forceinline__ bool row_chunk(const StepParams &P, const StepVar &V,
     return any_near;
 }
 
-template <int PM, bool EXACT, bool SAMPLE, bool COHERENT, bool I16>
+template <int PM, bool EXACT, bool SAMPLE, int GM, bool I16>
 __device__ __forceinline__ void row_careful(const StepParams &P, const StepVar &V, const RowSrc &R, const double *s_tab, int p, unsigned w,
                                          double2 xp, double &fx, double &fy, double &u) {
     fx = 0.0; fy = 0.0; u = 0.0;
@@ -337,7 +368,7 @@ __device__ __forceinline__ void row_careful(const StepParams &P, const StepVar &
     for (unsigned s = 0; s < w; ++s) {
         const unsigned so = s * kSlice;
         const int nb = I16 ? p + (int)R.nbr16[so] : R.nbr[so];
-        const double2 xq = gather_pos<COHERENT>(V, nb);
+        const double2 xq = gather_pos<GM>(V, nb);
         double k, r0, kr0, dx, dy, r2, g, ue;
         uint32_t thr;
         bool near;
@@ -367,15 +398,15 @@ __device__ __forceinline__ void row_careful(const StepParams &P, const StepVar &
     }
 }
 
-template <int PM, bool EXACT, bool SAMPLE, bool COHERENT, bool I16>
+template <int PM, bool EXACT, bool SAMPLE, int GM, bool I16>
 __device__ __forceinline__ void row_forces(const StepParams &P, const StepVar &V, const RowSrc &R, const double *s_tab, int p, unsigned w,
                                            double2 xp, double &fx, double &fy, double &u) {
     constexpr int CH = LSM_ROW_CH;
     unsigned s0 = 0;
     bool any_near = false;
-    for (; s0 + CH <= w; s0 += CH) any_near |= row_chunk<PM, EXACT, SAMPLE, COHERENT, I16, CH>(P, V, R, s_tab, p, s0, xp, fx, fy, u);
-    for (; s0 < w; ++s0) any_near |= row_chunk<PM, EXACT, SAMPLE, COHERENT, I16, 1>(P, V, R, s_tab, p, s0, xp, fx, fy, u);
-    if (any_near) row_careful<PM, EXACT, SAMPLE, COHERENT, I16>(P, V, R, s_tab, p, w, xp, fx, fy, u);
+    for (; s0 + CH <= w; s0 += CH) any_near |= row_chunk<PM, EXACT, SAMPLE, GM, I16, CH>(P, V, R, s_tab, p, s0, xp, fx, fy, u);
+    for (; s0 < w; ++s0) any_near |= row_chunk<PM, EXACT, SAMPLE, GM, I16, 1>(P, V, R, s_tab, p, s0, xp, fx, fy, u);
+    if (any_near) row_careful<PM, EXACT, SAMPLE, GM, I16>(P, V, R, s_tab, p, w, xp, fx, fy, u);
 }
 
 // Direct variant: block = tile, every stream read from global memory by the thread that needs it.
@@ -400,8 +431,8 @@ __global__ void __launch_bounds__(kBlock) k_gather_step(const StepParams P) {
     R.nbr = P.nbr + e0; R.nbr16 = nullptr; R.thr = P.sp.thr + e0; R.typ = P.sp.typ + e0; R.kF = P.sp.kF + e0; R.r0F = P.sp.r0F + e0;
     R.e0 = e0;
     double fx = 0.0, fy = 0.0, u = 0.0;
-    const StepVar V{P.pos_cur, P.pos_next, P.step};
-    row_forces<PM, EXACT, SAMPLE, false, false>(P, V, R, s_tab, (int)p, w, xp, fx, fy, u);
+    const StepVar V{P.pos_cur, P.pos_next, P.step, 0u};
+    row_forces<PM, EXACT, SAMPLE, GM_GLOBAL_NC, false>(P, V, R, s_tab, (int)p, w, xp, fx, fy, u);
     particle_update<EXACT, KICK2, ADVANCE, SAMPLE>(P, V, p, xp, vh, g, fx, fy, u);
 }
 
@@ -544,6 +575,7 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
         V.pos_cur = MULTI ? ((it & 1) ? M.pos_b : M.pos_a) : P.pos_cur;
         V.pos_next = MULTI ? ((it & 1) ? M.pos_a : M.pos_b) : P.pos_next;
         V.step = P.step + it;
+        V.pos_s = 0u;
         const bool kept = MULTI && M.resident && it > 0;   // tiles already in shared memory (stage i = i-th tile of this CTA)
         if (kept) { mbar_wait(go, (it - 1) & 1); s = 0; }
         for (long long t = blockIdx.x; t < P.T; t += gridDim.x) {
@@ -576,7 +608,7 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
                 } else {
                     const double2 xp = reinterpret_cast<const double2 *>(b + L.pos)[tid];
                     double fx = 0.0, fy = 0.0, uu = 0.0;
-                    row_forces<PM, EXACT, SAMPLE, MULTI, I16>(P, V, R, s_tab, (int)p, w, xp, fx, fy, uu);
+                    row_forces<PM, EXACT, SAMPLE, MULTI ? GM_GLOBAL_CG : GM_GLOBAL_NC, I16>(P, V, R, s_tab, (int)p, w, xp, fx, fy, uu);
                     const double2 vh = reinterpret_cast<const double2 *>(b + L.vel)[tid];
                     const uint8_t g = (b + L.grp)[tid];
                     if (MULTI && M.resident)
@@ -680,7 +712,7 @@ __global__ void __launch_bounds__(kBlock) k_integrate(const StepParams P) {
     const uint8_t g = P.grp[p];
     const double2 f = P.f[p];
     // in-place variant: pos_next == pos_cur for this path
-    particle_update<false, KICK2, ADVANCE, SAMPLE>(P, StepVar{P.pos_cur, P.pos_next, P.step}, p, xp, vh, g, f.x, f.y, 0.0);
+    particle_update<false, KICK2, ADVANCE, SAMPLE>(P, StepVar{P.pos_cur, P.pos_next, P.step, 0u}, p, xp, vh, g, f.x, f.y, 0.0);
     if (ADVANCE && !SAMPLE) P.f[p] = make_double2(0.0, 0.0);
 }
 

@@ -527,6 +527,90 @@ def test_step_fusion_fast_mode_config1():
     a.close(); b.close()
 
 
+# ---------------------------------------------------------------- cluster-resident stepping (NEXT-1)
+@pytest.mark.parametrize("cluster", [1, 2, 4, 8, 16])
+def test_resident_clusters_bit_identical_in_exact_mode(cluster):
+    """One thread-block cluster keeps the specimen in shared memory for whole runs of steps (ghosts through distributed
+    shared memory, cluster barrier per step): same row arithmetic in the same order, so exact mode must reproduce the
+    oracle bit for bit through a fracture run -- for every cluster size, with samples, compaction, odd / even run
+    lengths."""
+    p = _fracture_problem(n=48, du_y=6e-4, seed=11)
+    p.sample_every = 50
+    nsteps = 4000
+    o = OracleSim.from_problem(p); o.step(nsteps)
+    xo, vo = o.read_state(); bo, bso, nbo = o.read_broken()
+    assert nbo > 0
+    ho = o.read_stress()
+    g = lsm_create_from_problem(p, exact=True, step_fusion=lsm.FUSION_RESIDENT, cluster_size=cluster, compact_every=700)
+    inf = g.info()
+    assert inf["step_fusion"] == 2 and inf["cluster_size"] == cluster and 0 < inf["resident_smem_bytes"] <= 227 * 1024
+    g.step(1700); g.step(1); g.step(nsteps - 1701)
+    xg, vg = g.read_state(); bg, bsg, nbg = g.read_broken()
+    assert np.array_equal(xo, xg) and np.array_equal(vo, vg)
+    assert nbg == nbo and np.array_equal(bso, bsg)
+    hg = g.read_stress()
+    assert np.array_equal(ho["step"], hg["step"]) and np.array_equal(ho["n_broken"], hg["n_broken"])
+    assert np.allclose(hg["U"], ho["U"], rtol=1e-12) and np.allclose(hg["R"], ho["R"], rtol=1e-10, atol=1e-14)
+    assert g.info()["kernels_launched"] - inf["kernels_launched"] < 1200          # ~80 sample segments, not 4000 launches
+    g.close()
+
+
+def test_resident_ragged_batch_and_fast_mode():
+    """(a) a lattice whose particle count is not a multiple of 32 (ragged last slice), per-spring rc and typed k;
+    (b) a batch of 6 specimens (one cluster each) against the oracle stepping each alone, exact mode;
+    (c) fast arithmetic: resident == one launch per step bit for bit (same kernels' row code, same order)."""
+    x, si, sj, site, _ = triangular_lattice(37, 29)
+    row = site // 37
+    rng = np.random.default_rng(3)
+    x = x + rng.uniform(-0.02, 0.02, x.shape)
+    k = rng.choice([1.0, 2.0], si.size); rc = rng.uniform(1.03, 1.12, si.size)
+    bot = np.flatnonzero(row == 0).astype(np.int32); top = np.flatnonzero(row == 28).astype(np.int32)
+    o = OracleSim(x, si, sj, k, 1.0, rc, 0.03, gamma=0.02, sample_every=100)
+    o.set_boundary(0, bot, FIXED); o.set_boundary(1, top, MOVE, [1e-4, 5e-4])
+    o.step(1500)
+    xo, vo = o.read_state(); bso = o.read_broken()[1]
+    assert (bso >= 0).sum() > 0
+    for cl in (0, 2, 8):
+        g = lsm.lsm_create(x, si, sj, k, 1.0, rc, 0.03, gamma=0.02, sample_every=100, exact=True, step_fusion=lsm.FUSION_RESIDENT,
+                           cluster_size=cl)
+        g.set_boundary(0, bot, FIXED); g.set_boundary(1, top, MOVE, [1e-4, 5e-4])
+        assert g.info()["param_mode"] == 3 and g.info()["step_fusion"] == 2
+        g.step(1500)
+        xg, vg = g.read_state()
+        assert np.array_equal(xo, xg) and np.array_equal(vo, vg) and np.array_equal(bso, g.read_broken()[1])
+        g.close()
+    # (b)
+    B, n, nsteps = 6, 32, 3000
+    pb = config4(B=B, n=n); pb.sample_every = 100
+    g = lsm_create_from_problem(pb, exact=True, step_fusion=lsm.FUSION_RESIDENT)
+    assert g.info()["step_fusion"] == 2
+    g.step(nsteps)
+    xg, vg = g.read_state(); hg = g.read_stress(); bsg = g.read_broken()[1]
+    for b in range(B):
+        p1 = single_specimen(b, n); p1.sample_every = 100
+        o = OracleSim.from_problem(p1); o.step(nsteps)
+        xo, vo = o.read_state(); ho = o.read_stress()
+        sl = slice(pb.particle_offsets[b], pb.particle_offsets[b + 1]); ss = slice(pb.spring_offsets[b], pb.spring_offsets[b + 1])
+        assert np.array_equal(xg[sl], xo) and np.array_equal(vg[sl], vo) and np.array_equal(bsg[ss], o.read_broken()[1])
+        assert np.allclose(hg["U"][:, b], ho["U"][:, 0], rtol=1e-12) and np.array_equal(hg["n_broken"][:, b], ho["n_broken"][:, 0])
+    g.close()
+    # (c)
+    p = config1()
+    a = lsm_create_from_problem(p, step_fusion=lsm.FUSION_RESIDENT); a.step(3000)
+    b = lsm_create_from_problem(p, step_fusion=lsm.FUSION_OFF); b.step(3000)
+    c = lsm_create_from_problem(p); c.step(3000)
+    assert c.info()["step_fusion"] == 2                     # AUTO picks the resident kernel for a lattice that fits a cluster
+    xa, va = a.read_state(); xb, vb = b.read_state(); xc, vc = c.read_state()
+    assert np.array_equal(xa, xb) and np.array_equal(va, vb) and np.array_equal(xa, xc)
+    assert a.info()["kernels_launched"] < 300 < b.info()["kernels_launched"]
+    for s_ in (a, b, c):
+        s_.close()
+    # a lattice too large for one cluster is refused when RESIDENT is forced, and falls back under AUTO
+    with pytest.raises(lsm.LsmError) as ei:
+        lsm_create_from_problem(config2(n=640, n_blobs=40), step_fusion=lsm.FUSION_RESIDENT)
+    assert ei.value.status == -7
+
+
 # ---------------------------------------------------------------- full-size checks of the other configurations
 def test_full_size_config4_sampled_specimens():
     """BASELINE.json configs[3] at full size (1024 specimens, one launch): specimens sampled at random are compared
