@@ -12,21 +12,29 @@
 //     id range), double-buffered; its own half-step velocities and group bytes; its rows of the sliced-ELL lists.
 //   * A step reads buffer `cur` and writes buffer `cur ^ 1`.  A particle that is a ghost elsewhere is also written into
 //     the other CTA's window through distributed shared memory (st.shared::cluster on a mapa address).
-//   * Synchronisation per step: barrier.cluster.arrive (release) after the BOUNDARY slices (those exchanging ghosts) have
-//     been computed and pushed, then the interior slices, then __syncthreads; barrier.cluster.wait (acquire) only at the
-//     start of the next step, so the barrier's latency hides behind the interior work.  Interior slices read no ghost
-//     and are no ghost (the spring graph is symmetric), which is what makes the early arrive safe.
+//   * Synchronisation per step is by data flow, not by a barrier: a ghost is pushed with st.async ... mbarrier::complete_tx
+//     on the RECEIVING CTA's mbarrier, which that CTA armed with the byte count of all its ghosts; its boundary warps
+//     wait for the phase (~100 cycles when the data is there) before they read ghosts, interior warps never wait, and
+//     __syncthreads closes the step inside the CTA.  (A release / acquire barrier.cluster per step was measured at
+//     340-480 cycles on B200, a relaxed one at 75-140; the transaction barrier needs neither fence.)  Overwriting a
+//     ghost slot two steps later is safe because a CTA only receives the pushes of step n + 1 from a neighbour after
+//     that neighbour's boundary slices have read the ghosts of step n + 1 -- the spring graph is symmetric, so the
+//     slices that push to a CTA are exactly the slices that read its particles.
 //   * Row evaluation and the particle update are the functions of lsm_kernels.cuh (row_forces with GM_SMEM gathers,
 //     particle_math): the same arithmetic in the same order as the direct and streamed kernels, so exact mode stays
 //     bit-identical to the serial reference.  Breakage marks go to the global lists and to the resident copy.
 //   * Only plain time steps run here; sample steps, the last step of an lsm_step call and compaction are the streamed
 //     kernel's (one launch each), exactly as for the cooperative multi-step launch.
 #pragma once
+#include <type_traits>
+#include <utility>
 #include "lsm_kernels.cuh"
 
 namespace lsmk {
 
-constexpr int kResThreads = 512;       // 16 warps, one CTA per SM (the window fills most of its shared memory)
+constexpr int kResThreads = 512;       // 16 warps, one CTA per SM (the window fills most of its shared memory); measured on
+                                       // 128 specimens of 128^2: 512 threads 32.6 us per step, 768 34.3, 1024 33.6
+constexpr int kResCH = 6;              // springs of a row evaluated together
 constexpr int kResMaxPush = 6;         // other CTAs of the cluster a CTA has ghosts in (2 for a banded lattice numbering)
 constexpr int kResMaxCluster = 16;     // 8 portable, 16 with cudaFuncAttributeNonPortableClusterSizeAllowed
 
@@ -63,8 +71,9 @@ __device__ __forceinline__ uint32_t map_to_rank(uint32_t saddr, unsigned rank) {
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(saddr), "r"(rank));
     return r;
 }
-__device__ __forceinline__ void st_cluster_d2(uint32_t addr, double2 v) {
-    asm volatile("st.shared::cluster.v2.f64 [%0], {%1, %2};" ::"r"(addr), "d"(v.x), "d"(v.y) : "memory");
+// ghost push: the store and the completion of 16 transaction bytes on the receiver's mbarrier travel together
+__device__ __forceinline__ void st_async_d2(uint32_t addr, double2 v, uint32_t mbar) {
+    asm volatile("st.async.shared::cluster.mbarrier::complete_tx::bytes.v2.f64 [%0], {%1, %2}, [%3];" ::"r"(addr), "d"(v.x), "d"(v.y), "r"(mbar) : "memory");
 }
 __device__ __forceinline__ void sts_d2(uint32_t addr, double2 v) {
     asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(addr), "d"(v.x), "d"(v.y) : "memory");
@@ -88,6 +97,58 @@ __device__ __forceinline__ uint32_t lds_u8(uint32_t addr) {
     return v;
 }
 
+// ---- shared-memory row access with 32-bit addresses and immediate offsets (no generic-pointer arithmetic in the hot loop) ----
+template <int OFF> __device__ __forceinline__ int lds_s16o(uint32_t a) { int v; asm volatile("ld.shared.s16 %0, [%1+%2];" : "=r"(v) : "r"(a), "n"(OFF)); return v; }
+template <int OFF> __device__ __forceinline__ uint32_t lds_u16o(uint32_t a) { uint32_t v; asm volatile("ld.shared.u16 %0, [%1+%2];" : "=r"(v) : "r"(a), "n"(OFF)); return v; }
+template <int OFF> __device__ __forceinline__ uint32_t lds_u8o(uint32_t a) { uint32_t v; asm volatile("ld.shared.u8 %0, [%1+%2];" : "=r"(v) : "r"(a), "n"(OFF)); return v; }
+template <int OFF> __device__ __forceinline__ uint32_t lds_u32o(uint32_t a) { uint32_t v; asm volatile("ld.shared.u32 %0, [%1+%2];" : "=r"(v) : "r"(a), "n"(OFF)); return v; }
+template <int OFF> __device__ __forceinline__ double lds_f64o(uint32_t a) { double v; asm volatile("ld.shared.f64 %0, [%1+%2];" : "=d"(v) : "r"(a), "n"(OFF)); return v; }
+
+// compile-time loop 0 .. N-1 (the index is usable as a template argument: immediate offsets of the loads below)
+template <int N, int I = 0, class F> __device__ __forceinline__ void static_for(F &&f) {
+    if constexpr (I < N) { f(std::integral_constant<int, I>{}); static_for<N, I + 1>(f); }
+}
+
+struct RowS { uint32_t nbr, thr, typ, kF, r0F; };   // shared addresses of this lane's entry in the current slot of each row array
+
+// CH springs of one row from the resident copy: the arithmetic of row_chunk (slot_eval, same accumulation order), the
+// loads spelled as ld.shared [reg + immediate].  pos_p: shared address of the particle's own position in the current buffer.
+template <int PM, bool EXACT, int CH>
+__device__ __forceinline__ bool row_chunk_s(const StepParams &P, const RowS &A, uint32_t tab_s, uint32_t pos_p, double2 xp, double &fx, double &fy) {
+    constexpr bool kTab = (PM == PM_TYPED || PM == PM_KRT_RCF);
+    constexpr bool kHasThr = (PM == PM_RCF || PM == PM_KRT_RCF || PM == PM_FULL);
+    int nb[CH];
+    double2 xq[CH];
+    bool any_near = false;
+    static_for<CH>([&](auto ic) { constexpr int C = decltype(ic)::value; nb[C] = lds_s16o<C * kSlice * 2>(A.nbr); });
+#pragma unroll
+    for (int c = 0; c < CH; ++c) xq[c] = lds_d2(pos_p + (uint32_t)(nb[c] * 16));
+    static_for<CH>([&](auto ic) {
+        constexpr int C = decltype(ic)::value;
+        double k, r0 = 0.0, kr0, dx, dy, r2, g, ue;
+        uint32_t thr;
+        bool near;
+        if constexpr (kTab) {
+            const uint32_t ta = tab_s + lds_u8o<C * kSlice>(A.typ) * (uint32_t)(kTabStride * 8);
+            const double2 kk = lds_d2(ta);
+            k = kk.x; kr0 = kk.y;
+            if (EXACT) r0 = lds_f64o<24>(ta);
+            thr = PM == PM_TYPED ? lds_u32o<16>(ta) : P.sp.thr_base + lds_u16o<C * kSlice * 2>(A.thr) * P.sp.thr_mul;
+        } else if constexpr (PM == PM_FULL) {
+            k = lds_f64o<C * kSlice * 8>(A.kF); r0 = lds_f64o<C * kSlice * 8>(A.r0F); kr0 = k * r0;
+            thr = P.sp.thr_base + lds_u16o<C * kSlice * 2>(A.thr) * P.sp.thr_mul;
+        } else {
+            k = P.sp.k_u; r0 = P.sp.r0_u; kr0 = P.sp.kr0_u;
+            thr = kHasThr ? P.sp.thr_base + lds_u16o<C * kSlice * 2>(A.thr) * P.sp.thr_mul : P.sp.thr_u;
+        }
+        slot_eval<EXACT, false>(xq[C], xp, false, k, r0, kr0, thr, dx, dy, r2, g, ue, near);
+        fx = mad<EXACT>(g, dx, fx);
+        fy = mad<EXACT>(g, dy, fy);
+        any_near |= near;
+    });
+    return any_near;
+}
+
 template <int PM, bool EXACT>
 __global__ void __launch_bounds__(kResThreads, 1) k_resident(const StepParams P, const ResLayout L, const ResParams Q) {
     constexpr bool kTab = (PM == PM_TYPED || PM == PM_KRT_RCF);
@@ -95,9 +156,13 @@ __global__ void __launch_bounds__(kResThreads, 1) k_resident(const StepParams P,
     constexpr bool kHasKR = (PM == PM_FULL);
     extern __shared__ __align__(128) unsigned char smem[];
     __shared__ ResCta d;
+    __shared__ __align__(8) uint64_t ghost_bar[2];  // transaction barriers, alternating by step parity: a phase completes when all
+                                                    // ghosts of that step are in.  Two of them, so that the barrier a slow warp still has to
+                                                    // test cannot run a phase ahead (its next phase is armed only after the step's __syncthreads)
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     constexpr int nwarps = kResThreads / 32;
     if (tid < (int)(sizeof(ResCta) / 4)) reinterpret_cast<int32_t *>(&d)[tid] = reinterpret_cast<const int32_t *>(Q.desc + blockIdx.x)[tid];
+    if (tid == 0) { mbar_init(&ghost_bar[0], 1); mbar_init(&ghost_bar[1], 1); asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
     __syncthreads();
     // the hot loop keeps these in registers (d itself stays in shared memory for the push table)
     const int own_lo = d.own_lo, n_own = d.n_own, sl0 = d.sl0, n_sl = d.n_sl, wlo = d.wlo, wlen = d.wlen, n_boundary = d.n_boundary, n_push = d.n_push;
@@ -133,55 +198,82 @@ __global__ void __launch_bounds__(kResThreads, 1) k_resident(const StepParams P,
     cluster_wait();
 
     // ---------------- one slice of one step: lane = particle ----------------
-    auto do_slice = [&](int k, uint32_t pc, uint32_t pn, long long step, bool push) {
+    const uint32_t tab_s = smem_u32(s_tab), bar_s = smem_u32(&ghost_bar[0]);
+    const unsigned ghost_bytes = (unsigned)(wlen - n_own) * 16u;   // every window particle that is not mine is pushed to me each step
+    RowS lane_rows;    // shared addresses of this lane's entry in slot 0 of the CTA's row block
+    lane_rows.nbr = smem_u32(smem + L.nbr) + lane * 2; lane_rows.thr = smem_u32(smem + L.thr) + lane * 2; lane_rows.typ = smem_u32(smem + L.typ) + lane;
+    lane_rows.kF = smem_u32(smem + L.kF) + lane * 8; lane_rows.r0F = smem_u32(smem + L.r0F) + lane * 8;
+    auto do_slice = [&](int k, uint32_t pc, uint32_t pn, long long step, bool push, uint32_t push_bar) {
         const uint2 se = lds_u2(slice_s + (uint32_t)k * 8u);
         const int li = (int)(se.x & 0xFFFFu) * kSlice + lane;     // index among own particles
         if (li >= n_own) return;
         const int p = own_lo + li;
         const unsigned w = se.x >> 16;
-        const unsigned rel = se.y * kSlice + lane;
-        RowSrc R;
-        R.nbr = nullptr;
-        R.nbr16 = reinterpret_cast<const int16_t *>(smem + L.nbr) + rel;
-        R.thr = reinterpret_cast<const uint16_t *>(smem + L.thr) + rel;
-        R.typ = (smem + L.typ) + rel;
-        R.kF = reinterpret_cast<const double *>(smem + L.kF) + rel;
-        R.r0F = reinterpret_cast<const double *>(smem + L.r0F) + rel;
-        R.e0 = (size_t)(slot0 + se.y) * kSlice + lane;
-        StepVar V;
-        V.pos_cur = nullptr; V.pos_next = nullptr; V.step = step;
-        V.pos_s = pc - (uint32_t)wlo * 16u;
-        const double2 xp = lds_d2(V.pos_s + (uint32_t)p * 16u);
+        const uint32_t pos_p = pc + (uint32_t)(p - wlo) * 16u;
+        const double2 xp = lds_d2(pos_p);
         const double2 vh = lds_d2(vel_s + (uint32_t)li * 16u);
         const uint8_t g = (uint8_t)lds_u8(grp_s + (uint32_t)li);
-        double fx = 0.0, fy = 0.0, uu = 0.0;
-        row_forces<PM, EXACT, false, GM_SMEM, true>(P, V, R, s_tab, p, w, xp, fx, fy, uu);
+        RowS A;
+        A.nbr = lane_rows.nbr + se.y * (kSlice * 2); A.thr = lane_rows.thr + se.y * (kSlice * 2); A.typ = lane_rows.typ + se.y * kSlice;
+        A.kF = lane_rows.kF + se.y * (kSlice * 8); A.r0F = lane_rows.r0F + se.y * (kSlice * 8);
+        double fx = 0.0, fy = 0.0;
+        bool any_near = false;
+        constexpr int CH = kResCH;
+        unsigned s0 = 0;
+        for (; s0 + CH <= w; s0 += CH) {
+            any_near |= row_chunk_s<PM, EXACT, CH>(P, A, tab_s, pos_p, xp, fx, fy);
+            A.nbr += CH * kSlice * 2; A.thr += CH * kSlice * 2; A.typ += CH * kSlice; A.kF += CH * kSlice * 8; A.r0F += CH * kSlice * 8;
+        }
+        for (; s0 < w; ++s0) {
+            any_near |= row_chunk_s<PM, EXACT, 1>(P, A, tab_s, pos_p, xp, fx, fy);
+            A.nbr += kSlice * 2; A.thr += kSlice * 2; A.typ += kSlice; A.kF += kSlice * 8; A.r0F += kSlice * 8;
+        }
+        if (any_near) {   // rare: a spring came close to its breaking length -> redo the row deciding exactly (row_careful)
+            const unsigned rel = se.y * kSlice + lane;
+            RowSrc R;
+            R.nbr = nullptr;
+            R.nbr16 = reinterpret_cast<const int16_t *>(smem + L.nbr) + rel;
+            R.thr = reinterpret_cast<const uint16_t *>(smem + L.thr) + rel;
+            R.typ = (smem + L.typ) + rel;
+            R.kF = reinterpret_cast<const double *>(smem + L.kF) + rel;
+            R.r0F = reinterpret_cast<const double *>(smem + L.r0F) + rel;
+            R.e0 = (size_t)(slot0 + se.y) * kSlice + lane;
+            StepVar V;
+            V.pos_cur = nullptr; V.pos_next = nullptr; V.step = step;
+            V.pos_s = pc - (uint32_t)wlo * 16u;
+            double uu = 0.0;
+            row_careful<PM, EXACT, false, GM_SMEM, true>(P, V, R, s_tab, p, w, xp, fx, fy, uu);
+        }
         const Upd o = particle_math<EXACT, true, true, false>(P, step, p, xp, vh, g, fx, fy);
         sts_d2(pn + (uint32_t)(p - wlo) * 16u, o.xn);
         if (g == kFree) sts_d2(vel_s + (uint32_t)li * 16u, o.w);
         if (push) {
             for (int q = 0; q < n_push; ++q)
                 if (p >= d.push[q].lo && p < d.push[q].hi)
-                    st_cluster_d2(map_to_rank(pn + (uint32_t)(p - d.push[q].rwlo) * 16u, (unsigned)d.push[q].rank), o.xn);
+                    st_async_d2(map_to_rank(pn + (uint32_t)(p - d.push[q].rwlo) * 16u, (unsigned)d.push[q].rank), o.xn,
+                                map_to_rank(push_bar, (unsigned)d.push[q].rank));
         }
     };
 
     // ---------------- time steps ----------------
-    // Warp w takes entries w, w + 16, ... of the order list: its boundary slices first, then (after arriving on the
-    // cluster barrier) its interior ones -- every warp gets the same number of slices (+-1).
+    // Warp w takes entries w, w + 16, ... of the order list: its boundary slices first (they need this step's ghosts and
+    // push the next step's), then its interior ones -- every warp gets the same number of slices (+-1).
     bool cur = false;
     for (int it = 0; it < Q.nsteps; ++it) {
         const bool more = it + 1 < Q.nsteps;
         const uint32_t pc = cur ? posB : posA, pn = cur ? posA : posB;
-        if (it > 0) cluster_wait();                            // ghosts of this step have arrived; last step's readers are done
         int k = warp;
-        for (; k < n_boundary; k += nwarps) do_slice(k, pc, pn, P.step + it, more);
-        __syncwarp();
-        if (more) { if (warp < n_boundary) cluster_arrive(); else cluster_arrive_relaxed(); }   // release only what was pushed
-        for (; k < n_sl; k += nwarps) do_slice(k, pc, pn, P.step + it, false);
+        if (k < n_boundary) {
+            if (it > 0) mbar_wait(&ghost_bar[(it - 1) & 1], (unsigned)((it - 1) >> 1) & 1u);   // the ghosts pushed during step it - 1 are in
+            if (tid == 0 && more) mbar_expect_tx(&ghost_bar[it & 1], ghost_bytes);              // arm the phase that collects this step's pushes
+            for (; k < n_boundary; k += nwarps) do_slice(k, pc, pn, P.step + it, more, bar_s + (uint32_t)(it & 1) * 8u);
+        }
+        for (; k < n_sl; k += nwarps) do_slice(k, pc, pn, P.step + it, false, 0u);
         __syncthreads();                                       // own-region writes of this step before anyone's next step
         cur = !cur;
     }
+    cluster_arrive_relaxed();                                  // no CTA leaves while a neighbour may still be pushing into it
+    cluster_wait();
 
     // ---------------- store the own particles ----------------
     const double2 *res = reinterpret_cast<const double2 *>(smem + (cur ? L.pos1 : L.pos0)) + (own_lo - wlo);
