@@ -120,10 +120,13 @@ class ClockSampler:
                 "power_w_max": max(float(r[2]) for r in rows)}
 
 
-def time_oracle(p, n_steps, warm=1):
-    """Time the CPU oracle as it stands (serial, 1 thread) on `n_steps` time steps of problem p."""
+def time_oracle(p, n_steps, warm=1, threads=1):
+    """Time the CPU oracle as it stands on `n_steps` time steps of problem p: threads = 1 is the canonical serial loop,
+    threads > 1 its OpenMP variant (bit-equal to the serial loop: tests/test_oracle_pins.py)."""
     from oracle.olsm import OracleSim
     o = OracleSim.from_problem(p)
+    if threads > 1:
+        o.set_threads(threads)
     o.step(warm)
     t0 = time.perf_counter()
     o.step(n_steps)
@@ -131,6 +134,93 @@ def time_oracle(p, n_steps, warm=1):
     nb = o.read_broken()[2]
     o.close()
     return dt, nb
+
+
+def host_cores():
+    try:
+        return len(os.sched_getaffinity(0))
+    except Exception:
+        return os.cpu_count() or 1
+
+
+def oracle_legs(p, n_steps, what):
+    """The two reported CPU legs: 1 thread (the serial reference loop) and all host cores."""
+    nc = host_cores()
+    dt1, _ = time_oracle(p, n_steps)
+    out = {"value": p.M * n_steps / dt1, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": dt1,
+           "sample": "first %d time steps of %s (after 1 warm-up step), serial oracle" % (n_steps, what)}
+    if nc > 1:
+        dtn, _ = time_oracle(p, n_steps, threads=nc)
+        out["all_cores"] = {"value": p.M * n_steps / dtn, "unit": UNIT, "cores": nc, "kind": "oracle (OpenMP variant, bit-equal to the serial loop)",
+                            "seconds": dtn, "sample": "the same %d time steps on %d threads" % (n_steps, nc)}
+    return out
+
+
+def measure_device(p, inner, reps, warm, **create_kw):
+    """Device-resident throughput of one workload: `reps` lsm_step(inner) calls timed with CUDA events after `warm`
+    untimed calls.  Returns (seconds per time step, info, live springs at start, broken at end)."""
+    import torch
+    from paper_2201_04565_b200.binding import lsm_create_from_problem
+    sim = lsm_create_from_problem(p, **create_kw)
+    inf = sim.info()
+    alive0 = p.M - sim.n_broken()
+    for _ in range(warm):
+        sim.step(inner)
+    sim.read_stress()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    ev0.record()
+    for _ in range(reps):
+        sim.step(inner)
+    ev1.record()
+    torch.cuda.synchronize()
+    t = ev0.elapsed_time(ev1) * 1e-3 / (reps * inner)
+    nb = sim.n_broken()
+    sim.close()
+    return t, inf, alive0, nb
+
+
+def other_workloads_table(peak, budget_s, with_cpu):
+    """The other BASELINE.json configurations, measured in the same run with the library defaults:
+    us per time step, spring-updates/s, fraction of the HBM roofline by counted bytes (or "L2-resident"), and the two
+    oracle legs on the bounded windows SURVEY.md 8(d) names.  Stops adding rows when `budget_s` seconds are used up."""
+    import gc
+    import lsm_inputs as gen
+    import torch
+    t_begin = time.monotonic()
+    plan = [  # name, generator, time steps per call, timed calls, oracle steps, oracle problem (None = the same)
+        ("cfg1", lambda: gen.config1(), 2000, 5, 10000, None),
+        ("cfg2", lambda: gen.config2(), 1000, 5, 500, None),
+        ("cfg4", lambda: gen.config4(), 200, 3, 2000, lambda: gen.single_specimen(0)),
+        ("cfg5", lambda: gen.config5(), 50, 3, 3, None),
+    ]
+    rows = []
+    for name, make, inner, reps, n_cpu, make_cpu in plan:
+        if time.monotonic() - t_begin > budget_s:
+            rows.append({"workload": name, "skipped": "time budget of the default run used up"})
+            continue
+        if name == "cfg5" and torch.cuda.mem_get_info()[0] < 40e9:
+            rows.append({"workload": name, "skipped": "less than 40 GB of device memory free"})
+            continue
+        p = make()
+        p.sample_every = SAMPLE_EVERY
+        t, inf, alive0, nb = measure_device(p, inner, reps, 3, compact_every=1000, history_capacity=64)
+        pv = p_var_of(p)
+        bc = counted_bytes(p.N, alive0, pv, p.x.shape[1])
+        resident_l2 = 64.0 * p.N + inf["n_half_edges_stored"] * inf["bytes_per_half_edge"] < 100e6
+        row = {"workload": name, "N": p.N, "M": p.M, "n_batch": p.n_batch, "us_per_time_step": t * 1e6,
+               "spring_updates_per_s": alive0 * 1.0 / t, "broken_at_end": nb, "step_fusion": inf["step_fusion"],
+               "cluster_size": inf["cluster_size"], "param_mode": inf["param_mode"], "bytes_per_half_edge": inf["bytes_per_half_edge"],
+               "counted_bytes_per_time_step": bc, "p_var": pv,
+               "roofline": ("L2-resident / latency-bound: HBM roofline does not apply (t_roof by bytes %.2f us)" % (bc / peak / 1e3)) if resident_l2
+               else {"bound": "hbm", "achieved_GBs": bc / t / 1e9, "frac": min(1.0, bc / t / 1e9 / peak), "frac_uncapped": bc / t / 1e9 / peak}}
+        if with_cpu:
+            pc = make_cpu() if make_cpu else p
+            row["cpu_baseline"] = oracle_legs(pc, n_cpu, "one specimen of the batch" if make_cpu else name)
+        rows.append(row)
+        del p
+        gc.collect()
+    return rows
 
 
 def run_reference(args):
@@ -178,7 +268,12 @@ def main():
     ap.add_argument("--step-fusion", type=int, default=0, help="0 auto, 1 cooperative multi-step launches, 2 off, 3 cluster-resident")
     ap.add_argument("--cluster-size", type=int, default=0, help="cluster-resident stepping: CTAs per cluster (0 = library's choice)")
     ap.add_argument("--shuffle-ids", type=int, default=0, help="seed > 0: renumber particles / springs at random first (an arbitrary input-file order)")
+    ap.add_argument("--prebreak", type=float, default=0.0, help="fraction of springs dead from step 0 (rc < r0): the compaction window of SURVEY 8(d)")
+    ap.add_argument("--prebreak-mode", default="random", choices=["random", "band"], help="random springs, or every spring of a horizontal band")
+    ap.add_argument("--compact-now", type=int, default=0, help="1: run lsm_compact once before the timed region")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-table", action="store_true", help="skip the rows for the other BASELINE.json configurations (config.other_workloads)")
+    ap.add_argument("--table-budget", type=float, default=200.0, help="seconds after which no further row of that table is started")
     ap.add_argument("--cpu-steps", type=int, default=0, help="oracle time steps for cpu_baseline (0 = sized to ~15 s)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "b200":
@@ -213,11 +308,22 @@ def main():
         import lsm_inputs as gen
         p = gen.shuffle_ids(p, args.shuffle_ids)
         desc += " (ids shuffled, seed %d)" % args.shuffle_ids
+    if args.prebreak > 0:
+        if args.prebreak_mode == "random":
+            dead = np.random.default_rng(777).random(p.M) < args.prebreak
+        else:
+            ym = 0.5 * (p.x[p.spring_i, 1] + p.x[p.spring_j, 1])
+            H = p.x[:, 1].max()
+            dead = (ym > 0.3 * H) & (ym < (0.3 + args.prebreak) * H)
+        p.rc = np.where(dead, 0.5 * p.r0, p.rc)
+        desc += " (%.1f %% of the springs dead from step 0, %s)" % (100.0 * dead.mean(), args.prebreak_mode)
     p.sample_every = SAMPLE_EVERY
     fm = {"auto": lsm.FORCE_AUTO, "gather": lsm.FORCE_GATHER, "scatter": lsm.FORCE_SCATTER}[args.force_mode]
     sim = lsm_create_from_problem(p, device=local, force_mode=fm, reorder=args.reorder, compact_every=args.compact_every,
                                   exact=bool(args.exact), history_capacity=64, gather_variant=args.gather_variant, step_fusion=args.step_fusion,
                                   cluster_size=args.cluster_size)
+    if args.compact_now:
+        sim.compact()
     inf0 = sim.info()
     M_alive0 = p.M - sim.n_broken()
     S, K, W = args.inner, args.steps, args.warmup
@@ -287,6 +393,7 @@ def main():
         peak_src = "measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
         pv = p_var_of(p)
         bc = counted_bytes(p.N, M_alive0, pv, p.x.shape[1])
+        streamed = 64.0 * p.N + inf0["n_half_edges_stored"] * inf0["bytes_per_half_edge"] + 1.25 * p.N   # x, v in and out; slot streams; group bytes + tile headers
         t_launch = ms_max * 1e-3 / (K * S)     # upper bound of the step kernel's mean duration: every other launch in
         ach = bc / t_launch / 1e9              # the region (start/end, reductions, compaction) is charged to it
         value = units * S * K / (ms_max * 1e-3)
@@ -312,9 +419,14 @@ def main():
                          "peak_source": peak_src, "frac_of_nominal_8TBs": ach / 8000.0, "counted_bytes_per_time_step": bc,
                          "p_var": pv, "kernel": "fused step kernel (one launch per time step)",
                          "duration_us": t_launch * 1e6,
-                         "note": "achieved = counted (algorithmic) bytes / measured duration; the kernel streams fewer bytes than the "
-                                 "counted model (16-bit neighbour offsets and filter codes instead of int32 ids and fp64 rc), so "
-                                 "the uncapped ratio can pass 1; traffic = DRAM bytes per launch from the committed ncu capture"},
+                         # the second fraction: bytes the kernel streams BY DESIGN per launch (lsm_get_info) / time / peak
+                         "streamed_bytes_per_time_step": streamed, "achieved_streamed": streamed / t_launch / 1e9,
+                         "frac_streamed": streamed / t_launch / 1e9 / peak,
+                         "traffic_kind": "static: DRAM bytes per launch read from the committed ncu --set full capture (profiles/traffic_<workload>.txt), not measured by this run",
+                         "note": "frac = COUNTED (algorithmic) bytes / measured duration / peak, the headline of SURVEY 8(d); the kernel "
+                                 "streams fewer bytes than the counted model (16-bit neighbour offsets and filter codes instead of int32 "
+                                 "ids and fp64 rc), so the uncapped ratio can pass 1; frac_streamed = bytes the kernel moves by design / "
+                                 "duration / peak is the memory system's real utilisation"},
             "clocks": sampler.summary(tw0, tw1) if sampler else None,
         }
         tr = os.path.join(ROOT, "profiles", "traffic_%s.txt" % args.workload)
@@ -323,15 +435,16 @@ def main():
                 line["roofline"]["traffic"] = json.load(open(tr)).get("dram_bytes_per_launch")
             except Exception:
                 pass
+        sim.close()
+        sim = None
         if not args.no_cpu_baseline:
-            import lsm_inputs as gen
-            n_cpu = args.cpu_steps or max(2, int(15.0 * 1.1e8 / max(p.M, 1)))   # ~15 s of the serial oracle (1.1e8 spring-updates/s)
-            dt_o, _ = time_oracle(p, n_cpu)
-            line["cpu_baseline"] = {"value": p.M * n_cpu / dt_o, "unit": UNIT, "cores": 1, "kind": "oracle",
-                                    "sample": "first %d time steps of the same workload (after 1 warm-up step), serial oracle" % n_cpu,
-                                    "seconds": dt_o}
+            n_cpu = args.cpu_steps or max(2, int(8.0 * 1.1e8 / max(p.M, 1)))   # ~8 s of the serial oracle (1.1e8 spring-updates/s)
+            line["cpu_baseline"] = oracle_legs(p, n_cpu, "the same workload")
+        if world == 1 and args.workload == "cfg3" and not args.no_table:
+            line["config"]["other_workloads"] = other_workloads_table(peak, args.table_budget, not args.no_cpu_baseline)
         print(json.dumps(line))
-    sim.close()
+    if sim is not None:
+        sim.close()
     if dist is not None:
         dist.barrier()
         dist.destroy_process_group()

@@ -186,11 +186,15 @@ lsm_status lsm_read_stress(lsm_sim *sim, int64_t capacity, int64_t *n_samples, i
 lsm_status lsm_run_to_failure(lsm_sim *sim, int64_t max_steps, int32_t group, int32_t axis, double stop_fraction,
                               int64_t *steps_done, int32_t *failed, double *peak, int64_t *peak_step);
 
-/* Drop dead springs from the device lists now (also done every compact_every steps): stable, in-row, so every
- * particle keeps its summation order and no result changes (the paper keeps dead springs with k = 0, L196). */
+/* Drop dead springs from the device lists now (also done every compact_every steps; the paper keeps dead springs with
+ * k = 0, L196).  Two stages, both on the device and asynchronous: every row is compacted in place, stably (each particle
+ * keeps its summation order, so no result changes); then the slot storage is repacked (prefix sum of the slices' live
+ * widths, stable move) so that the streams the step kernel copies shrink.  A slice of 32 particles stores as many slots
+ * per particle as its longest row: bytes fall only where every row of a slice lost springs. */
 lsm_status lsm_compact(lsm_sim *sim);
 lsm_status lsm_sync(lsm_sim *sim);                                   /* cudaStreamSynchronize on the handle's stream */
-lsm_status lsm_get_info(lsm_sim *sim, lsm_info *info);               /* never fails on a valid handle, even after an error */
+lsm_status lsm_get_info(lsm_sim *sim, lsm_info *info);               /* never fails on a valid handle, even after an error;
+                                                                         synchronises the stream once after a compaction (slot count) */
 /* Device pointers of the current state in INTERNAL numbering, for zero-copy consumers (may change after lsm_step):
  * records of 2 doubles {x, y} per particle for dim = 2, of 4 doubles {x, y, z, 0} for dim = 3; owned by the handle. */
 lsm_status lsm_device_state(lsm_sim *sim, const double **pos_xy /* DEVICE */, const double **vel_xy /* DEVICE */);

@@ -68,6 +68,13 @@ struct lsm_sim {
     uint16_t *thr = nullptr;
     uint32_t thr_base = 0, thr_shift = 0;
     double *rcS = nullptr;
+    // repacking stage of the compaction (a7): scan scratch, one scratch array as large as the largest slot array
+    uint32_t *rp_new_off = nullptr, *rp_totals = nullptr;
+    unsigned long long *rp_state = nullptr;
+    unsigned int *rp_ticket = nullptr;
+    void *rp_scratch = nullptr;
+    long long E0 = 0;                // slots (x 32 entries) allocated at create
+    bool E_stale = false;            // the stored-slot count changed on the device since the host last read it
     int gather_variant = 0;          // resolved: 1 direct, 2 streamed
     StageLayout L;
     int stream_smem = 0, stream_grid = 0, stream_ctas_per_sm = 0;
@@ -625,13 +632,45 @@ lsm_status eval_initial(lsm_sim *s) {
     return LSM_OK;
 }
 
+template <class T> void repack_array(lsm_sim *s, const RepackParams &R, T *arr) {
+    if (!arr) return;
+    T *tmp = reinterpret_cast<T *>(s->rp_scratch);
+    k_repack_move<T><<<grid_for(R.nsl * kSlice), kBlock, 0, s->stream>>>(R, arr, tmp);
+    k_copy_back<T><<<2048, kBlock, 0, s->stream>>>(R, tmp, arr);
+    s->kernels_launched += 2;
+}
+
 lsm_status do_compact(lsm_sim *s) {
-    if (s->force_mode == LSM_FORCE_GATHER) {
+    if (s->force_mode == LSM_FORCE_GATHER && s->E0 > 0) {
         CompactParams C;
         C.hdr = s->hdr; C.nbr = s->nbr; C.nbr16 = s->nbr16; C.sid = s->sid; C.typ = s->typ; C.thr = s->thr;
         C.kF = s->kF; C.r0F = s->r0F; C.nslices = s->nslices;
         k_compact_ell<<<grid_for(s->nslices * kSlice), kBlock, 0, s->stream>>>(C);
         s->kernels_launched += 1;
+        CUDA_TRY(s, cudaGetLastError());
+        // repack: new slot offsets by a device-side scan of the live widths, stable move of every slot array
+        const long long nsl = s->T * kTileSlices;
+        const long long nblk = (nsl + kBlock - 1) / kBlock;
+        if (!s->rp_new_off) {
+            TRY(dev_alloc(s, &s->rp_new_off, (size_t)nsl + 1));
+            TRY(dev_alloc(s, &s->rp_state, (size_t)nblk));
+            TRY(dev_alloc(s, &s->rp_ticket, 1));
+            unsigned char *scr = nullptr;
+            TRY(dev_alloc(s, &scr, (size_t)s->E0 * kSlice * (s->kF ? 8 : 4)));
+            s->rp_scratch = scr;
+        }
+        RepackParams R;
+        R.hdr = s->hdr; R.nsl = nsl; R.new_off = s->rp_new_off; R.state = s->rp_state; R.ticket = s->rp_ticket; R.totals = s->rp_totals;
+        CUDA_TRY(s, cudaMemsetAsync(s->rp_state, 0, sizeof(unsigned long long) * nblk, s->stream));
+        CUDA_TRY(s, cudaMemsetAsync(s->rp_ticket, 0, sizeof(unsigned int), s->stream));
+        k_scan_widths<<<(unsigned)nblk, kBlock, 0, s->stream>>>(R);
+        s->kernels_launched += 1;
+        repack_array(s, R, s->nbr); repack_array(s, R, s->sid); repack_array(s, R, s->nbr16);
+        repack_array(s, R, s->typ); repack_array(s, R, s->thr); repack_array(s, R, s->kF); repack_array(s, R, s->r0F);
+        k_commit_offsets<<<grid_for(s->T), kBlock, 0, s->stream>>>(R);
+        k_commit_total<<<1, 1, 0, s->stream>>>(s->rp_totals);
+        s->kernels_launched += 2;
+        s->E_stale = true;
         CUDA_TRY(s, cudaGetLastError());
     }
     s->last_compact_step = s->step;
@@ -939,6 +978,12 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
         for (long long t = 0; t < T; ++t) s->max_tile_slots = std::max(s->max_tile_slots, hh[t].off[kTileSlices] - hh[t].off[0]);
         const size_t E = (size_t)off[T * kTileSlices] * kSlice;
         s->E = (long long)E;
+        s->E0 = (long long)off[T * kTileSlices];
+        {
+            std::vector<uint32_t> tot(2, off[T * kTileSlices]);
+            TRY(upload(s, &s->rp_totals, tot));
+            CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+        }
         std::vector<int32_t> hn(E), hs(E, -1);
         for (long long sl = 0; sl < T * kTileSlices; ++sl)       // padding slots point at their own particle
             for (size_t e = (size_t)off[sl] * kSlice; e < (size_t)off[sl + 1] * kSlice; ++e) hn[e] = (int32_t)(sl * kSlice + (e & 31));
@@ -1502,6 +1547,12 @@ lsm_status lsm_run_to_failure(lsm_sim *s, int64_t max_steps, int32_t group, int3
 lsm_status lsm_get_info(lsm_sim *s, lsm_info *info) {
     if (!s || !info) return LSM_E_INVALID;
     std::memset(info, 0, sizeof(*info));
+    if (s->E_stale && s->rp_totals && s->sticky == LSM_OK) {   // compaction repacked the lists on the device since the last query
+        DeviceScope scope(s->device);
+        uint32_t tot = 0;
+        if (cudaMemcpyAsync(&tot, s->rp_totals, sizeof(uint32_t), cudaMemcpyDeviceToHost, s->stream) == cudaSuccess &&
+            cudaStreamSynchronize(s->stream) == cudaSuccess) { s->E = (long long)tot * kSlice; s->E_stale = false; }
+    }
     info->n_particles = s->N; info->n_springs = s->M; info->n_half_edges_stored = s->E;
     static const int pbytes_scatter[5] = {0, 1, 8, 9, 24}, pbytes_gather[5] = {0, 1, 2, 3, 18};
     info->bytes_per_half_edge = s->force_mode == LSM_FORCE_GATHER ? (s->nbr16 && s->gather_variant == 2 ? 2 : 4) + pbytes_gather[s->pm] : 8 + pbytes_scatter[s->pm];

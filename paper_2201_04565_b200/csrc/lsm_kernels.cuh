@@ -810,9 +810,9 @@ __global__ void __launch_bounds__(kBlock) k_finalize_sample(const ReduceParams R
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-// Stream compaction of dead springs (a7).  Gather layout: every row is compacted in place, stably (the summation
-// order of the survivors is unchanged, so results are bit-identical), and the slice's live width shrinks to the
-// longest surviving row: dead columns are no longer read at all.
+// Stream compaction of dead springs (a7), first half.  Gather layout: every row is compacted in place, stably (the
+// summation order of the survivors is unchanged, so results are bit-identical), and the slice's live width shrinks to the
+// longest surviving row; the repacking stage below then removes the freed columns from the slot storage.
 // ---------------------------------------------------------------------------------------------------------------
 struct CompactParams {
     TileHdr *hdr;
@@ -856,6 +856,95 @@ __global__ void __launch_bounds__(kBlock) k_compact_ell(const CompactParams C) {
     for (int o = 16; o > 0; o >>= 1) wmax = max(wmax, __shfl_xor_sync(0xffffffffu, wmax, o));
     if (lane == 0) h->w[wi] = (uint8_t)wmax;
 }
+
+// Repacking (second half of a7): after the in-row pass the slices' live widths have shrunk; give every slice exactly its
+// live width in the slot storage, so that the streams the step kernels copy (and their byte counts: the producer sizes
+// each tile's bulk copies from off[8] - off[0]) shrink with it.  Three device-only stages, no host round trip:
+//   k_scan_widths   exclusive prefix sum of the live widths over all slices -> new slot offsets.  Single pass, decoupled
+//                   look-back: every block publishes its aggregate, then its inclusive prefix, in one 64-bit status word
+//                   (flag in the top two bits); blocks take their index from an atomic ticket so that every
+//                   predecessor a block may wait for is already running.
+//   k_repack_move   one warp per slice copies its live slots of one array to the new offsets in a scratch array (stable:
+//                   rows keep their order, so per-particle summation order and all results are unchanged);
+//   k_copy_back / k_commit_offsets   scratch -> array, then the tile headers take the new offsets.
+// All stages return at once when nothing shrank (new total == old total).
+struct RepackParams {
+    TileHdr *hdr;
+    long long nsl;                 // slices in the header table (tiles * 8)
+    uint32_t *new_off;             // [nsl + 1]
+    unsigned long long *state;     // [blocks] look-back status words, zeroed before the scan
+    unsigned int *ticket;          // zeroed before the scan
+    uint32_t *totals;              // [0] slots stored now, [1] slots after repacking
+};
+
+__global__ void __launch_bounds__(kBlock) k_scan_widths(const RepackParams R) {
+    __shared__ unsigned int bid_s;
+    __shared__ uint32_t wsum[kBlock / 32];
+    __shared__ uint32_t excl_s;
+    if (threadIdx.x == 0) bid_s = atomicAdd(R.ticket, 1u);
+    __syncthreads();
+    const unsigned bid = bid_s;
+    const long long sl = (long long)bid * kBlock + threadIdx.x;
+    const uint32_t w = sl < R.nsl ? R.hdr[sl >> 3].w[sl & 7] : 0u;
+    const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
+    uint32_t x = w;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+    if (lane == 31) wsum[wi] = x;
+    __syncthreads();
+    uint32_t before = 0, agg = 0;
+#pragma unroll
+    for (int q = 0; q < kBlock / 32; ++q) { if (q < wi) before += wsum[q]; agg += wsum[q]; }
+    const uint32_t incl = before + x;
+    if (threadIdx.x == 0) {
+        volatile unsigned long long *st = R.state;
+        uint32_t run = 0;
+        if (bid > 0) {
+            st[bid] = (1ull << 62) | agg;                         // aggregate available
+            for (long long j = (long long)bid - 1;; --j) {        // look back until a block with its inclusive prefix
+                unsigned long long v;
+                do { v = st[j]; } while ((v >> 62) == 0ull);
+                run += (uint32_t)v;
+                if ((v >> 62) == 2ull) break;
+            }
+        }
+        st[bid] = (2ull << 62) | (unsigned long long)(run + agg); // inclusive prefix available
+        excl_s = run;
+    }
+    __syncthreads();
+    if (sl < R.nsl) R.new_off[sl] = excl_s + incl - w;
+    if (sl == R.nsl - 1) { R.new_off[R.nsl] = excl_s + incl; R.totals[1] = excl_s + incl; }
+}
+
+template <class T>
+__global__ void __launch_bounds__(kBlock) k_repack_move(const RepackParams R, const T *src, T *dst) {
+    if (R.totals[1] == R.totals[0]) return;
+    const long long sl = ((long long)blockIdx.x * kBlock + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (sl >= R.nsl) return;
+    const TileHdr *h = R.hdr + (sl >> 3);
+    const unsigned w = h->w[sl & 7];
+    const size_t from = (size_t)h->off[sl & 7] * kSlice + lane, to = (size_t)R.new_off[sl] * kSlice + lane;
+    for (unsigned q = 0; q < w; ++q) dst[to + (size_t)q * kSlice] = src[from + (size_t)q * kSlice];
+}
+
+template <class T>
+__global__ void __launch_bounds__(kBlock) k_copy_back(const RepackParams R, const T *src, T *dst) {
+    if (R.totals[1] == R.totals[0]) return;
+    const size_t n = (size_t)R.totals[1] * kSlice;
+    for (size_t i = (size_t)blockIdx.x * kBlock + threadIdx.x; i < n; i += (size_t)gridDim.x * kBlock) dst[i] = src[i];
+}
+
+__global__ void __launch_bounds__(kBlock) k_commit_offsets(const RepackParams R) {
+    if (R.totals[1] == R.totals[0]) return;
+    const long long t = (long long)blockIdx.x * kBlock + threadIdx.x;      // tile
+    if (t * kTileSlices >= R.nsl) return;
+    TileHdr *h = R.hdr + t;
+#pragma unroll
+    for (int q = 0; q <= kTileSlices; ++q) h->off[q] = R.new_off[t * kTileSlices + q];
+}
+
+__global__ void k_commit_total(uint32_t *totals) { totals[0] = totals[1]; }
 
 // ---------------------------------------------------------------------------------------------------------------
 // Per-particle virial stress, Eq. 7 without 1/Omega:  S^k = 1/2 sum_l (x^l - x^k) (x) f^kl - m v (x) v,

@@ -527,6 +527,46 @@ def test_step_fusion_fast_mode_config1():
     a.close(); b.close()
 
 
+# ---------------------------------------------------------------- a7: compaction repacks the slot storage
+@pytest.mark.parametrize("kw", [dict(step_fusion=lsm.FUSION_OFF), dict(step_fusion=lsm.FUSION_ON), dict(step_fusion=lsm.FUSION_RESIDENT),
+                                dict(gather_variant=lsm.GATHER_DIRECT), dict(reorder=1, step_fusion=lsm.FUSION_OFF)],
+                         ids=["streamed", "coop", "resident", "direct", "morton"])
+def test_compaction_repacks_slot_storage_and_changes_no_result(kw):
+    """a7: a band of the specimen has all its springs dead from step 0 (rc < r0) and a seeded 20 % of the others too; the
+    rest is pulled to fracture.  Compaction (every 250 steps and once by hand) must shrink the stored slot count -- the
+    band's slices lose all their columns -- and change nothing: x, v, broken set, break steps bit-identical to the oracle
+    in exact mode, with every kernel family reading the repacked lists."""
+    p = _fracture_problem(n=64, du_y=2e-3, seed=5)
+    y = p.x[:, 1]
+    H = y.max()
+    ym = 0.5 * (y[p.spring_i] + y[p.spring_j])
+    rng = np.random.default_rng(9)
+    xm = 0.5 * (p.x[p.spring_i, 0] + p.x[p.spring_j, 0])
+    dead = ((ym > 0.30 * H) & (ym < 0.42 * H) & (xm > 30.0)) | (rng.random(p.M) < 0.2)     # the band: the right half (whole slices)
+    p.rc = np.where(dead, 0.5 * p.r0, p.rc)
+    p.sample_every = 100
+    o = OracleSim.from_problem(p)
+    assert o.read_broken()[2] == dead.sum()
+    g = lsm_create_from_problem(p, exact=True, compact_every=250, **kw)
+    e0 = g.info()["n_half_edges_stored"]
+    g.compact()
+    e1 = g.info()["n_half_edges_stored"]
+    # whole slices of the band emptied (row-major numbering: a slice is a row segment); random deaths alone free few columns
+    assert e1 <= e0 and (kw.get("reorder") or e1 < 0.98 * e0), (e0, e1)
+    assert np.array_equal(o.read_forces(), g.read_forces())
+    o.step(3000); g.step(1300); g.step(1); g.step(1699)
+    xo, vo = o.read_state(); xg, vg = g.read_state()
+    bo, bso, nbo = o.read_broken(); bg, bsg, nbg = g.read_broken()
+    assert nbo > dead.sum() + 5
+    assert np.array_equal(xo, xg) and np.array_equal(vo, vg) and np.array_equal(bso, bsg)
+    assert g.info()["n_half_edges_stored"] <= e1
+    ho, hg = o.read_stress(), g.read_stress()
+    assert np.array_equal(ho["n_broken"], hg["n_broken"]) and np.allclose(hg["U"], ho["U"], rtol=1e-12)
+    So, Sg = o.read_virial(), g.read_virial()
+    assert np.abs(Sg - So).max() <= 1e-11 * np.abs(So).max()
+    g.close()
+
+
 # ---------------------------------------------------------------- cluster-resident stepping (NEXT-1)
 @pytest.mark.parametrize("cluster", [1, 2, 4, 8, 16])
 def test_resident_clusters_bit_identical_in_exact_mode(cluster):
