@@ -260,7 +260,7 @@ def main():
     ap.add_argument("--ref-inner", type=int, default=2, help="time steps per bench step of --impl reference")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--workload", default="cfg3")
-    ap.add_argument("--force-mode", default="auto", choices=["auto", "gather", "scatter"])
+    ap.add_argument("--force-mode", default="auto", choices=["auto", "gather", "scatter", "scatter-warp", "scatter-tile"])
     ap.add_argument("--reorder", type=int, default=0)
     ap.add_argument("--compact-every", type=int, default=1000)
     ap.add_argument("--exact", type=int, default=0)
@@ -318,7 +318,8 @@ def main():
         p.rc = np.where(dead, 0.5 * p.r0, p.rc)
         desc += " (%.1f %% of the springs dead from step 0, %s)" % (100.0 * dead.mean(), args.prebreak_mode)
     p.sample_every = SAMPLE_EVERY
-    fm = {"auto": lsm.FORCE_AUTO, "gather": lsm.FORCE_GATHER, "scatter": lsm.FORCE_SCATTER}[args.force_mode]
+    fm = {"auto": lsm.FORCE_AUTO, "gather": lsm.FORCE_GATHER, "scatter": lsm.FORCE_SCATTER, "scatter-warp": lsm.FORCE_SCATTER_WARP,
+          "scatter-tile": lsm.FORCE_SCATTER_TILE}[args.force_mode]
     sim = lsm_create_from_problem(p, device=local, force_mode=fm, reorder=args.reorder, compact_every=args.compact_every,
                                   exact=bool(args.exact), history_capacity=64, gather_variant=args.gather_variant, step_fusion=args.step_fusion,
                                   cluster_size=args.cluster_size)

@@ -54,7 +54,13 @@ typedef enum {
 } lsm_status;
 
 enum { LSM_FIXED = 0, LSM_MOVE = 1 };                      /* boundary group modes */
-enum { LSM_FORCE_AUTO = 0, LSM_FORCE_SCATTER = 1, LSM_FORCE_GATHER = 2 };
+/* force accumulation.  GATHER (= AUTO): particle-centric, no atomics, deterministic -- the product path.  The three
+ * SCATTER modes are spring-centric as in the paper and are kept as measured comparisons:
+ * SCATTER = one fp64 RED per force component and endpoint (the paper's atomicAdd design); SCATTER_WARP = springs sorted
+ * by lower endpoint, segmented shuffle reduction, one RED pair per particle per warp; SCATTER_TILE = a CTA owns 1024
+ * particles, every spring is evaluated once into its own shared-memory slot, particles sum their slots, one RED pair
+ * per particle plus the spills across tile borders.  Fast arithmetic only (exact = 1 needs GATHER), dim = 2 only. */
+enum { LSM_FORCE_AUTO = 0, LSM_FORCE_SCATTER = 1, LSM_FORCE_GATHER = 2, LSM_FORCE_SCATTER_WARP = 3, LSM_FORCE_SCATTER_TILE = 4 };
 enum { LSM_REORDER_NONE = 0, LSM_REORDER_MORTON = 1, LSM_REORDER_RCM = 2,
        LSM_REORDER_BLOCKED = 3 /* 2-D only: bins of ~32 x 8 particles in row-major order, row-major inside a bin, so that a
                                   tile of 256 consecutive ids is a compact patch and neighbour offsets stay small */ };

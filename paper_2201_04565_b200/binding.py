@@ -14,7 +14,7 @@ import numpy as np
 from . import build as _build
 
 FIXED, MOVE = 0, 1
-FORCE_AUTO, FORCE_SCATTER, FORCE_GATHER = 0, 1, 2
+FORCE_AUTO, FORCE_SCATTER, FORCE_GATHER, FORCE_SCATTER_WARP, FORCE_SCATTER_TILE = 0, 1, 2, 3, 4
 REORDER_NONE, REORDER_MORTON, REORDER_RCM, REORDER_BLOCKED = 0, 1, 2, 3
 GATHER_AUTO, GATHER_DIRECT, GATHER_STREAMED = 0, 1, 2
 FUSION_AUTO, FUSION_ON, FUSION_OFF, FUSION_RESIDENT = 0, 1, 2, 3

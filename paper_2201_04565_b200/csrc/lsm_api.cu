@@ -91,6 +91,9 @@ struct lsm_sim {
     // scatter layout
     long long Ms = 0;
     int32_t *ssi = nullptr, *ssj = nullptr, *ssid = nullptr;
+    int scatter_variant = 0;         // 0 one RED per force component (the paper's design), 1 warp-aggregated, 2 shared-memory tiles
+    int32_t *s_own_off = nullptr, *s_jl_off = nullptr, *s_jl_idx = nullptr, *s_tile_off = nullptr;
+    int scatter_tiles = 0, scatter_tile_smem = 0;
     double *sUs = nullptr;
     long long *d_soff_list = nullptr;
     // parameters
@@ -247,6 +250,7 @@ ScatterParams scatter_params(const lsm_sim *s) {
     ScatterParams S;
     std::memset(&S, 0, sizeof(S));
     S.si = s->ssi; S.sj = s->ssj; S.sid = s->ssid; S.M = s->Ms; S.sUs = s->sUs;
+    S.own_off = s->s_own_off; S.jl_off = s->s_jl_off; S.jl_idx = s->s_jl_idx; S.tile_off = s->s_tile_off; S.N = s->N;
     S.sp.typ = s->typ; S.sp.kF = s->kF; S.sp.r0F = s->r0F; S.sp.rcF = s->rcF; S.sp.tab = s->tab; S.sp.ntypes = s->ntypes;
     S.sp.k_u = s->k_u; S.sp.r0_u = s->r0_u; S.sp.rc_u = s->rc_u;
     return S;
@@ -541,21 +545,29 @@ void launch_gather(lsm_sim *s, const StepParams &P, Variant v) {
     s->kernels_launched += 1;
 }
 
-template <int PM> void launch_scatter_pm(const StepParams &P, const ScatterParams &S, bool sample, cudaStream_t st) {
-    const unsigned grid = grid_for(S.M);
+template <int PM, bool SAMPLE> void launch_scatter_one(const lsm_sim *s, const StepParams &P, const ScatterParams &S) {
     if (S.M == 0) return;
-    if (sample) k_spring_scatter<PM, true><<<grid, kBlock, 0, st>>>(P, S);
-    else k_spring_scatter<PM, false><<<grid, kBlock, 0, st>>>(P, S);
+    if (s->scatter_variant == 1) k_spring_scatter_warp<PM, SAMPLE><<<grid_for(S.M), kBlock, 0, s->stream>>>(P, S);
+    else if (s->scatter_variant == 2) {
+        auto kern = k_spring_scatter_tile<PM, SAMPLE>;
+        if (s->scatter_tile_smem > 32 * 1024) cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, s->scatter_tile_smem);   // static + dynamic may pass 48 KB
+        kern<<<(unsigned)s->scatter_tiles, kScatterTileThreads, (size_t)s->scatter_tile_smem, s->stream>>>(P, S);
+    }
+    else k_spring_scatter<PM, SAMPLE><<<grid_for(S.M), kBlock, 0, s->stream>>>(P, S);
+}
+
+template <int PM> void launch_scatter_pm(const lsm_sim *s, const StepParams &P, const ScatterParams &S, bool sample) {
+    if (sample) launch_scatter_one<PM, true>(s, P, S); else launch_scatter_one<PM, false>(s, P, S);
 }
 
 void launch_scatter_force(lsm_sim *s, const StepParams &P, bool sample) {
     const ScatterParams S = scatter_params(s);
     switch (s->pm) {
-        case PM_UNIFORM: launch_scatter_pm<PM_UNIFORM>(P, S, sample, s->stream); break;
-        case PM_TYPED: launch_scatter_pm<PM_TYPED>(P, S, sample, s->stream); break;
-        case PM_RCF: launch_scatter_pm<PM_RCF>(P, S, sample, s->stream); break;
-        case PM_KRT_RCF: launch_scatter_pm<PM_KRT_RCF>(P, S, sample, s->stream); break;
-        default: launch_scatter_pm<PM_FULL>(P, S, sample, s->stream); break;
+        case PM_UNIFORM: launch_scatter_pm<PM_UNIFORM>(s, P, S, sample); break;
+        case PM_TYPED: launch_scatter_pm<PM_TYPED>(s, P, S, sample); break;
+        case PM_RCF: launch_scatter_pm<PM_RCF>(s, P, S, sample); break;
+        case PM_KRT_RCF: launch_scatter_pm<PM_KRT_RCF>(s, P, S, sample); break;
+        default: launch_scatter_pm<PM_FULL>(s, P, S, sample); break;
     }
     s->kernels_launched += 1;
 }
@@ -706,6 +718,8 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
     s->sample_every = d->sample_every; s->hist_cap = d->history_capacity > 0 ? d->history_capacity : 1024;
     s->compact_every = d->compact_every; s->reorder = d->reorder;
     s->force_mode = d->force_mode == LSM_FORCE_AUTO ? LSM_FORCE_GATHER : d->force_mode;
+    if (d->force_mode == LSM_FORCE_SCATTER_WARP) { s->force_mode = LSM_FORCE_SCATTER; s->scatter_variant = 1; }
+    if (d->force_mode == LSM_FORCE_SCATTER_TILE) { s->force_mode = LSM_FORCE_SCATTER; s->scatter_variant = 2; }
     s->exact = d->exact; s->step_fusion = d->step_fusion; s->cluster_size = d->cluster_size; s->gather_variant = d->gather_variant; s->device = d->device; s->stream = (cudaStream_t)d->stream;
     s->alloc = d->alloc; s->free_ = d->free_; s->alloc_user = d->alloc_user;
 
@@ -1126,6 +1140,26 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
         std::sort(order.begin(), order.end(), [&](int32_t x, int32_t y) { return a[x] != a[y] ? a[x] < a[y] : (b2[x] != b2[y] ? b2[x] < b2[y] : x < y); });
         std::vector<int32_t> hi(M), hj(M), hs(M);
         for (long long q = 0; q < M; ++q) { const int32_t e = order[q]; hi[q] = to_int(d->spring_i[e]); hj[q] = to_int(d->spring_j[e]); hs[q] = e; }
+        if (s->scatter_variant != 0) {   // aggregated variants: (lower endpoint, upper endpoint); f_lo += g d, f_hi -= g d with d = x_hi - x_lo
+            for (long long q = 0; q < M; ++q) if (hi[q] > hj[q]) std::swap(hi[q], hj[q]);
+            std::vector<int32_t> own(N + 1, 0), jlo(N + 1, 0), jli;
+            for (long long q = 0; q < M; ++q) own[hi[q] + 1]++;
+            for (long long p = 0; p < N; ++p) own[p + 1] += own[p];
+            const long long ntile = (N + kScatterTile - 1) / kScatterTile;
+            std::vector<int32_t> toff(ntile + 1, 0);
+            for (long long t = 0; t <= ntile; ++t) toff[t] = own[std::min<long long>(N, t * kScatterTile)];
+            long long cap = 0;
+            for (long long t = 0; t < ntile; ++t) cap = std::max<long long>(cap, toff[t + 1] - toff[t]);
+            // springs a particle is the UPPER endpoint of, lower endpoint in the same tile (the others spill with a RED)
+            for (long long q = 0; q < M; ++q) if (hi[q] / kScatterTile == hj[q] / kScatterTile) jlo[hj[q] + 1]++;
+            for (long long p = 0; p < N; ++p) jlo[p + 1] += jlo[p];
+            jli.resize(std::max<long long>(jlo[N], 1));
+            { std::vector<int32_t> fill(jlo.begin(), jlo.end() - 1); for (long long q = 0; q < M; ++q) if (hi[q] / kScatterTile == hj[q] / kScatterTile) jli[fill[hj[q]]++] = (int32_t)q; }
+            s->scatter_tiles = (int)ntile; s->scatter_tile_smem = (int)(cap * 16);
+            if (s->scatter_variant == 2 && s->scatter_tile_smem > 200 * 1024) return fail(s, LSM_E_UNSUPPORTED, "force_mode = SCATTER_TILE: a tile's springs do not fit in shared memory (degree too high)");
+            TRY(upload(s, &s->s_own_off, own)); TRY(upload(s, &s->s_jl_off, jlo)); TRY(upload(s, &s->s_jl_idx, jli)); TRY(upload(s, &s->s_tile_off, toff));
+            CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+        }
         s->Ms = M; s->E = M;
         TRY(upload(s, &s->ssi, hi)); TRY(upload(s, &s->ssj, hj)); TRY(upload(s, &s->ssid, hs));
         if (need_typ) { std::vector<uint8_t> ht(M); for (long long q = 0; q < M; ++q) ht[q] = stype[hs[q]]; TRY(upload(s, &s->typ, ht)); CUDA_TRY(s, cudaStreamSynchronize(s->stream)); }
@@ -1193,14 +1227,14 @@ lsm_status lsm_create(const lsm_desc *d, lsm_sim **out) {
     if (!d || !out) return fail(nullptr, LSM_E_INVALID, "desc / out is NULL");
     if (d->struct_size != sizeof(lsm_desc)) return fail(nullptr, LSM_E_INVALID, "lsm_desc.struct_size does not match this library (ABI mismatch)");
     if (d->dim != 2 && d->dim != 3) return fail(nullptr, LSM_E_INVALID, "dim must be 2 or 3");
-    if (d->dim == 3 && d->force_mode == LSM_FORCE_SCATTER) return fail(nullptr, LSM_E_UNSUPPORTED, "dim = 3 has no scatter path");
+    if (d->dim == 3 && (d->force_mode == LSM_FORCE_SCATTER || d->force_mode == LSM_FORCE_SCATTER_WARP || d->force_mode == LSM_FORCE_SCATTER_TILE)) return fail(nullptr, LSM_E_UNSUPPORTED, "dim = 3 has no scatter path");
     if (d->n_particles < 1 || d->n_springs < 0 || d->n_particles >= 2147483647LL || d->n_springs >= 2147483647LL) return fail(nullptr, LSM_E_INVALID, "need 1 <= N < 2^31-1 and 0 <= M < 2^31-1");
     if (d->n_batch < 1 || !d->x) return fail(nullptr, LSM_E_INVALID, "n_batch < 1 or x is NULL");
     if (!(d->dt > 0.0) || !(d->gamma >= 0.0) || !std::isfinite(d->dt) || !std::isfinite(d->gamma)) return fail(nullptr, LSM_E_INVALID, "need dt > 0 and gamma >= 0");
     if (d->sample_every < 0 || d->compact_every < 0 || d->history_capacity < 0) return fail(nullptr, LSM_E_INVALID, "negative sample_every / compact_every / history_capacity");
     if (d->reorder < LSM_REORDER_NONE || d->reorder > LSM_REORDER_BLOCKED) return fail(nullptr, LSM_E_INVALID, "bad reorder");
     if (d->reorder == LSM_REORDER_BLOCKED && d->dim != 2) return fail(nullptr, LSM_E_UNSUPPORTED, "reorder = BLOCKED is 2-D only");
-    if (d->force_mode < 0 || d->force_mode > 2) return fail(nullptr, LSM_E_INVALID, "bad force_mode");
+    if (d->force_mode < 0 || d->force_mode > LSM_FORCE_SCATTER_TILE) return fail(nullptr, LSM_E_INVALID, "bad force_mode");
     if (d->gather_variant < 0 || d->gather_variant > 2) return fail(nullptr, LSM_E_INVALID, "bad gather_variant");
     if (d->step_fusion < 0 || d->step_fusion > 3) return fail(nullptr, LSM_E_INVALID, "bad step_fusion");
     if (d->cluster_size != 0 && d->cluster_size != 1 && d->cluster_size != 2 && d->cluster_size != 4 && d->cluster_size != 8 && d->cluster_size != 16) return fail(nullptr, LSM_E_INVALID, "cluster_size must be 0 (auto), 1, 2, 4, 8 or 16");
@@ -1562,7 +1596,7 @@ lsm_status lsm_get_info(lsm_sim *s, lsm_info *info) {
     info->cluster_size = s->res_on ? s->res_cluster : 0;
     info->resident_smem_bytes = s->res_on ? s->RL.bytes : 0;
     info->stage_bytes = s->gather_variant == 2 ? s->L.bytes : 0;
-    info->param_mode = s->pm; info->n_types = s->ntypes; info->force_mode = s->force_mode; info->exact = s->exact;
+    info->param_mode = s->pm; info->n_types = s->ntypes; info->force_mode = s->force_mode == LSM_FORCE_SCATTER ? (s->scatter_variant == 1 ? LSM_FORCE_SCATTER_WARP : s->scatter_variant == 2 ? LSM_FORCE_SCATTER_TILE : LSM_FORCE_SCATTER) : s->force_mode; info->exact = s->exact;
     info->reorder = s->reorder; info->n_batch = s->B; info->device_bytes = s->device_bytes;
     info->kernels_launched = s->kernels_launched; info->current_step = s->step;
     return LSM_OK;

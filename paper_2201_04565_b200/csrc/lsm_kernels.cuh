@@ -668,7 +668,15 @@ struct ScatterParams {
     SpringParams sp;
     long long M;
     double *sUs;  // per-spring energy scratch (SAMPLE)
+    // aggregated variants (springs stored as (lower endpoint, upper endpoint), sorted by the lower one)
+    const int32_t *own_off;    // [N+1] springs whose lower endpoint is p: [own_off[p], own_off[p+1])
+    const int32_t *jl_off;     // [N+1] springs whose upper endpoint is p and whose lower endpoint lies in p's tile ...
+    const int32_t *jl_idx;     // ... as indices into the spring list
+    const int32_t *tile_off;   // [tiles+1] spring range of each tile of kScatterTile particles
+    long long N;
 };
+constexpr int kScatterTile = 1024;     // particles per CTA of the shared-memory tile variant
+constexpr int kScatterTileThreads = 512;
 
 template <int PM, bool SAMPLE>
 __global__ void __launch_bounds__(kBlock) k_spring_scatter(const StepParams P, const ScatterParams S) {
@@ -699,6 +707,120 @@ __global__ void __launch_bounds__(kBlock) k_spring_scatter(const StepParams P, c
         P.break_step[S.sid[e]] = P.step;
         atomicAdd(P.nbroken + spec_of(P.poff, P.B, i), 1ULL);
         if (SAMPLE) S.sUs[e] = 0.0;
+    }
+}
+
+// Scatter variant 2 (north_star: "warp-aggregated atomics"): springs are stored as (lower endpoint, upper endpoint) and
+// sorted by the lower one, so the ~3 springs of a particle sit in consecutive lanes.  Lower side: segmented shuffle
+// reduction over the run of equal ids, one RED pair per particle per warp.  Upper side: one RED pair per spring.  Same
+// arithmetic per spring as k_spring_scatter; the order of the REDs across warps is not fixed.
+template <int PM, bool SAMPLE>
+__global__ void __launch_bounds__(kBlock) k_spring_scatter_warp(const StepParams P, const ScatterParams S) {
+    constexpr bool kTab = (PM == PM_TYPED || PM == PM_KRT_RCF);
+    __shared__ double s_tab[kTab ? 3 * kMaxTypes : 1];
+    if (kTab) {
+        for (int i = threadIdx.x; i < 3 * S.sp.ntypes; i += kBlock) s_tab[i] = S.sp.tab[i];
+        __syncthreads();
+    }
+    const long long e = (long long)blockIdx.x * kBlock + threadIdx.x;
+    const unsigned lane = threadIdx.x & 31;
+    int i = -1, j = -1;
+    double gx = 0.0, gy = 0.0;
+    if (e < S.M) {
+        i = S.si[e];
+        if (i < 0) { if (SAMPLE) S.sUs[e] = 0.0; i = ~i; }          // dead: stays in its particle's run, contributes 0
+        else {
+            j = S.sj[e];
+            const double2 xi = P.pos_cur[i], xj = P.pos_cur[j];
+            double k, r0, rc;
+            load_params<PM>(S.sp, s_tab, (size_t)e, k, r0, rc);
+            const double dx = xj.x - xi.x, dy = xj.y - xi.y;
+            double gk, ext;
+            if (spring_eval<false>(dx, dy, k, r0, rc, gk, ext)) {
+                gx = gk * dx; gy = gk * dy;
+                if (SAMPLE) S.sUs[e] = 0.5 * k * ext * ext;
+            } else {
+                S.si[e] = ~i;
+                P.break_step[S.sid[e]] = P.step;
+                atomicAdd(P.nbroken + spec_of(P.poff, P.B, i), 1ULL);
+                if (SAMPLE) S.sUs[e] = 0.0;
+                j = -1;
+            }
+        }
+    }
+    // lower endpoint: runs of equal i are contiguous lanes (sorted list; dead springs keep their place) -> segmented
+    // reduction by shuffle-down
+    const unsigned run = __match_any_sync(0xffffffffu, i);
+    double ax = gx, ay = gy;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const double tx = __shfl_down_sync(0xffffffffu, ax, o), ty = __shfl_down_sync(0xffffffffu, ay, o);
+        if (lane + o < 32 && ((run >> (lane + o)) & 1u)) { ax += tx; ay += ty; }
+    }
+    if (i >= 0 && (lane == 0 || !((run >> (lane - 1)) & 1u))) {     // first lane of its run
+        double *fi = reinterpret_cast<double *>(P.f + i);
+        atomicAdd(fi, ax); atomicAdd(fi + 1, ay);
+    }
+    // upper endpoint: one RED pair per spring.  (Aggregating these too -- __match_any_sync on j, peers summed through
+    // __fns / __shfl loops -- halved the RED sectors again but quadrupled the instruction count: 129 us against 115 us
+    // for the plain kernel on config 3, profiles/r2_accumulation_variants.md.)
+    if (j >= 0) {
+        double *fj = reinterpret_cast<double *>(P.f + j);
+        atomicAdd(fj, -gx); atomicAdd(fj + 1, -gy);
+    }
+}
+
+// Scatter variant 3 (north_star: "shared-memory tile accumulation"): a CTA owns kScatterTile consecutive particles and
+// the springs whose lower endpoint is one of them (a contiguous range of the sorted list).  Phase A, one thread per
+// spring: evaluate it ONCE and park g*d in the spring's own shared-memory slot (plain STS: no shared-memory atomics,
+// which are compare-and-swap loops for fp64 on sm_100a); a spring whose upper endpoint belongs to another tile spills
+// its reaction with a global RED.  Phase B, one thread per particle: add the slots of the springs it is the lower
+// endpoint of (a contiguous run), subtract those it is the upper endpoint of (index list), one RED pair per particle
+// into f (other tiles' spills land there too).
+template <int PM, bool SAMPLE>
+__global__ void __launch_bounds__(kScatterTileThreads) k_spring_scatter_tile(const StepParams P, const ScatterParams S) {
+    constexpr bool kTab = (PM == PM_TYPED || PM == PM_KRT_RCF);
+    __shared__ double s_tab[kTab ? 3 * kMaxTypes : 1];
+    extern __shared__ __align__(16) unsigned char dyn[];
+    double2 *G = reinterpret_cast<double2 *>(dyn);
+    if (kTab) for (int i = threadIdx.x; i < 3 * S.sp.ntypes; i += kScatterTileThreads) s_tab[i] = S.sp.tab[i];
+    const long long p0 = (long long)blockIdx.x * kScatterTile, p1 = min(S.N, p0 + kScatterTile);
+    const int s0 = S.tile_off[blockIdx.x], s1 = S.tile_off[blockIdx.x + 1];
+    __syncthreads();
+    for (int e = s0 + threadIdx.x; e < s1; e += kScatterTileThreads) {
+        double2 gd = make_double2(0.0, 0.0);
+        const int i = S.si[e];
+        if (i < 0) { if (SAMPLE) S.sUs[e] = 0.0; }
+        else {
+            const int j = S.sj[e];
+            const double2 xi = P.pos_cur[i], xj = P.pos_cur[j];
+            double k, r0, rc;
+            load_params<PM>(S.sp, s_tab, (size_t)e, k, r0, rc);
+            const double dx = xj.x - xi.x, dy = xj.y - xi.y;
+            double gk, ext;
+            if (spring_eval<false>(dx, dy, k, r0, rc, gk, ext)) {
+                gd = make_double2(gk * dx, gk * dy);
+                if (SAMPLE) S.sUs[e] = 0.5 * k * ext * ext;
+                if (j >= p1) {                                    // upper endpoint in another tile: spill
+                    double *fj = reinterpret_cast<double *>(P.f + j);
+                    atomicAdd(fj, -gd.x); atomicAdd(fj + 1, -gd.y);
+                }
+            } else {
+                S.si[e] = ~i;
+                P.break_step[S.sid[e]] = P.step;
+                atomicAdd(P.nbroken + spec_of(P.poff, P.B, i), 1ULL);
+                if (SAMPLE) S.sUs[e] = 0.0;
+            }
+        }
+        G[e - s0] = gd;
+    }
+    __syncthreads();
+    for (long long p = p0 + threadIdx.x; p < p1; p += kScatterTileThreads) {
+        double fx = 0.0, fy = 0.0;
+        for (int e = S.own_off[p]; e < S.own_off[p + 1]; ++e) { const double2 g = G[e - s0]; fx += g.x; fy += g.y; }
+        for (int q = S.jl_off[p]; q < S.jl_off[p + 1]; ++q) { const double2 g = G[S.jl_idx[q] - s0]; fx -= g.x; fy -= g.y; }
+        double *fp = reinterpret_cast<double *>(P.f + p);
+        atomicAdd(fp, fx); atomicAdd(fp + 1, fy);
     }
 }
 

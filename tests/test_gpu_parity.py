@@ -18,8 +18,9 @@ from oracle.olsm import OracleSim
 from parity import check_forces, conditioning_floor, force_scale
 
 MODES = [dict(force_mode=lsm.FORCE_GATHER, exact=False), dict(force_mode=lsm.FORCE_GATHER, exact=True),
-         dict(force_mode=lsm.FORCE_SCATTER, exact=False)]
-MODE_IDS = ["gather-fast", "gather-exact", "scatter"]
+         dict(force_mode=lsm.FORCE_SCATTER, exact=False), dict(force_mode=lsm.FORCE_SCATTER_WARP, exact=False),
+         dict(force_mode=lsm.FORCE_SCATTER_TILE, exact=False)]
+MODE_IDS = ["gather-fast", "gather-exact", "scatter", "scatter-warp", "scatter-tile"]
 
 
 @pytest.fixture(autouse=True)
@@ -99,7 +100,7 @@ def _peak_and_failure(step, sig, du_y, H0):
     return sig[ip], step[ip] * du_y / H0, eps_f
 
 
-@pytest.mark.parametrize("mode", [MODES[0], MODES[2]], ids=["gather-fast", "scatter"])
+@pytest.mark.parametrize("mode", [MODES[0], MODES[2], MODES[3], MODES[4]], ids=["gather-fast", "scatter", "scatter-warp", "scatter-tile"])
 def test_T3_T4_T5_fracture_curve(mode):
     p = _fracture_problem()
     nsteps = 9000
