@@ -192,6 +192,17 @@ lsm_status lsm_read_stress(lsm_sim *sim, int64_t capacity, int64_t *n_samples, i
 lsm_status lsm_run_to_failure(lsm_sim *sim, int64_t max_steps, int32_t group, int32_t axis, double stop_fraction,
                               int64_t *steps_done, int32_t *failed, double *peak, int64_t *peak_step);
 
+/* Strain-rate control of the paper's protocol ("boundary particles were displaced apart ... at the strain
+ * rate of 1e-6"): groups group_lo and group_hi (both already defined with lsm_set_boundary) become MOVE groups pulled
+ * apart along `axis` so that the gauge length H0 -- the distance between the two groups' mean positions along the axis
+ * at this call -- grows by strain_per_step * H0 per step: symmetric != 0 moves group_lo by -du/2 and group_hi by +du/2
+ * per step (both grips, as in the paper), symmetric == 0 holds group_lo and moves group_hi by du.  ramp != 0 also gives
+ * every free particle, along the axis, the velocity e (x - c) / dt of the affine field (c = the point that stays at rest)
+ * so that the pull starts without a grip shock, and refreshes the held forces as lsm_write_state does.  *gauge_length
+ * (may be NULL) returns H0: strain after n steps = n * strain_per_step.  dim = 2.  Synchronises the stream. */
+lsm_status lsm_set_strain_rate(lsm_sim *sim, int32_t group_lo, int32_t group_hi, int32_t axis, double strain_per_step,
+                               int32_t symmetric, int32_t ramp, double *gauge_length);
+
 /* Drop dead springs from the device lists now (also done every compact_every steps; the paper keeps dead springs with
  * k = 0, L196).  Two stages, both on the device and asynchronous: every row is compacted in place, stably (each particle
  * keeps its summation order, so no result changes); then the slot storage is repacked (prefix sum of the slices' live

@@ -21,7 +21,7 @@ FUSION_AUTO, FUSION_ON, FUSION_OFF, FUSION_RESIDENT = 0, 1, 2, 3
 MAX_GROUPS = 8
 
 EXPORTS = ["lsm_create", "lsm_set_boundary", "lsm_step", "lsm_write_state", "lsm_read_state", "lsm_read_forces",
-           "lsm_read_broken", "lsm_read_energy", "lsm_read_virial", "lsm_read_stress", "lsm_run_to_failure", "lsm_compact", "lsm_sync", "lsm_get_info",
+           "lsm_read_broken", "lsm_read_energy", "lsm_read_virial", "lsm_read_stress", "lsm_run_to_failure", "lsm_set_strain_rate", "lsm_compact", "lsm_sync", "lsm_get_info",
            "lsm_device_state", "lsm_last_error", "lsm_destroy", "lsm_abi_version"]
 
 _ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
@@ -90,6 +90,7 @@ def library():
         L.lsm_read_energy.argtypes = [C.c_void_p, d, d]
         L.lsm_read_stress.argtypes = [C.c_void_p, C.c_int64, i64, i64, d, d, d, i64]
         L.lsm_run_to_failure.argtypes = [C.c_void_p, C.c_int64, C.c_int32, C.c_int32, C.c_double, i64, i32, d, i64]
+        L.lsm_set_strain_rate.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_double, C.c_int32, C.c_int32, d]
         L.lsm_compact.argtypes = [C.c_void_p]
         L.lsm_sync.argtypes = [C.c_void_p]
         L.lsm_get_info.argtypes = [C.c_void_p, C.POINTER(LsmInfo)]
@@ -228,6 +229,13 @@ class LsmSim:
                                                  C.byref(n), C.byref(failed), _ptr(peak, C.c_double), _ptr(pstep, C.c_int64)))
         return int(n.value), bool(failed.value), peak, pstep
 
+    def set_strain_rate(self, group_lo, group_hi, axis, strain_per_step, symmetric=True, ramp=True):
+        """Returns the gauge length H0."""
+        h0 = C.c_double(0.0)
+        self._check(library().lsm_set_strain_rate(self._h, int(group_lo), int(group_hi), int(axis), float(strain_per_step),
+                                                  int(bool(symmetric)), int(bool(ramp)), C.byref(h0)))
+        return float(h0.value)
+
     def info(self):
         inf = LsmInfo()
         self._check(library().lsm_get_info(self._h, C.byref(inf)))
@@ -338,6 +346,7 @@ def lsm_read_broken(sim): return sim.read_broken()
 def lsm_read_energy(sim): return sim.read_energy()
 def lsm_read_stress(sim, capacity=None): return sim.read_stress(capacity)
 def lsm_run_to_failure(sim, max_steps, group=1, axis=1, stop_fraction=0.1): return sim.run_to_failure(max_steps, group, axis, stop_fraction)
+def lsm_set_strain_rate(sim, group_lo, group_hi, axis, strain_per_step, symmetric=True, ramp=True): return sim.set_strain_rate(group_lo, group_hi, axis, strain_per_step, symmetric, ramp)
 def lsm_compact(sim): return sim.compact()
 def lsm_sync(sim): return sim.sync()
 def lsm_get_info(sim): return sim.info()

@@ -1578,6 +1578,51 @@ lsm_status lsm_run_to_failure(lsm_sim *s, int64_t max_steps, int32_t group, int3
     return LSM_OK;
 }
 
+// Strain-rate control of the paper's protocol: host logic around lsm_set_boundary plus one ramp kernel.
+lsm_status lsm_set_strain_rate(lsm_sim *s, int32_t g_lo, int32_t g_hi, int32_t axis, double strain_per_step, int32_t symmetric, int32_t ramp,
+                               double *gauge_length) {
+    CHECK_SIM(s);
+    if (s->dim != 2) { s->err = "lsm_set_strain_rate: dim = 2 only"; return LSM_E_UNSUPPORTED; }
+    if (g_lo < 0 || g_lo >= kMaxGroups || g_hi < 0 || g_hi >= kMaxGroups || g_lo == g_hi || axis < 0 || axis >= s->dim || !std::isfinite(strain_per_step)) { s->err = "bad arguments"; return LSM_E_INVALID; }
+    Group &lo = s->groups[g_lo], &hi = s->groups[g_hi];
+    if (!lo.set || !hi.set || lo.ids.empty() || hi.ids.empty()) { s->err = "lsm_set_strain_rate: both groups must have been defined with lsm_set_boundary"; return LSM_E_INVALID; }
+    // gauge length = distance between the groups' mean positions along the axis, now (sums in ascending caller id)
+    std::vector<double> x((size_t)s->N * 2);
+    TRY(lsm_read_state(s, x.data(), nullptr));
+    auto mean_of = [&](const Group &g) {
+        std::vector<int32_t> c(g.ids.size());
+        for (size_t q = 0; q < g.ids.size(); ++q) c[q] = s->perm.empty() ? g.ids[q] : s->perm[g.ids[q]];
+        std::sort(c.begin(), c.end());
+        double sum = 0.0;
+        for (int32_t id : c) sum += x[(size_t)id * 2 + axis];
+        return sum / (double)c.size();
+    };
+    const double m_lo = mean_of(lo), m_hi = mean_of(hi), H0 = m_hi - m_lo;
+    if (!(H0 > 0.0)) { s->err = "lsm_set_strain_rate: group_hi must lie above group_lo along the axis"; return LSM_E_INVALID; }
+    if (gauge_length) *gauge_length = H0;
+    const double du = strain_per_step * H0;
+    double d_lo[3] = {0.0, 0.0, 0.0}, d_hi[3] = {0.0, 0.0, 0.0};
+    d_lo[axis] = symmetric ? -0.5 * du : 0.0;
+    d_hi[axis] = symmetric ? 0.5 * du : du;
+    auto caller_ids = [&](const Group &g) {
+        std::vector<int32_t> c(g.ids.size());
+        for (size_t q = 0; q < g.ids.size(); ++q) c[q] = s->perm.empty() ? g.ids[q] : s->perm[g.ids[q]];
+        return c;
+    };
+    const std::vector<int32_t> c_lo = caller_ids(lo), c_hi = caller_ids(hi);
+    TRY(lsm_set_boundary(s, g_lo, c_lo.data(), (int64_t)c_lo.size(), LSM_MOVE, d_lo));
+    TRY(lsm_set_boundary(s, g_hi, c_hi.data(), (int64_t)c_hi.size(), LSM_MOVE, d_hi));
+    if (ramp) {
+        const double c = symmetric ? 0.5 * (m_lo + m_hi) : m_lo;
+        k_velocity_ramp<<<grid_for(s->N), kBlock, 0, s->stream>>>(s->pos[s->cur], s->vel, s->grp, s->N, axis, strain_per_step, c, s->dt);
+        s->kernels_launched += 1;
+        CUDA_TRY(s, cudaGetLastError());
+        TRY(eval_initial(s));          // the held total force f - gamma v follows the new velocities (as after lsm_write_state)
+        CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    }
+    return LSM_OK;
+}
+
 lsm_status lsm_get_info(lsm_sim *s, lsm_info *info) {
     if (!s || !info) return LSM_E_INVALID;
     std::memset(info, 0, sizeof(*info));

@@ -1168,6 +1168,18 @@ __global__ void __launch_bounds__(kBlock) k_group_assign(const int32_t *ids, lon
     sKE[p] = 0.0;           // kinematic particles carry no KE (Q6)
 }
 
+// Velocity ramp of the strain-rate protocol (lsm_set_strain_rate): every free particle takes, along `axis`, the velocity
+// of the affine field that moves the grips apart, v = e (x - c) / dt (e = strain per step, c = the fixed point).
+__global__ void __launch_bounds__(kBlock) k_velocity_ramp(const double2 *pos, double2 *vel, const uint8_t *grp, long long N, int axis, double e, double c, double dt) {
+    const long long p = (long long)blockIdx.x * kBlock + threadIdx.x;
+    if (p >= N || grp[p] != kFree) return;
+    const double2 x = pos[p];
+    double2 v = vel[p];
+    const double r = __ddiv_rn(__dmul_rn(e, __dsub_rn(axis == 0 ? x.x : x.y, c)), dt);
+    if (axis == 0) v.x = r; else v.y = r;
+    vel[p] = v;
+}
+
 __global__ void __launch_bounds__(kBlock) k_broken_from_steps(const long long *break_step, uint8_t *broken, long long M) {
     const long long e = (long long)blockIdx.x * kBlock + threadIdx.x;
     if (e < M) broken[e] = break_step[e] >= 0;

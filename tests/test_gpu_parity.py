@@ -778,6 +778,58 @@ def test_symmetric_grips_run_to_failure_matches_oracle():
     g.close(); f.close()
 
 
+def test_strain_rate_control_with_velocity_ramp_matches_oracle():
+    """NEXT-2 tail ("displaced apart ... at the strain rate of 1e-6"): lsm_set_strain_rate turns two FIXED grip
+    rows into a symmetric pull at a given strain per step and starts the free particles on the affine velocity ramp.
+    The same protocol spelled with the oracle's set_boundary / write_state (gauge length from sequential sums, ramp
+    (e (y - c)) / dt): identical gauge length, state and -- through lsm_run_to_failure -- stop step, peak step, broken set in
+    exact mode; the one-sided, ramp-free variant too."""
+    p = _fracture_problem(n=48, du_y=3e-4, seed=11)
+    p.sample_every = 100
+    for g_ in p.groups:
+        g_.mode = FIXED; g_.du = np.zeros(2)
+    p.v = np.zeros_like(p.x)
+    bot, top = p.groups[0].ids, p.groups[1].ids
+    e = 1.5e-5
+    def seq_mean(a):
+        t = 0.0
+        for v_ in a:
+            t += float(v_)
+        return t / len(a)
+    for symmetric, ramp in ((True, True), (False, False)):
+        o = OracleSim.from_problem(p)
+        g = lsm_create_from_problem(p, exact=True, history_capacity=512)
+        H0g = g.set_strain_rate(0, 1, 1, e, symmetric=symmetric, ramp=ramp)
+        x0, v0 = o.read_state()
+        m_lo, m_hi = seq_mean(x0[np.sort(bot), 1]), seq_mean(x0[np.sort(top), 1])
+        H0 = m_hi - m_lo
+        assert H0g == H0
+        du = e * H0
+        o.set_boundary(0, bot, MOVE, [0.0, -0.5 * du if symmetric else 0.0])
+        o.set_boundary(1, top, MOVE, [0.0, 0.5 * du if symmetric else du])
+        if ramp:
+            c = 0.5 * (m_lo + m_hi) if symmetric else m_lo
+            free = np.ones(p.N, dtype=bool); free[bot] = False; free[top] = False
+            v = v0.copy(); v[free, 1] = (e * (x0[free, 1] - c)) / p.dt
+            o.write_state(x0, v)
+        xo, vo = o.read_state(); xg, vg = g.read_state()
+        assert np.array_equal(xo, xg) and np.array_equal(vo, vg)
+        peak, peak_step, steps, failed = 0.0, -1, 0, False
+        while steps < 12000 and not failed:
+            o.step(100); steps += 100
+            r = abs(o.read_stress()["R"][-1, 0, 1, 1])
+            if r > peak:
+                peak, peak_step = r, steps
+            elif peak > 0 and r < 0.1 * peak:
+                failed = True
+        n, gf, gpeak, gstep = g.run_to_failure(12000, group=1, axis=1, stop_fraction=0.1)
+        assert failed and gf and n == steps and gstep[0] == peak_step and abs(gpeak[0] / peak - 1) <= 1e-12
+        assert np.array_equal(o.read_broken()[1], g.read_broken()[1]) and o.read_broken()[2] > 0
+        xo, vo = o.read_state(); xg, vg = g.read_state()
+        assert np.array_equal(xo, xg) and np.array_equal(vo, vg)
+        g.close()
+
+
 # ---------------------------------------------------------------- D = 3 (the layout of the paper's kernel listing, L93-L97)
 def _problem_3d(n=(9, 8, 7), seed=5, rc_spread=True):
     from lsm_inputs import cubic_lattice_3d
