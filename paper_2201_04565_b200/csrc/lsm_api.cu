@@ -1208,8 +1208,8 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
         CUDA_TRY(s, cudaStreamSynchronize(s->stream));
         TRY(dev_alloc(s, &s->part, (size_t)s->nchunks * 2));
         TRY(dev_alloc(s, &s->sU, (size_t)N)); TRY(dev_alloc(s, &s->sKE, (size_t)N));
-        TRY(dev_alloc(s, &s->flags, 1));
-        CUDA_TRY(s, cudaMemsetAsync(s->flags, 0, sizeof(int), s->stream));
+        TRY(dev_alloc(s, &s->flags, 2));               // [0] sticky device-side error bits, [1] scratch of the input validation
+        CUDA_TRY(s, cudaMemsetAsync(s->flags, 0, 2 * sizeof(int), s->stream));
         TRY(dev_alloc(s, &s->cur_U, (size_t)B)); TRY(dev_alloc(s, &s->cur_KE, (size_t)B));
         const size_t cap = (size_t)s->hist_cap;
         TRY(dev_alloc(s, &s->hist_step, cap)); TRY(dev_alloc(s, &s->hist_nb, cap * B));
@@ -1403,21 +1403,24 @@ lsm_status lsm_sync(lsm_sim *s) {
 lsm_status lsm_write_state(lsm_sim *s, const double *x, const double *v) {
     CHECK_SIM(s);
     if (!x) { s->err = "x is NULL"; return LSM_E_INVALID; }
-    for (long long q = 0; q < s->dim * s->N; ++q)
-        if (!std::isfinite(x[q]) || (v && !std::isfinite(v[q]))) { s->err = "non-finite position / velocity"; return LSM_E_NONFINITE; }
-    if (s->dim == 3) {
-        CUDA_TRY(s, cudaMemcpyAsync(s->stage3[0], x, sizeof(double) * 3 * s->N, cudaMemcpyHostToDevice, s->stream));
-        if (v) CUDA_TRY(s, cudaMemcpyAsync(s->stage3[1], v, sizeof(double) * 3 * s->N, cudaMemcpyHostToDevice, s->stream));
-        k3_from_caller<<<grid_for(s->N), kBlock, 0, s->stream>>>(s->stage3[0], v ? s->stage3[1] : nullptr, s->pos3[s->cur], s->vel3, s->d_inv, s->N, s->grp);
-    } else {
-        CUDA_TRY(s, cudaMemcpyAsync(s->stage[0], x, sizeof(double2) * s->N, cudaMemcpyHostToDevice, s->stream));
-        if (v) CUDA_TRY(s, cudaMemcpyAsync(s->stage[1], v, sizeof(double2) * s->N, cudaMemcpyHostToDevice, s->stream));
-        k_from_caller<<<grid_for(s->N), kBlock, 0, s->stream>>>(s->stage[0], v ? s->stage[1] : nullptr, s->pos[s->cur], s->vel, s->d_inv, s->N, s->grp);
-    }
+    // stage the caller's arrays, validate them on the device, and only then touch the state
+    double *sx = s->dim == 3 ? s->stage3[0] : reinterpret_cast<double *>(s->stage[0]);
+    double *sv = s->dim == 3 ? s->stage3[1] : reinterpret_cast<double *>(s->stage[1]);
+    const long long n = (long long)s->dim * s->N;
+    CUDA_TRY(s, cudaMemcpyAsync(sx, x, sizeof(double) * n, cudaMemcpyHostToDevice, s->stream));
+    if (v) CUDA_TRY(s, cudaMemcpyAsync(sv, v, sizeof(double) * n, cudaMemcpyHostToDevice, s->stream));
+    CUDA_TRY(s, cudaMemsetAsync(s->flags + 1, 0, sizeof(int), s->stream));
+    k_check_finite<<<(unsigned)std::min<long long>(2048, (n + kBlock - 1) / kBlock), kBlock, 0, s->stream>>>(sx, v ? sv : nullptr, n, s->flags + 1);
+    s->kernels_launched += 1;
+    int bad = 0;
+    CUDA_TRY(s, cudaMemcpyAsync(&bad, s->flags + 1, sizeof(int), cudaMemcpyDeviceToHost, s->stream));
+    CUDA_TRY(s, cudaStreamSynchronize(s->stream));   // x / v are borrowed for the duration of the call only (lsm.h): consumed here
+    if (bad) { s->err = "non-finite position / velocity"; return LSM_E_NONFINITE; }
+    if (s->dim == 3) k3_from_caller<<<grid_for(s->N), kBlock, 0, s->stream>>>(s->stage3[0], v ? s->stage3[1] : nullptr, s->pos3[s->cur], s->vel3, s->d_inv, s->N, s->grp);
+    else k_from_caller<<<grid_for(s->N), kBlock, 0, s->stream>>>(s->stage[0], v ? s->stage[1] : nullptr, s->pos[s->cur], s->vel, s->d_inv, s->N, s->grp);
     s->kernels_launched += 1;
     for (int g = 0; g < kMaxGroups; ++g) s->groups[g].n0 = s->step;
     TRY(eval_initial(s));
-    CUDA_TRY(s, cudaStreamSynchronize(s->stream));   // x / v are borrowed for the duration of the call only (lsm.h)
     return LSM_OK;
 }
 

@@ -1135,6 +1135,14 @@ __global__ void __launch_bounds__(kBlock) k_to_caller(const double2 *src, double
     dst[c] = v;
 }
 
+// Input validation of lsm_write_state on the device (the staged copies of the caller's arrays): *bad |= 1 on NaN / Inf.
+__global__ void __launch_bounds__(kBlock) k_check_finite(const double *a, const double *b, long long n, int *bad) {
+    bool ok = true;
+    for (long long q = (long long)blockIdx.x * kBlock + threadIdx.x; q < n; q += (long long)gridDim.x * kBlock)
+        ok = ok && isfinite(a[q]) && (!b || isfinite(b[q]));
+    if (!ok) atomicOr(bad, 1);
+}
+
 __global__ void __launch_bounds__(kBlock) k_from_caller(const double2 *srcx, const double2 *srcv, double2 *pos, double2 *vel,
                                                         const int32_t *inv, long long N, const uint8_t *grp) {
     const long long c = (long long)blockIdx.x * kBlock + threadIdx.x;

@@ -287,6 +287,16 @@ def test_invalid_inputs_are_rejected():
         g.set_boundary(1, [0], FIXED)                      # already in group 0
     with pytest.raises(lsm.LsmError):
         g.set_boundary(9, [1], FIXED)
+    xs, vs = g.read_state()                                    # lsm_write_state validates on the device before touching the state
+    xn = x.copy(); xn[2, 0] = np.nan
+    with pytest.raises(lsm.LsmError) as ei:
+        g.write_state(xn)
+    assert ei.value.status == -3
+    with pytest.raises(lsm.LsmError) as ei:
+        g.write_state(x, np.full(x.shape, np.inf))
+    assert ei.value.status == -3
+    assert np.array_equal(g.read_state()[0], xs) and np.array_equal(g.read_state()[1], vs)
+    g.step(3)                                                  # not sticky: the handle is still usable
     g.close()
     # springs must not cross specimens
     with pytest.raises(lsm.LsmError) as ei:
