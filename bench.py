@@ -266,6 +266,7 @@ def main():
     ap.add_argument("--exact", type=int, default=0)
     ap.add_argument("--gather-variant", type=int, default=0, help="0 auto, 1 direct, 2 streamed")
     ap.add_argument("--step-fusion", type=int, default=0, help="0 auto, 1 cooperative multi-step launches, 2 off, 3 cluster-resident")
+    ap.add_argument("--gather-window", type=int, default=0, help="0 auto, 1 on, 2 off: neighbour windows staged in shared memory")
     ap.add_argument("--cluster-size", type=int, default=0, help="cluster-resident stepping: CTAs per cluster (0 = library's choice)")
     ap.add_argument("--shuffle-ids", type=int, default=0, help="seed > 0: renumber particles / springs at random first (an arbitrary input-file order)")
     ap.add_argument("--prebreak", type=float, default=0.0, help="fraction of springs dead from step 0 (rc < r0): the compaction window of SURVEY 8(d)")
@@ -322,7 +323,7 @@ def main():
           "scatter-tile": lsm.FORCE_SCATTER_TILE}[args.force_mode]
     sim = lsm_create_from_problem(p, device=local, force_mode=fm, reorder=args.reorder, compact_every=args.compact_every,
                                   exact=bool(args.exact), history_capacity=64, gather_variant=args.gather_variant, step_fusion=args.step_fusion,
-                                  cluster_size=args.cluster_size)
+                                  cluster_size=args.cluster_size, gather_window=args.gather_window)
     if args.compact_now:
         sim.compact()
     inf0 = sim.info()
@@ -406,7 +407,7 @@ def main():
             "config": {"workload": desc, "N": p.N, "M": p.M, "M_alive_at_start": M_alive0, "broken_at_end": nb_after,
                        "time_steps_per_bench_step": S, "ns_per_time_step": 1e6 * ms_max / (K * S), "sample_every": SAMPLE_EVERY,
                        "compact_every": args.compact_every, "force_mode": inf0["force_mode"], "param_mode": inf0["param_mode"],
-                       "exact": inf0["exact"], "reorder": inf0["reorder"], "gather_variant": inf0["gather_variant"], "step_fusion": inf0["step_fusion"], "cluster_size": inf0["cluster_size"], "pipeline_stages": inf0["pipeline_stages"], "stage_bytes": inf0["stage_bytes"], "bytes_per_half_edge": inf0["bytes_per_half_edge"],
+                       "exact": inf0["exact"], "reorder": inf0["reorder"], "gather_variant": inf0["gather_variant"], "step_fusion": inf0["step_fusion"], "cluster_size": inf0["cluster_size"], "window_particles": inf0["window_particles"], "window_stages": inf0["window_stages"], "pipeline_stages": inf0["pipeline_stages"], "stage_bytes": inf0["stage_bytes"], "bytes_per_half_edge": inf0["bytes_per_half_edge"],
                        "half_edges_stored": inf0["n_half_edges_stored"], "device_bytes": inf0["device_bytes"],
                        "l2": "inputs larger than L2 (%.0f MB streamed per time step vs 126 MB L2)"
                              % ((64.0 * p.N + inf0["n_half_edges_stored"] * inf0["bytes_per_half_edge"] + 1.25 * p.N) / 1e6),

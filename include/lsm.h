@@ -37,7 +37,7 @@ extern "C" {
 #endif
 
 #define LSM_MAX_GROUPS 8
-#define LSM_ABI_VERSION 4
+#define LSM_ABI_VERSION 5
 
 typedef struct lsm_sim lsm_sim; /* opaque */
 
@@ -67,6 +67,10 @@ enum { LSM_REORDER_NONE = 0, LSM_REORDER_MORTON = 1, LSM_REORDER_RCM = 2,
 /* kernels of the gather path: DIRECT = one thread per particle reading global memory; STREAMED = persistent CTAs,
  * bulk-async-copy (TMA engine) staging of the tile streams through a shared-memory mbarrier pipeline */
 enum { LSM_GATHER_AUTO = 0, LSM_GATHER_DIRECT = 1, LSM_GATHER_STREAMED = 2 };
+/* plain time steps of the streamed kernel: AUTO / ON = the producer also stages the tile's neighbour id ranges (its
+ * "window": <= 4 contiguous ranges with a banded numbering) and the consumers gather from shared memory; OFF = gathers
+ * from global memory (L1 / L2).  ON fails with LSM_E_UNSUPPORTED where AUTO would fall back to OFF. */
+enum { LSM_WINDOW_AUTO = 0, LSM_WINDOW_ON = 1, LSM_WINDOW_OFF = 2 };
 /* several time steps per launch: ON = one cooperative launch with a grid barrier between steps (state stays in L2 /
  * the CTAs' pipeline stages); RESIDENT = one thread-block cluster per specimen keeps it in shared memory for the whole
  * run of steps, ghosts exchanged through distributed shared memory, cluster barrier per step (needs dim = 2, 16-bit
@@ -107,7 +111,9 @@ typedef struct lsm_desc {
                                          spring list (GATHER only).  0: fast arithmetic (FMA, rsqrt)              */
     int32_t step_fusion;              /* LSM_FUSION_* (above)                                                     */
     int32_t gather_variant;           /* LSM_GATHER_*: AUTO = STREAMED when a tile's rows fit in shared memory    */
+    int32_t gather_window;            /* LSM_WINDOW_*                                                             */
     int32_t device;                   /* CUDA device ordinal                                                      */
+    int32_t _pad1;
     int32_t cluster_size;             /* RESIDENT stepping: CTAs per cluster, 0 = chosen by the library, else 1, 2, 4, 8, 16 */
     void *stream;                     /* cudaStream_t, NULL = the default stream                                  */
     lsm_alloc_fn alloc;               /* NULL -> cudaMalloc / cudaFree                                            */
@@ -135,6 +141,8 @@ typedef struct lsm_info {
     int32_t step_fusion;              /* 0: one launch per step; 1: cooperative multi-step launches; 2: cluster-resident */
     int32_t cluster_size;             /* cluster-resident stepping: CTAs per cluster (0 otherwise)                */
     int64_t resident_smem_bytes;      /* cluster-resident stepping: dynamic shared memory per CTA                 */
+    int32_t window_particles;         /* windowed gathers: largest tile window in particles (0 = gathers from global memory) */
+    int32_t window_stages;            /* windowed gathers: pipeline stages                                        */
 } lsm_info;
 
 /* Build a simulation from particle / spring arrays.  Copies everything (the caller may free its inputs afterwards),

@@ -17,6 +17,7 @@ FIXED, MOVE = 0, 1
 FORCE_AUTO, FORCE_SCATTER, FORCE_GATHER, FORCE_SCATTER_WARP, FORCE_SCATTER_TILE = 0, 1, 2, 3, 4
 REORDER_NONE, REORDER_MORTON, REORDER_RCM, REORDER_BLOCKED = 0, 1, 2, 3
 GATHER_AUTO, GATHER_DIRECT, GATHER_STREAMED = 0, 1, 2
+WINDOW_AUTO, WINDOW_ON, WINDOW_OFF = 0, 1, 2
 FUSION_AUTO, FUSION_ON, FUSION_OFF, FUSION_RESIDENT = 0, 1, 2, 3
 MAX_GROUPS = 8
 
@@ -41,7 +42,8 @@ class LsmDesc(C.Structure):
         ("dt", C.c_double), ("gamma", C.c_double),
         ("sample_every", C.c_int32), ("history_capacity", C.c_int32), ("compact_every", C.c_int32),
         ("reorder", C.c_int32), ("force_mode", C.c_int32), ("exact", C.c_int32), ("step_fusion", C.c_int32),
-        ("gather_variant", C.c_int32), ("device", C.c_int32), ("cluster_size", C.c_int32), ("stream", C.c_void_p),
+        ("gather_variant", C.c_int32), ("gather_window", C.c_int32), ("device", C.c_int32), ("_pad1", C.c_int32), ("cluster_size", C.c_int32),
+        ("stream", C.c_void_p),
         ("alloc", _ALLOC_FN), ("free_", _FREE_FN), ("alloc_user", C.c_void_p),
     ]
 
@@ -54,6 +56,7 @@ class LsmInfo(C.Structure):
         ("device_bytes", C.c_int64), ("kernels_launched", C.c_int64), ("current_step", C.c_int64),
         ("gather_variant", C.c_int32), ("pipeline_stages", C.c_int32), ("stage_bytes", C.c_int64),
         ("step_fusion", C.c_int32), ("cluster_size", C.c_int32), ("resident_smem_bytes", C.c_int64),
+        ("window_particles", C.c_int32), ("window_stages", C.c_int32),
     ]
 
 
@@ -260,7 +263,7 @@ class LsmSim:
 
 def lsm_create(x, spring_i, spring_j, k, r0, rc, dt, gamma=0.0, v=None, mass=1.0, n_batch=1, particle_offsets=None,
                spring_offsets=None, sample_every=0, history_capacity=0, compact_every=0, reorder=REORDER_NONE,
-               force_mode=FORCE_AUTO, exact=False, step_fusion=0, gather_variant=GATHER_AUTO, cluster_size=0, device=0, stream=None, use_torch_allocator=True):
+               force_mode=FORCE_AUTO, exact=False, step_fusion=0, gather_variant=GATHER_AUTO, gather_window=0, cluster_size=0, device=0, stream=None, use_torch_allocator=True):
     """lsm_create: build a simulation from HOST arrays.  k / r0 / rc may be scalars (uniform) or [M] arrays."""
     L = library()
     x = np.ascontiguousarray(x, dtype=np.float64)
@@ -297,7 +300,7 @@ def lsm_create(x, spring_i, spring_j, k, r0, rc, dt, gamma=0.0, v=None, mass=1.0
     d.dt = float(dt); d.gamma = float(gamma)
     d.sample_every = int(sample_every); d.history_capacity = int(history_capacity); d.compact_every = int(compact_every)
     d.reorder = int(reorder); d.force_mode = int(force_mode); d.exact = int(bool(exact)); d.step_fusion = int(step_fusion)
-    d.gather_variant = int(gather_variant); d.cluster_size = int(cluster_size)
+    d.gather_variant = int(gather_variant); d.gather_window = int(gather_window); d.cluster_size = int(cluster_size)
     d.device = int(device)
     allocator = None
     try:

@@ -16,6 +16,7 @@
 #include "lsm_kernels.cuh"
 #include "lsm_kernels3.cuh"
 #include "lsm_resident.cuh"
+#include "lsm_window.cuh"
 
 using namespace lsmk;
 
@@ -81,6 +82,11 @@ struct lsm_sim {
     uint32_t max_tile_slots = 0;
     double *virial = nullptr;        // [N][3] output buffer of lsm_read_virial (allocated on first use)
     int multi_on = 0;                // fuse runs of plain time steps into one cooperative launch
+    // windowed streamed kernel (lsm_window.cuh): neighbour ranges of every tile staged in shared memory by the producer
+    int win_on = 0, win_cap = 0, win_smem = 0, win_grid = 0;
+    StageLayout LW;
+    TileWin *d_win = nullptr;
+    uint16_t *widx = nullptr;
     // cluster-resident stepping (lsm_resident.cuh): one thread-block cluster per unit (specimen / small lattice)
     int res_on = 0, res_cluster = 0, res_grid = 0, res_active_clusters = 0;
     ResLayout RL;
@@ -236,7 +242,7 @@ StepParams step_params(const lsm_sim *s, long long step) {
     P.mass_u = s->mass_u; P.inv_mass_u = 1.0 / s->mass_u;
     P.dt = s->dt; P.hdt = 0.5 * s->dt; P.gamma = s->gamma;
     P.N = s->N; P.step = step;
-    P.hdr = s->hdr; P.T = s->T; P.nbr = s->nbr; P.nbr16 = s->nbr16; P.sid = s->sid;
+    P.hdr = s->hdr; P.T = s->T; P.nbr = s->nbr; P.nbr16 = s->nbr16; P.widx = s->widx; P.sid = s->sid;
     P.sp.typ = s->typ; P.sp.kF = s->kF; P.sp.r0F = s->r0F; P.sp.rcF = s->rcF; P.sp.tab = s->tab; P.sp.ntypes = s->ntypes;
     P.sp.thr = s->thr; P.sp.thr_base = s->thr_base; P.sp.thr_mul = 1u << s->thr_shift; P.sp.rcS = s->rcS; P.sp.kr0_u = s->k_u * s->r0_u; P.sp.thr_u = thr_of(s->rc_u);
     P.sp.k_u = s->k_u; P.sp.r0_u = s->r0_u; P.sp.rc_u = s->rc_u;
@@ -524,6 +530,26 @@ template <bool EXACT> cudaError_t launch_resident_pm(const lsm_sim *s, const Ste
     }
 }
 
+template <int PM, bool EXACT> void launch_win_one(const lsm_sim *s, const StepParams &P, const WinParams &W) {
+    auto kern = k_gather_win<PM, EXACT>;
+    static thread_local OptIn configured_for;
+    int &have = configured_for.bytes[s->device < kMaxDevices ? s->device : kMaxDevices - 1];
+    if (have < s->win_smem || s->device >= kMaxDevices - 1) {
+        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, s->win_smem) == cudaSuccess) have = s->win_smem;
+    }
+    kern<<<s->win_grid, kTile + 32, s->win_smem, s->stream>>>(P, s->LW, W);
+}
+
+template <bool EXACT> void launch_win_pm(const lsm_sim *s, const StepParams &P, const WinParams &W) {
+    switch (s->pm) {
+        case PM_UNIFORM: launch_win_one<PM_UNIFORM, EXACT>(s, P, W); break;
+        case PM_TYPED: launch_win_one<PM_TYPED, EXACT>(s, P, W); break;
+        case PM_RCF: launch_win_one<PM_RCF, EXACT>(s, P, W); break;
+        case PM_KRT_RCF: launch_win_one<PM_KRT_RCF, EXACT>(s, P, W); break;
+        default: launch_win_one<PM_FULL, EXACT>(s, P, W); break;
+    }
+}
+
 // nsteps plain time steps, first force evaluation = step `step`, state resident in the clusters' shared memory.
 cudaError_t launch_resident(lsm_sim *s, long long step, int nsteps) {
     const StepParams P = step_params(s, step);
@@ -534,7 +560,11 @@ cudaError_t launch_resident(lsm_sim *s, long long step, int nsteps) {
 
 void launch_gather(lsm_sim *s, const StepParams &P, Variant v) {
     if (s->dim == 3 && s->gather_variant != 2) { launch_gather3(s, P.step, v); return; }
-    if (s->gather_variant == 2) {
+    if (s->win_on && v == V_MID) {       // plain time step: neighbour windows staged by the producer, gathers from shared memory
+        WinParams W;
+        W.win = s->d_win; W.widx = s->widx; W.win_off = s->LW.pos;
+        if (s->exact) launch_win_pm<true>(s, P, W); else launch_win_pm<false>(s, P, W);
+    } else if (s->gather_variant == 2) {
         if (s->exact) launch_stream_pm<true>(s, P, v);
         else launch_stream_pm<false>(s, P, v);
     } else {
@@ -656,7 +686,7 @@ lsm_status do_compact(lsm_sim *s) {
     if (s->force_mode == LSM_FORCE_GATHER && s->E0 > 0) {
         CompactParams C;
         C.hdr = s->hdr; C.nbr = s->nbr; C.nbr16 = s->nbr16; C.sid = s->sid; C.typ = s->typ; C.thr = s->thr;
-        C.kF = s->kF; C.r0F = s->r0F; C.nslices = s->nslices;
+        C.kF = s->kF; C.r0F = s->r0F; C.nslices = s->nslices; C.widx = s->widx;
         k_compact_ell<<<grid_for(s->nslices * kSlice), kBlock, 0, s->stream>>>(C);
         s->kernels_launched += 1;
         CUDA_TRY(s, cudaGetLastError());
@@ -677,7 +707,7 @@ lsm_status do_compact(lsm_sim *s) {
         CUDA_TRY(s, cudaMemsetAsync(s->rp_ticket, 0, sizeof(unsigned int), s->stream));
         k_scan_widths<<<(unsigned)nblk, kBlock, 0, s->stream>>>(R);
         s->kernels_launched += 1;
-        repack_array(s, R, s->nbr); repack_array(s, R, s->sid); repack_array(s, R, s->nbr16);
+        repack_array(s, R, s->nbr); repack_array(s, R, s->sid); repack_array(s, R, s->nbr16); repack_array(s, R, s->widx);
         repack_array(s, R, s->typ); repack_array(s, R, s->thr); repack_array(s, R, s->kF); repack_array(s, R, s->r0F);
         k_commit_offsets<<<grid_for(s->T), kBlock, 0, s->stream>>>(R);
         k_commit_total<<<1, 1, 0, s->stream>>>(s->rp_totals);
@@ -1093,6 +1123,77 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
             const long long fuse_below = 1 << 18;   // measured: 64^2 5.8 -> 3.6 us per step, 512^2 8.4 -> 8.3, 2.1 M particles 39.1 -> 40.4
             if (s->step_fusion == LSM_FUSION_ON && !(coop && s->gather_variant == 2)) return fail(s, LSM_E_UNSUPPORTED, "step_fusion = ON needs the streamed gather kernel and cooperative launch support");
             s->multi_on = coop && s->gather_variant == 2 && (s->step_fusion == LSM_FUSION_ON || ((s->step_fusion == LSM_FUSION_AUTO || s->step_fusion == LSM_FUSION_RESIDENT) && N <= fuse_below));
+            // ---- windowed gathers: the neighbour id ranges of every tile (lsm_window.cuh) ----
+            if (D == 2 && s->nbr16 && s->gather_variant == 2 && d->gather_window != LSM_WINDOW_OFF) {
+                std::vector<TileWin> tw(T);
+                std::vector<uint16_t> hw(E);
+                std::vector<int32_t> ids;
+                bool ok = true;
+                long long cap = 0;
+                for (long long t = 0; t < T && ok; ++t) {
+                    const long long p0 = t * kTile, p1 = std::min<long long>(s->Npad, p0 + kTile);
+                    const size_t e_lo = (size_t)hh[t].off[0] * kSlice, e_hi = (size_t)hh[t].off[kTileSlices] * kSlice;
+                    ids.clear();
+                    for (size_t e = e_lo; e < e_hi; ++e) ids.push_back(hn[e]);
+                    ids.push_back((int32_t)p0); ids.push_back((int32_t)(p1 - 1));
+                    std::sort(ids.begin(), ids.end());
+                    ids.erase(std::unique(ids.begin(), ids.end()), ids.end());
+                    // ranges: cut where more than 32 ids are skipped (never inside the own particles p0 .. p1-1); if that gives
+                    // more than kWinMaxSeg ranges, the smallest gaps are bridged
+                    TileWin &w = tw[t];
+                    std::memset(&w, 0, sizeof(w));
+                    std::vector<std::pair<long long, size_t>> cuts;      // (gap, index of the first id after the cut)
+                    for (size_t q = 1; q < ids.size(); ++q) {
+                        const bool own_gap = ids[q - 1] >= p0 && ids[q] < p1;
+                        if (ids[q] - ids[q - 1] > 32 && !own_gap) cuts.push_back({(long long)ids[q] - ids[q - 1], q});
+                    }
+                    if ((int)cuts.size() > kWinMaxSeg - 1) {
+                        std::sort(cuts.begin(), cuts.end(), [](const auto &a, const auto &b) { return a.first > b.first; });
+                        cuts.resize(kWinMaxSeg - 1);
+                    }
+                    std::sort(cuts.begin(), cuts.end(), [](const auto &a, const auto &b) { return a.second < b.second; });
+                    int nseg = 0;
+                    long long tot = 0;
+                    size_t first = 0;
+                    for (size_t c = 0; c <= cuts.size(); ++c) {
+                        const size_t last = (c < cuts.size() ? cuts[c].second : ids.size()) - 1;
+                        const long long len = (long long)ids[last] - ids[first] + 1;
+                        if (len > 65535) { ok = false; break; }
+                        w.start[nseg] = ids[first]; w.len[nseg] = (uint16_t)len; tot += len; ++nseg;
+                        first = last + 1;
+                    }
+                    if (tot > 4096) ok = false;                          // a window this wide would not leave two pipeline stages
+                    if (!ok || tot > 65535) { ok = false; break; }
+                    cap = std::max(cap, tot);
+                    auto index_of = [&](int32_t id) { long long o = 0; for (int q = 0; q < nseg; ++q) { if (id >= w.start[q] && id < w.start[q] + (int32_t)w.len[q]) return (uint16_t)(o + id - w.start[q]); o += w.len[q]; } return (uint16_t)0; };
+                    w.own_base = index_of((int32_t)p0);
+                    uint16_t ob = w.own_base;
+                    std::memcpy(hh[t].pad, &ob, 2);
+                    for (size_t e = e_lo; e < e_hi; ++e) hw[e] = index_of(hn[e]);
+                }
+                if (d->gather_window == LSM_WINDOW_ON && !ok) return fail(s, LSM_E_UNSUPPORTED, "gather_window = ON: a tile's neighbours do not form <= 4 short id ranges (numbering not banded)");
+                if (ok) {
+                    StageLayout LW = s->L;
+                    const int extra = ((int)((cap * 16 + 127) & ~127LL)) - kTile * 16;      // the window replaces the own-position block
+                    LW.vel += extra; LW.hdr += extra; LW.grp += extra; LW.nbr += extra; LW.thr += extra; LW.typ += extra; LW.kF += extra; LW.r0F += extra;
+                    LW.bytes += extra;
+                    int ctas = s->stream_ctas_per_sm;
+                    for (;; --ctas) {
+                        const int budget = std::min(dev_smem, (dev_smem + 1024) / ctas - 1024) - LW.first;
+                        LW.stages = std::min<int>(max_stages, budget / std::max(LW.bytes, 1));
+                        if (LW.stages >= 2 || ctas == 1) break;
+                    }
+                    if (LW.stages >= 2) {
+                        s->win_on = 1; s->win_cap = (int)cap; s->LW = LW;
+                        s->win_smem = LW.first + LW.stages * LW.bytes;
+                        s->win_grid = (int)std::min<long long>(T, (long long)ctas * n_sm);
+                        CUDA_TRY(s, cudaMemcpyAsync(s->hdr, hh.data(), sizeof(TileHdr) * T, cudaMemcpyHostToDevice, s->stream));   // own_base in the pad bytes
+                        TRY(upload(s, &s->d_win, tw));
+                        TRY(upload(s, &s->widx, hw));
+                        CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+                    } else if (d->gather_window == LSM_WINDOW_ON) return fail(s, LSM_E_UNSUPPORTED, "gather_window = ON: the windows do not fit two pipeline stages");
+                }
+            } else if (d->gather_window == LSM_WINDOW_ON) return fail(s, LSM_E_UNSUPPORTED, "gather_window = ON needs dim = 2, the streamed gather kernel and 16-bit neighbour offsets");
             // cluster-resident stepping: units (specimens) small enough for one thread-block cluster's shared memory
             const bool want_res = s->step_fusion == LSM_FUSION_RESIDENT || s->step_fusion == LSM_FUSION_AUTO;
             if (want_res && D == 2 && s->nbr16 && s->gather_variant == 2 && N <= 0x7FFFFFFF) {
@@ -1236,6 +1337,7 @@ lsm_status lsm_create(const lsm_desc *d, lsm_sim **out) {
     if (d->reorder == LSM_REORDER_BLOCKED && d->dim != 2) return fail(nullptr, LSM_E_UNSUPPORTED, "reorder = BLOCKED is 2-D only");
     if (d->force_mode < 0 || d->force_mode > LSM_FORCE_SCATTER_TILE) return fail(nullptr, LSM_E_INVALID, "bad force_mode");
     if (d->gather_variant < 0 || d->gather_variant > 2) return fail(nullptr, LSM_E_INVALID, "bad gather_variant");
+    if (d->gather_window < 0 || d->gather_window > 2) return fail(nullptr, LSM_E_INVALID, "bad gather_window");
     if (d->step_fusion < 0 || d->step_fusion > 3) return fail(nullptr, LSM_E_INVALID, "bad step_fusion");
     if (d->cluster_size != 0 && d->cluster_size != 1 && d->cluster_size != 2 && d->cluster_size != 4 && d->cluster_size != 8 && d->cluster_size != 16) return fail(nullptr, LSM_E_INVALID, "cluster_size must be 0 (auto), 1, 2, 4, 8 or 16");
     if ((d->alloc == nullptr) != (d->free_ == nullptr)) return fail(nullptr, LSM_E_INVALID, "alloc and free_ must be given together");
@@ -1642,6 +1744,8 @@ lsm_status lsm_get_info(lsm_sim *s, lsm_info *info) {
     info->pipeline_stages = s->gather_variant == 2 ? s->L.stages : 0;
     info->step_fusion = s->res_on ? 2 : s->multi_on;
     info->cluster_size = s->res_on ? s->res_cluster : 0;
+    info->window_particles = s->win_on ? s->win_cap : 0;
+    info->window_stages = s->win_on ? s->LW.stages : 0;
     info->resident_smem_bytes = s->res_on ? s->RL.bytes : 0;
     info->stage_bytes = s->gather_variant == 2 ? s->L.bytes : 0;
     info->param_mode = s->pm; info->n_types = s->ntypes; info->force_mode = s->force_mode == LSM_FORCE_SCATTER ? (s->scatter_variant == 1 ? LSM_FORCE_SCATTER_WARP : s->scatter_variant == 2 ? LSM_FORCE_SCATTER_TILE : LSM_FORCE_SCATTER) : s->force_mode; info->exact = s->exact;

@@ -50,7 +50,7 @@ enum ParamMode { PM_UNIFORM = 0, PM_TYPED = 1, PM_RCF = 2, PM_KRT_RCF = 3, PM_FU
 struct __align__(16) TileHdr {          // 64 bytes per tile of 256 particles
     uint32_t off[kTileSlices + 1];     // slot offset (units of 32 entries) of each slice, and the end of the tile
     uint8_t w[kTileSlices];            // live width of each slice (shrinks under compaction)
-    uint8_t pad[20];
+    uint8_t pad[20];                   // pad[0..1]: window index of the tile's first particle (lsm_window.cuh)
 };
 static_assert(sizeof(TileHdr) == 64, "TileHdr must be 64 bytes");
 
@@ -105,6 +105,7 @@ struct StepParams {
     long long T;  // tiles
     int32_t *nbr;
     int16_t *nbr16;   // same list as 16-bit offsets (neighbour - self), present when every offset fits: the streamed copy
+    uint16_t *widx;   // same list as window indices (lsm_window.cuh), or NULL; kept consistent by whoever kills a spring
     const int32_t *sid;
     SpringParams sp;
     // breakage bookkeeping
@@ -383,6 +384,7 @@ __device__ __forceinline__ void row_careful(const StepParams &P, const StepVar &
             if (__dsqrt_rn(r2) > rc) {   // strict '>' (Q1)
                 P.nbr[e] = p;                             // dead from now on: the slot points at its own particle
                 if (P.nbr16) P.nbr16[e] = 0;
+                if (P.widx) { uint16_t ob; memcpy(&ob, P.hdr[p >> 8].pad, 2); P.widx[e] = (uint16_t)(ob + (p & (kTile - 1))); }
                 if (I16) const_cast<int16_t *>(R.nbr16)[so] = 0;   // and the staged copy (resident tiles are not reloaded)
                 else const_cast<int32_t *>(R.nbr)[so] = p;
                 if (p < nb) {
@@ -944,6 +946,7 @@ struct CompactParams {
     uint16_t *thr;
     double *kF, *r0F;
     long long nslices;
+    uint16_t *widx;        // window indices of the windowed kernel (NULL when unused); a free slot holds the particle's own index
 };
 
 __global__ void __launch_bounds__(kBlock) k_compact_ell(const CompactParams C) {
@@ -964,6 +967,7 @@ __global__ void __launch_bounds__(kBlock) k_compact_ell(const CompactParams C) {
                 const size_t d = e0 + (size_t)j * kSlice;
                 C.nbr[d] = nb; C.sid[d] = C.sid[e];
                 if (C.nbr16) C.nbr16[d] = C.nbr16[e];
+                if (C.widx) C.widx[d] = C.widx[e];
                 if (C.typ) C.typ[d] = C.typ[e];
                 if (C.thr) C.thr[d] = C.thr[e];
                 if (C.kF) C.kF[d] = C.kF[e];
@@ -972,7 +976,13 @@ __global__ void __launch_bounds__(kBlock) k_compact_ell(const CompactParams C) {
             ++j;
         }
     }
-    for (unsigned s = j; s < w; ++s) { C.nbr[e0 + (size_t)s * kSlice] = self; if (C.nbr16) C.nbr16[e0 + (size_t)s * kSlice] = 0; }
+    uint16_t own_idx = 0;
+    if (C.widx) { uint16_t ob; memcpy(&ob, h->pad, 2); own_idx = (uint16_t)(ob + wi * kSlice + lane); }   // TileHdr.pad[0..1] = window index of the tile's first particle
+    for (unsigned s = j; s < w; ++s) {
+        C.nbr[e0 + (size_t)s * kSlice] = self;
+        if (C.nbr16) C.nbr16[e0 + (size_t)s * kSlice] = 0;
+        if (C.widx) C.widx[e0 + (size_t)s * kSlice] = own_idx;
+    }
     unsigned wmax = j;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) wmax = max(wmax, __shfl_xor_sync(0xffffffffu, wmax, o));

@@ -25,7 +25,7 @@ def test_library_exports_every_declared_symbol():
     assert set(names) == set(lsm.EXPORTS)
     for n in names:
         assert hasattr(L, n), n
-    assert lsm.lsm_abi_version() == 4
+    assert lsm.lsm_abi_version() == 5
 
 
 def test_desc_layout_matches_header_field_order():

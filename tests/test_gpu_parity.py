@@ -509,11 +509,14 @@ def test_gather_variants_and_step_fusion_bit_identical_in_exact_mode():
     xo, vo = o.read_state(); bo, bso, nbo = o.read_broken()
     assert nbo > 0
     ho = o.read_stress()
-    for kw in (dict(gather_variant=lsm.GATHER_DIRECT), dict(gather_variant=lsm.GATHER_STREAMED, step_fusion=lsm.FUSION_OFF),
+    for kw in (dict(gather_variant=lsm.GATHER_DIRECT), dict(gather_variant=lsm.GATHER_STREAMED, step_fusion=lsm.FUSION_OFF, gather_window=lsm.WINDOW_OFF),
+               dict(gather_variant=lsm.GATHER_STREAMED, step_fusion=lsm.FUSION_OFF, gather_window=lsm.WINDOW_ON, compact_every=450),
+               dict(gather_variant=lsm.GATHER_STREAMED, step_fusion=lsm.FUSION_OFF, gather_window=lsm.WINDOW_ON, reorder=2),
                dict(gather_variant=lsm.GATHER_STREAMED, step_fusion=lsm.FUSION_ON)):
         g = lsm_create_from_problem(p, exact=True, **kw)
         inf = g.info()
         assert inf["step_fusion"] == (1 if kw.get("step_fusion") == lsm.FUSION_ON else 0)
+        assert (inf["window_particles"] > 0) == (kw.get("gather_window") == lsm.WINDOW_ON or kw.get("step_fusion") == lsm.FUSION_ON)
         g.step(1700); g.step(1); g.step(nsteps - 1701)        # odd / even run lengths, a 1-step call
         xg, vg = g.read_state(); bg, bsg, nbg = g.read_broken()
         assert np.array_equal(xo, xg) and np.array_equal(vo, vg)
@@ -702,6 +705,30 @@ def test_large_config5_first_steps(n):
     eps = np.finfo(np.float64).eps
     assert np.abs(xg - xo).max() <= 32 * eps * np.abs(xo).max() and np.abs(vg - vo).max() <= 1e-12
     assert g.n_broken() == o.read_broken()[2] == 0
+    g.close()
+
+
+def test_windowed_gathers_fast_mode_and_refusal():
+    """Neighbour windows staged in shared memory (lsm_window.cuh) vs gathers from global memory: the same arithmetic on
+    the same numbers, so fast mode is bit-identical too, through breakage and compaction, per-spring rc (config 3
+    recipe) and typed parameters in a batch; a shuffled numbering has no windows: ON is refused, AUTO falls back."""
+    for p, kw in ((config3(n=256, strain_per_step=1.2e-5), dict()), (config4(B=3, n=64), dict(step_fusion=lsm.FUSION_OFF))):
+        p.sample_every = 100
+        a = lsm_create_from_problem(p, gather_window=lsm.WINDOW_ON, compact_every=500, step_fusion=lsm.FUSION_OFF)
+        b = lsm_create_from_problem(p, gather_window=lsm.WINDOW_OFF, compact_every=500, step_fusion=lsm.FUSION_OFF)
+        assert a.info()["window_particles"] > 256 and b.info()["window_particles"] == 0
+        a.step(3500); b.step(3500)
+        xa, va = a.read_state(); xb, vb = b.read_state()
+        assert np.array_equal(xa, xb) and np.array_equal(va, vb) and np.array_equal(a.read_broken()[1], b.read_broken()[1])
+        ha, hb = a.read_stress(), b.read_stress()
+        assert np.array_equal(ha["U"], hb["U"]) and np.array_equal(ha["R"], hb["R"])
+        a.close(); b.close()
+    q = shuffle_ids(config2(n=256, n_blobs=40), 5)
+    with pytest.raises(lsm.LsmError) as ei:
+        lsm_create_from_problem(q, gather_window=lsm.WINDOW_ON)
+    assert ei.value.status == -7
+    g = lsm_create_from_problem(q)
+    assert g.info()["window_particles"] == 0
     g.close()
 
 
