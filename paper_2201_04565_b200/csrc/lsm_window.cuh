@@ -55,6 +55,7 @@ __device__ __forceinline__ void row_careful_w(const StepParams &P, const WinPara
                 P.nbr[e] = p;                                 // dead from now on: every copy of the slot points at its own particle
                 P.nbr16[e] = 0;
                 W.widx[e] = (uint16_t)own_idx;
+                reinterpret_cast<uint16_t *>(const_cast<int16_t *>(R.nbr16))[so] = (uint16_t)own_idx;   // and the staged copy
                 if (p < nb) {
                     P.break_step[P.sid[e]] = step;
                     atomicAdd(P.nbroken + spec_of(P.poff, P.B, p), 1ULL);
