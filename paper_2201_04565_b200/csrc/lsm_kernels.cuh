@@ -23,6 +23,8 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <type_traits>
+#include <utility>
 
 namespace lsmk {
 
@@ -250,6 +252,34 @@ __device__ __forceinline__ void particle_update(const StepParams &P, const StepV
 // Two kernels share the row evaluation below: k_gather_step reads the slot streams straight from global memory;
 // k_gather_stream (the product path) stages them tile by tile through shared memory with bulk async copies.
 // ---------------------------------------------------------------------------------------------------------------
+// ---- shared-memory row access with 32-bit addresses and immediate offsets (no generic-pointer arithmetic in the hot loop) ----
+template <int OFF> __device__ __forceinline__ int lds_s16o(uint32_t a) { int v; asm volatile("ld.shared.s16 %0, [%1+%2];" : "=r"(v) : "r"(a), "n"(OFF)); return v; }
+template <int OFF> __device__ __forceinline__ uint32_t lds_u16o(uint32_t a) { uint32_t v; asm volatile("ld.shared.u16 %0, [%1+%2];" : "=r"(v) : "r"(a), "n"(OFF)); return v; }
+template <int OFF> __device__ __forceinline__ uint32_t lds_u8o(uint32_t a) { uint32_t v; asm volatile("ld.shared.u8 %0, [%1+%2];" : "=r"(v) : "r"(a), "n"(OFF)); return v; }
+template <int OFF> __device__ __forceinline__ uint32_t lds_u32o(uint32_t a) { uint32_t v; asm volatile("ld.shared.u32 %0, [%1+%2];" : "=r"(v) : "r"(a), "n"(OFF)); return v; }
+template <int OFF> __device__ __forceinline__ double lds_f64o(uint32_t a) { double v; asm volatile("ld.shared.f64 %0, [%1+%2];" : "=d"(v) : "r"(a), "n"(OFF)); return v; }
+
+// compile-time loop 0 .. N-1 (the index is usable as a template argument: immediate offsets of the loads below)
+template <int N, int I = 0, class F> __device__ __forceinline__ void static_for(F &&f) {
+    if constexpr (I < N) { f(std::integral_constant<int, I>{}); static_for<N, I + 1>(f); }
+}
+
+struct RowS { uint32_t nbr, thr, typ, kF, r0F; };   // shared addresses of this lane's entry in the current slot of each row array
+
+__device__ __forceinline__ uint2 lds_u2(uint32_t addr) {
+    uint2 v;
+    asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ uint32_t lds_u8(uint32_t addr) {
+    uint32_t v;
+    asm volatile("ld.shared.u8 %0, [%1];" : "=r"(v) : "r"(addr));
+    return v;
+}
+
+__device__ __forceinline__ int lds_s32_at(uint32_t a) { int v; asm volatile("ld.shared.s32 %0, [%1];" : "=r"(v) : "r"(a)); return v; }
+template <int OFF> __device__ __forceinline__ int lds_s32o(uint32_t a) { int v; asm volatile("ld.shared.s32 %0, [%1+%2];" : "=r"(v) : "r"(a), "n"(OFF)); return v; }
+
 struct RowSrc {            // where one particle's row lives: pointers already offset to (slice offset)*32 + lane
     const int32_t *nbr;    // slot s at nbr[s*32]  (global memory, or the staged shared-memory copy)
     const int16_t *nbr16;  // I16: the staged copy holds 16-bit offsets (neighbour - self) instead
@@ -409,6 +439,51 @@ __device__ __forceinline__ void row_forces(const StepParams &P, const StepVar &V
     for (; s0 + CH <= w; s0 += CH) any_near |= row_chunk<PM, EXACT, SAMPLE, GM, I16, CH>(P, V, R, s_tab, p, s0, xp, fx, fy, u);
     for (; s0 < w; ++s0) any_near |= row_chunk<PM, EXACT, SAMPLE, GM, I16, 1>(P, V, R, s_tab, p, s0, xp, fx, fy, u);
     if (any_near) row_careful<PM, EXACT, SAMPLE, GM, I16>(P, V, R, s_tab, p, w, xp, fx, fy, u);
+}
+
+// The same chunk for the streamed kernel's consumers: the row comes from the pipeline stage through 32-bit shared
+// addresses with immediate offsets (no generic-pointer arithmetic per slot), the neighbour positions from global memory.
+template <int PM, bool EXACT, bool SAMPLE, int GM, bool I16, int CH>
+__device__ __forceinline__ bool row_chunk_g(const StepParams &P, const StepVar &V, const RowS &A, uint32_t tab_s, int p, double2 xp,
+                                            double &fx, double &fy, double &u) {
+    constexpr bool kTab = (PM == PM_TYPED || PM == PM_KRT_RCF);
+    constexpr bool kHasThr = (PM == PM_RCF || PM == PM_KRT_RCF || PM == PM_FULL);
+    int nb[CH];
+    double2 xq[CH];
+    bool any_near = false;
+    const double2 *own = V.pos_cur + p;
+    asm("" : "+l"(own));   // keep the own address in a register pair: each gather address is then one wide multiply-add
+    static_for<CH>([&](auto ic) { constexpr int C = decltype(ic)::value; nb[C] = I16 ? lds_s16o<C * kSlice * 2>(A.nbr) : lds_s32o<C * kSlice * 4>(A.nbr); });
+#pragma unroll
+    for (int c = 0; c < CH; ++c) {
+        xq[c] = I16 ? (GM == GM_GLOBAL_CG ? __ldcg(own + nb[c]) : __ldg(own + nb[c])) : gather_pos<GM>(V, nb[c]);
+        if (I16) nb[c] += p;
+    }
+    static_for<CH>([&](auto ic) {
+        constexpr int C = decltype(ic)::value;
+        double k, r0 = 0.0, kr0, dx, dy, r2, g, ue;
+        uint32_t thr;
+        bool near;
+        if constexpr (kTab) {
+            const uint32_t ta = tab_s + lds_u8o<C * kSlice>(A.typ) * (uint32_t)(kTabStride * 8);
+            const double2 kk = lds_d2(ta);
+            k = kk.x; kr0 = kk.y;
+            if (EXACT || SAMPLE) r0 = lds_f64o<24>(ta);
+            thr = PM == PM_TYPED ? lds_u32o<16>(ta) : P.sp.thr_base + lds_u16o<C * kSlice * 2>(A.thr) * P.sp.thr_mul;
+        } else if constexpr (PM == PM_FULL) {
+            k = lds_f64o<C * kSlice * 8>(A.kF); r0 = lds_f64o<C * kSlice * 8>(A.r0F); kr0 = k * r0;
+            thr = P.sp.thr_base + lds_u16o<C * kSlice * 2>(A.thr) * P.sp.thr_mul;
+        } else {
+            k = P.sp.k_u; r0 = P.sp.r0_u; kr0 = P.sp.kr0_u;
+            thr = kHasThr ? P.sp.thr_base + lds_u16o<C * kSlice * 2>(A.thr) * P.sp.thr_mul : P.sp.thr_u;
+        }
+        slot_eval<EXACT, SAMPLE>(xq[C], xp, p < nb[C], k, r0, kr0, thr, dx, dy, r2, g, ue, near);
+        fx = mad<EXACT>(g, dx, fx);
+        fy = mad<EXACT>(g, dy, fy);
+        if (SAMPLE) u = add<EXACT>(u, ue);
+        any_near |= near;
+    });
+    return any_near;
 }
 
 // Direct variant: block = tile, every stream read from global memory by the thread that needs it.
@@ -610,7 +685,29 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
                 } else {
                     const double2 xp = reinterpret_cast<const double2 *>(b + L.pos)[tid];
                     double fx = 0.0, fy = 0.0, uu = 0.0;
-                    row_forces<PM, EXACT, SAMPLE, MULTI ? GM_GLOBAL_CG : GM_GLOBAL_NC, I16>(P, V, R, s_tab, (int)p, w, xp, fx, fy, uu);
+                    if constexpr (MULTI) {   // cooperative multi-step launches: measured 3.5 % faster with the generic-pointer row code
+                        row_forces<PM, EXACT, SAMPLE, GM_GLOBAL_CG, I16>(P, V, R, s_tab, (int)p, w, xp, fx, fy, uu);
+                    } else {   // the row: chunks of LSM_ROW_CH springs through 32-bit shared addresses, then the careful pass if needed
+                        constexpr int GMv = GM_GLOBAL_NC;
+                        constexpr unsigned kIdB = I16 ? 2 : 4;
+                        const uint32_t b_s = smem_u32(b);
+                        RowS A;
+                        A.nbr = b_s + (uint32_t)L.nbr + rel * kIdB; A.thr = b_s + (uint32_t)L.thr + rel * 2; A.typ = b_s + (uint32_t)L.typ + rel;
+                        A.kF = b_s + (uint32_t)L.kF + rel * 8; A.r0F = b_s + (uint32_t)L.r0F + rel * 8;
+                        const uint32_t tab_s = smem_u32(s_tab);
+                        constexpr int CH = LSM_ROW_CH;
+                        bool any_near = false;
+                        unsigned s0 = 0;
+                        for (; s0 + CH <= w; s0 += CH) {
+                            any_near |= row_chunk_g<PM, EXACT, SAMPLE, GMv, I16, CH>(P, V, A, tab_s, (int)p, xp, fx, fy, uu);
+                            A.nbr += CH * kSlice * kIdB; A.thr += CH * kSlice * 2; A.typ += CH * kSlice; A.kF += CH * kSlice * 8; A.r0F += CH * kSlice * 8;
+                        }
+                        for (; s0 < w; ++s0) {
+                            any_near |= row_chunk_g<PM, EXACT, SAMPLE, GMv, I16, 1>(P, V, A, tab_s, (int)p, xp, fx, fy, uu);
+                            A.nbr += kSlice * kIdB; A.thr += kSlice * 2; A.typ += kSlice; A.kF += kSlice * 8; A.r0F += kSlice * 8;
+                        }
+                        if (any_near) row_careful<PM, EXACT, SAMPLE, GMv, I16>(P, V, R, s_tab, (int)p, w, xp, fx, fy, uu);
+                    }
                     const double2 vh = reinterpret_cast<const double2 *>(b + L.vel)[tid];
                     const uint8_t g = (b + L.grp)[tid];
                     if (MULTI && M.resident)

@@ -26,8 +26,6 @@
 //   * Only plain time steps run here; sample steps, the last step of an lsm_step call and compaction are the streamed
 //     kernel's (one launch each), exactly as for the cooperative multi-step launch.
 #pragma once
-#include <type_traits>
-#include <utility>
 #include "lsm_kernels.cuh"
 
 namespace lsmk {
@@ -86,30 +84,6 @@ template <class T> __device__ __forceinline__ void res_copy16(void *dst, const T
 }
 
 __device__ __forceinline__ void cluster_arrive_relaxed() { asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory"); }
-__device__ __forceinline__ uint2 lds_u2(uint32_t addr) {
-    uint2 v;
-    asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr));
-    return v;
-}
-__device__ __forceinline__ uint32_t lds_u8(uint32_t addr) {
-    uint32_t v;
-    asm volatile("ld.shared.u8 %0, [%1];" : "=r"(v) : "r"(addr));
-    return v;
-}
-
-// ---- shared-memory row access with 32-bit addresses and immediate offsets (no generic-pointer arithmetic in the hot loop) ----
-template <int OFF> __device__ __forceinline__ int lds_s16o(uint32_t a) { int v; asm volatile("ld.shared.s16 %0, [%1+%2];" : "=r"(v) : "r"(a), "n"(OFF)); return v; }
-template <int OFF> __device__ __forceinline__ uint32_t lds_u16o(uint32_t a) { uint32_t v; asm volatile("ld.shared.u16 %0, [%1+%2];" : "=r"(v) : "r"(a), "n"(OFF)); return v; }
-template <int OFF> __device__ __forceinline__ uint32_t lds_u8o(uint32_t a) { uint32_t v; asm volatile("ld.shared.u8 %0, [%1+%2];" : "=r"(v) : "r"(a), "n"(OFF)); return v; }
-template <int OFF> __device__ __forceinline__ uint32_t lds_u32o(uint32_t a) { uint32_t v; asm volatile("ld.shared.u32 %0, [%1+%2];" : "=r"(v) : "r"(a), "n"(OFF)); return v; }
-template <int OFF> __device__ __forceinline__ double lds_f64o(uint32_t a) { double v; asm volatile("ld.shared.f64 %0, [%1+%2];" : "=d"(v) : "r"(a), "n"(OFF)); return v; }
-
-// compile-time loop 0 .. N-1 (the index is usable as a template argument: immediate offsets of the loads below)
-template <int N, int I = 0, class F> __device__ __forceinline__ void static_for(F &&f) {
-    if constexpr (I < N) { f(std::integral_constant<int, I>{}); static_for<N, I + 1>(f); }
-}
-
-struct RowS { uint32_t nbr, thr, typ, kF, r0F; };   // shared addresses of this lane's entry in the current slot of each row array
 
 // CH springs of one row from the resident copy: the arithmetic of row_chunk (slot_eval, same accumulation order), the
 // loads spelled as ld.shared [reg + immediate].  pos_p: shared address of the particle's own position in the current buffer.
