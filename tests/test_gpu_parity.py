@@ -161,10 +161,14 @@ def test_T7_reorder_compaction_shuffle_transparent(mode):
     xo, vo = o.read_state(); bo, bso, nbo = o.read_broken()
     assert nbo > 0
     first = bso[bso >= 0].min()
+    oq = OracleSim.from_problem(q); oq.step(nsteps)         # the oracle on the shuffled arrays themselves (its own summation order)
+    xoq, voq = oq.read_state(); bsoq = oq.read_broken()[1]
     for prob, reorder, compact in [(p, 1, 0), (p, 0, 300), (q, 1, 300), (q, 0, 0), (q, 2, 300), (p, 2, 0), (q, 3, 300), (p, 3, 0)]:
         g = lsm_create_from_problem(prob, reorder=reorder, compact_every=compact, **mode)
         g.step(nsteps)
         xg, vg = g.read_state(); bg, bsg, nbg = g.read_broken()
+        if mode["exact"] and prob is q:     # bit-identical to the oracle run on the same (shuffled) input, whatever the renumbering
+            assert np.array_equal(xg, xoq) and np.array_equal(vg, voq) and np.array_equal(bsg, bsoq)
         if prob is q:       # translate back to p's numbering
             xg2 = np.empty_like(xg); xg2[q.meta["perm"]] = xg; xg = xg2
             bs2 = np.empty_like(bsg); bs2[q.meta["spring_perm"]] = bsg; bsg = bs2
