@@ -227,4 +227,154 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_win(const St
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// Several plain time steps in ONE cooperative launch for L2-resident lattices, with windows (k_coop_win).
+// Every CTA keeps its tiles' rows, velocities and group bytes in its pipeline stages for the whole launch (as the resident
+// mode of k_gather_stream<MULTI> does) and re-fetches only the position WINDOW of each tile per step, by bulk async copy
+// from the position buffer all CTAs have just written -- after the same grid barrier (one global arrival counter).  The
+// consumers then gather from shared memory instead of paying an L2 round trip per tile behind the barrier.
+// ---------------------------------------------------------------------------------------------------------------
+struct CoopWinParams {
+    const TileWin *win;
+    uint16_t *widx;
+    unsigned long long *gbar;          // global arrival counter (monotonic across launches)
+    unsigned long long gbar_base;      // its value before this launch
+    double2 *pos_a, *pos_b;            // step i reads pos_a / writes pos_b when i is even, the reverse when odd
+    int nsteps;
+};
+
+template <int PM, bool EXACT>
+__global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_coop_win(const StepParams P, const StageLayout L, const CoopWinParams Q) {
+    constexpr bool kTab = (PM == PM_TYPED || PM == PM_KRT_RCF);
+    constexpr bool kHasThr = (PM == PM_RCF || PM == PM_KRT_RCF || PM == PM_FULL);
+    constexpr bool kHasKR = (PM == PM_FULL);
+    extern __shared__ __align__(128) unsigned char smem[];
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem);          // [kMaxStages] window (and, first, whole tile) landed
+    uint64_t *stepdone = full + 2 * kMaxStages;                    // all consumer warps finished the step
+    double *s_tab = reinterpret_cast<double *>(smem + kStreamHdrBytes);
+    unsigned char *stage0 = smem + L.first;
+    const int tid = threadIdx.x, wi = tid >> 5, lane = tid & 31;
+    if (tid == 0) {
+        for (int s = 0; s < L.stages; ++s) mbar_init(full + s, 1);
+        mbar_init(stepdone, kTileSlices);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (kTab) for (int i = tid; i < kTabStride * P.sp.ntypes; i += kTile + 32) s_tab[i] = P.sp.tab[i];
+    __syncthreads();
+    const WinParams W{Q.win, Q.widx, L.pos};
+
+    if (wi == kTileSlices) {  // ---------------- producer warp ----------------
+        for (int it = 0; it < Q.nsteps; ++it) {
+            const double2 *pos_cur = (it & 1) ? Q.pos_b : Q.pos_a;
+            if (it > 0 && lane == 0) {   // grid barrier: every CTA has finished (and published) step it - 1
+                mbar_wait(stepdone, (unsigned)(it - 1) & 1u);
+                __threadfence();
+                atomicAdd(Q.gbar, 1ULL);
+                const unsigned long long target = Q.gbar_base + (unsigned long long)it * gridDim.x;
+                while (*reinterpret_cast<volatile unsigned long long *>(Q.gbar) < target) { }
+                __threadfence();
+                asm volatile("fence.proxy.async;" ::: "memory");          // their generic-proxy stores before our bulk copies
+            }
+            if (lane == 0) {
+                int s = 0;
+                for (long long t = blockIdx.x; t < P.T; t += gridDim.x, ++s) {
+                    const TileWin tw = Q.win[t];
+                    unsigned nwin = 0;
+#pragma unroll
+                    for (int q = 0; q < kWinMaxSeg; ++q) nwin += tw.len[q];
+                    unsigned char *b = stage0 + (size_t)s * L.bytes;
+                    unsigned bytes = nwin * 16;
+                    const TileHdr *h = P.hdr + t;
+                    const uint32_t o0 = h->off[0], ns = h->off[kTileSlices] - h->off[0];
+                    if (it == 0) {
+                        bytes += kTile * 16 + kTile + 64 + ns * (kSlice * 2);
+                        if (kHasThr) bytes += ns * (kSlice * 2);
+                        if (kTab) bytes += ns * kSlice;
+                        if (kHasKR) bytes += 2 * ns * (kSlice * 8);
+                    }
+                    mbar_expect_tx(full + s, bytes);
+                    unsigned woff = 0;
+#pragma unroll
+                    for (int q = 0; q < kWinMaxSeg; ++q)
+                        if (tw.len[q]) { bulk_g2s(b + L.pos + woff * 16, pos_cur + tw.start[q], tw.len[q] * 16u, full + s); woff += tw.len[q]; }
+                    if (it == 0) {   // rows, velocities and group bytes stay for the whole launch
+                        bulk_g2s(b + L.vel, reinterpret_cast<const char *>(P.vel) + t * (kTile * 16), kTile * 16, full + s);
+                        bulk_g2s(b + L.grp, P.grp + t * kTile, kTile, full + s);
+                        bulk_g2s(b + L.hdr, h, 64, full + s);
+                        if (ns) {
+                            const size_t e = (size_t)o0 * kSlice;
+                            bulk_g2s(b + L.nbr, Q.widx + e, ns * (kSlice * 2), full + s);
+                            if (kHasThr) bulk_g2s(b + L.thr, P.sp.thr + e, ns * (kSlice * 2), full + s);
+                            if (kTab) bulk_g2s(b + L.typ, P.sp.typ + e, ns * kSlice, full + s);
+                            if (kHasKR) {
+                                bulk_g2s(b + L.kF, P.sp.kF + e, ns * (kSlice * 8), full + s);
+                                bulk_g2s(b + L.r0F, P.sp.r0F + e, ns * (kSlice * 8), full + s);
+                            }
+                        }
+                    }
+                }
+            }
+            __syncwarp();
+        }
+        return;
+    }
+    // ---------------- consumer warps: thread = particle ----------------
+    const uint32_t stage_s0 = smem_u32(stage0), tab_s = smem_u32(s_tab);
+    for (int it = 0; it < Q.nsteps; ++it) {
+        StepVar V;
+        V.pos_cur = (it & 1) ? Q.pos_b : Q.pos_a; V.pos_next = (it & 1) ? Q.pos_a : Q.pos_b; V.step = P.step + it; V.pos_s = 0u;
+        const bool last = it + 1 == Q.nsteps;
+        int s = 0;
+        for (long long t = blockIdx.x; t < P.T; t += gridDim.x, ++s) {
+            mbar_wait(full + s, (unsigned)it & 1u);
+            const uint32_t b_s = stage_s0 + (uint32_t)s * (uint32_t)L.bytes;
+            const long long p = t * kTile + tid;
+            if (p < P.N) {
+                const uint32_t hdr_s = b_s + (uint32_t)L.hdr;
+                const unsigned w = lds_u8(hdr_s + 36u + (uint32_t)wi);
+                const uint32_t off_w = lds_u32o<0>(hdr_s + (uint32_t)wi * 4u), off_0 = lds_u32o<0>(hdr_s);
+                const unsigned own_idx = (lds_u32o<44>(hdr_s) & 0xFFFFu) + (unsigned)tid;
+                const unsigned rel = (off_w - off_0) * kSlice + lane;
+                const uint32_t win_s = b_s + (uint32_t)L.pos;
+                const uint32_t vel_a = b_s + (uint32_t)L.vel + (uint32_t)tid * 16u;
+                const double2 xp = lds_d2(win_s + own_idx * 16u);
+                const double2 vh = lds_d2(vel_a);
+                const uint8_t g = (uint8_t)lds_u8(b_s + (uint32_t)L.grp + (uint32_t)tid);
+                RowS A;
+                A.nbr = b_s + (uint32_t)L.nbr + rel * 2; A.thr = b_s + (uint32_t)L.thr + rel * 2; A.typ = b_s + (uint32_t)L.typ + rel;
+                A.kF = b_s + (uint32_t)L.kF + rel * 8; A.r0F = b_s + (uint32_t)L.r0F + rel * 8;
+                double fx = 0.0, fy = 0.0;
+                bool any_near = false;
+                constexpr int CH = LSM_ROW_CH;
+                unsigned s0 = 0;
+                for (; s0 + CH <= w; s0 += CH) {
+                    any_near |= row_chunk_w<PM, EXACT, CH>(P, A, tab_s, win_s, xp, fx, fy);
+                    A.nbr += CH * kSlice * 2; A.thr += CH * kSlice * 2; A.typ += CH * kSlice; A.kF += CH * kSlice * 8; A.r0F += CH * kSlice * 8;
+                }
+                for (; s0 < w; ++s0) {
+                    any_near |= row_chunk_w<PM, EXACT, 1>(P, A, tab_s, win_s, xp, fx, fy);
+                    A.nbr += kSlice * 2; A.thr += kSlice * 2; A.typ += kSlice; A.kF += kSlice * 8; A.r0F += kSlice * 8;
+                }
+                if (any_near) {
+                    unsigned char *b = stage0 + (size_t)s * L.bytes;
+                    RowSrc R;
+                    R.nbr = nullptr;
+                    R.nbr16 = reinterpret_cast<const int16_t *>(b + L.nbr) + rel;
+                    R.thr = reinterpret_cast<const uint16_t *>(b + L.thr) + rel;
+                    R.typ = (b + L.typ) + rel;
+                    R.kF = reinterpret_cast<const double *>(b + L.kF) + rel;
+                    R.r0F = reinterpret_cast<const double *>(b + L.r0F) + rel;
+                    R.e0 = (size_t)off_w * kSlice + lane;
+                    row_careful_w<PM, EXACT>(P, W, V.step, R, s_tab, win_s, (int)p, own_idx, w, xp, fx, fy);
+                }
+                const Upd o = particle_math<EXACT, true, true, false>(P, V.step, p, xp, vh, g, fx, fy);
+                V.pos_next[p] = o.xn;                                   // the neighbours' (and our own) next windows come from here
+                if (g == kFree) { sts_d2(vel_a, o.w); if (last) P.vel[p] = o.w; }
+            }
+            __syncwarp();
+        }
+        if (!last) { __syncwarp(); if (lane == 0) mbar_arrive(stepdone); }
+    }
+}
+
 }  // namespace lsmk

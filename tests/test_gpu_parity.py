@@ -949,6 +949,29 @@ def test_3d_oscillator_and_unsupported_combinations():
         assert ei.value.status == -7
 
 
+def test_cooperative_launch_with_windows_bit_identical():
+    """A lattice with more tiles than CTAs under cooperative multi-step launches: the windows of every tile are re-fetched
+    by bulk copy after each grid barrier (k_coop_win) instead of gathering from L2.  Exact mode through fracture,
+    compaction and odd / even run lengths; fast mode == one launch per step bit for bit."""
+    p = config2(n=384, seed=11, n_blobs=80, du_y=8e-3)
+    p.sample_every = 50
+    nsteps = 1200
+    o = OracleSim.from_problem(p); o.set_threads(8); o.step(nsteps)
+    xo, vo = o.read_state(); bso, nbo = o.read_broken()[1:]
+    assert nbo > 0
+    g = lsm_create_from_problem(p, exact=True, step_fusion=lsm.FUSION_ON, compact_every=350)
+    inf = g.info()
+    assert inf["step_fusion"] == 1 and inf["window_particles"] > 0 and (p.N + 255) // 256 > 3 * 148
+    g.step(601); g.step(1); g.step(nsteps - 602)
+    xg, vg = g.read_state()
+    assert np.array_equal(xo, xg) and np.array_equal(vo, vg) and np.array_equal(bso, g.read_broken()[1])
+    g.close()
+    a = lsm_create_from_problem(p, step_fusion=lsm.FUSION_ON); a.step(700)
+    b = lsm_create_from_problem(p, step_fusion=lsm.FUSION_OFF); b.step(700)
+    assert np.array_equal(a.read_state()[0], b.read_state()[0]) and np.array_equal(a.read_state()[1], b.read_state()[1])
+    a.close(); b.close()
+
+
 def test_step_fusion_non_resident_pipeline_large_lattice():
     """Forced step fusion on a lattice too large for its tiles to stay resident in shared memory (T > CTAs x stages):
     the fused launch then refills its pipeline from global memory after every grid barrier (generic-proxy stores ->
