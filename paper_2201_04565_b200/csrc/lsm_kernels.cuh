@@ -538,6 +538,14 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned by
                  ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
+// Grid barrier of the cooperative multi-step launches, one thread per CTA: a release-add on a global arrival counter (this
+// CTA's stores, observed through its step barrier, become visible first), then acquire-polls until every CTA has arrived.
+__device__ __forceinline__ void grid_arrive_and_wait(unsigned long long *ctr, unsigned long long target) {
+    asm volatile("red.release.gpu.global.add.u64 [%0], 1;" ::"l"(ctr) : "memory");
+    unsigned long long v;
+    do { asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(ctr) : "memory"); } while (v < target);
+}
+
 struct StageLayout {      // byte offsets of the staged arrays inside one pipeline stage (all multiples of 128)
     int pos, vel, hdr, grp, nbr, thr, typ, kF, r0F;
     int bytes;            // stage size
@@ -602,11 +610,7 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
                 const double2 *pos_cur = MULTI ? ((it & 1) ? M.pos_b : M.pos_a) : P.pos_cur;
                 if (MULTI && it > 0) {  // grid barrier: every CTA has finished (and published) step it-1
                     mbar_wait(stepdone, (it - 1) & 1);
-                    __threadfence();
-                    atomicAdd(M.gbar, 1ULL);
-                    const unsigned long long target = M.gbar_base + (unsigned long long)it * gridDim.x;
-                    while (*reinterpret_cast<volatile unsigned long long *>(M.gbar) < target) { }
-                    __threadfence();
+                    grid_arrive_and_wait(M.gbar, M.gbar_base + (unsigned long long)it * gridDim.x);
                     asm volatile("fence.proxy.async;" ::: "memory");
                     if (M.resident) { mbar_arrive(go); continue; }   // nothing to copy: the consumers own the staged tiles
                 }

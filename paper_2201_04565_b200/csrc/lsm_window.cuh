@@ -268,11 +268,7 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_coop_win(const Step
             const double2 *pos_cur = (it & 1) ? Q.pos_b : Q.pos_a;
             if (it > 0 && lane == 0) {   // grid barrier: every CTA has finished (and published) step it - 1
                 mbar_wait(stepdone, (unsigned)(it - 1) & 1u);
-                __threadfence();
-                atomicAdd(Q.gbar, 1ULL);
-                const unsigned long long target = Q.gbar_base + (unsigned long long)it * gridDim.x;
-                while (*reinterpret_cast<volatile unsigned long long *>(Q.gbar) < target) { }
-                __threadfence();
+                grid_arrive_and_wait(Q.gbar, Q.gbar_base + (unsigned long long)it * gridDim.x);
                 asm volatile("fence.proxy.async;" ::: "memory");          // their generic-proxy stores before our bulk copies
             }
             if (lane == 0) {
