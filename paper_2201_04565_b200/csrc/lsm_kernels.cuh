@@ -33,13 +33,9 @@ constexpr int kSlice = 32;
 constexpr int kTile = 256;            // particles per tile (= kBlock): 8 slices
 constexpr int kTileSlices = kTile / kSlice;
 constexpr int kMaxStages = 8;
-#ifndef LSM_STREAM_MINB
-#define LSM_STREAM_MINB 3      // resident CTAs per SM the streamed kernel is compiled for (register budget)
-#endif
-#ifndef LSM_ROW_CH
-#define LSM_ROW_CH 6           // springs of a row evaluated together (instruction-level parallelism vs registers)
-#endif
-constexpr int kStreamMinB = LSM_STREAM_MINB;
+constexpr int kStreamMinB = 3;         // resident CTAs per SM the streamed kernels are compiled for (register budget)
+constexpr int kRowCH = 6;              // springs of a row evaluated together (instruction-level parallelism vs registers)
+constexpr int kRowCH3 = 3;             // D = 3 (32-byte positions): three at a time keep the register budget of 3 CTAs per SM
 constexpr int kStreamHdrBytes = 256;   // mbarriers at the front of the streamed kernel's dynamic shared memory
 constexpr uint8_t kFree = 0xFF;
 constexpr int kMaxGroups = 8;
@@ -433,7 +429,7 @@ __device__ __forceinline__ void row_careful(const StepParams &P, const StepVar &
 template <int PM, bool EXACT, bool SAMPLE, int GM, bool I16>
 __device__ __forceinline__ void row_forces(const StepParams &P, const StepVar &V, const RowSrc &R, const double *s_tab, int p, unsigned w,
                                            double2 xp, double &fx, double &fy, double &u) {
-    constexpr int CH = LSM_ROW_CH;
+    constexpr int CH = kRowCH;
     unsigned s0 = 0;
     bool any_near = false;
     for (; s0 + CH <= w; s0 += CH) any_near |= row_chunk<PM, EXACT, SAMPLE, GM, I16, CH>(P, V, R, s_tab, p, s0, xp, fx, fy, u);
@@ -691,7 +687,7 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
                     double fx = 0.0, fy = 0.0, uu = 0.0;
                     if constexpr (MULTI) {   // cooperative multi-step launches: measured 3.5 % faster with the generic-pointer row code
                         row_forces<PM, EXACT, SAMPLE, GM_GLOBAL_CG, I16>(P, V, R, s_tab, (int)p, w, xp, fx, fy, uu);
-                    } else {   // the row: chunks of LSM_ROW_CH springs through 32-bit shared addresses, then the careful pass if needed
+                    } else {   // the row: chunks of kRowCH springs through 32-bit shared addresses, then the careful pass if needed
                         constexpr int GMv = GM_GLOBAL_NC;
                         constexpr unsigned kIdB = I16 ? 2 : 4;
                         const uint32_t b_s = smem_u32(b);
@@ -699,7 +695,7 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
                         A.nbr = b_s + (uint32_t)L.nbr + rel * kIdB; A.thr = b_s + (uint32_t)L.thr + rel * 2; A.typ = b_s + (uint32_t)L.typ + rel;
                         A.kF = b_s + (uint32_t)L.kF + rel * 8; A.r0F = b_s + (uint32_t)L.r0F + rel * 8;
                         const uint32_t tab_s = smem_u32(s_tab);
-                        constexpr int CH = LSM_ROW_CH;
+                        constexpr int CH = kRowCH;
                         bool any_near = false;
                         unsigned s0 = 0;
                         for (; s0 + CH <= w; s0 += CH) {

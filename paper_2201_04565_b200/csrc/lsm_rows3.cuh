@@ -113,10 +113,7 @@ __device__ __forceinline__ void row_careful3(const StepParams &P, const StepVar 
 template <int PM, bool EXACT, bool SAMPLE, bool COHERENT, bool I16>
 __device__ __forceinline__ void row_forces3(const StepParams &P, const StepVar &V, const RowSrc &R, const double *s_tab, int p, unsigned w,
                                             double4 xp, double &fx, double &fy, double &fz, double &u) {
-#ifndef LSM_ROW3_CH
-#define LSM_ROW3_CH 3      // 32-byte positions: three springs at a time keep the register budget of 3 CTAs per SM
-#endif
-    constexpr int CH = LSM_ROW3_CH;
+    constexpr int CH = kRowCH3;
     unsigned s0 = 0;
     bool any_near = false;
     for (; s0 + CH <= w; s0 += CH) any_near |= row_chunk3<PM, EXACT, SAMPLE, COHERENT, I16, CH>(P, V, R, s_tab, p, s0, xp, fx, fy, fz, u);

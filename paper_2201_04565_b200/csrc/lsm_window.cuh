@@ -197,7 +197,7 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_win(const St
             A.kF = b_s + (uint32_t)L.kF + rel * 8; A.r0F = b_s + (uint32_t)L.r0F + rel * 8;
             double fx = 0.0, fy = 0.0;
             bool any_near = false;
-            constexpr int CH = LSM_ROW_CH;
+            constexpr int CH = kRowCH;
             unsigned s0 = 0;
             for (; s0 + CH <= w; s0 += CH) {
                 any_near |= row_chunk_w<PM, EXACT, CH>(P, A, tab_s, win_s, xp, fx, fy);
@@ -341,7 +341,7 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_coop_win(const Step
                 A.kF = b_s + (uint32_t)L.kF + rel * 8; A.r0F = b_s + (uint32_t)L.r0F + rel * 8;
                 double fx = 0.0, fy = 0.0;
                 bool any_near = false;
-                constexpr int CH = LSM_ROW_CH;
+                constexpr int CH = kRowCH;
                 unsigned s0 = 0;
                 for (; s0 + CH <= w; s0 += CH) {
                     any_near |= row_chunk_w<PM, EXACT, CH>(P, A, tab_s, win_s, xp, fx, fy);
