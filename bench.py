@@ -214,6 +214,13 @@ def other_workloads_table(peak, budget_s, with_cpu):
                "counted_bytes_per_time_step": bc, "p_var": pv,
                "roofline": ("L2-resident / latency-bound: HBM roofline does not apply (t_roof by bytes %.2f us)" % (bc / peak / 1e3)) if resident_l2
                else {"bound": "hbm", "achieved_GBs": bc / t / 1e9, "frac": min(1.0, bc / t / 1e9 / peak), "frac_uncapped": bc / t / 1e9 / peak}}
+        if name == "cfg4":   # the batch both ways: resident clusters (default) and one streamed sweep per step
+            t2, inf2, _, _ = measure_device(p, inner, reps, 3, compact_every=1000, history_capacity=64, step_fusion=2)
+            row["streamed_single_sweep"] = {"us_per_time_step": t2 * 1e6, "spring_updates_per_s": alive0 * 1.0 / t2,
+                                            "frac": min(1.0, bc / t2 / 1e9 / peak), "frac_uncapped": bc / t2 / 1e9 / peak,
+                                            "window_particles": inf2["window_particles"],
+                                            "note": "step_fusion = OFF: every step streams the whole batch through HBM (1.35 GB of DRAM traffic per step "
+                                                    "against 14 MB for the resident clusters, profiles/r2_cfg4_cfg5_resident.md)"}
         if with_cpu:
             pc = make_cpu() if make_cpu else p
             row["cpu_baseline"] = oracle_legs(pc, n_cpu, "one specimen of the batch" if make_cpu else name)
