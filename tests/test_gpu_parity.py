@@ -669,6 +669,71 @@ def test_resident_ragged_batch_and_fast_mode():
     assert ei.value.status == -7
 
 
+@pytest.mark.parametrize("seed", [1, 2, 3, 4])
+def test_random_networks_every_kernel_family_exact(seed):
+    """Differential test on irregular networks (nothing lattice-like for the layouts to lean on): jittered points,
+    springs to random near neighbours plus a few long ones, degrees 0..~14, three specimens of different sizes in one
+    batch (sizes multiples of 32 so that the resident kernel may take them), random per-spring k / r0 / rc, per-particle
+    masses, damping, a FIXED and a MOVE group per specimen.  Exact mode: every kernel family must reproduce the oracle bit
+    for bit through breakage, samples and compaction."""
+    rng = np.random.default_rng(1000 + seed)
+    xs, sis, sjs, poff, soff, groups_fix, groups_mov = [], [], [], [0], [0], [], []
+    for n in (rng.integers(10, 40) * 32, rng.integers(3, 12) * 32, rng.integers(20, 60) * 32):
+        side = int(np.ceil(np.sqrt(n)))
+        pts = np.stack([np.arange(n) % side, np.arange(n) // side], 1).astype(float) + rng.uniform(-0.3, 0.3, (n, 2))
+        order = np.argsort(pts[:, 1] * 3.0 + pts[:, 0] * 0.01 + rng.uniform(0, 2, n))      # a loosely banded numbering
+        pts = pts[order]
+        ii, jj = [], []
+        for p_ in range(n):
+            d2 = ((pts - pts[p_]) ** 2).sum(1)
+            near = np.argsort(d2)[1:1 + rng.integers(0, 6)]
+            for q in near:
+                if q != p_:
+                    ii.append(p_); jj.append(int(q))
+        for _ in range(n // 20):                                                           # long springs
+            a, b = rng.integers(0, n, 2)
+            if a != b:
+                ii.append(int(a)); jj.append(int(b))
+        base = poff[-1]
+        xs.append(pts); sis.append(np.array(ii) + base); sjs.append(np.array(jj) + base)
+        ysort = np.argsort(pts[:, 1])
+        groups_fix.append(ysort[:side] + base); groups_mov.append(ysort[-side:] + base)
+        poff.append(base + n); soff.append(soff[-1] + len(ii))
+    x = np.concatenate(xs); si = np.concatenate(sis).astype(np.int32); sj = np.concatenate(sjs).astype(np.int32)
+    M = si.size
+    r = np.linalg.norm(x[sj] - x[si], axis=1)
+    k = rng.uniform(0.5, 2.0, M); r0 = r * rng.uniform(0.97, 1.03, M); rc = r0 * rng.uniform(1.05, 1.25, M)
+    mass = rng.choice([0.5, 1.0, 2.0], x.shape[0])
+    fix = np.concatenate(groups_fix).astype(np.int32); mov = np.concatenate(groups_mov).astype(np.int32)
+    kw0 = dict(gamma=0.05, mass=mass, n_batch=3, particle_offsets=poff, spring_offsets=soff, sample_every=50)
+    o = OracleSim(x, si, sj, k, r0, rc, 0.02, **kw0)
+    o.set_boundary(0, fix, FIXED); o.set_boundary(1, mov, MOVE, [1e-3, 4e-3])
+    o.step(900)
+    xo, vo = o.read_state(); bso, nbo = o.read_broken()[1:]; ho = o.read_stress()
+    assert nbo > 0
+    for kw in (dict(), dict(step_fusion=lsm.FUSION_OFF), dict(step_fusion=lsm.FUSION_OFF, gather_window=lsm.WINDOW_OFF, reorder=2),
+               dict(step_fusion=lsm.FUSION_ON, reorder=1), dict(gather_variant=lsm.GATHER_DIRECT, reorder=3), dict(step_fusion=lsm.FUSION_OFF, reorder=2)):
+        g = lsm.lsm_create(x, si, sj, k, r0, rc, 0.02, exact=True, compact_every=170, **kw0, **kw)
+        g.set_boundary(0, fix, FIXED); g.set_boundary(1, mov, MOVE, [1e-3, 4e-3])
+        g.step(333); g.step(1); g.step(566)
+        xg, vg = g.read_state()
+        assert np.array_equal(xo, xg) and np.array_equal(vo, vg) and np.array_equal(bso, g.read_broken()[1]), (kw, g.info())
+        hg = g.read_stress()
+        assert np.array_equal(ho["n_broken"], hg["n_broken"]) and np.allclose(hg["U"], ho["U"], rtol=1e-11) and np.allclose(hg["KE"], ho["KE"], rtol=1e-11)
+        g.close()
+    for cl in (2, 8):      # resident clusters, where the numbering allows them
+        try:
+            g = lsm.lsm_create(x, si, sj, k, r0, rc, 0.02, exact=True, compact_every=170, step_fusion=lsm.FUSION_RESIDENT, cluster_size=cl, reorder=2, **kw0)
+        except lsm.LsmError as e:
+            assert e.status == -7
+            continue
+        g.set_boundary(0, fix, FIXED); g.set_boundary(1, mov, MOVE, [1e-3, 4e-3])
+        g.step(900)
+        xg, vg = g.read_state()
+        assert np.array_equal(xo, xg) and np.array_equal(vo, vg) and np.array_equal(bso, g.read_broken()[1]), (cl, g.info())
+        g.close()
+
+
 # ---------------------------------------------------------------- full-size checks of the other configurations
 def test_full_size_config4_sampled_specimens():
     """BASELINE.json configs[3] at full size (1024 specimens, one launch): specimens sampled at random are compared
