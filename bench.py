@@ -10,7 +10,7 @@ target ("the 4M-particle lattice", >= 60 % of HBM) is quoted on.  Synthetic and 
 A bench "step" is one lsm_step(S) call: S = --inner consecutive time steps of the whole hot path (boundary
 displacement, kick + drift, spring forces + breakage, damping + kick, the sample reductions every 100 time steps and
 the scheduled compaction), on state already resident in HBM.  value = live springs x time steps / second over all
-ranks.  The per-step traffic (~262 MB streamed by the kernel) is larger than the 126 MB L2, so consecutive time steps cannot serve each other
+ranks.  The per-step traffic (~244 MB streamed by the kernel) is larger than the 126 MB L2, so consecutive time steps cannot serve each other
 from cache (config.l2: "inputs larger than L2").
 
 e2e: the same K bench steps through the C ABI with HOST buffers inside the timed region: lsm_write_state from pinned
@@ -433,7 +433,7 @@ def main():
                          "frac_streamed": streamed / t_launch / 1e9 / peak,
                          "traffic_kind": "static: DRAM bytes per launch read from the committed ncu --set full capture (profiles/traffic_<workload>.txt), not measured by this run",
                          "note": "frac = COUNTED (algorithmic) bytes / measured duration / peak, the headline of SURVEY 8(d); the kernel "
-                                 "streams fewer bytes than the counted model (16-bit neighbour offsets and filter codes instead of int32 "
+                                 "streams fewer bytes than the counted model (16-bit window indices and 8-bit filter codes instead of int32 "
                                  "ids and fp64 rc), so the uncapped ratio can pass 1; frac_streamed = bytes the kernel moves by design / "
                                  "duration / peak is the memory system's real utilisation"},
             "clocks": sampler.summary(tw0, tw1) if sampler else None,

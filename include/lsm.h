@@ -127,8 +127,8 @@ typedef struct lsm_info {
     int64_t n_half_edges_stored;      /* gather: ELL slots incl. padding; scatter: list length                    */
     int64_t bytes_per_half_edge;      /* id (2 B offset, or 4 B when an offset does not fit) + parameter bytes per slot */
     int32_t param_mode;               /* 0 uniform, 1 typed (1 B), 2 k,r0 uniform + rc per spring, 3 k,r0 typed + rc per
-                                         spring, 4 k, r0, rc all per spring.  Gather layout: a per-spring rc costs 2 B
-                                         per half-edge (a conservative 16-bit filter on r^2; the exact fp64 rc is
+                                         spring, 4 k, r0, rc all per spring.  Gather layout: a per-spring rc costs 1 B
+                                         per half-edge (a conservative 8-bit filter on r^2; the exact fp64 rc is
                                          read only when r is close to it, so the decision is always the fp64 one)  */
     int32_t n_types;
     int32_t force_mode, exact, reorder, n_batch;

@@ -66,7 +66,7 @@ struct lsm_sim {
     TileHdr *hdr = nullptr;
     int32_t *nbr = nullptr, *sid = nullptr;
     int16_t *nbr16 = nullptr;
-    uint16_t *thr = nullptr;
+    thr_t *thr = nullptr;
     uint32_t thr_base = 0, thr_shift = 0;
     double *rcS = nullptr;
     // repacking stage of the compaction (a7): scan scratch, one scratch array as large as the largest slot array
@@ -488,7 +488,7 @@ ResPlan plan_resident(const lsm_sim *s, int C, const std::vector<int32_t> &nbmin
     L.grp = (int)o; o += up(sl_cap * kSlice);
     L.sl_off = (int)o; o += up(sl_cap * 8);        // {slice | width << 16, slot offset} per entry of the order list
     L.nbr = (int)o; o += up(slot_cap * kSlice * 2);
-    L.thr = (int)o; if (need_thr) o += up(slot_cap * kSlice * 2);
+    L.thr = (int)o; if (need_thr) o += up(slot_cap * kSlice * kThrB);
     L.typ = (int)o; if (need_typ) o += up(slot_cap * kSlice);
     L.kF = (int)o; if (need_kr) o += up(slot_cap * kSlice * 8);
     L.r0F = (int)o; if (need_kr) o += up(slot_cap * kSlice * 8);
@@ -1080,16 +1080,16 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
         }
         if (need_typ) { std::vector<uint8_t> ht(E, 0); for (size_t e = 0; e < E; ++e) if (hs[e] >= 0) ht[e] = stype[hs[e]]; TRY(upload(s, &s->typ, ht)); CUDA_TRY(s, cudaStreamSynchronize(s->stream)); }
         if (need_rcF) {
-            // 16-bit code of the filter word: base = the smallest word, shift = as few bits as make the spread fit;
+            // 8-bit code of the filter word: base = the smallest word, shift = as few bits as make the spread fit;
             // codes are rounded DOWN (a lower threshold only sends a few more springs to the exact decision)
             uint32_t lo = 0xFFFFFFFFu, hi = 0;
             for (long long e = 0; e < M; ++e) { const uint32_t t = thr_of(getrc(e)); lo = std::min(lo, t); hi = std::max(hi, t); }
             if (M == 0) lo = hi = 0;
             uint32_t shift = 0;
-            while (((hi - lo) >> shift) > 0xFFFFu) ++shift;
+            while (((hi - lo) >> shift) > 0xFFu) ++shift;
             s->thr_base = lo; s->thr_shift = shift;
-            std::vector<uint16_t> h(E, 0xFFFFu);
-            for (size_t e = 0; e < E; ++e) if (hs[e] >= 0) h[e] = (uint16_t)((thr_of(getrc(hs[e])) - lo) >> shift);
+            std::vector<thr_t> h(E, (thr_t)0xFFu);
+            for (size_t e = 0; e < E; ++e) if (hs[e] >= 0) h[e] = (thr_t)((thr_of(getrc(hs[e])) - lo) >> shift);
             TRY(upload(s, &s->thr, h)); CUDA_TRY(s, cudaStreamSynchronize(s->stream));
             std::vector<double> hr(M);
             for (long long e = 0; e < M; ++e) hr[e] = getrc(e);
@@ -1117,7 +1117,7 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
             L.hdr = o; o += 128;
             L.grp = o; o += kTile;
             L.nbr = o; o += up(cap * kSlice * (s->nbr16 ? 2 : 4));
-            L.thr = o; if (need_rcF) o += up(cap * kSlice * 2);
+            L.thr = o; if (need_rcF) o += up(cap * kSlice * kThrB);
             L.typ = o; if (need_typ) o += up(cap * kSlice);
             L.kF = o; if (need_krF) o += up(cap * kSlice * 8);
             L.r0F = o; if (need_krF) o += up(cap * kSlice * 8);
@@ -1781,7 +1781,7 @@ lsm_status lsm_get_info(lsm_sim *s, lsm_info *info) {
             cudaStreamSynchronize(s->stream) == cudaSuccess) { s->E = (long long)tot * kSlice; s->E_stale = false; }
     }
     info->n_particles = s->N; info->n_springs = s->M; info->n_half_edges_stored = s->E;
-    static const int pbytes_scatter[5] = {0, 1, 8, 9, 24}, pbytes_gather[5] = {0, 1, 2, 3, 18};
+    static const int pbytes_scatter[5] = {0, 1, 8, 9, 24}, pbytes_gather[5] = {0, 1, 1, 2, 17};
     info->bytes_per_half_edge = s->force_mode == LSM_FORCE_GATHER ? (s->nbr16 && s->gather_variant == 2 ? 2 : 4) + pbytes_gather[s->pm] : 8 + pbytes_scatter[s->pm];
     info->gather_variant = s->force_mode == LSM_FORCE_GATHER ? s->gather_variant : 0;
     info->pipeline_stages = s->gather_variant == 2 ? s->L.stages : 0;

@@ -11,7 +11,7 @@
 //     nbr[E] int32 neighbour id; a padding slot or a dead spring holds the particle's OWN id (a spring never joins a
 //     particle to itself): its gather is legal, gives r = 0 and therefore contributes nothing, with no validity test,
 //     sid[E] caller spring id (cold: read only when a spring breaks or comes within the filter margin of rc),
-//     per-slot parameters by ParamMode: typ[E] uint8, thr[E] uint16 = 16-bit code of (high word of rc*rc) - 1 (a
+//     per-slot parameters by ParamMode: typ[E] uint8, thr[E] uint8 = 8-bit code of (high word of rc*rc) - 1 (a
 //     conservative integer filter on r^2; anything above it is decided by the exact fp64 rcS[sid]: the decision is the
 //     fp64 one), kF/r0F[E].  nbr16[E] int16: the neighbour list again as offsets (neighbour - self), streamed instead
 //     of nbr when every offset fits in 16 bits.
@@ -35,6 +35,8 @@ constexpr int kTileSlices = kTile / kSlice;
 constexpr int kMaxStages = 8;
 constexpr int kStreamMinB = 3;         // resident CTAs per SM the streamed kernels are compiled for (register budget)
 constexpr int kRowCH = 6;              // springs of a row evaluated together (instruction-level parallelism vs registers)
+typedef uint8_t thr_t;                 // per-half-edge code of the breakage filter (round 1: 16 bits; the filter only has to be
+constexpr int kThrB = 1;               // conservative, so 8 bits stream half the bytes and send a few more rows to the exact pass)
 constexpr int kRowCH3 = 3;             // D = 3 (32-byte positions): three at a time keep the register budget of 3 CTAs per SM
 constexpr int kStreamHdrBytes = 256;   // mbarriers at the front of the streamed kernel's dynamic shared memory
 constexpr uint8_t kFree = 0xFF;
@@ -60,7 +62,7 @@ struct GroupTab {
 struct SpringParams {  // parameter encoding shared by the gather (per half-edge) and scatter (per spring) layouts
     const uint8_t *typ;
     const double *kF, *r0F, *rcF;      // rcF: scatter layout only
-    const uint16_t *thr;               // gather layout: breakage filter per half-edge, 16 bits: the filter word
+    const thr_t *thr;                  // gather layout: breakage filter per half-edge, 8 bits: the filter word
                                        // (high word of rc*rc) - 1 is thr_base + thr[e] * thr_mul, rounded down
     uint32_t thr_base, thr_mul;       // thr_mul = 1 << shift (decode = one multiply-add)
     const double *rcS;                 // gather layout: exact rc per spring, caller numbering
@@ -279,7 +281,7 @@ template <int OFF> __device__ __forceinline__ int lds_s32o(uint32_t a) { int v; 
 struct RowSrc {            // where one particle's row lives: pointers already offset to (slice offset)*32 + lane
     const int32_t *nbr;    // slot s at nbr[s*32]  (global memory, or the staged shared-memory copy)
     const int16_t *nbr16;  // I16: the staged copy holds 16-bit offsets (neighbour - self) instead
-    const uint16_t *thr;
+    const thr_t *thr;
     const uint8_t *typ;
     const double *kF, *r0F;
     size_t e0;                // global entry index of slot 0 of this lane (for the cold paths)
@@ -465,13 +467,13 @@ __device__ __forceinline__ bool row_chunk_g(const StepParams &P, const StepVar &
             const double2 kk = lds_d2(ta);
             k = kk.x; kr0 = kk.y;
             if (EXACT || SAMPLE) r0 = lds_f64o<24>(ta);
-            thr = PM == PM_TYPED ? lds_u32o<16>(ta) : P.sp.thr_base + lds_u16o<C * kSlice * 2>(A.thr) * P.sp.thr_mul;
+            thr = PM == PM_TYPED ? lds_u32o<16>(ta) : P.sp.thr_base + lds_u8o<C * kSlice * kThrB>(A.thr) * P.sp.thr_mul;
         } else if constexpr (PM == PM_FULL) {
             k = lds_f64o<C * kSlice * 8>(A.kF); r0 = lds_f64o<C * kSlice * 8>(A.r0F); kr0 = k * r0;
-            thr = P.sp.thr_base + lds_u16o<C * kSlice * 2>(A.thr) * P.sp.thr_mul;
+            thr = P.sp.thr_base + lds_u8o<C * kSlice * kThrB>(A.thr) * P.sp.thr_mul;
         } else {
             k = P.sp.k_u; r0 = P.sp.r0_u; kr0 = P.sp.kr0_u;
-            thr = kHasThr ? P.sp.thr_base + lds_u16o<C * kSlice * 2>(A.thr) * P.sp.thr_mul : P.sp.thr_u;
+            thr = kHasThr ? P.sp.thr_base + lds_u8o<C * kSlice * kThrB>(A.thr) * P.sp.thr_mul : P.sp.thr_u;
         }
         slot_eval<EXACT, SAMPLE>(xq[C], xp, p < nb[C], k, r0, kr0, thr, dx, dy, r2, g, ue, near);
         fx = mad<EXACT>(g, dx, fx);
@@ -619,7 +621,7 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
                     if (u > 0) mbar_wait(empty + s, (u - 1) & 1);
                     constexpr unsigned kIdB = I16 ? 2 : 4;   // bytes per streamed neighbour id
                     unsigned bytes = 2 * kTile * kVB + kTile + 64 + ns * (kSlice * kIdB);
-                    if (kHasThr) bytes += ns * (kSlice * 2);
+                    if (kHasThr) bytes += ns * (kSlice * kThrB);
                     if (kHasTyp) bytes += ns * kSlice;
                     if (kHasKR) bytes += 2 * ns * (kSlice * 8);
                     unsigned char *b = stage0 + (size_t)s * L.bytes;
@@ -632,7 +634,7 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
                         const size_t e = (size_t)o0 * kSlice;
                         if (I16) bulk_g2s(b + L.nbr, P.nbr16 + e, ns * (kSlice * 2), full + s);
                         else bulk_g2s(b + L.nbr, P.nbr + e, ns * (kSlice * 4), full + s);
-                        if (kHasThr) bulk_g2s(b + L.thr, P.sp.thr + e, ns * (kSlice * 2), full + s);
+                        if (kHasThr) bulk_g2s(b + L.thr, P.sp.thr + e, ns * (kSlice * kThrB), full + s);
                         if (kHasTyp) bulk_g2s(b + L.typ, P.sp.typ + e, ns * kSlice, full + s);
                         if (kHasKR) {
                             bulk_g2s(b + L.kF, P.sp.kF + e, ns * (kSlice * 8), full + s);
@@ -666,7 +668,7 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
                 RowSrc R;
                 R.nbr = reinterpret_cast<const int32_t *>(b + L.nbr) + rel;
                 R.nbr16 = reinterpret_cast<const int16_t *>(b + L.nbr) + rel;
-                R.thr = reinterpret_cast<const uint16_t *>(b + L.thr) + rel;
+                R.thr = reinterpret_cast<const thr_t *>(b + L.thr) + rel;
                 R.typ = (b + L.typ) + rel;
                 R.kF = reinterpret_cast<const double *>(b + L.kF) + rel;
                 R.r0F = reinterpret_cast<const double *>(b + L.r0F) + rel;
@@ -692,7 +694,7 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
                         constexpr unsigned kIdB = I16 ? 2 : 4;
                         const uint32_t b_s = smem_u32(b);
                         RowS A;
-                        A.nbr = b_s + (uint32_t)L.nbr + rel * kIdB; A.thr = b_s + (uint32_t)L.thr + rel * 2; A.typ = b_s + (uint32_t)L.typ + rel;
+                        A.nbr = b_s + (uint32_t)L.nbr + rel * kIdB; A.thr = b_s + (uint32_t)L.thr + rel * kThrB; A.typ = b_s + (uint32_t)L.typ + rel;
                         A.kF = b_s + (uint32_t)L.kF + rel * 8; A.r0F = b_s + (uint32_t)L.r0F + rel * 8;
                         const uint32_t tab_s = smem_u32(s_tab);
                         constexpr int CH = kRowCH;
@@ -700,11 +702,11 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_stream(const
                         unsigned s0 = 0;
                         for (; s0 + CH <= w; s0 += CH) {
                             any_near |= row_chunk_g<PM, EXACT, SAMPLE, GMv, I16, CH>(P, V, A, tab_s, (int)p, xp, fx, fy, uu);
-                            A.nbr += CH * kSlice * kIdB; A.thr += CH * kSlice * 2; A.typ += CH * kSlice; A.kF += CH * kSlice * 8; A.r0F += CH * kSlice * 8;
+                            A.nbr += CH * kSlice * kIdB; A.thr += CH * kSlice * kThrB; A.typ += CH * kSlice; A.kF += CH * kSlice * 8; A.r0F += CH * kSlice * 8;
                         }
                         for (; s0 < w; ++s0) {
                             any_near |= row_chunk_g<PM, EXACT, SAMPLE, GMv, I16, 1>(P, V, A, tab_s, (int)p, xp, fx, fy, uu);
-                            A.nbr += kSlice * kIdB; A.thr += kSlice * 2; A.typ += kSlice; A.kF += kSlice * 8; A.r0F += kSlice * 8;
+                            A.nbr += kSlice * kIdB; A.thr += kSlice * kThrB; A.typ += kSlice; A.kF += kSlice * 8; A.r0F += kSlice * 8;
                         }
                         if (any_near) row_careful<PM, EXACT, SAMPLE, GMv, I16>(P, V, R, s_tab, (int)p, w, xp, fx, fy, uu);
                     }
@@ -1040,7 +1042,7 @@ struct CompactParams {
     int32_t *nbr, *sid;
     int16_t *nbr16;
     uint8_t *typ;
-    uint16_t *thr;
+    thr_t *thr;
     double *kF, *r0F;
     long long nslices;
     uint16_t *widx;        // window indices of the windowed kernel (NULL when unused); a free slot holds the particle's own index

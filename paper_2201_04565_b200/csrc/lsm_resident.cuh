@@ -107,13 +107,13 @@ __device__ __forceinline__ bool row_chunk_s(const StepParams &P, const RowS &A, 
             const double2 kk = lds_d2(ta);
             k = kk.x; kr0 = kk.y;
             if (EXACT) r0 = lds_f64o<24>(ta);
-            thr = PM == PM_TYPED ? lds_u32o<16>(ta) : P.sp.thr_base + lds_u16o<C * kSlice * 2>(A.thr) * P.sp.thr_mul;
+            thr = PM == PM_TYPED ? lds_u32o<16>(ta) : P.sp.thr_base + lds_u8o<C * kSlice * kThrB>(A.thr) * P.sp.thr_mul;
         } else if constexpr (PM == PM_FULL) {
             k = lds_f64o<C * kSlice * 8>(A.kF); r0 = lds_f64o<C * kSlice * 8>(A.r0F); kr0 = k * r0;
-            thr = P.sp.thr_base + lds_u16o<C * kSlice * 2>(A.thr) * P.sp.thr_mul;
+            thr = P.sp.thr_base + lds_u8o<C * kSlice * kThrB>(A.thr) * P.sp.thr_mul;
         } else {
             k = P.sp.k_u; r0 = P.sp.r0_u; kr0 = P.sp.kr0_u;
-            thr = kHasThr ? P.sp.thr_base + lds_u16o<C * kSlice * 2>(A.thr) * P.sp.thr_mul : P.sp.thr_u;
+            thr = kHasThr ? P.sp.thr_base + lds_u8o<C * kSlice * kThrB>(A.thr) * P.sp.thr_mul : P.sp.thr_u;
         }
         slot_eval<EXACT, false>(xq[C], xp, false, k, r0, kr0, thr, dx, dy, r2, g, ue, near);
         fx = mad<EXACT>(g, dx, fx);
@@ -156,7 +156,7 @@ __global__ void __launch_bounds__(kResThreads, 1) k_resident(const StepParams P,
         const uint32_t slot1 = (sl_end & 7) ? __ldg(&P.hdr[sl_end >> 3].off[sl_end & 7]) : __ldg(&P.hdr[(sl_end >> 3) - 1].off[kTileSlices]);
         const size_t e0 = (size_t)slot0 * kSlice, ne = (size_t)(slot1 - slot0) * kSlice;
         res_copy16(smem + L.nbr, P.nbr16 + e0, ne * 2, tid);
-        if (kHasThr) res_copy16(smem + L.thr, P.sp.thr + e0, ne * 2, tid);
+        if (kHasThr) res_copy16(smem + L.thr, P.sp.thr + e0, ne * kThrB, tid);
         if (kTab) res_copy16(smem + L.typ, P.sp.typ + e0, ne, tid);
         if (kHasKR) { res_copy16(smem + L.kF, P.sp.kF + e0, ne * 8, tid); res_copy16(smem + L.r0F, P.sp.r0F + e0, ne * 8, tid); }
     }
@@ -175,7 +175,7 @@ __global__ void __launch_bounds__(kResThreads, 1) k_resident(const StepParams P,
     const uint32_t tab_s = smem_u32(s_tab), bar_s = smem_u32(&ghost_bar[0]);
     const unsigned ghost_bytes = (unsigned)(wlen - n_own) * 16u;   // every window particle that is not mine is pushed to me each step
     RowS lane_rows;    // shared addresses of this lane's entry in slot 0 of the CTA's row block
-    lane_rows.nbr = smem_u32(smem + L.nbr) + lane * 2; lane_rows.thr = smem_u32(smem + L.thr) + lane * 2; lane_rows.typ = smem_u32(smem + L.typ) + lane;
+    lane_rows.nbr = smem_u32(smem + L.nbr) + lane * 2; lane_rows.thr = smem_u32(smem + L.thr) + lane * kThrB; lane_rows.typ = smem_u32(smem + L.typ) + lane;
     lane_rows.kF = smem_u32(smem + L.kF) + lane * 8; lane_rows.r0F = smem_u32(smem + L.r0F) + lane * 8;
     auto do_slice = [&](int k, uint32_t pc, uint32_t pn, long long step, bool push, uint32_t push_bar) {
         const uint2 se = lds_u2(slice_s + (uint32_t)k * 8u);
@@ -188,7 +188,7 @@ __global__ void __launch_bounds__(kResThreads, 1) k_resident(const StepParams P,
         const double2 vh = lds_d2(vel_s + (uint32_t)li * 16u);
         const uint8_t g = (uint8_t)lds_u8(grp_s + (uint32_t)li);
         RowS A;
-        A.nbr = lane_rows.nbr + se.y * (kSlice * 2); A.thr = lane_rows.thr + se.y * (kSlice * 2); A.typ = lane_rows.typ + se.y * kSlice;
+        A.nbr = lane_rows.nbr + se.y * (kSlice * 2); A.thr = lane_rows.thr + se.y * (kSlice * kThrB); A.typ = lane_rows.typ + se.y * kSlice;
         A.kF = lane_rows.kF + se.y * (kSlice * 8); A.r0F = lane_rows.r0F + se.y * (kSlice * 8);
         double fx = 0.0, fy = 0.0;
         bool any_near = false;
@@ -196,18 +196,18 @@ __global__ void __launch_bounds__(kResThreads, 1) k_resident(const StepParams P,
         unsigned s0 = 0;
         for (; s0 + CH <= w; s0 += CH) {
             any_near |= row_chunk_s<PM, EXACT, CH>(P, A, tab_s, pos_p, xp, fx, fy);
-            A.nbr += CH * kSlice * 2; A.thr += CH * kSlice * 2; A.typ += CH * kSlice; A.kF += CH * kSlice * 8; A.r0F += CH * kSlice * 8;
+            A.nbr += CH * kSlice * 2; A.thr += CH * kSlice * kThrB; A.typ += CH * kSlice; A.kF += CH * kSlice * 8; A.r0F += CH * kSlice * 8;
         }
         for (; s0 < w; ++s0) {
             any_near |= row_chunk_s<PM, EXACT, 1>(P, A, tab_s, pos_p, xp, fx, fy);
-            A.nbr += kSlice * 2; A.thr += kSlice * 2; A.typ += kSlice; A.kF += kSlice * 8; A.r0F += kSlice * 8;
+            A.nbr += kSlice * 2; A.thr += kSlice * kThrB; A.typ += kSlice; A.kF += kSlice * 8; A.r0F += kSlice * 8;
         }
         if (any_near) {   // rare: a spring came close to its breaking length -> redo the row deciding exactly (row_careful)
             const unsigned rel = se.y * kSlice + lane;
             RowSrc R;
             R.nbr = nullptr;
             R.nbr16 = reinterpret_cast<const int16_t *>(smem + L.nbr) + rel;
-            R.thr = reinterpret_cast<const uint16_t *>(smem + L.thr) + rel;
+            R.thr = reinterpret_cast<const thr_t *>(smem + L.thr) + rel;
             R.typ = (smem + L.typ) + rel;
             R.kF = reinterpret_cast<const double *>(smem + L.kF) + rel;
             R.r0F = reinterpret_cast<const double *>(smem + L.r0F) + rel;

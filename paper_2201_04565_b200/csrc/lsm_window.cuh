@@ -89,13 +89,13 @@ __device__ __forceinline__ bool row_chunk_w(const StepParams &P, const RowS &A, 
             const double2 kk = lds_d2(ta);
             k = kk.x; kr0 = kk.y;
             if (EXACT) r0 = lds_f64o<24>(ta);
-            thr = PM == PM_TYPED ? lds_u32o<16>(ta) : P.sp.thr_base + lds_u16o<C * kSlice * 2>(A.thr) * P.sp.thr_mul;
+            thr = PM == PM_TYPED ? lds_u32o<16>(ta) : P.sp.thr_base + lds_u8o<C * kSlice * kThrB>(A.thr) * P.sp.thr_mul;
         } else if constexpr (PM == PM_FULL) {
             k = lds_f64o<C * kSlice * 8>(A.kF); r0 = lds_f64o<C * kSlice * 8>(A.r0F); kr0 = k * r0;
-            thr = P.sp.thr_base + lds_u16o<C * kSlice * 2>(A.thr) * P.sp.thr_mul;
+            thr = P.sp.thr_base + lds_u8o<C * kSlice * kThrB>(A.thr) * P.sp.thr_mul;
         } else {
             k = P.sp.k_u; r0 = P.sp.r0_u; kr0 = P.sp.kr0_u;
-            thr = kHasThr ? P.sp.thr_base + lds_u16o<C * kSlice * 2>(A.thr) * P.sp.thr_mul : P.sp.thr_u;
+            thr = kHasThr ? P.sp.thr_base + lds_u8o<C * kSlice * kThrB>(A.thr) * P.sp.thr_mul : P.sp.thr_u;
         }
         slot_eval<EXACT, false>(xq[C], xp, false, k, r0, kr0, thr, dx, dy, r2, g, ue, near);
         fx = mad<EXACT>(g, dx, fx);
@@ -147,7 +147,7 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_win(const St
                 if (u > 0) mbar_wait(empty + s, (u - 1) & 1);
                 const unsigned nwin = ln[0] + ln[1] + ln[2] + ln[3];
                 unsigned bytes = nwin * 16 + kTile * 16 + kTile + 64 + ns * (kSlice * 2);
-                if (kHasThr) bytes += ns * (kSlice * 2);
+                if (kHasThr) bytes += ns * (kSlice * kThrB);
                 if (kTab) bytes += ns * kSlice;
                 if (kHasKR) bytes += 2 * ns * (kSlice * 8);
                 unsigned char *b = stage0 + (size_t)s * L.bytes;
@@ -162,7 +162,7 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_win(const St
                 if (ns) {
                     const size_t e = (size_t)o0 * kSlice;
                     bulk_g2s(b + L.nbr, W.widx + e, ns * (kSlice * 2), full + s);
-                    if (kHasThr) bulk_g2s(b + L.thr, P.sp.thr + e, ns * (kSlice * 2), full + s);
+                    if (kHasThr) bulk_g2s(b + L.thr, P.sp.thr + e, ns * (kSlice * kThrB), full + s);
                     if (kTab) bulk_g2s(b + L.typ, P.sp.typ + e, ns * kSlice, full + s);
                     if (kHasKR) {
                         bulk_g2s(b + L.kF, P.sp.kF + e, ns * (kSlice * 8), full + s);
@@ -193,7 +193,7 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_win(const St
             const double2 vh = lds_d2(b_s + (uint32_t)L.vel + (uint32_t)tid * 16u);
             const uint8_t g = (uint8_t)lds_u8(b_s + (uint32_t)L.grp + (uint32_t)tid);
             RowS A;
-            A.nbr = b_s + (uint32_t)L.nbr + rel * 2; A.thr = b_s + (uint32_t)L.thr + rel * 2; A.typ = b_s + (uint32_t)L.typ + rel;
+            A.nbr = b_s + (uint32_t)L.nbr + rel * 2; A.thr = b_s + (uint32_t)L.thr + rel * kThrB; A.typ = b_s + (uint32_t)L.typ + rel;
             A.kF = b_s + (uint32_t)L.kF + rel * 8; A.r0F = b_s + (uint32_t)L.r0F + rel * 8;
             double fx = 0.0, fy = 0.0;
             bool any_near = false;
@@ -201,18 +201,18 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_gather_win(const St
             unsigned s0 = 0;
             for (; s0 + CH <= w; s0 += CH) {
                 any_near |= row_chunk_w<PM, EXACT, CH>(P, A, tab_s, win_s, xp, fx, fy);
-                A.nbr += CH * kSlice * 2; A.thr += CH * kSlice * 2; A.typ += CH * kSlice; A.kF += CH * kSlice * 8; A.r0F += CH * kSlice * 8;
+                A.nbr += CH * kSlice * 2; A.thr += CH * kSlice * kThrB; A.typ += CH * kSlice; A.kF += CH * kSlice * 8; A.r0F += CH * kSlice * 8;
             }
             for (; s0 < w; ++s0) {
                 any_near |= row_chunk_w<PM, EXACT, 1>(P, A, tab_s, win_s, xp, fx, fy);
-                A.nbr += kSlice * 2; A.thr += kSlice * 2; A.typ += kSlice; A.kF += kSlice * 8; A.r0F += kSlice * 8;
+                A.nbr += kSlice * 2; A.thr += kSlice * kThrB; A.typ += kSlice; A.kF += kSlice * 8; A.r0F += kSlice * 8;
             }
             if (any_near) {   // rare: redo the row deciding exactly
                 unsigned char *b = stage0 + (size_t)s * L.bytes;
                 RowSrc R;
                 R.nbr = nullptr;
                 R.nbr16 = reinterpret_cast<const int16_t *>(b + L.nbr) + rel;
-                R.thr = reinterpret_cast<const uint16_t *>(b + L.thr) + rel;
+                R.thr = reinterpret_cast<const thr_t *>(b + L.thr) + rel;
                 R.typ = (b + L.typ) + rel;
                 R.kF = reinterpret_cast<const double *>(b + L.kF) + rel;
                 R.r0F = reinterpret_cast<const double *>(b + L.r0F) + rel;
@@ -284,7 +284,7 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_coop_win(const Step
                     const uint32_t o0 = h->off[0], ns = h->off[kTileSlices] - h->off[0];
                     if (it == 0) {
                         bytes += kTile * 16 + kTile + 64 + ns * (kSlice * 2);
-                        if (kHasThr) bytes += ns * (kSlice * 2);
+                        if (kHasThr) bytes += ns * (kSlice * kThrB);
                         if (kTab) bytes += ns * kSlice;
                         if (kHasKR) bytes += 2 * ns * (kSlice * 8);
                     }
@@ -300,7 +300,7 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_coop_win(const Step
                         if (ns) {
                             const size_t e = (size_t)o0 * kSlice;
                             bulk_g2s(b + L.nbr, Q.widx + e, ns * (kSlice * 2), full + s);
-                            if (kHasThr) bulk_g2s(b + L.thr, P.sp.thr + e, ns * (kSlice * 2), full + s);
+                            if (kHasThr) bulk_g2s(b + L.thr, P.sp.thr + e, ns * (kSlice * kThrB), full + s);
                             if (kTab) bulk_g2s(b + L.typ, P.sp.typ + e, ns * kSlice, full + s);
                             if (kHasKR) {
                                 bulk_g2s(b + L.kF, P.sp.kF + e, ns * (kSlice * 8), full + s);
@@ -337,7 +337,7 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_coop_win(const Step
                 const double2 vh = lds_d2(vel_a);
                 const uint8_t g = (uint8_t)lds_u8(b_s + (uint32_t)L.grp + (uint32_t)tid);
                 RowS A;
-                A.nbr = b_s + (uint32_t)L.nbr + rel * 2; A.thr = b_s + (uint32_t)L.thr + rel * 2; A.typ = b_s + (uint32_t)L.typ + rel;
+                A.nbr = b_s + (uint32_t)L.nbr + rel * 2; A.thr = b_s + (uint32_t)L.thr + rel * kThrB; A.typ = b_s + (uint32_t)L.typ + rel;
                 A.kF = b_s + (uint32_t)L.kF + rel * 8; A.r0F = b_s + (uint32_t)L.r0F + rel * 8;
                 double fx = 0.0, fy = 0.0;
                 bool any_near = false;
@@ -345,18 +345,18 @@ __global__ void __launch_bounds__(kTile + 32, kStreamMinB) k_coop_win(const Step
                 unsigned s0 = 0;
                 for (; s0 + CH <= w; s0 += CH) {
                     any_near |= row_chunk_w<PM, EXACT, CH>(P, A, tab_s, win_s, xp, fx, fy);
-                    A.nbr += CH * kSlice * 2; A.thr += CH * kSlice * 2; A.typ += CH * kSlice; A.kF += CH * kSlice * 8; A.r0F += CH * kSlice * 8;
+                    A.nbr += CH * kSlice * 2; A.thr += CH * kSlice * kThrB; A.typ += CH * kSlice; A.kF += CH * kSlice * 8; A.r0F += CH * kSlice * 8;
                 }
                 for (; s0 < w; ++s0) {
                     any_near |= row_chunk_w<PM, EXACT, 1>(P, A, tab_s, win_s, xp, fx, fy);
-                    A.nbr += kSlice * 2; A.thr += kSlice * 2; A.typ += kSlice; A.kF += kSlice * 8; A.r0F += kSlice * 8;
+                    A.nbr += kSlice * 2; A.thr += kSlice * kThrB; A.typ += kSlice; A.kF += kSlice * 8; A.r0F += kSlice * 8;
                 }
                 if (any_near) {
                     unsigned char *b = stage0 + (size_t)s * L.bytes;
                     RowSrc R;
                     R.nbr = nullptr;
                     R.nbr16 = reinterpret_cast<const int16_t *>(b + L.nbr) + rel;
-                    R.thr = reinterpret_cast<const uint16_t *>(b + L.thr) + rel;
+                    R.thr = reinterpret_cast<const thr_t *>(b + L.thr) + rel;
                     R.typ = (b + L.typ) + rel;
                     R.kF = reinterpret_cast<const double *>(b + L.kF) + rel;
                     R.r0F = reinterpret_cast<const double *>(b + L.r0F) + rel;
