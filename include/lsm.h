@@ -73,9 +73,11 @@ enum { LSM_GATHER_AUTO = 0, LSM_GATHER_DIRECT = 1, LSM_GATHER_STREAMED = 2 };
 enum { LSM_WINDOW_AUTO = 0, LSM_WINDOW_ON = 1, LSM_WINDOW_OFF = 2 };
 /* several time steps per launch: ON = one cooperative launch with a grid barrier between steps (state stays in L2 /
  * the CTAs' pipeline stages); RESIDENT = one thread-block cluster per specimen keeps it in shared memory for the whole
- * run of steps, ghosts exchanged through distributed shared memory, cluster barrier per step (needs dim = 2, 16-bit
- * neighbour offsets, specimens starting on multiples of 32 particles and fitting one cluster; else LSM_E_UNSUPPORTED);
- * AUTO = RESIDENT where it applies, else ON for L2-resident launch-bound problems, else one launch per step */
+ * run of steps, ghosts pushed through distributed shared memory onto the receiver's transaction barrier (needs dim = 2,
+ * 16-bit neighbour offsets, specimens starting on multiples of 32 particles and fitting one cluster; else
+ * LSM_E_UNSUPPORTED); AUTO = RESIDENT where the clusters fill the GPU or the lattice is tiny, else ON for L2-resident
+ * launch-bound problems (up to 2^18 particles), else one launch per step.  gather_window = AUTO also applies only up to
+ * 2^25 particles (above, the bulk-copied neighbour ranges miss L2: DESIGN.md). */
 enum { LSM_FUSION_AUTO = 0, LSM_FUSION_ON = 1, LSM_FUSION_OFF = 2, LSM_FUSION_RESIDENT = 3 };
 
 /* Optional device allocator (the Python binding passes PyTorch's caching allocator). */
