@@ -88,6 +88,7 @@ static void force_eval(olsm_sim *s)
     const int D = s->D;
     memset(s->f, 0, sizeof(double) * (size_t)(s->N * D));
     for (int b = 0; b < s->B; ++b) s->U[b] = 0.0;
+    s->U_stale = 0;                                       /* U[] is summed right here: nothing left over from force_eval_threads() */
     for (int64_t e = 0; e < s->M; ++e) {
         if (!s->alive[e]) continue;                       /* irreversible: L98, L196 (Q2) */
         const int64_t i = s->si[e], j = s->sj[e];

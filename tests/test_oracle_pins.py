@@ -649,7 +649,11 @@ def test_threaded_variant_is_bit_equal_to_the_serial_loop():
     p.sample_every = 50
     a = OracleSim.from_problem(p); b = OracleSim.from_problem(p)
     b.set_threads(4)
-    a.step(4000); b.step(1500); b.set_threads(1); b.step(500); b.set_threads(3); b.step(2000)
+    # the threaded -> serial switch falls BETWEEN two sample steps (samples every 50), and U is read right after it and again
+    # at the next sample: a serial evaluation must not be overwritten by the per-spring energies of the last threaded one
+    a.step(1470); b.step(1470); b.set_threads(1); a.step(10); b.step(10)
+    assert np.array_equal(a.read_energy()[0], b.read_energy()[0]) and np.array_equal(a.read_energy()[1], b.read_energy()[1])
+    a.step(2520); b.step(520); b.set_threads(3); b.step(2000)
     assert a.read_broken()[2] > 10
     for u, w in zip(a.read_state() + (a.read_forces(),) + a.read_broken()[:2], b.read_state() + (b.read_forces(),) + b.read_broken()[:2]):
         assert np.array_equal(u, w)
