@@ -229,6 +229,56 @@ const char *lsm_last_error(const lsm_sim *sim); /* sim NULL: error of the last f
 void lsm_destroy(lsm_sim *sim);
 int32_t lsm_abi_version(void);
 
+/* ---- The one entry point that allocates nothing ----------------------------------------------------------------------
+ * Elastic energy U = sum over unbroken springs of k (r - r0)^2 / 2 (Eq. 1; the quantity of Fig. 4B, which
+ * the paper sums on the CPU, L113) of a spring list the caller already holds ON THE DEVICE, without an lsm_sim handle.
+ *
+ * Why it exists: every other call needs a handle, and lsm_create makes dozens of device allocations.  This one is for
+ * callers that cannot ask CUDA for memory at the point where they need the number: a process whose GPU memory was all
+ * given to one arena or framework pool at start-up (cudaMalloc fails there, or eats what the pool's owner budgeted); a
+ * monitor running beside asynchronous lsm_step work (cudaFree waits for the whole device and cudaMalloc may, which stalls
+ * the step pipeline); a long unattended sweep whose memory footprint must be fixed when the library loads.  The function
+ * calls neither cudaMalloc nor cudaFree nor any allocating library routine.  Its only scratch -- the per-block partial
+ * sums of a deterministic two-level reduction -- lives in a fixed array inside the library: 524,544 bytes that every GPU
+ * which loads liblsm_b200.so holds until the process exits, whether or not this function is ever called.
+ *
+ * The limit: n_springs <= LSM_STATIC_MAX_SPRINGS (2^28; one partial per 8192 springs, 32768 partials).  A longer list is
+ * rejected with LSM_E_RANGE before anything is enqueued and U is left untouched: split the list and add the parts, or
+ * use lsm_create + lsm_read_energy.
+ *
+ * Arguments (DEVICE pointers are memory of `device`, in the CALLER's numbering; nothing is copied or kept):
+ *   device, stream   CUDA device ordinal (made current for the call, the caller's device restored) and cudaStream_t
+ *                    (NULL = default stream).  The call only enqueues a 8-byte memset and two kernels on `stream`.
+ *   dim              2 or 3; x is interleaved [n_particles*dim] as everywhere in this header.
+ *   spring_i/j       [n_springs] endpoints (the paper's atom_i / atom_j, L91-L92); may be NULL when n_springs == 0.
+ *   k, r0            [n_springs], or NULL to take k_uniform / r0_uniform.
+ *   broken           [n_springs] bytes, non-zero = the spring is dead and contributes nothing (what lsm_read_broken
+ *                    returns, uploaded); NULL = all alive.  Breakage is irreversible (L98, L196): this function does not
+ *                    test r > rc itself, the flags are the caller's record of it.
+ *   U                DEVICE [1]: the energy.  Summation order is fixed by the list alone (same bits on every GPU).
+ *   counts           DEVICE [2] or NULL: {springs summed, springs skipped because an endpoint is outside
+ *                    [0, n_particles) or i == j}.  Bad ids are skipped and counted on the device, never dereferenced.
+ *   errbuf           HOST buffer of errbuf_len bytes for the message of a failed call (may be NULL); lsm_last_error
+ *                    does not cover this function.
+ * Returns LSM_OK once the work is enqueued (read U after synchronising the stream); LSM_E_INVALID (bad dim / sizes /
+ * NULL pointers / device ordinal outside [0, 64)), LSM_E_RANGE (list too long), LSM_E_CUDA (no device, launch failure).
+ *
+ * Sharing: all calls on one device use the same array, and it keeps whatever the previous call left in it.  The function
+ * clears the one word that must start at zero (the bad-id counter) itself, on `stream`, and every partial it reads was
+ * written by the same call, so calls that follow each other on one stream, or that are otherwise ordered, are
+ * independent of each other.  Two calls that may run on the GPU at the same time (different streams or host threads
+ * without an event or synchronisation between them) race on the array and both results are garbage: order them.
+ *
+ * First call on each device: looks up the device address of the array (cudaGetSymbolAddress, once per device, under a
+ * host mutex).  Make that first call on an ordinary stream, before any stream capture is begun. */
+#define LSM_STATIC_MAX_SPRINGS 268435456
+lsm_status lsm_spring_energy_static(int32_t device, void *stream, int32_t dim, int64_t n_particles, int64_t n_springs,
+                                    const double *x /* DEVICE */, const int32_t *spring_i /* DEVICE */, const int32_t *spring_j /* DEVICE */,
+                                    const double *k /* DEVICE or NULL */, const double *r0 /* DEVICE or NULL */,
+                                    double k_uniform, double r0_uniform, const uint8_t *broken /* DEVICE or NULL */,
+                                    double *U /* DEVICE [1] */, int64_t *counts /* DEVICE [2] or NULL */,
+                                    char *errbuf /* HOST */, size_t errbuf_len);
+
 #ifdef __cplusplus
 }
 #endif

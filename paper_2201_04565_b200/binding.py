@@ -23,7 +23,8 @@ MAX_GROUPS = 8
 
 EXPORTS = ["lsm_create", "lsm_set_boundary", "lsm_step", "lsm_write_state", "lsm_read_state", "lsm_read_forces",
            "lsm_read_broken", "lsm_read_energy", "lsm_read_virial", "lsm_read_stress", "lsm_run_to_failure", "lsm_set_strain_rate", "lsm_compact", "lsm_sync", "lsm_get_info",
-           "lsm_device_state", "lsm_last_error", "lsm_destroy", "lsm_abi_version"]
+           "lsm_device_state", "lsm_last_error", "lsm_destroy", "lsm_abi_version", "lsm_spring_energy_static"]
+STATIC_MAX_SPRINGS = 1 << 28
 
 _ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
 _FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)
@@ -103,6 +104,9 @@ def library():
         L.lsm_destroy.argtypes = [C.c_void_p]
         L.lsm_destroy.restype = None
         L.lsm_abi_version.restype = C.c_int32
+        L.lsm_spring_energy_static.argtypes = [C.c_int32, C.c_void_p, C.c_int32, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p,
+                                               C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p,
+                                               C.c_char_p, C.c_size_t]
         for n in EXPORTS:
             if n not in ("lsm_last_error", "lsm_destroy", "lsm_abi_version"):
                 getattr(L, n).restype = C.c_int32
@@ -356,3 +360,37 @@ def lsm_get_info(sim): return sim.info()
 def lsm_destroy(sim): return sim.close()
 def lsm_last_error(sim=None): return (library().lsm_last_error(sim._h if sim is not None else None) or b"").decode()
 def lsm_abi_version(): return int(library().lsm_abi_version())
+
+
+def lsm_spring_energy_static(x, spring_i, spring_j, k, r0, U, broken=None, counts=None, stream=None):
+    """lsm_spring_energy_static: elastic energy (Eq. 1) of a spring list that already sits on the GPU, for callers that
+    cannot allocate there (see include/lsm.h for who they are).  Marshalling only, and in keeping with the entry point
+    this wrapper creates no tensor either: every array is a CUDA tensor the caller made earlier -- x [N, dim] float64,
+    spring_i / spring_j [M] int32, k / r0 [M] float64 or Python scalars (uniform), broken [M] uint8 or None, U [1] float64
+    (output), counts [2] int64 or None (output: springs summed, springs skipped for bad ids).  Contiguous tensors on one
+    device; the work is enqueued on `stream` (default: torch's current stream on that device) and U is valid once that
+    stream has been synchronised.  Raises LsmError(-2) for more than STATIC_MAX_SPRINGS springs."""
+    import torch
+    dev = x.device.index if x.device.index is not None else torch.cuda.current_device()
+
+    def dptr(t, dtype, n, name):
+        if t is None:
+            return None
+        if not (t.is_cuda and t.device.index == dev and t.dtype == dtype and t.is_contiguous() and t.numel() == n):
+            raise LsmError(-1, "%s must be a contiguous %s CUDA tensor with %d entries on device %d" % (name, dtype, n, dev))
+        return C.c_void_p(t.data_ptr())
+
+    if x.dim() != 2:
+        raise LsmError(-1, "x must be [N, dim]")
+    N, D, M = int(x.shape[0]), int(x.shape[1]), int(spring_i.numel())
+    k_t, k_u = (None, float(k)) if not hasattr(k, "data_ptr") else (k, 0.0)
+    r0_t, r0_u = (None, float(r0)) if not hasattr(r0, "data_ptr") else (r0, 0.0)
+    if stream is None:
+        stream = torch.cuda.current_stream(dev).cuda_stream
+    err = C.create_string_buffer(512)
+    st = library().lsm_spring_energy_static(
+        dev, C.c_void_p(stream or 0), D, N, M, dptr(x, torch.float64, N * D, "x"), dptr(spring_i, torch.int32, M, "spring_i"),
+        dptr(spring_j, torch.int32, M, "spring_j"), dptr(k_t, torch.float64, M, "k"), dptr(r0_t, torch.float64, M, "r0"), k_u, r0_u,
+        dptr(broken, torch.uint8, M, "broken"), dptr(U, torch.float64, 1, "U"), dptr(counts, torch.int64, 2, "counts"), err, len(err))
+    if st != 0:
+        raise LsmError(st, err.value.decode())

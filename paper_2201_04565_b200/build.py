@@ -12,7 +12,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "liblsm_b200.so")
-SOURCES = [os.path.join(CSRC, "lsm_api.cu")]
+SOURCES = [os.path.join(CSRC, "lsm_api.cu"), os.path.join(CSRC, "lsm_static.cu")]
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 
 
