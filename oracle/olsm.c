@@ -15,7 +15,10 @@
  *   samples       U and KE (L113), boundary reaction sums and broken count (BASELINE.json north_star item 4).
  *   olsm_read_virial()  per-particle virial stress, Eq. 7 (L147), pinned by P13 (virial = Cauchy stress in a homogeneous
  *                 static state; kinetic term; sum over particles = sum over springs of g d (x) d).
- * Readings where the paper is silent are those of SURVEY.md 8(c) / DESIGN.md "Readings" (Q1..Q20), named inline.
+ *   olsm_read_strain()  per-particle Lagrangian strain, Eq. 8 (L150, L156), reading Q21; pinned by P15 (homogeneous
+ *                 deformation gives exactly (F^T F - I)/2, rigid rotation gives 0, small-strain limit of P3's state,
+ *                 rank-deficient neighbourhoods are flagged, a transposed J fails).
+ * Readings where the paper is silent are those of SURVEY.md 8(c) / DESIGN.md "Readings" (Q1..Q21), named inline.
  *
  * Pins (tests/test_oracle_pins.py, all run without a GPU): P1 paper's worked oscillator example (L123-L127) against
  * the closed form of velocity Verlet and the analytic ODE solution; P2 two free particles (reduced mass period);
@@ -54,6 +57,7 @@ typedef struct olsm_sim {
     int32_t B;                      /* n_batch */
     int64_t *poff, *soff;           /* [B+1] */
     double *x, *v, *f, *fd, *m;     /* [N*D] x4, [N] */
+    double *xref;                   /* [N*D] positions at olsm_create: the reference configuration of Eq. 8 (Q21) */
     int32_t *si, *sj;
     double *k, *r0, *rc;
     uint8_t *alive;
@@ -234,6 +238,7 @@ olsm_sim *olsm_create(int32_t D, int64_t N, int64_t M, int32_t B, const int64_t 
     else { memcpy(s->poff, poff, sizeof(int64_t) * (size_t)(B + 1)); memcpy(s->soff, soff, sizeof(int64_t) * (size_t)(B + 1)); }
     const size_t nd = (size_t)(N * D);
     s->x = malloc(sizeof(double) * nd); memcpy(s->x, x, sizeof(double) * nd);
+    s->xref = malloc(sizeof(double) * nd); memcpy(s->xref, x, sizeof(double) * nd);
     s->v = calloc(nd, sizeof(double)); if (v) memcpy(s->v, v, sizeof(double) * nd);
     s->f = calloc(nd, sizeof(double)); s->fd = calloc(nd, sizeof(double));
     s->m = malloc(sizeof(double) * (size_t)N);
@@ -463,6 +468,76 @@ int32_t olsm_read_virial(const olsm_sim *s, double *out)
     return 0;
 }
 
+/* Per-particle Lagrangian strain, Eq. 8: eps^L = (J J^T - delta) / 2 with "J the locally affine
+ * transformation matrix considering the relative displacement of particle with its first nearest neighbors" (L156; the
+ * method of Shimizu et al. 2007 cited at L145).  The printed index form "J_ij J_ji" has lost its summation: reading Q21.
+ *   neighbours of p   the particles joined to p by a spring that is alive now (its "first nearest neighbours" in a
+ *                     spring network are the particles it is bonded to; a broken bond is no longer one);
+ *   reference         the positions given to olsm_create, d0 = xref_l - xref_p;  current d = x_l - x_p;
+ *   J                 Shimizu's row-vector map d0 J ~ d in the least-squares sense: J = V^-1 W, V = sum d0^T d0,
+ *                     W = sum d0^T d.  In column-vector language F = J^T = (sum d (x) d0) V^-1 is the deformation
+ *                     gradient and J J^T = F^T F, so eps = (F^T F - I)/2, the Green-Lagrange strain; symmetric.
+ *   rank deficiency   fewer than D independent reference bonds (det V <= 1e-12 (tr V / D)^D): eps = 0 and ok[p] = 0.
+ * out[p] = {e_xx, e_yy, e_xy} in 2-D, {e_xx, e_yy, e_zz, e_xy, e_yz, e_zx} in 3-D (the layout of olsm_read_virial);
+ * ok may be NULL.  Serial loop over the alive springs in caller order, then one solve per particle. */
+int32_t olsm_read_strain(const olsm_sim *s, double *out, uint8_t *ok)
+{
+    if (!s || !out) return -1;
+    const int D = s->D, C = D == 2 ? 3 : 6;
+    double *V = calloc((size_t)(s->N * 9), sizeof(double)), *W = calloc((size_t)(s->N * 9), sizeof(double));
+    if (!V || !W) { free(V); free(W); return -2; }
+    for (int64_t e = 0; e < s->M; ++e) {
+        if (!s->alive[e]) continue;
+        const int64_t i = s->si[e], j = s->sj[e];
+        double d0[3] = {0.0, 0.0, 0.0}, d[3] = {0.0, 0.0, 0.0};
+        for (int c = 0; c < D; ++c) { d0[c] = s->xref[D * j + c] - s->xref[D * i + c]; d[c] = s->x[D * j + c] - s->x[D * i + c]; }
+        /* the bond seen from j is (-d0, -d): the same dyads, so both ends add the same terms */
+        for (int a = 0; a < D; ++a)
+            for (int b = 0; b < D; ++b) {
+                V[9 * i + 3 * a + b] += d0[a] * d0[b]; V[9 * j + 3 * a + b] += d0[a] * d0[b];
+                W[9 * i + 3 * a + b] += d[a] * d0[b];  W[9 * j + 3 * a + b] += d[a] * d0[b];      /* W = sum d (x) d0 */
+            }
+    }
+    for (int64_t p = 0; p < s->N; ++p) {
+        const double *v = V + 9 * p, *w = W + 9 * p;
+        double inv[9], F[9], det, tr;
+        for (int c = 0; c < C; ++c) out[C * p + c] = 0.0;
+        if (ok) ok[p] = 0;
+        if (D == 2) {
+            det = v[0] * v[4] - v[1] * v[3];
+            tr = 0.5 * (v[0] + v[4]);
+            if (!(det > 1e-12 * tr * tr)) continue;
+            inv[0] = v[4] / det; inv[1] = -v[1] / det; inv[3] = -v[3] / det; inv[4] = v[0] / det;
+        } else {
+            const double c00 = v[4] * v[8] - v[5] * v[7], c01 = v[5] * v[6] - v[3] * v[8], c02 = v[3] * v[7] - v[4] * v[6];
+            det = v[0] * c00 + v[1] * c01 + v[2] * c02;
+            tr = (v[0] + v[4] + v[8]) / 3.0;
+            if (!(det > 1e-12 * tr * tr * tr)) continue;
+            inv[0] = c00 / det; inv[1] = (v[2] * v[7] - v[1] * v[8]) / det; inv[2] = (v[1] * v[5] - v[2] * v[4]) / det;
+            inv[3] = c01 / det; inv[4] = (v[0] * v[8] - v[2] * v[6]) / det; inv[5] = (v[2] * v[3] - v[0] * v[5]) / det;
+            inv[6] = c02 / det; inv[7] = (v[1] * v[6] - v[0] * v[7]) / det; inv[8] = (v[0] * v[4] - v[1] * v[3]) / det;
+        }
+        for (int a = 0; a < D; ++a)
+            for (int b = 0; b < D; ++b) {
+                double t = 0.0;
+                for (int c = 0; c < D; ++c) t += w[3 * a + c] * inv[3 * c + b];                   /* F = W V^-1 */
+                F[3 * a + b] = t;
+            }
+        double E[9];
+        for (int a = 0; a < D; ++a)
+            for (int b = 0; b < D; ++b) {
+                double t = 0.0;
+                for (int c = 0; c < D; ++c) t += F[3 * c + a] * F[3 * c + b];                     /* (F^T F)_ab = (J J^T)_ab */
+                E[3 * a + b] = 0.5 * (t - (a == b ? 1.0 : 0.0));
+            }
+        if (D == 2) { out[3 * p] = E[0]; out[3 * p + 1] = E[4]; out[3 * p + 2] = E[1]; }
+        else { out[6 * p] = E[0]; out[6 * p + 1] = E[4]; out[6 * p + 2] = E[8]; out[6 * p + 3] = E[1]; out[6 * p + 4] = E[5]; out[6 * p + 5] = E[6]; }
+        if (ok) ok[p] = 1;
+    }
+    free(V); free(W);
+    return 0;
+}
+
 int64_t olsm_n_samples(const olsm_sim *s) { return s ? s->ns : -1; }
 int64_t olsm_current_step(const olsm_sim *s) { return s ? s->step : -1; }
 
@@ -488,7 +563,7 @@ void olsm_destroy(olsm_sim *s)
 {
     if (!s) return;
     for (int gi = 0; gi < OLSM_MAX_GROUPS; ++gi) { free(s->g[gi].ids); free(s->g[gi].x0); }
-    free(s->poff); free(s->soff); free(s->x); free(s->v); free(s->f); free(s->fd); free(s->m);
+    free(s->poff); free(s->soff); free(s->x); free(s->xref); free(s->v); free(s->f); free(s->fd); free(s->m);
     free(s->si); free(s->sj); free(s->k); free(s->r0); free(s->rc); free(s->alive); free(s->break_step);
     free(s->nbroken); free(s->U); free(s->spec_of_spring); free(s->spec_of_particle); free(s->group_of);
     free(s->h_step); free(s->h_R); free(s->h_U); free(s->h_KE); free(s->h_nb);

@@ -47,6 +47,7 @@ def lib():
         L.olsm_read_broken.argtypes = [C.c_void_p, u8, i64, i64]
         L.olsm_read_energy.argtypes = [C.c_void_p, d, d]
         L.olsm_read_virial.argtypes = [C.c_void_p, d]
+        L.olsm_read_strain.argtypes = [C.c_void_p, d, u8]
         L.olsm_read_stress.argtypes = [C.c_void_p, C.c_int64, i64, i64, d, d, d, i64]
         L.olsm_n_samples.restype = C.c_int64
         L.olsm_n_samples.argtypes = [C.c_void_p]
@@ -143,6 +144,14 @@ class OracleSim:
         if lib().olsm_read_virial(self._h, _p(S, C.c_double)) != 0:
             raise ValueError("olsm_read_virial failed")
         return S
+
+    def read_strain(self):
+        """Per-particle Lagrangian strain (Eq. 8, reading Q21): ([N,3] = e_xx, e_yy, e_xy; 3-D: [N,6] = xx, yy, zz, xy, yz,
+        zx), ok[N] bool (False: fewer than D independent bonds, strain reported as 0)."""
+        E = np.empty((self.N, 3 if self.D == 2 else 6)); ok = np.empty(self.N, dtype=np.uint8)
+        if lib().olsm_read_strain(self._h, _p(E, C.c_double), _p(ok, C.c_uint8)) != 0:
+            raise ValueError("olsm_read_strain failed")
+        return E, ok.astype(bool)
 
     @property
     def current_step(self):

@@ -393,6 +393,110 @@ def test_P13_virial_kinetic_term_and_sum_rule():
     assert np.allclose((S[:, 0] + S[:, 1]).sum(), (k * (r - r0) * r).sum(), rtol=1e-12)
 
 
+# ---------------------------------------------------------------- P15: Lagrangian strain field, Eq. 8 (L150, L156), reading Q21
+def _green_lagrange(F):
+    F = np.asarray(F, dtype=float)
+    E = 0.5 * (F.T @ F - np.eye(F.shape[0]))
+    return np.array([E[0, 0], E[1, 1], E[0, 1]]) if F.shape[0] == 2 else np.array([E[0, 0], E[1, 1], E[2, 2], E[0, 1], E[1, 2], E[2, 0]])
+
+
+def test_P15_strain_of_a_homogeneous_deformation_is_green_lagrange():
+    """x -> F x + t with a NON-symmetric F (stretch + shear + rotation part): the local affine fit recovers F at every
+    particle that has two independent bonds -- interior, edge and corner alike -- so eps = (F^T F - I)/2 everywhere.
+    F F^T (a transposed J), F^T F without the 1/2, the small-strain (F + F^T)/2 - I: all differ from it by > 1e-2."""
+    nx, ny = 9, 7
+    x, si, sj, site, _ = triangular_lattice(nx, ny)
+    F = np.array([[1.25, 0.5], [0.125, 0.875]])
+    s = OracleSim(x, si, sj, 1.0, 1.0, 10.0, 0.01)
+    s.write_state(x @ F.T + np.array([3.0, -2.0]))
+    E, ok = s.read_strain()
+    want = _green_lagrange(F)
+    assert ok.all() and np.abs(E - want).max() <= 1e-13
+    wrong = [_green_lagrange(F.T), 2 * want, np.array([F[0, 0] - 1, F[1, 1] - 1, 0.5 * (F[0, 1] + F[1, 0])])]
+    assert min(np.abs(w - want).max() for w in wrong) > 1e-2
+    # rigid motion: rotation by 0.7 rad + translation -> zero strain
+    c, sn = np.cos(0.7), np.sin(0.7)
+    s.write_state(x @ np.array([[c, -sn], [sn, c]]).T + np.array([-1.0, 4.0]))
+    E, ok = s.read_strain()
+    assert ok.all() and np.abs(E).max() <= 1e-14
+    # the reference is the configuration given at create, not the last written state: undeformed again -> 0 (V V^-1 rounds)
+    s.write_state(x)
+    assert np.abs(s.read_strain()[0]).max() <= 1e-15
+
+
+@pytest.mark.parametrize("eps", [1e-3, 1e-6])
+def test_P15_small_strain_limit_of_the_uniaxial_state(eps):
+    """P3's affine state x * (1 - eps/3, 1 + eps) (Poisson's ratio 1/3): e_yy = eps + eps^2/2, e_xx = -eps/3 + eps^2/18,
+    e_xy = 0; to first order the symmetric displacement gradient (eps_yy = eps, eps_xx = -eps/3)."""
+    x, si, sj, site, _ = triangular_lattice(16, 12)
+    s = OracleSim(x * np.array([1.0 - eps / 3.0, 1.0 + eps]), si, sj, 1.0, 1.0, 2.0, 0.01)
+    assert np.abs(s.read_strain()[0]).max() <= 1e-15            # created in that state: it IS the reference
+    s = OracleSim(x, si, sj, 1.0, 1.0, 2.0, 0.01)
+    s.write_state(x * np.array([1.0 - eps / 3.0, 1.0 + eps]))
+    E, ok = s.read_strain()
+    assert ok.all()
+    assert np.abs(E[:, 1] - (eps + eps ** 2 / 2)).max() <= 1e-14 and np.abs(E[:, 0] - (-eps / 3 + eps ** 2 / 18)).max() <= 1e-14
+    assert np.abs(E[:, 2]).max() <= 1e-14
+    assert np.abs(E[:, 1] - eps).max() <= eps ** 2 and np.abs(E[:, 0] + eps / 3).max() <= eps ** 2
+
+
+def test_P15_least_squares_against_numpy_and_bond_selection():
+    """(a) a NON-affine displacement: per particle, J from numpy's lstsq (SVD) on the stacked bond vectors d0 J ~ d (the
+    row-vector form of Shimizu et al.), eps = (J J^T - I)/2 -- another routine, the paper's own index order;
+    (b) only bonds alive now count: a neighbour whose spring has broken (r > rc) does not enter the fit;
+    (c) fewer than two independent bonds (none, one, two collinear): flagged, reported as 0, never NaN."""
+    x, si, sj, site, _ = triangular_lattice(8, 6)
+    rng = np.random.default_rng(21)
+    s = OracleSim(x, si, sj, 1.0, 1.0, 10.0, 0.01)
+    xc = x @ np.array([[1.1, 0.2], [-0.1, 0.95]]).T + rng.uniform(-0.05, 0.05, x.shape)
+    s.write_state(xc)
+    E, ok = s.read_strain()
+    assert ok.all()
+    for p in range(x.shape[0]):
+        nb = np.concatenate([sj[si == p], si[sj == p]])
+        J = np.linalg.lstsq(x[nb] - x[p], xc[nb] - xc[p], rcond=None)[0]
+        G = 0.5 * (J @ J.T - np.eye(2))
+        assert np.abs(E[p] - [G[0, 0], G[1, 1], G[0, 1]]).max() <= 1e-13
+    # (b) centre 0 with neighbours 1, 2 (moved by F1) and 3 (torn away: its spring breaks at create + write_state)
+    F1 = np.array([[1.5, 0.25], [0.0, 0.75]])
+    x4 = np.array([[0.0, 0.0], [1.0, 0.0], [0.0, 1.0], [-1.0, -1.0], [5.0, 5.0], [6.0, 5.0], [7.0, 5.0], [9.0, 9.0]])
+    si4, sj4 = [0, 0, 0, 4, 5], [1, 2, 3, 5, 6]
+    s = OracleSim(x4, si4, sj4, 1.0, np.array([1.0, 1.0, np.sqrt(2.0), 1.0, 1.0]), np.array([9.0, 9.0, 2.0, 9.0, 9.0]), 0.01)
+    x4c = x4 @ F1.T
+    x4c[3] = [-4.0, -4.0]                                           # |d| = 5.66 > rc = 2: broken
+    x4c[4:7] = x4[4:7] * 1.5                                        # a collinear chain, stretched
+    s.write_state(x4c)
+    assert s.read_broken()[0].tolist() == [False, False, True, False, False]
+    E, ok = s.read_strain()
+    assert ok.tolist() == [True, False, False, False, False, False, False, False]
+    assert np.abs(E[0] - _green_lagrange(F1)).max() <= 1e-15        # from bonds 0-1 and 0-2 alone
+    assert np.all(E[1:] == 0.0) and np.isfinite(E).all()            # one bond (1, 2, 4, 6), none (3, 7), two collinear (5)
+
+
+def test_P15_strain_3d():
+    """D = 3: a non-symmetric homogeneous F on a cubic network with face diagonals -> (F^T F - I)/2 in the order
+    {xx, yy, zz, xy, yz, zx}; a rotation about a skew axis -> 0; a plain cubic network's corner (3 orthogonal bonds) is
+    still full rank, a particle with bonds in one plane only is flagged."""
+    from lsm_inputs import cubic_lattice_3d
+    x, si, sj, r0 = cubic_lattice_3d(4, 3, 5)
+    F = np.array([[1.25, 0.5, 0.0], [0.125, 0.875, 0.25], [-0.25, 0.0, 1.5]])
+    s = OracleSim(x, si, sj, 1.0, r0, 10.0 * r0, 0.01)
+    s.write_state(x @ F.T + np.array([1.0, 2.0, 3.0]))
+    E, ok = s.read_strain()
+    assert ok.all() and np.abs(E - _green_lagrange(F)).max() <= 1e-13
+    assert np.abs(_green_lagrange(F.T) - _green_lagrange(F)).max() > 1e-2
+    n = np.array([1.0, 2.0, 2.0]) / 3.0
+    K = np.array([[0, -n[2], n[1]], [n[2], 0, -n[0]], [-n[1], n[0], 0]])
+    R = np.eye(3) + np.sin(0.9) * K + (1 - np.cos(0.9)) * K @ K
+    s.write_state(x @ R.T)
+    assert np.abs(s.read_strain()[0]).max() <= 1e-14
+    xs, si2, sj2, r02 = cubic_lattice_3d(2, 2, 1, diagonals=False)   # a single square in the plane z = 0
+    s = OracleSim(xs, si2, sj2, 1.0, r02, 10.0 * r02, 0.01)
+    s.write_state(xs * 1.1)
+    E, ok = s.read_strain()
+    assert not ok.any() and np.all(E == 0.0)
+
+
 # ---------------------------------------------------------------- P14: the oracle's D = 3 branch (the paper's listing is 3-D, L93-L97)
 def test_P14_3d_oscillator_along_a_skew_axis_and_invariants():
     """(a) P1's worked example rotated onto the axis (1,2,2)/3: the 3-D trajectory must be the 1-D closed form along
