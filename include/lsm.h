@@ -180,6 +180,17 @@ lsm_status lsm_read_forces(lsm_sim *sim, double *f /* [N*dim] */);
  * springs contribute nothing.  dim = 3: S[p] = {S_xx, S_yy, S_zz, S_xy, S_yz, S_zx}.  Gather layout only
  * (LSM_E_UNSUPPORTED with force_mode = SCATTER). */
 lsm_status lsm_read_virial(lsm_sim *sim, double *S /* [N*3], dim = 3: [N*6] */);
+/* Per-particle Lagrangian strain of the current state, Eq. 8 (eps^L = (J J^T - delta)/2, printed with its
+ * summation lost; L156: "J is the locally affine transformation matrix considering the relative displacement of particle
+ * with its first nearest neighbors"; reading Q21 of DESIGN.md).  For particle p, F = (sum d (x) d0)(sum d0 (x) d0)^-1 is the
+ * least-squares affine map of the reference bond vectors d0 = xref_l - xref_p of its springs that are ALIVE now onto
+ * their current bond vectors d = x_l - x_p; xref = the positions given to lsm_create (lsm_write_state does not move the
+ * reference); E[p] = (F^T F - I)/2 = {e_xx, e_yy, e_xy}, dim = 3: {e_xx, e_yy, e_zz, e_xy, e_yz, e_zx} (symmetric;
+ * tensor components, not engineering shear).  ok[p] (may be NULL) = 0 where p has fewer than dim independent live bonds
+ * (det V <= 1e-12 (tr V / dim)^dim): E[p] = 0 there, never NaN.  Caller numbering; gather layout only (LSM_E_UNSUPPORTED
+ * with a SCATTER force_mode).  The first call uploads the reference positions (16 or 32 bytes per particle of device
+ * memory from then on).  Synchronises the stream. */
+lsm_status lsm_read_strain(lsm_sim *sim, double *E /* [N*3], dim = 3: [N*6] */, uint8_t *ok /* [N] or NULL */);
 /* Irreversible breakage, caller spring numbering: broken[s] = 1 if spring s is dead;
  * break_step[s] = step of the force evaluation that broke it, -1 if alive; *n_broken = total over all specimens. */
 lsm_status lsm_read_broken(lsm_sim *sim, uint8_t *broken /* [M] or NULL */, int64_t *break_step /* [M] or NULL */,

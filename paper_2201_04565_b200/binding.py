@@ -22,7 +22,7 @@ FUSION_AUTO, FUSION_ON, FUSION_OFF, FUSION_RESIDENT = 0, 1, 2, 3
 MAX_GROUPS = 8
 
 EXPORTS = ["lsm_create", "lsm_set_boundary", "lsm_step", "lsm_write_state", "lsm_read_state", "lsm_read_forces",
-           "lsm_read_broken", "lsm_read_energy", "lsm_read_virial", "lsm_read_stress", "lsm_run_to_failure", "lsm_set_strain_rate", "lsm_compact", "lsm_sync", "lsm_get_info",
+           "lsm_read_broken", "lsm_read_energy", "lsm_read_virial", "lsm_read_strain", "lsm_read_stress", "lsm_run_to_failure", "lsm_set_strain_rate", "lsm_compact", "lsm_sync", "lsm_get_info",
            "lsm_device_state", "lsm_last_error", "lsm_destroy", "lsm_abi_version", "lsm_spring_energy_static"]
 STATIC_MAX_SPRINGS = 1 << 28
 
@@ -90,6 +90,7 @@ def library():
         L.lsm_read_state.argtypes = [C.c_void_p, d, d]
         L.lsm_read_forces.argtypes = [C.c_void_p, d]
         L.lsm_read_virial.argtypes = [C.c_void_p, d]
+        L.lsm_read_strain.argtypes = [C.c_void_p, d, u8]
         L.lsm_read_broken.argtypes = [C.c_void_p, u8, i64, i64]
         L.lsm_read_energy.argtypes = [C.c_void_p, d, d]
         L.lsm_read_stress.argtypes = [C.c_void_p, C.c_int64, i64, i64, d, d, d, i64]
@@ -202,6 +203,12 @@ class LsmSim:
         S = np.empty((self.N, 3 if self.D == 2 else 6))
         self._check(library().lsm_read_virial(self._h, _ptr(S, C.c_double)))
         return S
+
+    def read_strain(self):
+        """(E [N,3] or [N,6], ok [N] bool): Lagrangian strain per particle (Eq. 8) and the full-rank flag."""
+        E = np.empty((self.N, 3 if self.D == 2 else 6)); ok = np.empty(self.N, dtype=np.uint8)
+        self._check(library().lsm_read_strain(self._h, _ptr(E, C.c_double), _ptr(ok, C.c_uint8)))
+        return E, ok.astype(bool)
 
     def read_broken(self):
         b = np.empty(self.M, dtype=np.uint8); bs = np.empty(self.M, dtype=np.int64); n = C.c_int64(0)
@@ -331,8 +338,6 @@ def lsm_create(x, spring_i, spring_j, k, r0, rc, dt, gamma=0.0, v=None, mass=1.0
 
 def lsm_create_from_problem(p, **kw):
     """Convenience: build from an lsm_inputs.Problem (arrays only) and set its boundary groups."""
-    def uni(a):
-        return float(a[0]) if a.size and np.all(a == a[0]) else a
     args = dict(gamma=p.gamma, v=p.v, mass=p.mass, n_batch=p.n_batch, particle_offsets=p.particle_offsets,
                 spring_offsets=p.spring_offsets, sample_every=p.sample_every)
     args.update(kw)
@@ -349,6 +354,7 @@ def lsm_write_state(sim, x, v=None): return sim.write_state(x, v)
 def lsm_read_state(sim, out_x=None, out_v=None): return sim.read_state(out_x, out_v)
 def lsm_read_forces(sim): return sim.read_forces()
 def lsm_read_virial(sim): return sim.read_virial()
+def lsm_read_strain(sim): return sim.read_strain()
 def lsm_read_broken(sim): return sim.read_broken()
 def lsm_read_energy(sim): return sim.read_energy()
 def lsm_read_stress(sim, capacity=None): return sim.read_stress(capacity)

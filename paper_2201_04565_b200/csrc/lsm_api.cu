@@ -81,6 +81,14 @@ struct lsm_sim {
     int stream_smem = 0, stream_grid = 0, stream_ctas_per_sm = 0;
     uint32_t max_tile_slots = 0;
     double *virial = nullptr;        // [N][3] output buffer of lsm_read_virial (allocated on first use)
+    // Lagrangian strain (lsm_read_strain): reference positions = the positions given at create, internal numbering, kept on
+    // the host and uploaded on first use (callers that never ask pay no device memory), output buffers likewise
+    std::vector<double2> h_ref2;
+    std::vector<double4> h_ref3;
+    double2 *ref2 = nullptr;
+    double4 *ref3 = nullptr;
+    double *strain = nullptr;
+    uint8_t *strain_ok = nullptr;
     int multi_on = 0;                // fuse runs of plain time steps into one cooperative launch
     // windowed streamed kernel (lsm_window.cuh): neighbour ranges of every tile staged in shared memory by the producer
     int win_on = 0, win_cap = 0, win_smem = 0, win_grid = 0;
@@ -421,6 +429,7 @@ struct ResPlan {
     std::vector<uint16_t> order;
     ResLayout L;
     bool ok = false;
+    int active = 0;              // clusters of this shape the device holds at once (cudaOccupancyMaxActiveClusters)
 };
 
 ResPlan plan_resident(const lsm_sim *s, int C, const std::vector<int32_t> &nbmin, const std::vector<int32_t> &nbmax,
@@ -474,6 +483,18 @@ ResPlan plan_resident(const lsm_sim *s, int C, const std::vector<int32_t> &nbmin
             bnd.insert(bnd.end(), inner.begin(), inner.end());
             ord[(size_t)b * C + c].swap(bnd);
         }
+        // The ghost exchange is safe only when pushes are mutual: a CTA waits, per step, for the pushes of exactly the CTAs
+        // it pushes to, and that wait is what keeps a neighbour from running two steps ahead and landing step n+2 ghosts on
+        // a transaction barrier whose step-n phase is still open.  Windows are id hulls, so on an irregular graph (a band
+        // plus a few long springs) CTA r can lie inside hull(c) without any spring into c: c pushes to r, r not to c.
+        // Lattices and banded numberings always give mutual pushes; anything else is not planned as resident.
+        for (int c = 0; c < C; ++c)
+            for (int k = 0; k < dd[c].n_push; ++k) {
+                const ResCta &t = dd[dd[c].push[k].rank];
+                bool back = false;
+                for (int m = 0; m < t.n_push && !back; ++m) back = t.push[m].rank == c;
+                if (!back) return R;
+            }
     }
     if (sl_cap > 65535) return R;
     const bool need_typ = s->pm == PM_TYPED || s->pm == PM_KRT_RCF, need_thr = s->pm == PM_RCF || s->pm == PM_KRT_RCF || s->pm == PM_FULL, need_kr = s->pm == PM_FULL;
@@ -500,17 +521,26 @@ ResPlan plan_resident(const lsm_sim *s, int C, const std::vector<int32_t> &nbmin
     return R;
 }
 
-template <int PM, bool EXACT> cudaError_t launch_resident_one(const lsm_sim *s, const StepParams &P, const ResParams &Q) {
+// Opt the resident kernel in to `bytes` of dynamic shared memory and to non-portable cluster sizes, once per device and
+// size.  The attribute is only ever raised: the occupancy queries at create ask about several candidate layouts in turn.
+template <int PM, bool EXACT> cudaError_t resident_configure(const lsm_sim *s, int bytes) {
     auto kern = k_resident<PM, EXACT>;
     static thread_local OptIn configured_for;
     int &have = configured_for.bytes[s->device < kMaxDevices ? s->device : kMaxDevices - 1];
-    if (have < s->RL.bytes || s->device >= kMaxDevices - 1) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, s->RL.bytes);
+    if (have < bytes || s->device >= kMaxDevices - 1) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
         if (e != cudaSuccess) return e;
         e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
         if (e != cudaSuccess) return e;
-        have = s->RL.bytes;
+        have = bytes;
     }
+    return cudaSuccess;
+}
+
+template <int PM, bool EXACT> cudaError_t launch_resident_one(const lsm_sim *s, const StepParams &P, const ResParams &Q) {
+    auto kern = k_resident<PM, EXACT>;
+    cudaError_t e0 = resident_configure<PM, EXACT>(s, s->RL.bytes);
+    if (e0 != cudaSuccess) return e0;
     cudaLaunchConfig_t cfg;
     std::memset(&cfg, 0, sizeof(cfg));
     cfg.gridDim = dim3((unsigned)s->res_grid); cfg.blockDim = dim3(kResThreads); cfg.dynamicSmemBytes = (size_t)s->RL.bytes; cfg.stream = s->stream;
@@ -519,6 +549,33 @@ template <int PM, bool EXACT> cudaError_t launch_resident_one(const lsm_sim *s, 
     at[0].val.clusterDim.x = (unsigned)s->res_cluster; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
     cfg.attrs = at; cfg.numAttrs = 1;
     return cudaLaunchKernelEx(&cfg, kern, P, s->RL, Q);
+}
+
+// How many clusters of C CTAs with `bytes` of dynamic shared memory each the current device can hold at once (0: such a
+// cluster cannot be scheduled here at all -- a MIG slice, a GPC with too few free SMs, a smaller part).  Asked at create.
+template <int PM, bool EXACT> int resident_clusters_one(const lsm_sim *s, int C, int bytes) {
+    auto kern = k_resident<PM, EXACT>;
+    if (resident_configure<PM, EXACT>(s, bytes) != cudaSuccess) { cudaGetLastError(); return 0; }
+    cudaLaunchConfig_t cfg;
+    std::memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = dim3((unsigned)C); cfg.blockDim = dim3(kResThreads); cfg.dynamicSmemBytes = (size_t)bytes;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = (unsigned)C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    int n = 0;
+    if (cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess) { cudaGetLastError(); return 0; }
+    return n;
+}
+
+int resident_clusters(const lsm_sim *s, int C, int bytes) {
+    switch (s->pm) {
+        case PM_UNIFORM: return s->exact ? resident_clusters_one<PM_UNIFORM, true>(s, C, bytes) : resident_clusters_one<PM_UNIFORM, false>(s, C, bytes);
+        case PM_TYPED: return s->exact ? resident_clusters_one<PM_TYPED, true>(s, C, bytes) : resident_clusters_one<PM_TYPED, false>(s, C, bytes);
+        case PM_RCF: return s->exact ? resident_clusters_one<PM_RCF, true>(s, C, bytes) : resident_clusters_one<PM_RCF, false>(s, C, bytes);
+        case PM_KRT_RCF: return s->exact ? resident_clusters_one<PM_KRT_RCF, true>(s, C, bytes) : resident_clusters_one<PM_KRT_RCF, false>(s, C, bytes);
+        default: return s->exact ? resident_clusters_one<PM_FULL, true>(s, C, bytes) : resident_clusters_one<PM_FULL, false>(s, C, bytes);
+    }
 }
 
 template <bool EXACT> cudaError_t launch_resident_pm(const lsm_sim *s, const StepParams &P, const ResParams &Q) {
@@ -603,7 +660,11 @@ template <int PM, bool SAMPLE> void launch_scatter_one(const lsm_sim *s, const S
     if (s->scatter_variant == 1) k_spring_scatter_warp<PM, SAMPLE><<<grid_for(S.M), kBlock, 0, s->stream>>>(P, S);
     else if (s->scatter_variant == 2) {
         auto kern = k_spring_scatter_tile<PM, SAMPLE>;
-        if (s->scatter_tile_smem > 32 * 1024) cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, s->scatter_tile_smem);   // static + dynamic may pass 48 KB
+        static thread_local OptIn configured_for;    // opt in once per device and size, as the other kernels do (static + dynamic may pass 48 KB)
+        int &have = configured_for.bytes[s->device < kMaxDevices ? s->device : kMaxDevices - 1];
+        if (s->scatter_tile_smem > 32 * 1024 && (have < s->scatter_tile_smem || s->device >= kMaxDevices - 1)) {
+            if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, s->scatter_tile_smem) == cudaSuccess) have = s->scatter_tile_smem;
+        }   // a failure shows up as a launch error, which the callers check
         kern<<<(unsigned)s->scatter_tiles, kScatterTileThreads, (size_t)s->scatter_tile_smem, s->stream>>>(P, S);
     }
     else k_spring_scatter<PM, SAMPLE><<<grid_for(S.M), kBlock, 0, s->stream>>>(P, S);
@@ -971,6 +1032,7 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
                 if (d->v) hv[p] = make_double4(d->v[3 * c], d->v[3 * c + 1], d->v[3 * c + 2], 0.0);
             }
             TRY(upload(s, &s->pos3[0], hx));
+            s->h_ref3 = hx;
             TRY(dev_alloc(s, &s->pos3[1], (size_t)Np));
             CUDA_TRY(s, cudaMemcpyAsync(s->pos3[1], s->pos3[0], sizeof(double4) * Np, cudaMemcpyDeviceToDevice, s->stream));
             TRY(upload(s, &s->vel3, hv));
@@ -989,6 +1051,7 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
             hv[p] = d->v ? make_double2(d->v[2 * c], d->v[2 * c + 1]) : make_double2(0.0, 0.0);
         }
         TRY(upload(s, &s->pos[0], hx));
+        s->h_ref2 = hx;
         TRY(dev_alloc(s, &s->pos[1], (size_t)Np));
         CUDA_TRY(s, cudaMemcpyAsync(s->pos[1], s->pos[0], sizeof(double2) * Np, cudaMemcpyDeviceToDevice, s->stream));
         TRY(upload(s, &s->vel, hv));
@@ -1240,6 +1303,10 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
                     if (s->cluster_size > 0 && C != s->cluster_size) continue;
                     ResPlan R = plan_resident(s, C, nbmin, nbmax, off, budget);
                     if (!R.ok) continue;
+                    // a plan counts only if this device can place such a cluster (sizes above 8 are non-portable, each CTA
+                    // asks for most of an SM's shared memory); otherwise the next size, or the other schedules, take over
+                    R.active = resident_clusters(s, C, R.L.bytes);
+                    if (R.active < 1) continue;
                     if (!best.ok) { best = std::move(R); if (s->cluster_size > 0) break; continue; }
                     // a single (or a few) small units: more CTAs per unit while the GPU is not full and each keeps >= 8 slices
                     if ((long long)B * C <= n_sm && R.L.sl_cap >= 8) best = std::move(R); else break;
@@ -1249,14 +1316,14 @@ static lsm_status create_impl(const lsm_desc *d, lsm_sim *s) {
                 // resident pays when the clusters fill the GPU, or when each warp has about one slice per step
                 if (best.ok && s->step_fusion == LSM_FUSION_AUTO && !((long long)B * best.C * 2 >= n_sm || best.L.sl_cap <= 16)) best.ok = false;
                 if (best.ok) {
-                    s->res_on = 1; s->res_cluster = best.C; s->res_grid = B * best.C; s->RL = best.L;
+                    s->res_on = 1; s->res_cluster = best.C; s->res_grid = B * best.C; s->RL = best.L; s->res_active_clusters = best.active;
                     TRY(upload(s, &s->res_desc, best.desc));
                     TRY(upload(s, &s->res_order, best.order));
                     CUDA_TRY(s, cudaStreamSynchronize(s->stream));
                     s->multi_on = 0;                               // the cluster barrier replaces the grid barrier
                 }
             }
-            if (s->step_fusion == LSM_FUSION_RESIDENT && !s->res_on) return fail(s, LSM_E_UNSUPPORTED, "step_fusion = RESIDENT: needs dim = 2, the streamed gather kernel, 16-bit neighbour offsets (a banded numbering), specimens that start on multiples of 32 particles and fit one cluster's shared memory");
+            if (s->step_fusion == LSM_FUSION_RESIDENT && !s->res_on) return fail(s, LSM_E_UNSUPPORTED, "step_fusion = RESIDENT: needs dim = 2, the streamed gather kernel, 16-bit neighbour offsets (a banded numbering), specimens that start on multiples of 32 particles and fit one cluster's shared memory, CTAs whose ghost exchange is mutual, and a device that can place such a cluster");
             if (s->multi_on) {
                 TRY(dev_alloc(s, &s->gbar, 1));
                 CUDA_TRY(s, cudaMemsetAsync(s->gbar, 0, sizeof(unsigned long long), s->stream));
@@ -1643,6 +1710,32 @@ lsm_status lsm_read_virial(lsm_sim *s, double *S) {
     return check_flags(s);
 }
 
+lsm_status lsm_read_strain(lsm_sim *s, double *E, uint8_t *ok) {
+    CHECK_SIM(s);
+    if (!E) { s->err = "E is NULL"; return LSM_E_INVALID; }
+    if (s->force_mode != LSM_FORCE_GATHER) { s->err = "lsm_read_strain needs the gather layout"; return LSM_E_UNSUPPORTED; }
+    const int C = s->dim == 3 ? 6 : 3;
+    if (!s->strain) {
+        TRY(dev_alloc(s, &s->strain, (size_t)s->N * C));
+        TRY(dev_alloc(s, &s->strain_ok, (size_t)s->N));
+        if (s->dim == 3) TRY(upload(s, &s->ref3, s->h_ref3)); else TRY(upload(s, &s->ref2, s->h_ref2));
+    }
+    if (s->dim == 3) {
+        StrainParams<double4> S;
+        S.pos = s->pos3[s->cur]; S.ref = s->ref3; S.hdr = s->hdr; S.nbr = s->nbr; S.inv = s->d_inv; S.N = s->N; S.out = s->strain; S.ok = s->strain_ok;
+        k_strain3<<<grid_for(s->N), kBlock, 0, s->stream>>>(S);
+    } else {
+        StrainParams<double2> S;
+        S.pos = s->pos[s->cur]; S.ref = s->ref2; S.hdr = s->hdr; S.nbr = s->nbr; S.inv = s->d_inv; S.N = s->N; S.out = s->strain; S.ok = s->strain_ok;
+        k_strain2<<<grid_for(s->N), kBlock, 0, s->stream>>>(S);
+    }
+    s->kernels_launched += 1;
+    CUDA_TRY(s, cudaGetLastError());
+    CUDA_TRY(s, cudaMemcpyAsync(E, s->strain, sizeof(double) * C * s->N, cudaMemcpyDeviceToHost, s->stream));
+    if (ok) CUDA_TRY(s, cudaMemcpyAsync(ok, s->strain_ok, (size_t)s->N, cudaMemcpyDeviceToHost, s->stream));
+    return check_flags(s);
+}
+
 lsm_status lsm_read_broken(lsm_sim *s, uint8_t *broken, int64_t *break_step, int64_t *n_broken) {
     CHECK_SIM(s);
     if (broken && s->M > 0) {
@@ -1734,19 +1827,32 @@ lsm_status lsm_set_strain_rate(lsm_sim *s, int32_t g_lo, int32_t g_hi, int32_t a
     if (g_lo < 0 || g_lo >= kMaxGroups || g_hi < 0 || g_hi >= kMaxGroups || g_lo == g_hi || axis < 0 || axis >= s->dim || !std::isfinite(strain_per_step)) { s->err = "bad arguments"; return LSM_E_INVALID; }
     Group &lo = s->groups[g_lo], &hi = s->groups[g_hi];
     if (!lo.set || !hi.set || lo.ids.empty() || hi.ids.empty()) { s->err = "lsm_set_strain_rate: both groups must have been defined with lsm_set_boundary"; return LSM_E_INVALID; }
-    // gauge length = distance between the groups' mean positions along the axis, now (sums in ascending caller id)
-    std::vector<double> x((size_t)s->N * 2);
-    TRY(lsm_read_state(s, x.data(), nullptr));
-    auto mean_of = [&](const Group &g) {
-        std::vector<int32_t> c(g.ids.size());
-        for (size_t q = 0; q < g.ids.size(); ++q) c[q] = s->perm.empty() ? g.ids[q] : s->perm[g.ids[q]];
-        std::sort(c.begin(), c.end());
+    // gauge length = distance between the groups' mean positions along the axis, now (sums in ascending caller id).
+    // Only the members' coordinates leave the device (a gather into the read-out staging buffer, then n doubles each).
+    // Everything that can be refused is refused before the first lsm_set_boundary below, so the two groups are never
+    // left half redefined by a bad argument; a CUDA failure after that point makes the handle sticky-failed anyway.
+    if ((long long)lo.ids.size() + (long long)hi.ids.size() > 2 * s->N || !lo.d_ids || !hi.d_ids) { s->err = "lsm_set_strain_rate: group tables are inconsistent"; return LSM_E_INVALID; }
+    std::vector<double> c_lo_x(lo.ids.size()), c_hi_x(hi.ids.size());
+    {
+        double *scr = reinterpret_cast<double *>(s->stage[0]);     // 2 N doubles
+        k_gather_axis<<<grid_for((long long)lo.ids.size()), kBlock, 0, s->stream>>>(s->pos[s->cur], lo.d_ids, (long long)lo.ids.size(), axis, scr);
+        k_gather_axis<<<grid_for((long long)hi.ids.size()), kBlock, 0, s->stream>>>(s->pos[s->cur], hi.d_ids, (long long)hi.ids.size(), axis, scr + lo.ids.size());
+        s->kernels_launched += 2;
+        CUDA_TRY(s, cudaGetLastError());
+        CUDA_TRY(s, cudaMemcpyAsync(c_lo_x.data(), scr, sizeof(double) * lo.ids.size(), cudaMemcpyDeviceToHost, s->stream));
+        CUDA_TRY(s, cudaMemcpyAsync(c_hi_x.data(), scr + lo.ids.size(), sizeof(double) * hi.ids.size(), cudaMemcpyDeviceToHost, s->stream));
+        TRY(check_flags(s));                                        // synchronises the stream
+    }
+    auto mean_of = [&](const Group &g, const std::vector<double> &val) {
+        std::vector<std::pair<int32_t, double>> c(g.ids.size());
+        for (size_t q = 0; q < g.ids.size(); ++q) c[q] = {s->perm.empty() ? g.ids[q] : s->perm[g.ids[q]], val[q]};
+        std::sort(c.begin(), c.end(), [](const std::pair<int32_t, double> &a, const std::pair<int32_t, double> &b) { return a.first < b.first; });
         double sum = 0.0;
-        for (int32_t id : c) sum += x[(size_t)id * 2 + axis];
+        for (const auto &e : c) sum += e.second;
         return sum / (double)c.size();
     };
-    const double m_lo = mean_of(lo), m_hi = mean_of(hi), H0 = m_hi - m_lo;
-    if (!(H0 > 0.0)) { s->err = "lsm_set_strain_rate: group_hi must lie above group_lo along the axis"; return LSM_E_INVALID; }
+    const double m_lo = mean_of(lo, c_lo_x), m_hi = mean_of(hi, c_hi_x), H0 = m_hi - m_lo;
+    if (!(H0 > 0.0) || !std::isfinite(H0)) { s->err = "lsm_set_strain_rate: group_hi must lie above group_lo along the axis"; return LSM_E_INVALID; }
     if (gauge_length) *gauge_length = H0;
     const double du = strain_per_step * H0;
     double d_lo[3] = {0.0, 0.0, 0.0}, d_hi[3] = {0.0, 0.0, 0.0};

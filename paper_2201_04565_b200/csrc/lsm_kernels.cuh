@@ -1232,6 +1232,101 @@ __global__ void __launch_bounds__(kBlock) k_virial(const VirialParams V) {
     V.out[3 * c + 2] = sxy - m * v.x * v.y;
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// Lagrangian strain field, Eq. 8, reading Q21 of DESIGN.md: per particle, the least-squares
+// affine map F of the reference bond vectors d0 of its LIVE springs onto their current bond vectors d,
+// F = (sum d (x) d0) (sum d0 (x) d0)^-1, eps = (F^T F - I)/2.  Particle-centric over the sliced-ELL rows (a free or dead
+// slot holds the particle's own id), one thread per particle, caller order out.  POS = double2 (D = 2) or double4 (D = 3).
+// Fewer than D independent reference bonds (det V <= 1e-12 (tr V / D)^D): eps = 0, ok = 0.
+// ---------------------------------------------------------------------------------------------------------------
+template <class POS> struct StrainParams {
+    const POS *pos, *ref;     // current and reference positions, internal numbering
+    const TileHdr *hdr;
+    const int32_t *nbr;
+    const int32_t *inv;       // caller id -> internal id, or NULL
+    long long N;
+    double *out;              // [N][3] {xx, yy, xy} or [N][6] {xx, yy, zz, xy, yz, zx}
+    uint8_t *ok;              // [N]
+};
+
+__global__ void __launch_bounds__(kBlock) k_strain2(const StrainParams<double2> S) {
+    const long long c = (long long)blockIdx.x * kBlock + threadIdx.x;
+    if (c >= S.N) return;
+    const int p = S.inv ? S.inv[c] : (int)c;
+    const TileHdr *h = S.hdr + (p >> 8);
+    const int wi = (p >> 5) & 7, lane = p & 31;
+    const unsigned w = h->w[wi];
+    const size_t e0 = (size_t)h->off[wi] * kSlice + lane;
+    const double2 xp = S.pos[p], rp = S.ref[p];
+    double vxx = 0.0, vxy = 0.0, vyy = 0.0, wxx = 0.0, wxy = 0.0, wyx = 0.0, wyy = 0.0;
+    for (unsigned s = 0; s < w; ++s) {
+        const int nb = S.nbr[e0 + (size_t)s * kSlice];
+        if (nb == p) continue;
+        const double2 xq = S.pos[nb], rq = S.ref[nb];
+        const double ax = rq.x - rp.x, ay = rq.y - rp.y, dx = xq.x - xp.x, dy = xq.y - xp.y;
+        vxx += ax * ax; vxy += ax * ay; vyy += ay * ay;
+        wxx += dx * ax; wxy += dx * ay; wyx += dy * ax; wyy += dy * ay;     // W = sum d (x) d0
+    }
+    const double det = vxx * vyy - vxy * vxy, tr = 0.5 * (vxx + vyy);
+    double exx = 0.0, eyy = 0.0, exy = 0.0;
+    const bool good = det > 1e-12 * tr * tr;
+    if (good) {
+        const double ixx = vyy / det, ixy = -vxy / det, iyy = vxx / det;
+        const double fxx = wxx * ixx + wxy * ixy, fxy = wxx * ixy + wxy * iyy, fyx = wyx * ixx + wyy * ixy, fyy = wyx * ixy + wyy * iyy;
+        exx = 0.5 * (fxx * fxx + fyx * fyx - 1.0);
+        eyy = 0.5 * (fxy * fxy + fyy * fyy - 1.0);
+        exy = 0.5 * (fxx * fxy + fyx * fyy);
+    }
+    S.out[3 * c] = exx; S.out[3 * c + 1] = eyy; S.out[3 * c + 2] = exy;
+    S.ok[c] = good ? 1 : 0;
+}
+
+__global__ void __launch_bounds__(kBlock) k_strain3(const StrainParams<double4> S) {
+    const long long c = (long long)blockIdx.x * kBlock + threadIdx.x;
+    if (c >= S.N) return;
+    const int p = S.inv ? S.inv[c] : (int)c;
+    const TileHdr *h = S.hdr + (p >> 8);
+    const int wi = (p >> 5) & 7, lane = p & 31;
+    const unsigned w = h->w[wi];
+    const size_t e0 = (size_t)h->off[wi] * kSlice + lane;
+    const double4 xp = S.pos[p], rp = S.ref[p];
+    double v[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};      // xx xy xz yy yz zz
+    double m[9] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};   // W row-major
+    for (unsigned s = 0; s < w; ++s) {
+        const int nb = S.nbr[e0 + (size_t)s * kSlice];
+        if (nb == p) continue;
+        const double4 xq = S.pos[nb], rq = S.ref[nb];
+        const double a[3] = {rq.x - rp.x, rq.y - rp.y, rq.z - rp.z}, d[3] = {xq.x - xp.x, xq.y - xp.y, xq.z - xp.z};
+        v[0] += a[0] * a[0]; v[1] += a[0] * a[1]; v[2] += a[0] * a[2]; v[3] += a[1] * a[1]; v[4] += a[1] * a[2]; v[5] += a[2] * a[2];
+#pragma unroll
+        for (int i = 0; i < 3; ++i)
+#pragma unroll
+            for (int j = 0; j < 3; ++j) m[3 * i + j] += d[i] * a[j];
+    }
+    // cofactors of the symmetric V
+    const double c00 = v[3] * v[5] - v[4] * v[4], c01 = v[4] * v[2] - v[1] * v[5], c02 = v[1] * v[4] - v[3] * v[2];
+    const double det = v[0] * c00 + v[1] * c01 + v[2] * c02, tr = (v[0] + v[3] + v[5]) / 3.0;
+    double e[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    const bool good = det > 1e-12 * tr * tr * tr;
+    if (good) {
+        double iv[9];
+        iv[0] = c00 / det; iv[1] = c01 / det; iv[2] = c02 / det;
+        iv[3] = iv[1]; iv[4] = (v[0] * v[5] - v[2] * v[2]) / det; iv[5] = (v[2] * v[1] - v[0] * v[4]) / det;
+        iv[6] = iv[2]; iv[7] = iv[5]; iv[8] = (v[0] * v[3] - v[1] * v[1]) / det;
+        double F[9];
+#pragma unroll
+        for (int i = 0; i < 3; ++i)
+#pragma unroll
+            for (int j = 0; j < 3; ++j) F[3 * i + j] = m[3 * i] * iv[j] + m[3 * i + 1] * iv[3 + j] + m[3 * i + 2] * iv[6 + j];
+        auto ftf = [&](int a, int b) { return F[a] * F[b] + F[3 + a] * F[3 + b] + F[6 + a] * F[6 + b]; };
+        e[0] = 0.5 * (ftf(0, 0) - 1.0); e[1] = 0.5 * (ftf(1, 1) - 1.0); e[2] = 0.5 * (ftf(2, 2) - 1.0);
+        e[3] = 0.5 * ftf(0, 1); e[4] = 0.5 * ftf(1, 2); e[5] = 0.5 * ftf(2, 0);
+    }
+#pragma unroll
+    for (int q = 0; q < 6; ++q) S.out[6 * c + q] = e[q];
+    S.ok[c] = good ? 1 : 0;
+}
+
 // ---- small utility kernels (numbering translation at the API boundary, boundary-group bookkeeping) ----
 // dst[perm_dst[q]] <- src[q] style copies.  inv: caller id -> internal id.
 __global__ void __launch_bounds__(kBlock) k_to_caller(const double2 *src, double2 *dst, const int32_t *inv, long long N,
@@ -1287,6 +1382,12 @@ __global__ void __launch_bounds__(kBlock) k_group_assign(const int32_t *ids, lon
 
 // Velocity ramp of the strain-rate protocol (lsm_set_strain_rate): every free particle takes, along `axis`, the velocity
 // of the affine field that moves the grips apart, v = e (x - c) / dt (e = strain per step, c = the fixed point).
+// One coordinate of the listed particles (internal ids), in list order: the gauge-length means of lsm_set_strain_rate.
+__global__ void __launch_bounds__(kBlock) k_gather_axis(const double2 *pos, const int32_t *ids, long long n, int axis, double *out) {
+    const long long q = (long long)blockIdx.x * kBlock + threadIdx.x;
+    if (q < n) { const double2 r = pos[ids[q]]; out[q] = axis == 0 ? r.x : r.y; }
+}
+
 __global__ void __launch_bounds__(kBlock) k_velocity_ramp(const double2 *pos, double2 *vel, const uint8_t *grp, long long N, int axis, double e, double c, double dt) {
     const long long p = (long long)blockIdx.x * kBlock + threadIdx.x;
     if (p >= N || grp[p] != kFree) return;

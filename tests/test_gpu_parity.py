@@ -59,7 +59,13 @@ def test_T1_forces_single_evaluation(make, mode, reorder):
     if mode["exact"]:
         assert np.array_equal(fo, fg)
     else:
-        check_forces(fg, fo, sc)
+        # Q11 as written.  The R4 floor is added only where the input itself says the bound cannot be met by ANY fp64
+        # evaluation: a particle for which ONE ulp in r (k r eps per spring) already exceeds 1e-12 of its own contributions
+        # (cfg3-160 has two such particles: all their live springs are within 1e-3 of rest length).  Measured errors:
+        # DESIGN.md "Tolerances".
+        one_ulp = conditioning_floor(p.x, p.spring_i, p.spring_j, p.k, ~bo, ulps=1.0)
+        ill = bool((one_ulp > 1e-12 * sc)[sc > 0].any())
+        check_forces(fg, fo, sc, floor=conditioning_floor(p.x, p.spring_i, p.spring_j, p.k, ~bo) if ill else None, label="T1 " + p.name)
     Uo, KEo = o.read_energy(); Ug, KEg = g.read_energy()
     assert np.allclose(Ug, Uo, rtol=1e-12, atol=0) and np.allclose(KEg, KEo, rtol=1e-12, atol=1e-300)
     g.close()
@@ -388,7 +394,7 @@ def test_full_size_config3_bench_configuration():
     fo, fg = o.read_forces(), g.read_forces()
     bo = o.read_broken()[0]
     sc = force_scale(xo, p.spring_i, p.spring_j, p.k, p.r0, ~bo)
-    check_forces(fg, fo, sc, floor=conditioning_floor(xo, p.spring_i, p.spring_j, p.k, ~bo))
+    check_forces(fg, fo, sc, floor=conditioning_floor(xo, p.spring_i, p.spring_j, p.k, ~bo), label="cfg3-full step 200")
     assert np.abs(fg.sum(axis=0)).max() <= 1e-9 * np.abs(fg).sum()
     g.close()
 
@@ -436,7 +442,7 @@ def test_config2_at_its_own_size():
     g = lsm_create_from_problem(p)
     e = lsm_create_from_problem(p, exact=True)
     assert g.info()["step_fusion"] == 1 and g.info()["param_mode"] == 1
-    check_forces(g.read_forces(), f0, sc0, floor=conditioning_floor(p.x, p.spring_i, p.spring_j, p.k))
+    check_forces(g.read_forces(), f0, sc0, floor=conditioning_floor(p.x, p.spring_i, p.spring_j, p.k), label="cfg2-full step 0")
     assert np.array_equal(e.read_forces(), f0)
     o.step(200); g.step(200); e.step(200)
     xo, vo = o.read_state(); xg, vg = g.read_state(); xe, ve = e.read_state()
@@ -613,6 +619,35 @@ def test_resident_clusters_bit_identical_in_exact_mode(cluster):
     g.close()
 
 
+def test_resident_refuses_one_sided_ghost_exchange():
+    """A band plus a few long springs: a CTA's window is the id hull of its neighbours, so CTA 0 (which owns an end of a
+    long spring) sees CTA 2's particles as ghosts while CTA 2 reads nothing of CTA 0.  CTA 2 would push to CTA 0 and never
+    wait for it -- the per-step wait that keeps neighbours within one step of each other is missing.  Such a plan must not
+    be made: explicit RESIDENT with 4 or 8 CTAs is refused, one CTA (no exchange) and AUTO stay bit-identical."""
+    nx, ny = 32, 64
+    x, si, sj, site, _ = triangular_lattice(nx, ny)
+    long_i = np.array([2 * nx + 5, 10 * nx + 3, 5 * nx + 20], dtype=np.int32)
+    long_j = np.array([60 * nx + 7, 50 * nx + 1, 40 * nx + 9], dtype=np.int32)
+    si = np.concatenate([si, long_i]); sj = np.concatenate([sj, long_j])
+    r0 = np.ones(si.size); r0[-3:] = np.linalg.norm(x[long_j] - x[long_i], axis=1) * 0.999      # slightly stretched tie rods
+    x = x + np.random.default_rng(8).uniform(-0.02, 0.02, x.shape)
+    rc = 1.5 * r0
+    bot = np.flatnonzero(site // nx == 0).astype(np.int32)
+    o = OracleSim(x, si, sj, 1.0, r0, rc, 0.03, gamma=0.01); o.set_boundary(0, bot, FIXED); o.step(800)
+    xo, vo = o.read_state()
+    for C in (4, 8):
+        with pytest.raises(lsm.LsmError) as ei:
+            lsm.lsm_create(x, si, sj, 1.0, r0, rc, 0.03, gamma=0.01, exact=True, step_fusion=lsm.FUSION_RESIDENT, cluster_size=C)
+        assert ei.value.status == -7
+    for kw in (dict(step_fusion=lsm.FUSION_RESIDENT, cluster_size=1), dict()):
+        g = lsm.lsm_create(x, si, sj, 1.0, r0, rc, 0.03, gamma=0.01, exact=True, **kw)
+        g.set_boundary(0, bot, FIXED); g.step(800)
+        assert g.info()["cluster_size"] <= 1 or "step_fusion" not in kw
+        xg, vg = g.read_state()
+        assert np.array_equal(xo, xg) and np.array_equal(vo, vg)
+        g.close()
+
+
 def test_resident_ragged_batch_and_fast_mode():
     """(a) a lattice whose particle count is not a multiple of 32 (ragged last slice), per-spring rc and typed k;
     (b) a batch of 6 specimens (one cluster each) against the oracle stepping each alone, exact mode;
@@ -747,14 +782,16 @@ def test_full_size_config4_sampled_specimens():
     xg, vg = g.read_state(); hg = g.read_stress()
     assert hg["U"].shape == (3, B)
     po = pb.particle_offsets
-    for b in np.random.default_rng(4).choice(B, 4, replace=False):
+    for b in np.random.default_rng(4).choice(B, 8, replace=False):     # 8 randomly chosen specimens
         ps = single_specimen(int(b)); ps.sample_every = 100
         o = OracleSim.from_problem(ps); o.step(nsteps)
         xo, vo = o.read_state(); ho = o.read_stress()
         sl = slice(po[b], po[b + 1])
         assert np.abs(xg[sl] - xo).max() <= 1e-11 and np.abs(vg[sl] - vo).max() <= 1e-11
         assert np.allclose(hg["U"][:, b], ho["U"][:, 0], rtol=1e-10) and np.allclose(hg["KE"][:, b], ho["KE"][:, 0], rtol=1e-10)
-        assert np.allclose(hg["R"][:, b], ho["R"][:, 0], rtol=1e-9, atol=1e-13)
+        # T2's norm for the sampled reactions: 1e-9 of the specimen's largest reaction.  (A per-component relative bound is
+        # not meaningful for R_x of a grip, a sum of ~128 lateral forces that cancel to 1e-3 of R_y.)
+        assert np.abs(hg["R"][:, b] - ho["R"][:, 0]).max() <= 1e-9 * np.abs(ho["R"][:, 0]).max()
     g.close()
 
 
@@ -768,8 +805,8 @@ def test_large_config5_first_steps(n):
     assert g.info()["param_mode"] == 0 and g.info()["bytes_per_half_edge"] == 2     # uniform parameters, 16-bit neighbour offsets
     fo, fg = o.read_forces(), g.read_forces()
     sc = force_scale(p.x, p.spring_i, p.spring_j, p.k, p.r0)
-    check_forces(fg, fo, sc, floor=conditioning_floor(p.x, p.spring_i, p.spring_j, p.k))
-    o.step(5); g.step(5)
+    check_forces(fg, fo, sc, floor=conditioning_floor(p.x, p.spring_i, p.spring_j, p.k), label="cfg5-%d" % n)
+    o.step(20); g.step(20)                                     # config 5's 20 parity steps
     xo, vo = o.read_state(); xg, vg = g.read_state()
     eps = np.finfo(np.float64).eps
     assert np.abs(xg - xo).max() <= 32 * eps * np.abs(xo).max() and np.abs(vg - vo).max() <= 1e-12
@@ -847,6 +884,83 @@ def test_virial_stress_matches_oracle(reorder):
     So, Sg = o.read_virial(), g.read_virial()
     assert np.abs(Sg - So).max() <= 1e-12 * np.abs(So).max()
     g.close()
+
+
+# ---------------------------------------------------------------- NEXT-4 second half: Lagrangian strain field (Eq. 8)
+def _check_strain(Eg, okg, Eo, oko):
+    """Element by element.  The flag is an fp64 decision both sides take with the same formula; the strain of a
+    well-conditioned neighbourhood agrees to rounding, |dE| <= 1e-11 max(1, |E|) (near a crack a particle may keep two
+    almost collinear bonds: V is then badly conditioned, which the bound's |E| term -- E grows as 1/det -- absorbs)."""
+    assert np.array_equal(okg, oko)
+    assert np.all(Eg[~okg] == 0.0) and np.isfinite(Eg).all()
+    assert np.all(np.abs(Eg - Eo) <= 1e-11 * np.maximum(1.0, np.abs(Eo).max(axis=1, keepdims=True)))
+
+
+@pytest.mark.parametrize("reorder", [0, 1, 2, 3])
+def test_strain_field_matches_oracle(reorder):
+    """lsm_read_strain against the oracle's Eq. 8 (reading Q21): (a) a homogeneous non-symmetric deformation written with
+    lsm_write_state gives (F^T F - I)/2 at every particle through the CUDA path too; (b) a specimen pulled until it has
+    cracked (exact mode, so both sides hold the same positions and the same broken set), with and without compaction:
+    every particle's strain and full-rank flag, under every renumbering; the strain is large only next to the crack;
+    (c) a batch with per-spring rc in fast mode right after create: all zero."""
+    x, si, sj, site, _ = triangular_lattice(37, 29)
+    F = np.array([[1.25, 0.5], [0.125, 0.875]])
+    g = lsm.lsm_create(x, si, sj, 1.0, 1.0, 10.0, 0.01, reorder=reorder)
+    g.write_state(x @ F.T + np.array([3.0, -2.0]))
+    E, ok = g.read_strain()
+    G = 0.5 * (F.T @ F - np.eye(2))
+    assert ok.all() and np.abs(E - [G[0, 0], G[1, 1], G[0, 1]]).max() <= 1e-13
+    g.close()
+    p = _fracture_problem(n=48, du_y=6e-4, seed=11)
+    o = OracleSim.from_problem(p); o.step(3700)
+    Eo, oko = o.read_strain()
+    bo, _, nbo = o.read_broken()
+    assert nbo > 0 and np.abs(Eo).max() > 0.05 and np.median(np.abs(Eo[:, 1])) < 0.05
+    for compact in (0, 500):
+        g = lsm_create_from_problem(p, reorder=reorder, exact=True, compact_every=compact); g.step(3700)
+        assert np.array_equal(g.read_state()[0], o.read_state()[0]) and np.array_equal(bo, g.read_broken()[0])
+        Eg, okg = g.read_strain()
+        _check_strain(Eg, okg, Eo, oko)
+        g.step(10); o2 = None                                   # a second call after more steps reuses the uploaded reference
+        Eg2, _ = g.read_strain()
+        assert not np.array_equal(Eg2, Eg)
+        g.close()
+    q = config3(n=96)
+    g = lsm_create_from_problem(q, reorder=reorder)
+    E, ok = g.read_strain()
+    oq = OracleSim.from_problem(q)
+    assert np.array_equal(ok, oq.read_strain()[1]) and np.abs(E).max() <= 1e-15
+    g.close()
+    with pytest.raises(lsm.LsmError) as ei:
+        lsm_create_from_problem(config1(), force_mode=lsm.FORCE_SCATTER).read_strain()
+    assert ei.value.status == -7
+
+
+def test_strain_field_3d_matches_oracle():
+    """D = 3: homogeneous F through lsm_write_state, then the pulled, partly broken 3-D network of the 3-D parity test."""
+    x, si, sj, k, r0, rc, bot, top = _problem_3d()
+    F = np.array([[1.25, 0.5, 0.0], [0.125, 0.875, 0.25], [-0.25, 0.0, 1.5]])
+    o = OracleSim(x, si, sj, k, r0, 50.0 * r0, 0.02); g = lsm.lsm_create(x, si, sj, k, r0, 50.0 * r0, 0.02)
+    xf = x @ F.T
+    o.write_state(xf); g.write_state(xf)
+    Eo, oko = o.read_strain(); Eg, okg = g.read_strain()
+    G = 0.5 * (F.T @ F - np.eye(3))
+    assert oko.all() and np.abs(Eo - [G[0, 0], G[1, 1], G[2, 2], G[0, 1], G[1, 2], G[2, 0]]).max() <= 1e-12
+    _check_strain(Eg, okg, Eo, oko)
+    g.close()
+    du = np.array([0.0, 1e-4, 4e-4])
+    o = OracleSim(x, si, sj, k, r0, rc, 0.02, gamma=0.02); o.set_boundary(0, bot, FIXED); o.set_boundary(1, top, MOVE, du)
+    o.step(2500)
+    assert o.read_broken()[2] > 5
+    Eo, oko = o.read_strain()
+    for reorder in (0, 1):
+        g = lsm.lsm_create(x, si, sj, k, r0, rc, 0.02, gamma=0.02, exact=True, reorder=reorder, compact_every=300)
+        g.set_boundary(0, bot, FIXED); g.set_boundary(1, top, MOVE, du)
+        g.step(2500)
+        assert np.array_equal(g.read_state()[0], o.read_state()[0])
+        Eg, okg = g.read_strain()
+        _check_strain(Eg, okg, Eo, oko)
+        g.close()
 
 
 # ---------------------------------------------------------------- the paper's protocol: both grips displaced apart, run to failure
@@ -1021,7 +1135,7 @@ def test_cooperative_launch_with_windows_bit_identical():
     p = config2(n=384, seed=11, n_blobs=80, du_y=8e-3)
     p.sample_every = 50
     nsteps = 1200
-    o = OracleSim.from_problem(p); o.set_threads(8); o.step(nsteps)
+    o = OracleSim.from_problem(p); o.step(nsteps)            # the serial reference loop, as in every parity test
     xo, vo = o.read_state(); bso, nbo = o.read_broken()[1:]
     assert nbo > 0
     g = lsm_create_from_problem(p, exact=True, step_fusion=lsm.FUSION_ON, compact_every=350)
