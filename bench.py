@@ -156,7 +156,20 @@ def oracle_legs(p, n_steps, what):
     return out
 
 
-def measure_device(p, inner, reps, warm, **create_kw):
+def step_kernel_name(inf):
+    """The kernel that carries the plain time steps of a handle, from lsm_get_info (the names of csrc/)."""
+    if inf["force_mode"] != 2:
+        return {1: "k_spring_scatter", 3: "k_spring_scatter_warp", 4: "k_spring_scatter_tile"}.get(inf["force_mode"], "k_spring_scatter")
+    if inf["step_fusion"] == 2:
+        return "k_resident"
+    if inf["gather_variant"] == 1:
+        return "k_gather_step"
+    if inf["window_particles"] > 0:
+        return "k_coop_win" if inf["step_fusion"] == 1 else "k_gather_win"
+    return "k_gather_stream"
+
+
+def measure_device(p, inner, reps, warm, compact_now=False, **create_kw):
     """Device-resident throughput of one workload: `reps` lsm_step(inner) calls timed with CUDA events after `warm`
     untimed calls.  Returns (seconds per time step, info, live springs at start, broken at end)."""
     import torch
@@ -164,6 +177,9 @@ def measure_device(p, inner, reps, warm, **create_kw):
     sim = lsm_create_from_problem(p, **create_kw)
     inf = sim.info()
     alive0 = p.M - sim.n_broken()
+    if compact_now:
+        sim.compact()
+        inf = dict(inf, n_half_edges_stored_before_compaction=inf["n_half_edges_stored"], n_half_edges_stored=sim.info()["n_half_edges_stored"])
     for _ in range(warm):
         sim.step(inner)
     sim.read_stress()
@@ -212,7 +228,12 @@ def other_workloads_table(peak, budget_s, with_cpu):
                "spring_updates_per_s": alive0 * 1.0 / t, "broken_at_end": nb, "step_fusion": inf["step_fusion"],
                "cluster_size": inf["cluster_size"], "param_mode": inf["param_mode"], "bytes_per_half_edge": inf["bytes_per_half_edge"],
                "counted_bytes_per_time_step": bc, "p_var": pv,
+               "step_kernel": step_kernel_name(inf),
                "roofline": ("L2-resident / latency-bound: HBM roofline does not apply (t_roof by bytes %.2f us)" % (bc / peak / 1e3)) if resident_l2
+               else {"bound": "smem/issue (cluster-resident: ~1 % of the counted bytes reach DRAM, profiles/r2_cfg4_cfg5_resident.md)",
+                     "counted_bytes_equiv_frac": bc / t / 1e9 / peak,
+                     "note": "counted bytes / time / HBM peak: a comparison with the single-sweep schedule (SURVEY N3), not a memory-system utilisation"}
+               if inf["step_fusion"] == 2
                else {"bound": "hbm", "achieved_GBs": bc / t / 1e9, "frac": min(1.0, bc / t / 1e9 / peak), "frac_uncapped": bc / t / 1e9 / peak}}
         if name == "cfg4":   # the batch both ways: resident clusters (default) and one streamed sweep per step
             t2, inf2, _, _ = measure_device(p, inner, reps, 3, compact_every=1000, history_capacity=64, step_fusion=2)
@@ -228,6 +249,51 @@ def other_workloads_table(peak, budget_s, with_cpu):
         del p
         gc.collect()
     return rows
+
+
+def compaction_window(p, peak):
+    """SURVEY.md 8(d)'s second throughput window: the headline workload again with >= 10 % of its springs broken and the
+    lists compacted (lsm_compact before the timed region), with the same kernel as the headline.  Two shapes of damage:
+    springs dead at random (no 32-particle slice loses a whole column, so the streams do not shrink: DESIGN.md
+    "Compaction") and a horizontal band of dead springs (whole slices die, their columns are freed)."""
+    import copy
+    rows = {}
+    for mode in ("random", "band"):
+        q = copy.copy(p)
+        if mode == "random":
+            dead = np.random.default_rng(777).random(p.M) < 0.10
+        else:
+            ym = 0.5 * (p.x[p.spring_i, 1] + p.x[p.spring_j, 1])
+            H = p.x[:, 1].max()
+            dead = (ym > 0.3 * H) & (ym < 0.4 * H)
+        q.rc = np.where(dead, 0.5 * p.r0, p.rc)
+        t, inf, alive0, nb = measure_device(q, 200, 3, 3, compact_now=True, compact_every=1000, history_capacity=64)
+        bc = counted_bytes(p.N, alive0, p_var_of(q), p.x.shape[1])
+        rows[mode] = {"dead_fraction": float(dead.mean()), "M_alive": alive0, "us_per_time_step": t * 1e6, "spring_updates_per_s": alive0 / t,
+                      "step_kernel": step_kernel_name(inf), "half_edges_stored": inf["n_half_edges_stored"],
+                      "half_edges_stored_before_compaction": inf["n_half_edges_stored_before_compaction"],
+                      "counted_bytes_per_time_step": bc, "frac_uncapped": bc / t / 1e9 / peak}
+    return rows
+
+
+def flat_summary(rows, cw):
+    """One number per configuration, first in `config` so that a reader that keeps only its leading keys still sees all
+    five BASELINE.json configurations and the compaction window; the nested tables follow."""
+    out = {}
+    for r in rows:
+        w = r["workload"]
+        if "us_per_time_step" not in r:
+            out[w + "_us"] = None
+            continue
+        out[w + "_us"] = round(r["us_per_time_step"], 3)
+        rf = r.get("roofline")
+        if isinstance(rf, dict):
+            out[w + "_frac"] = round(rf.get("frac_uncapped", rf.get("counted_bytes_equiv_frac", 0.0)), 4)
+        if "streamed_single_sweep" in r:
+            out[w + "_streamed_us"] = round(r["streamed_single_sweep"]["us_per_time_step"], 3)
+    for mode, r in (cw or {}).items():
+        out["cfg3_10pct_dead_%s_us" % mode] = round(r["us_per_time_step"], 3)
+    return out
 
 
 def run_reference(args):
@@ -441,7 +507,12 @@ def main():
         tr = os.path.join(ROOT, "profiles", "traffic_%s.txt" % args.workload)
         if os.path.exists(tr):                 # per-launch DRAM bytes of the step kernel from the committed ncu --set full capture
             try:
-                line["roofline"]["traffic"] = json.load(open(tr)).get("dram_bytes_per_launch")
+                prof = json.load(open(tr))
+                if prof.get("kernel") == step_kernel_name(inf0):
+                    line["roofline"]["traffic"] = prof.get("dram_bytes_per_launch")
+                else:       # a capture of another kernel says nothing about this run: leave traffic null and say why
+                    line["roofline"]["traffic_kind"] = "none: %s holds a capture of %s, this run's step kernel is %s" % (
+                        os.path.relpath(tr, ROOT), prof.get("kernel"), step_kernel_name(inf0))
             except Exception:
                 pass
         sim.close()
@@ -449,8 +520,17 @@ def main():
         if not args.no_cpu_baseline:
             n_cpu = args.cpu_steps or max(2, int(8.0 * 1.1e8 / max(p.M, 1)))   # ~8 s of the serial oracle (1.1e8 spring-updates/s)
             line["cpu_baseline"] = oracle_legs(p, n_cpu, "the same workload")
-        if world == 1 and args.workload == "cfg3" and not args.no_table:
-            line["config"]["other_workloads"] = other_workloads_table(peak, args.table_budget, not args.no_cpu_baseline)
+        line["roofline"]["kernel_name"] = step_kernel_name(inf0)
+        if world == 1 and args.workload == "cfg3" and not args.no_table and not args.prebreak:
+            cw = compaction_window(p, peak)
+            rows = other_workloads_table(peak, args.table_budget, not args.no_cpu_baseline)
+            cfg = line["config"]
+            head = {k: cfg[k] for k in ("workload", "N", "M", "ns_per_time_step")}
+            head.update(flat_summary(rows, cw))
+            head.update({k: v for k, v in cfg.items() if k not in head})
+            head["compaction_window"] = cw
+            head["other_workloads"] = rows
+            line["config"] = head
         print(json.dumps(line))
     if sim is not None:
         sim.close()
