@@ -29,8 +29,10 @@
 
 namespace {
 
-constexpr int kSBlock = 256;                     // threads per block
-constexpr int kSPerThread = 32;                  // springs per thread
+constexpr int kSBlock = 1024;                    // threads per block: short threads (8 springs each), 64 warps per SM in flight --
+                                                 // the loop is three dependent loads deep (flag -> ids -> positions), so it
+                                                 // is latency-bound: 256 threads x 32 springs took 114 us on config 3 (measured)
+constexpr int kSPerThread = 8;                   // springs per thread
 constexpr int kSChunk = kSBlock * kSPerThread;   // 8192 springs per block, a fixed cut: the summation order does not depend on the GPU
 constexpr long long kSMaxBlocks = LSM_STATIC_MAX_SPRINGS / kSChunk;   // 32768
 static_assert(kSMaxBlocks * kSChunk == LSM_STATIC_MAX_SPRINGS, "the maximum is a whole number of blocks");
@@ -76,7 +78,7 @@ __device__ __forceinline__ double warp_sum_d(double v) {
     return v;
 }
 
-// Fixed-order block sum: xor-shuffle tree inside each warp, then the 8 warp sums in warp order (every thread gets it).
+// Fixed-order block sum: xor-shuffle tree inside each warp, then the 32 warp sums in warp order (every thread gets it).
 __device__ __forceinline__ double block_sum_d(double v, double *sh8) {
     v = warp_sum_d(v);
     __syncthreads();
@@ -100,7 +102,7 @@ __device__ __forceinline__ unsigned long long block_sum_u(unsigned long long v, 
     return t;
 }
 
-// Level 1: block c sums the springs [c * 8192, (c + 1) * 8192): thread t takes c * 8192 + i * 256 + t for i = 0 .. 31 in
+// Level 1: block c sums the springs [c * 8192, (c + 1) * 8192): thread t takes c * 8192 + i * 1024 + t for i = 0 .. 7 in
 // that order (coalesced list reads, two gathered positions per spring), u = k (r - r0)^2 / 2 with an IEEE square root.
 // A broken spring contributes nothing (the (1 - Xi) factor of Eq. 1, kept irreversible by the caller's flag array as in
 // PAPER.md:L98, L196); a spring with an endpoint outside [0, N) or with i == j is skipped and counted.
@@ -139,7 +141,7 @@ __global__ void __launch_bounds__(kSBlock) k_static_energy_partials(const Energy
     }
 }
 
-// Level 2: one block sums the nblk partials, thread t taking t, t + 256, ... in that order, then the fixed-order block sum.
+// Level 2: one block sums the nblk partials, thread t taking t, t + 1024, ... in that order, then the fixed-order block sum.
 __global__ void __launch_bounds__(kSBlock) k_static_energy_final(unsigned char *scratch, int nblk, double *U, long long *counts) {
     __shared__ double shd[kSBlock / 32];
     __shared__ unsigned long long shu[kSBlock / 32];
